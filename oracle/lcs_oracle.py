@@ -1,0 +1,213 @@
+"""ctypes wrapper of the CPU oracle (oracle/lcs_oracle.c).  TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+import this module.  It never imports the CUDA binding (paper_2209_13775_b200.lcs) and shares no
+code with it.  Argument marshalling only: all arithmetic is in lcs_oracle.c.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "lcs_oracle.c")
+_LIB = os.path.join(_HERE, "liblcs_oracle.so")
+
+
+def build(force: bool = False) -> str:
+    """gcc -O2 -ffp-contract=off -fopenmp -shared -fPIC (no FMA contraction, OpenMP over seeds)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + ".tmp.%d" % os.getpid()
+        subprocess.check_call(["gcc", "-O2", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC",
+                               "-o", tmp, _SRC, "-lm"])
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+class _Field(C.Structure):
+    _fields_ = [("dim", C.c_int32), ("kind", C.c_int32),
+                ("n", C.c_int32 * 3), ("periodic", C.c_int32 * 3),
+                ("origin", C.c_double * 3), ("spacing", C.c_double * 3),
+                ("nv", C.c_int64), ("nc", C.c_int64),
+                ("verts", C.c_void_p), ("cells", C.c_void_p), ("neigh", C.c_void_p),
+                ("ns", C.c_int32), ("vel_f32", C.c_int32),
+                ("times", C.c_void_p), ("vel", C.c_void_p)]
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(build())
+        _lib.orc_eigmax_sym2.restype = C.c_double
+        _lib.orc_eigmax_sym2.argtypes = [C.c_double] * 3
+        _lib.orc_eigmax_sym3.restype = C.c_double
+        _lib.orc_eigmax_sym3.argtypes = [C.c_double] * 6
+        _lib.orc_simplex_build_neighbours.restype = C.c_int
+        _lib.orc_max_threads.restype = C.c_int
+    return _lib
+
+
+def _p(a):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+class OracleField:
+    """Field description for the oracle.  Keeps numpy arrays alive; builds the face-neighbour table
+    of a simplex mesh with the oracle's own routine."""
+
+    def __init__(self, dim, kind, times, vel, n=(1, 1, 1), origin=(0, 0, 0), spacing=(1, 1, 1),
+                 periodic=(0, 0, 0), vertices=None, cells=None):
+        self.dim, self.kind = int(dim), int(kind)
+        self.times = np.ascontiguousarray(times, dtype=np.float64)
+        assert vel.dtype in (np.float32, np.float64)
+        self.vel = np.ascontiguousarray(vel)
+        self.verts = None if vertices is None else np.ascontiguousarray(vertices, dtype=np.float64)
+        self.cells = None if cells is None else np.ascontiguousarray(cells, dtype=np.int32)
+        self.neigh = None
+        f = _Field()
+        f.dim, f.kind = self.dim, self.kind
+        for a in range(3):
+            f.n[a] = int(n[a]) if a < len(n) else 1
+            f.periodic[a] = int(periodic[a]) if a < len(periodic) else 0
+            f.origin[a] = float(origin[a]) if a < len(origin) else 0.0
+            f.spacing[a] = float(spacing[a]) if a < len(spacing) else 1.0
+        if self.kind == 1:
+            f.nv, f.nc = self.verts.shape[0], self.cells.shape[0]
+            self.neigh = np.empty_like(self.cells)
+            rc = lib().orc_simplex_build_neighbours(C.c_int32(self.dim), C.c_int64(f.nc),
+                                                    _p(self.cells), _p(self.neigh))
+            if rc != 0:
+                raise ValueError("mesh error %d" % rc)
+            assert self.vel.shape[1] == f.nv
+        else:
+            f.nv = f.n[0] * f.n[1] * f.n[2]
+            assert self.vel.shape[1] == f.nv, (self.vel.shape, f.nv)
+        f.verts, f.cells, f.neigh = _p(self.verts), _p(self.cells), _p(self.neigh)
+        f.ns = len(self.times)
+        f.vel_f32 = 1 if self.vel.dtype == np.float32 else 0
+        f.times, f.vel = _p(self.times), _p(self.vel)
+        self._f = f
+
+    @classmethod
+    def from_workload(cls, w):
+        return cls(w.dim, w.kind, w.times, w.vel, n=w.n, origin=w.origin, spacing=w.spacing,
+                   periodic=w.periodic, vertices=w.vertices, cells=w.cells)
+
+    # ---- location ---------------------------------------------------------------------------
+    def cart_locate(self, pos):
+        pos = np.ascontiguousarray(pos, dtype=np.float64)
+        n = pos.shape[0]
+        cell = np.empty(n, dtype=np.int32)
+        w = np.zeros((n, self.dim), dtype=np.float64)
+        lib().orc_cart_locate(C.byref(self._f), C.c_int64(n), _p(pos), _p(cell), _p(w))
+        return cell, w
+
+    def locate_brute(self, pos):
+        pos = np.ascontiguousarray(pos, dtype=np.float64)
+        n = pos.shape[0]
+        cell = np.empty(n, dtype=np.int32)
+        count = np.empty(n, dtype=np.int32)
+        lib().orc_simplex_locate_brute(C.byref(self._f), C.c_int64(n), _p(pos), _p(cell), _p(count))
+        return cell, count
+
+    def accepts(self, pos, cell):
+        pos = np.ascontiguousarray(pos, dtype=np.float64)
+        cell = np.ascontiguousarray(cell, dtype=np.int32)
+        ok = np.empty(pos.shape[0], dtype=np.int32)
+        lib().orc_simplex_accepts(C.byref(self._f), C.c_int64(pos.shape[0]), _p(pos), _p(cell), _p(ok))
+        return ok.astype(bool)
+
+    def locate_walk(self, pos, start=None):
+        pos = np.ascontiguousarray(pos, dtype=np.float64)
+        n = pos.shape[0]
+        if start is None:
+            start = self.start_hint(pos)
+        start = np.ascontiguousarray(start, dtype=np.int32)
+        cell = np.empty(n, dtype=np.int32)
+        lib().orc_simplex_locate_walk(C.byref(self._f), C.c_int64(n), _p(pos), _p(start), _p(cell))
+        return cell
+
+    def start_hint(self, pos):
+        """A start cell for the walk: any cell incident on the nearest mesh vertex (scipy cKDTree, a
+        library primitive).  The walk's result does not depend on it (canonical predicate => unique)."""
+        from scipy.spatial import cKDTree
+        if not hasattr(self, "_tree"):
+            self._tree = cKDTree(self.verts)
+            v2c = np.zeros(self.verts.shape[0], dtype=np.int32)
+            ids = np.repeat(np.arange(self.cells.shape[0], dtype=np.int32), self.dim + 1)
+            v2c[self.cells.ravel()] = ids
+            self._v2c = v2c
+        _, nearest = self._tree.query(np.asarray(pos, dtype=np.float64), workers=-1)
+        return self._v2c[nearest]
+
+    def locate(self, pos):
+        """-1 = outside.  Cartesian: O2 formula; simplex: canonical-predicate walk (fast mode)."""
+        if self.kind == 0:
+            return self.cart_locate(pos)[0]
+        return self.locate_walk(pos)
+
+    # ---- interpolation ----------------------------------------------------------------------
+    def velocity(self, pos, t, start=None):
+        pos = np.ascontiguousarray(pos, dtype=np.float64)
+        n = pos.shape[0]
+        if self.kind == 1 and start is None:
+            start = self.start_hint(pos)
+        st = None if start is None else np.ascontiguousarray(start, dtype=np.int32)
+        u = np.empty((n, self.dim), dtype=np.float64)
+        inside = np.empty(n, dtype=np.int32)
+        lib().orc_velocity(C.byref(self._f), C.c_int64(n), _p(pos), C.c_double(t), _p(st), _p(u), _p(inside))
+        return u, inside.astype(bool)
+
+    # ---- RK4 flow map -----------------------------------------------------------------------
+    def advect(self, seeds, t0, tf, h, rec_every=0):
+        seeds = np.ascontiguousarray(seeds, dtype=np.float64)      # fp32 seeds are widened exactly
+        n = seeds.shape[0]
+        cell0 = self.locate_walk(seeds) if self.kind == 1 else None
+        F = np.empty_like(seeds)
+        flag = np.empty(n, dtype=np.uint8)
+        es = np.empty(n, dtype=np.int32)
+        traj = None
+        if rec_every > 0:
+            N = int(round((tf - t0) / h))
+            traj = np.empty((N // rec_every, n, self.dim), dtype=np.float64)
+        lib().orc_advect(C.byref(self._f), C.c_int64(n), _p(seeds), C.c_double(t0), C.c_double(tf),
+                         C.c_double(h), _p(cell0), _p(F), _p(flag), _p(es), C.c_int32(rec_every), _p(traj))
+        if rec_every > 0:
+            return F, flag, es, traj
+        return F, flag, es
+
+
+def cg_ftle(dim, ng, seed_spacing, seed_periodic, period, flowmap, exit_flag, T):
+    """Returns (cg [n][3|6], ftle [n], status [n])."""
+    F = np.ascontiguousarray(flowmap, dtype=np.float64)
+    n = F.shape[0]
+    ng_ = np.asarray(list(ng) + [1] * (3 - len(ng)), dtype=np.int32)
+    dx = np.asarray(list(seed_spacing) + [1.0] * (3 - len(seed_spacing)), dtype=np.float64)
+    sp = np.asarray(list(seed_periodic) + [0] * (3 - len(seed_periodic)), dtype=np.int32)
+    per = np.asarray(list(period) + [0.0] * (3 - len(period)), dtype=np.float64)
+    assert n == int(ng_[0]) * int(ng_[1]) * (int(ng_[2]) if dim == 3 else 1)
+    fl = None if exit_flag is None else np.ascontiguousarray(exit_flag, dtype=np.uint8)
+    cg = np.empty((n, 3 if dim == 2 else 6), dtype=np.float64)
+    ftle = np.empty(n, dtype=np.float64)
+    status = np.empty(n, dtype=np.uint8)
+    lib().orc_cg_ftle(C.c_int32(dim), _p(ng_), _p(dx), _p(sp), _p(per), _p(F), _p(fl), C.c_double(T),
+                      _p(cg), _p(ftle), _p(status))
+    return cg, ftle, status
+
+
+def eigmax_sym2(c11, c12, c22):
+    return lib().orc_eigmax_sym2(c11, c12, c22)
+
+
+def eigmax_sym3(c11, c12, c13, c22, c23, c33):
+    return lib().orc_eigmax_sym3(c11, c12, c13, c22, c23, c33)
+
+
+def max_threads():
+    return int(lib().orc_max_threads())
