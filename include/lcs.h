@@ -1,0 +1,149 @@
+/* lcs.h -- C-ABI of liblcs.so: the B200 (sm_100a) hot path of the LCS pipeline of arXiv 2209.13775.
+ *
+ *   velocity snapshots on a mesh --lcs_field_create/lcs_field_set_snapshot--> resident field
+ *   seeds --lcs_advect (RK4, Eq. 1.2)--> flow map F_{t0}^{tf} + exit flags
+ *   flow map --lcs_cg_ftle (central differences, Eq. 1.1)--> Cauchy-Green tensor C, FTLE
+ *   positions --lcs_locate--> containing mesh cell
+ *
+ * Conventions
+ *  - Plain C, no exceptions or aborts cross the boundary; every call returns an lcs_status and
+ *    lcs_last_error() gives a thread-local message.  A tracer leaving the domain is DATA (flags).
+ *  - "device" pointers are CUDA device pointers of the current device, allocated and owned by the
+ *    caller (the Python binding uses torch tensors); "host" pointers are ordinary memory.  The library
+ *    owns only what lives behind lcs_field (mesh, snapshots, tracer scratch).
+ *  - The hot calls (lcs_locate, lcs_advect, lcs_cg_ftle) are asynchronous on `cuda_stream` (a
+ *    cudaStream_t passed as void*, NULL = default stream); the caller synchronises.
+ *  - Every step of the path runs in CUDA kernels; there is no CPU fallback.
+ * Citations are PAPER.md lines (the paper text) and DESIGN.md readings where the paper is silent.
+ */
+#ifndef LCS_H
+#define LCS_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct lcs_field lcs_field;           /* opaque; owns device copies of mesh + snapshots */
+
+typedef enum {
+    LCS_OK = 0,
+    LCS_ERR_INVALID_ARG = 1,
+    LCS_ERR_TIME_RANGE = 2,                   /* [t0,tf] not inside the snapshot times            */
+    LCS_ERR_MESH = 3,                         /* bad connectivity / index out of range            */
+    LCS_ERR_OOM = 4,
+    LCS_ERR_CUDA = 5,
+    LCS_ERR_NOT_READY = 6                     /* a snapshot needed by the call was never set      */
+} lcs_status;
+
+typedef enum { LCS_F32 = 0, LCS_F64 = 1 } lcs_dtype;
+typedef enum { LCS_MESH_CARTESIAN = 0, LCS_MESH_SIMPLEX = 1 } lcs_mesh_kind;
+
+/* Description of gridded, time-sampled velocity data u(x,t): a Cartesian grid or a
+ * simplicial mesh (triangles / tetrahedra) plus the snapshot times.               */
+typedef struct {
+    int32_t dim;                              /* 2 or 3                                           */
+    int32_t kind;                             /* lcs_mesh_kind                                    */
+    /* Cartesian: n[a] nodes on axis a, node i at origin[a] + i*spacing[a]; periodic[a] != 0 => n[a]
+     * cells on that axis and node n[a] == node 0, else n[a]-1 cells.  Node index = i0 + n0*(i1 + n1*i2). */
+    int32_t n[3];
+    int32_t periodic[3];
+    double origin[3];
+    double spacing[3];
+    /* Simplex: HOST pointers, copied during create.  vertices [n_vertices][dim] fp64; cells
+     * [n_cells][dim+1] int32 of any orientation.  The library builds face adjacency and a uniform bin
+     * grid on the device.                                                                          */
+    int64_t n_vertices;
+    int64_t n_cells;
+    const double *vertices;
+    const int32_t *cells;
+    /* Time: strictly increasing and uniformly spaced, n_snapshots >= 2.  HOST pointer, copied.      */
+    int32_t n_snapshots;
+    int32_t vel_dtype;                        /* lcs_dtype: storage type of the velocity data     */
+    const double *times;
+    int32_t compute_dtype;                    /* lcs_dtype: type of seeds / flow map and of the
+                                                 arithmetic inside lcs_advect                      */
+    int32_t max_resident_snapshots;           /* 0 = keep every snapshot on the device; k >= 3 = ring of
+                                                 k device slots fed from host memory on a side stream
+                                                 (the temporal window of PAPER.md:57, 61, 85)      */
+} lcs_field_desc;
+
+/* Creates the field: uploads the mesh, orients cells, builds adjacency + bins (simplex).  Snapshots are
+ * supplied afterwards.  *out is NULL on error.                                                     */
+lcs_status lcs_field_create(const lcs_field_desc *desc, lcs_field **out);
+
+/* Velocity of snapshot s (0-based), layout [node][dim] of vel_dtype, node order = mesh vertex order
+ * (Cartesian: i0 fastest).  `vel` is a host pointer (pinned memory makes the copy asynchronous) or, with
+ * is_device_ptr != 0, a device pointer.  The data is copied / re-laid-out on the library's side stream;
+ * with max_resident_snapshots == 0 the caller may free `vel` after lcs_field_sync.  In ring mode the
+ * HOST pointer is retained and must stay valid until lcs_field_destroy (snapshots are re-streamed
+ * from it whenever the window moves; "loaded into GPU memory only when a new file is needed"). */
+lcs_status lcs_field_set_snapshot(lcs_field *f, int32_t s, const void *vel, int32_t is_device_ptr);
+lcs_status lcs_field_sync(lcs_field *f);
+void lcs_field_destroy(lcs_field *f);
+
+/* Integer options.  Keys: "integrator" 0 = auto, 1 = fused (one persistent per-seed loop per snapshot
+ * window), 2 = split (one short kernel per RK4 stage, tracers advance synchronously: PAPER.md:85);
+ * "sort_seeds" 0/1 = process tracers in cell order (results are returned in the caller's order);
+ * "resort_every" k = re-bundle tracers by cell every k snapshot windows (0 = never).   */
+lcs_status lcs_field_set_option(lcs_field *f, const char *key, int64_t value);
+lcs_status lcs_field_get_info(const lcs_field *f, const char *key, int64_t *value);
+
+/* Cell containing each position ("computes which cell ... each seed point is located in";
+ * PAPER.md:87 cell search).  pos: device [n][dim] fp64.  cell: device [n] int32, -1 = outside.
+ * Cartesian: arithmetic indexing, cell id = i0 + nc0*(i1 + nc1*i2), upper boundary closed.
+ * Simplex: bin grid -> start cell -> walk across faces with the canonical fp64 face predicate (vertices
+ * of a face sorted by id, every product and sum rounded separately, ties broken as if the point were
+ * p + (eps, eps^2, eps^3)); the result is the unique owner, bit-exact against the oracle.
+ * bary (optional, may be NULL): device [n][dim] Cartesian weights or [n][dim+1] barycentric weights. */
+lcs_status lcs_locate(lcs_field *f, int64_t n, const double *pos, int32_t *cell, double *bary,
+                      void *cuda_stream);
+
+/* Flow map by classical RK4 of dx/dt = u(x,t) (Eq. 1.2) with bi/trilinear or
+ * barycentric interpolation in space and linear interpolation in time between the two bracketing
+ * snapshots.  N = round((tf-t0)/h) steps; h < 0 integrates backward in time.
+ * seeds, flowmap: device [n][dim] of compute_dtype; flowmap may alias seeds.
+ * exit_flag (device [n] u8, may be NULL): 0 = inside the domain up to tf; 1 = left during integration
+ *   (any of the four RK4 evaluation points outside; flowmap = position at the start of that step;
+ *   PAPER.md:65); 2 = seed outside at t0 (flowmap = seed).
+ * exit_step (device [n] i32, may be NULL): completed steps (N for flag 0, 0 for flag 2).
+ * Errors: LCS_ERR_INVALID_ARG if h == 0, sign(h) != sign(tf-t0) or |N*h-(tf-t0)| > 1e-9*|tf-t0|;
+ * LCS_ERR_TIME_RANGE if [t0,tf] leaves [times[0], times[ns-1]] by more than 1e-9 snapshot intervals.   */
+lcs_status lcs_advect(lcs_field *f, int64_t n, const void *seeds, double t0, double tf, double h,
+                      void *flowmap, uint8_t *exit_flag, int32_t *exit_step, void *cuda_stream);
+
+/* Central-difference flow-map gradient G_ab = dF_a/dx_b on the structured seed grid,
+ * Cauchy-Green tensor C = G^T G (Eq. 1.1), its largest eigenvalue (closed form) and
+ * FTLE = ln(lambda_max) / (2|T|), fused in one kernel.
+ * Seed index = i0 + ng0*(i1 + ng1*i2); seed_spacing per axis; seed_periodic[a] != 0 => differences wrap
+ * on that axis, adding +-period[a] to component a of the wrapped neighbour.
+ * flowmap: device [n][dim] of `dtype`; exit_flag: device [n] u8 or NULL (all valid).
+ * A neighbour is valid if it is inside the grid (or reached by wrap) and its flag is 0.  Both valid:
+ * central difference; one valid and the seed valid: one-sided, status bit 1; seed invalid or no valid
+ * neighbour on some axis: C, FTLE = NaN, status bit 0.
+ * cg: device [n][3] (C11,C12,C22) or [n][6] (C11,C12,C13,C22,C23,C33) of `dtype`, may be NULL.
+ * ftle: device [n] of `dtype`.  status: device [n] u8, may be NULL.  Arithmetic is fp64 throughout. */
+lcs_status lcs_cg_ftle(int32_t dim, int32_t dtype, const int32_t ng[3], const double seed_spacing[3],
+                       const int32_t seed_periodic[3], const double period[3],
+                       const void *flowmap, const uint8_t *exit_flag, double T,
+                       void *cg, void *ftle, uint8_t *status, void *cuda_stream);
+
+/* End-to-end convenience with HOST buffers: copies the seeds to the device, runs lcs_advect and
+ * lcs_cg_ftle and copies flow map (optional), flags (optional) and FTLE back; synchronous.
+ * seeds_host/flowmap_host: [n][dim] of the field's compute_dtype; ftle_host: [n] of compute_dtype.
+ * Pinned host memory makes the copies asynchronous with respect to each other.                      */
+lcs_status lcs_ftle_host(lcs_field *f, const int32_t ng[3], const double seed_spacing[3],
+                         const int32_t seed_periodic[3], const double period[3],
+                         const void *seeds_host, double t0, double tf, double h,
+                         void *flowmap_host, uint8_t *exit_flag_host, void *ftle_host);
+
+/* Number of kernels this library has launched in this process (bench.py's gpu_launches).           */
+int64_t lcs_kernel_launch_count(void);
+
+const char *lcs_last_error(void);             /* thread-local, static storage                       */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LCS_H */

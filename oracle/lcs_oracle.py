@@ -1,8 +1,8 @@
 """ctypes wrapper of the CPU oracle (oracle/lcs_oracle.c).  TEST INFRASTRUCTURE ONLY.
 
-Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
-import this module.  It never imports the CUDA binding (paper_2209_13775_b200.lcs) and shares no
-code with it.  Argument marshalling only: all arithmetic is in lcs_oracle.c.
+Allowed users of this module: tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+--impl reference legs, nothing else.  The CUDA binding (paper_2209_13775_b200.lcs) is never loaded
+from here and no code is shared with it.  Argument marshalling only: all arithmetic is in lcs_oracle.c.
 """
 from __future__ import annotations
 

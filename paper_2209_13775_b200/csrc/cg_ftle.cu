@@ -1,0 +1,141 @@
+// cg_ftle.cu -- fused finite-difference gradient (row a5), Cauchy-Green tensor and closed-form largest
+// eigenvalue / FTLE (row a6) on the structured seed grid, for sm_100a.
+//
+// Paper: "standard central difference formula for the flow map gradient" on the seed grid;
+// C = grad F^T grad F (Eq. 1.1); FTLE from the largest eigenvalue of C.
+// The paper does not describe a GPU kernel for this stage (its GPU section covers the flow map only);
+// here it is one HBM-streaming kernel: every flow-map element is read from DRAM once (the 2*dim stencil
+// reads of neighbouring threads hit L1/L2), all arithmetic is fp64 (once per seed, far below the
+// streaming time), outputs are written once.
+#include <math.h>
+
+#include "lcs_internal.cuh"
+
+namespace {
+
+struct CgGrid {
+    int ng[3];
+    int per[3];
+    double inv_dx[3];     // 1/dx
+    double period[3];
+    double inv_2T;        // 1 / (2|T|)
+};
+
+__device__ __forceinline__ double eigmax_sym2(double c11, double c12, double c22)
+{
+    double hd = 0.5 * (c11 - c22);
+    return 0.5 * (c11 + c22) + sqrt(hd * hd + c12 * c12);
+}
+
+// trigonometric closed form for the largest eigenvalue of a symmetric 3x3 matrix
+__device__ __forceinline__ double eigmax_sym3(double c11, double c12, double c13, double c22, double c23, double c33)
+{
+    double q = (c11 + c22 + c33) / 3.0;
+    double p1 = c12 * c12 + c13 * c13 + c23 * c23;
+    double d1 = c11 - q, d2 = c22 - q, d3 = c33 - q;
+    double p2 = d1 * d1 + d2 * d2 + d3 * d3 + 2.0 * p1;
+    if (p2 == 0.0) return q;
+    double p = sqrt(p2 / 6.0);
+    double ip = 1.0 / p;
+    double b11 = d1 * ip, b22 = d2 * ip, b33 = d3 * ip, b12 = c12 * ip, b13 = c13 * ip, b23 = c23 * ip;
+    double det = b11 * (b22 * b33 - b23 * b23) - b12 * (b12 * b33 - b23 * b13) + b13 * (b12 * b23 - b22 * b13);
+    double r = fmin(1.0, fmax(-1.0, 0.5 * det));
+    return q + 2.0 * p * cos(acos(r) / 3.0);
+}
+
+template <int DIM, typename T>
+__global__ void __launch_bounds__(256) cg_ftle_kernel(const __grid_constant__ CgGrid g, const T *__restrict__ F,
+                                                       const uint8_t *__restrict__ flag, T *__restrict__ cg,
+                                                       T *__restrict__ ftle, uint8_t *__restrict__ status, int64_t n)
+{
+    int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= n) return;
+    const int64_t n0 = g.ng[0], n1 = g.ng[1];
+    int ijk[3] = {(int)(idx % n0), (int)((idx / n0) % n1), (int)(idx / (n0 * n1))};
+    const int64_t stride[3] = {1, n0, n0 * n1};
+    constexpr int NCG = (DIM == 2) ? 3 : 6;
+    uint8_t st = 0;
+    if (flag && flag[idx] != 0) st = 1;
+    double F0[DIM];
+#pragma unroll
+    for (int a = 0; a < DIM; ++a) F0[a] = (double)F[idx * DIM + a];
+    double G[DIM][DIM];
+#pragma unroll
+    for (int b = 0; b < DIM; ++b) {
+        int ip = ijk[b] + 1, im = ijk[b] - 1;
+        double shp = 0.0, shm = 0.0;
+        bool okp = true, okm = true;
+        if (ip >= g.ng[b]) { if (g.per[b]) { ip -= g.ng[b]; shp = g.period[b]; } else okp = false; }
+        if (im < 0) { if (g.per[b]) { im += g.ng[b]; shm = -g.period[b]; } else okm = false; }
+        int64_t jp = idx + (int64_t)(ip - ijk[b]) * stride[b], jm = idx + (int64_t)(im - ijk[b]) * stride[b];
+        if (okp && flag && flag[jp] != 0) okp = false;
+        if (okm && flag && flag[jm] != 0) okm = false;
+#pragma unroll
+        for (int a = 0; a < DIM; ++a) {
+            double Fp = okp ? (double)F[jp * DIM + a] + (a == b ? shp : 0.0) : 0.0;
+            double Fm = okm ? (double)F[jm * DIM + a] + (a == b ? shm : 0.0) : 0.0;
+            double v = 0.0;
+            if (okp && okm) v = (Fp - Fm) * (0.5 * g.inv_dx[b]);
+            else if (okp) v = (Fp - F0[a]) * g.inv_dx[b];
+            else if (okm) v = (F0[a] - Fm) * g.inv_dx[b];
+            G[a][b] = v;
+        }
+        if (!okp && !okm) st |= 1;
+        else if (!(okp && okm)) st |= 2;
+    }
+    double C[NCG], lam;
+    if (st & 1) {
+#pragma unroll
+        for (int i = 0; i < NCG; ++i) C[i] = nan("");
+        lam = nan("");
+    } else if constexpr (DIM == 2) {
+        C[0] = G[0][0] * G[0][0] + G[1][0] * G[1][0];
+        C[1] = G[0][0] * G[0][1] + G[1][0] * G[1][1];
+        C[2] = G[0][1] * G[0][1] + G[1][1] * G[1][1];
+        lam = eigmax_sym2(C[0], C[1], C[2]);
+    } else {
+        int m = 0;
+#pragma unroll
+        for (int b = 0; b < 3; ++b)
+#pragma unroll
+            for (int c = b; c < 3; ++c) C[m++] = G[0][b] * G[0][c] + G[1][b] * G[1][c] + G[2][b] * G[2][c];
+        lam = eigmax_sym3(C[0], C[1], C[2], C[3], C[4], C[5]);
+    }
+    if (cg) {
+#pragma unroll
+        for (int i = 0; i < NCG; ++i) cg[idx * NCG + i] = (T)C[i];
+    }
+    ftle[idx] = (st & 1) ? (T)nan("") : (T)(log(lam) * g.inv_2T);
+    if (status) status[idx] = st;
+}
+
+}  // namespace
+
+extern "C" lcs_status lcs_cg_ftle(int32_t dim, int32_t dtype, const int32_t ng[3], const double seed_spacing[3],
+                                  const int32_t seed_periodic[3], const double period[3], const void *flowmap,
+                                  const uint8_t *exit_flag, double T, void *cg, void *ftle, uint8_t *status, void *cuda_stream)
+{
+    if ((dim != 2 && dim != 3) || !ng || !seed_spacing || !flowmap || !ftle) { lcs_set_error("null argument or bad dim"); return LCS_ERR_INVALID_ARG; }
+    if (dtype != LCS_F32 && dtype != LCS_F64) { lcs_set_error("bad dtype"); return LCS_ERR_INVALID_ARG; }
+    if (!(T != 0.0) || !isfinite(T)) { lcs_set_error("T must be finite and non-zero"); return LCS_ERR_INVALID_ARG; }
+    CgGrid g;
+    int64_t n = 1;
+    for (int a = 0; a < 3; ++a) {
+        g.ng[a] = a < dim ? ng[a] : 1;
+        g.per[a] = (a < dim && seed_periodic) ? (seed_periodic[a] != 0) : 0;
+        g.period[a] = (a < dim && period) ? period[a] : 0.0;
+        if (a < dim && (ng[a] < 1 || !(seed_spacing[a] > 0))) { lcs_set_error("bad seed grid on axis %d", a); return LCS_ERR_INVALID_ARG; }
+        g.inv_dx[a] = a < dim ? 1.0 / seed_spacing[a] : 1.0;
+        n *= g.ng[a];
+    }
+    g.inv_2T = 1.0 / (2.0 * fabs(T));
+    if (n == 0) return LCS_OK;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const unsigned grid = lcs_blocks(n, 256);
+    if (dim == 2 && dtype == LCS_F64) LCS_LAUNCH((cg_ftle_kernel<2, double>), grid, 256, 0, st, g, (const double *)flowmap, exit_flag, (double *)cg, (double *)ftle, status, n);
+    else if (dim == 2) LCS_LAUNCH((cg_ftle_kernel<2, float>), grid, 256, 0, st, g, (const float *)flowmap, exit_flag, (float *)cg, (float *)ftle, status, n);
+    else if (dtype == LCS_F64) LCS_LAUNCH((cg_ftle_kernel<3, double>), grid, 256, 0, st, g, (const double *)flowmap, exit_flag, (double *)cg, (double *)ftle, status, n);
+    else LCS_LAUNCH((cg_ftle_kernel<3, float>), grid, 256, 0, st, g, (const float *)flowmap, exit_flag, (float *)cg, (float *)ftle, status, n);
+    LCS_CUDA_OK(cudaGetLastError());
+    return LCS_OK;
+}

@@ -1,0 +1,426 @@
+// field.cu -- lcs_field life cycle, the resident snapshot window (row a0), window planning and the
+// C-ABI entry points that dispatch to the Cartesian / simplex kernels.
+//
+// Snapshot window (PAPER.md:57 Cache filter, "a window of velocity data frames (nominally two
+// ...) are loaded on the GPU's memory", "velocity data is loaded into GPU memory only every
+// time a new velocity data file is needed"): raw snapshots live in device slots (all of them, or a ring of
+// k fed from host memory on a side stream); the two snapshots bracketing the current window are fused
+// into one "pair record" array {a, b-a} per node that the integrator kernels gather from.
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+
+#include "lcs_internal.cuh"
+
+std::atomic<int64_t> g_lcs_launches{0};
+static thread_local char g_err[512] = "";
+
+void lcs_set_error(const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof g_err, fmt, ap);
+    va_end(ap);
+}
+
+extern "C" const char *lcs_last_error(void) { return g_err; }
+extern "C" int64_t lcs_kernel_launch_count(void) { return g_lcs_launches.load(); }
+
+// ---------------------------------------------------------------------------------------------
+// pair-record build: rec[node] = { a[0..dim), 0.., (b-a)[0..dim), 0.. }   (HBM streaming, once per window)
+// TV = storage type of the raw snapshot, TR = record type = the wider of storage and compute type, so that with
+// fp32 data and fp64 arithmetic the difference b - a is formed in fp64 exactly as the oracle forms it.
+template <int DIM, typename TV, typename TR>
+__global__ void __launch_bounds__(256) build_pair_kernel(const TV *__restrict__ a, const TV *__restrict__ b,
+                                                          PairRec<DIM, TR> *__restrict__ rec, int64_t nnodes)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= nnodes) return;
+    PairRec<DIM, TR> r;
+#pragma unroll
+    for (int c = 0; c < PadOf<DIM>::P; ++c) {
+        TR va = (c < DIM) ? (TR)a[i * DIM + c] : TR(0);
+        TR vb = (c < DIM) ? (TR)b[i * DIM + c] : TR(0);
+        r.a[c] = va;
+        r.d[c] = vb - va;
+    }
+    rec[i] = r;
+}
+
+static int rec_dtype(const lcs_field *f) { return (f->vel_dtype == LCS_F64 || f->compute_dtype == LCS_F64) ? LCS_F64 : LCS_F32; }
+static size_t pair_bytes(const lcs_field *f) { return (size_t)f->nnodes * 2 * f->P * lcs_esize(rec_dtype(f)); }
+static size_t raw_bytes(const lcs_field *f) { return (size_t)f->nnodes * f->dim * lcs_esize(f->vel_dtype); }
+
+// Makes snapshot s resident in some raw slot (enqueueing the upload on the side stream if needed) and
+// returns the slot.  `keep0/keep1` are snapshots that must not be evicted.
+static lcs_status ensure_slot(lcs_field *f, int s, int keep0, int keep1, int *slot_out)
+{
+    if (s < 0 || s >= f->ns) { lcs_set_error("snapshot %d out of range", s); return LCS_ERR_INVALID_ARG; }
+    if (!f->snap_set[s]) { lcs_set_error("snapshot %d was never set", s); return LCS_ERR_NOT_READY; }
+    if (f->snap_slot[s] >= 0) { *slot_out = f->snap_slot[s]; return LCS_OK; }
+    // ring mode only: pick an empty slot, else the resident snapshot farthest from s
+    int best = -1, best_d = -1;
+    for (int k = 0; k < f->nslots; ++k) {
+        int held = f->slot_snap[k];
+        if (held < 0) { best = k; break; }
+        if (held == keep0 || held == keep1) continue;
+        int d = abs(held - s);
+        if (d > best_d) { best_d = d; best = k; }
+    }
+    if (best < 0) { lcs_set_error("no free snapshot slot"); return LCS_ERR_INVALID_ARG; }
+    if (f->slot_snap[best] >= 0) f->snap_slot[f->slot_snap[best]] = -1;
+    if (!f->slot[best]) LCS_CUDA_OK(cudaMalloc(&f->slot[best], raw_bytes(f)));
+    // do not overwrite the slot before its last reader (a pair build on the compute stream) is done
+    if (f->slot_free_valid[best]) LCS_CUDA_OK(cudaStreamWaitEvent(f->side, f->slot_free[best], 0));
+    LCS_CUDA_OK(cudaMemcpyAsync(f->slot[best], f->host_src[s], raw_bytes(f), cudaMemcpyHostToDevice, f->side));
+    LCS_CUDA_OK(cudaEventRecord(f->slot_ready[best], f->side));
+    f->info_h2d_bytes += (int64_t)raw_bytes(f);
+    f->slot_snap[best] = s;
+    f->snap_slot[s] = best;
+    *slot_out = best;
+    return LCS_OK;
+}
+
+lcs_status lcs_field_prefetch(lcs_field *f, int s)
+{
+    if (!f->ring || s < 0 || s >= f->ns || !f->snap_set[s]) return LCS_OK;
+    int slot;
+    // keep the neighbours of s (the pair that is most likely in use)
+    return ensure_slot(f, s, s - 1, s + 1, &slot);
+}
+
+template <int DIM, typename TV, typename TR>
+static void launch_build_pair(const void *a, const void *b, void *rec, int64_t nnodes, cudaStream_t st)
+{
+    LCS_LAUNCH((build_pair_kernel<DIM, TV, TR>), lcs_blocks(nnodes, 256), 256, 0, st, (const TV *)a, (const TV *)b,
+               (PairRec<DIM, TR> *)rec, nnodes);
+}
+
+lcs_status lcs_field_require_pair(lcs_field *f, int s, cudaStream_t st, const void **pair)
+{
+    if (s < 0 || s + 1 >= f->ns) { lcs_set_error("pair %d out of range", s); return LCS_ERR_INVALID_ARG; }
+    f->pair_clock++;
+    for (int k = 0; k < lcs_field::kPairCache; ++k)
+        if (f->pair_snap[k] == s && f->pair_buf[k]) { f->pair_age[k] = f->pair_clock; *pair = f->pair_buf[k]; return LCS_OK; }
+    int s0, s1;
+    lcs_status rc = ensure_slot(f, s, s, s + 1, &s0);
+    if (rc != LCS_OK) return rc;
+    rc = ensure_slot(f, s + 1, s, s + 1, &s1);
+    if (rc != LCS_OK) return rc;
+    int k = 0;
+    for (int j = 1; j < lcs_field::kPairCache; ++j)
+        if (f->pair_age[j] < f->pair_age[k]) k = j;
+    if (!f->pair_buf[k]) LCS_CUDA_OK(cudaMalloc(&f->pair_buf[k], pair_bytes(f)));
+    LCS_CUDA_OK(cudaStreamWaitEvent(st, f->slot_ready[s0], 0));
+    LCS_CUDA_OK(cudaStreamWaitEvent(st, f->slot_ready[s1], 0));
+    const bool v64 = f->vel_dtype == LCS_F64, r64 = rec_dtype(f) == LCS_F64;
+    const void *A = f->slot[s0], *B = f->slot[s1];
+    void *R = f->pair_buf[k];
+    if (f->dim == 2) {
+        if (v64) launch_build_pair<2, double, double>(A, B, R, f->nnodes, st);
+        else if (r64) launch_build_pair<2, float, double>(A, B, R, f->nnodes, st);
+        else launch_build_pair<2, float, float>(A, B, R, f->nnodes, st);
+    } else {
+        if (v64) launch_build_pair<3, double, double>(A, B, R, f->nnodes, st);
+        else if (r64) launch_build_pair<3, float, double>(A, B, R, f->nnodes, st);
+        else launch_build_pair<3, float, float>(A, B, R, f->nnodes, st);
+    }
+    LCS_CUDA_OK(cudaGetLastError());
+    if (f->ring) {
+        LCS_CUDA_OK(cudaEventRecord(f->slot_free[s0], st));
+        LCS_CUDA_OK(cudaEventRecord(f->slot_free[s1], st));
+        f->slot_free_valid[s0] = f->slot_free_valid[s1] = 1;
+    }
+    f->pair_snap[k] = s;
+    f->pair_age[k] = f->pair_clock;
+    *pair = f->pair_buf[k];
+    return LCS_OK;
+}
+
+lcs_status lcs_scratch_reserve(lcs_field *f, size_t bytes)
+{
+    if (f->scratch.bytes >= bytes) return LCS_OK;
+    if (f->scratch.buf) { cudaDeviceSynchronize(); cudaFree(f->scratch.buf); f->scratch.buf = nullptr; f->scratch.bytes = 0; }
+    LCS_CUDA_OK(cudaMalloc(&f->scratch.buf, bytes));
+    f->scratch.bytes = bytes;
+    return LCS_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Window plan.  Stage times by multiplication (DESIGN reading #16): ta = t0 + n h, tb = t0 + (n+1/2) h,
+// tc = t0 + (n+1) h.  The snapshot interval is that of the step's midpoint when both ends lie in it (to a
+// tolerance of 1e-9 intervals: a stage time that lands on a snapshot is evaluated with tau = 1 in the
+// earlier interval instead of tau = 0 in the later one -- the same value, reading #17); otherwise each
+// stage time takes its own interval s = clamp(floor((t - times[0]) / dt), 0, ns-2) as the oracle does.
+lcs_status lcs_plan_windows(const lcs_field *f, double t0, double h, int64_t N, std::vector<StepWindow> &windows,
+                            std::vector<double> &tau)
+{
+    const double T0 = f->times[0], dt = f->dt_snap, eps = 1e-9 * dt;
+    auto bracket = [&](double t) {
+        double q = floor((t - T0) / dt);
+        int s = q < 0.0 ? 0 : (q > (double)(f->ns - 2) ? f->ns - 2 : (int)q);
+        return s;
+    };
+    windows.clear();
+    tau.resize((size_t)3 * N);
+    for (int64_t n = 0; n < N; ++n) {
+        double t[3] = {t0 + (double)n * h, t0 + ((double)n + 0.5) * h, t0 + ((double)n + 1.0) * h};
+        int sm = bracket(t[1]);
+        double lo = f->times[sm] - eps, hi = f->times[sm + 1] + eps;
+        int s[3];
+        if (t[0] >= lo && t[0] <= hi && t[2] >= lo && t[2] <= hi) s[0] = s[1] = s[2] = sm;
+        else for (int k = 0; k < 3; ++k) s[k] = bracket(t[k]);
+        for (int k = 0; k < 3; ++k) tau[3 * n + k] = (t[k] - f->times[s[k]]) / (f->times[s[k] + 1] - f->times[s[k]]);
+        if (!windows.empty()) {
+            StepWindow &w = windows.back();
+            if (w.s[0] == s[0] && w.s[1] == s[1] && w.s[2] == s[2] && w.count < (1 << 30)) { w.count++; continue; }
+        }
+        StepWindow w;
+        w.first = n; w.count = 1; w.s[0] = s[0]; w.s[1] = s[1]; w.s[2] = s[2];
+        windows.push_back(w);
+    }
+    return LCS_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+extern "C" lcs_status lcs_field_create(const lcs_field_desc *d, lcs_field **out)
+{
+    if (out) *out = nullptr;
+    if (!d || !out) { lcs_set_error("null argument"); return LCS_ERR_INVALID_ARG; }
+    if (d->dim != 2 && d->dim != 3) { lcs_set_error("dim must be 2 or 3"); return LCS_ERR_INVALID_ARG; }
+    if (d->kind != LCS_MESH_CARTESIAN && d->kind != LCS_MESH_SIMPLEX) { lcs_set_error("bad mesh kind"); return LCS_ERR_INVALID_ARG; }
+    if (d->n_snapshots < 2 || !d->times) { lcs_set_error("need >= 2 snapshot times"); return LCS_ERR_INVALID_ARG; }
+    if ((d->vel_dtype != LCS_F32 && d->vel_dtype != LCS_F64) || (d->compute_dtype != LCS_F32 && d->compute_dtype != LCS_F64)) {
+        lcs_set_error("bad dtype"); return LCS_ERR_INVALID_ARG;
+    }
+    if (d->max_resident_snapshots != 0 && d->max_resident_snapshots < 3) {
+        lcs_set_error("max_resident_snapshots must be 0 or >= 3"); return LCS_ERR_INVALID_ARG;
+    }
+    double dt = d->times[1] - d->times[0];
+    if (!(dt > 0)) { lcs_set_error("times must increase"); return LCS_ERR_INVALID_ARG; }
+    for (int s = 1; s < d->n_snapshots; ++s)
+        if (fabs((d->times[s] - d->times[s - 1]) - dt) > 1e-9 * dt) { lcs_set_error("snapshot times must be uniformly spaced"); return LCS_ERR_INVALID_ARG; }
+
+    int dev_count = 0;
+    if (cudaGetDeviceCount(&dev_count) != cudaSuccess || dev_count == 0) {
+        lcs_set_error("no CUDA device: liblcs has no CPU fallback");
+        return LCS_ERR_CUDA;
+    }
+    lcs_field *f = new (std::nothrow) lcs_field();
+    if (!f) return LCS_ERR_OOM;
+    f->dim = d->dim; f->kind = d->kind; f->vel_dtype = d->vel_dtype; f->compute_dtype = d->compute_dtype;
+    f->P = (d->dim == 2) ? 2 : 4;
+    f->times.assign(d->times, d->times + d->n_snapshots);
+    f->dt_snap = dt;
+    f->ns = d->n_snapshots;
+    lcs_status rc = LCS_OK;
+    if (d->kind == LCS_MESH_CARTESIAN) {
+        int64_t nn = 1;
+        for (int a = 0; a < 3; ++a) {
+            int32_t na = (a < d->dim) ? d->n[a] : 1;
+            if (a < d->dim && (na < 2 || !(d->spacing[a] > 0))) { lcs_set_error("bad Cartesian grid on axis %d", a); delete f; return LCS_ERR_INVALID_ARG; }
+            f->cart.n[a] = na;
+            f->cart.periodic[a] = (a < d->dim) ? (d->periodic[a] != 0) : 0;
+            f->cart.pow2[a] = (na & (na - 1)) == 0;
+            f->cart.origin[a] = (a < d->dim) ? d->origin[a] : 0.0;
+            f->cart.spacing[a] = (a < d->dim) ? d->spacing[a] : 1.0;
+            f->cart.inv[a] = 1.0 / f->cart.spacing[a];
+            nn *= na;
+        }
+        if (nn >= (1LL << 31)) { lcs_set_error("grid too large for int32 node ids"); delete f; return LCS_ERR_INVALID_ARG; }
+        f->nnodes = nn;
+    } else {
+        if (d->n_vertices < d->dim + 1 || d->n_cells < 1 || !d->vertices || !d->cells || d->n_vertices >= (1LL << 31) ||
+            d->n_cells >= (1LL << 31) / (d->dim + 1)) {
+            lcs_set_error("bad simplex mesh sizes / null pointers"); delete f; return LCS_ERR_INVALID_ARG;
+        }
+        f->nnodes = d->n_vertices;
+        f->mesh.nv = d->n_vertices; f->mesh.nc = d->n_cells;
+        rc = lcs_simplex_build(f, d->vertices, d->cells);
+        if (rc != LCS_OK) { lcs_field_destroy(f); return rc; }
+    }
+    f->ring = d->max_resident_snapshots != 0 && d->max_resident_snapshots < d->n_snapshots;
+    f->nslots = f->ring ? d->max_resident_snapshots : d->n_snapshots;
+    f->slot.assign(f->nslots, nullptr);
+    f->slot_snap.assign(f->nslots, -1);
+    f->slot_ready.assign(f->nslots, nullptr);
+    f->slot_free.assign(f->nslots, nullptr);
+    f->slot_free_valid.assign(f->nslots, 0);
+    f->snap_slot.assign(f->ns, -1);
+    f->snap_set.assign(f->ns, 0);
+    f->host_src.assign(f->ns, nullptr);
+    cudaError_t e = cudaStreamCreateWithFlags(&f->side, cudaStreamNonBlocking);
+    for (int k = 0; k < f->nslots && e == cudaSuccess; ++k) {
+        e = cudaEventCreateWithFlags(&f->slot_ready[k], cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&f->slot_free[k], cudaEventDisableTiming);
+    }
+    if (e != cudaSuccess) { lcs_set_error("stream/event creation failed: %s", cudaGetErrorString(e)); lcs_field_destroy(f); return LCS_ERR_CUDA; }
+    *out = f;
+    return LCS_OK;
+}
+
+extern "C" void lcs_field_destroy(lcs_field *f)
+{
+    if (!f) return;
+    cudaDeviceSynchronize();
+    for (void *p : f->slot) if (p) cudaFree(p);
+    for (cudaEvent_t ev : f->slot_ready) if (ev) cudaEventDestroy(ev);
+    for (cudaEvent_t ev : f->slot_free) if (ev) cudaEventDestroy(ev);
+    for (cudaEvent_t ev : f->win_ev) cudaEventDestroy(ev);
+    for (int k = 0; k < lcs_field::kPairCache; ++k) if (f->pair_buf[k]) cudaFree(f->pair_buf[k]);
+    if (f->scratch.buf) cudaFree(f->scratch.buf);
+    if (f->h_seeds) cudaFree(f->h_seeds);
+    if (f->h_flow) cudaFree(f->h_flow);
+    if (f->h_ftle) cudaFree(f->h_ftle);
+    if (f->h_flag) cudaFree(f->h_flag);
+    lcs_simplex_free(f);
+    if (f->side) cudaStreamDestroy(f->side);
+    delete f;
+}
+
+extern "C" lcs_status lcs_field_set_snapshot(lcs_field *f, int32_t s, const void *vel, int32_t is_device_ptr)
+{
+    if (!f || !vel) { lcs_set_error("null argument"); return LCS_ERR_INVALID_ARG; }
+    if (s < 0 || s >= f->ns) { lcs_set_error("snapshot index %d out of range", s); return LCS_ERR_INVALID_ARG; }
+    // any cached pair built from the old contents is stale
+    for (int k = 0; k < lcs_field::kPairCache; ++k)
+        if (f->pair_snap[k] == s || f->pair_snap[k] == s - 1) f->pair_snap[k] = -1;
+    if (f->ring) {
+        if (is_device_ptr) { lcs_set_error("ring mode streams snapshots from HOST memory"); return LCS_ERR_INVALID_ARG; }
+        f->host_src[s] = vel;
+        f->snap_set[s] = 1;
+        if (f->snap_slot[s] >= 0) { f->slot_snap[f->snap_slot[s]] = -1; f->snap_slot[s] = -1; }
+        return LCS_OK;
+    }
+    if (!f->slot[s]) LCS_CUDA_OK(cudaMalloc(&f->slot[s], raw_bytes(f)));
+    LCS_CUDA_OK(cudaMemcpyAsync(f->slot[s], vel, raw_bytes(f), is_device_ptr ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, f->side));
+    LCS_CUDA_OK(cudaEventRecord(f->slot_ready[s], f->side));
+    if (!is_device_ptr) f->info_h2d_bytes += (int64_t)raw_bytes(f);
+    f->slot_snap[s] = s;
+    f->snap_slot[s] = s;
+    f->snap_set[s] = 1;
+    return LCS_OK;
+}
+
+extern "C" lcs_status lcs_field_sync(lcs_field *f)
+{
+    if (!f) { lcs_set_error("null field"); return LCS_ERR_INVALID_ARG; }
+    LCS_CUDA_OK(cudaStreamSynchronize(f->side));
+    return LCS_OK;
+}
+
+extern "C" lcs_status lcs_field_set_option(lcs_field *f, const char *key, int64_t value)
+{
+    if (!f || !key) { lcs_set_error("null argument"); return LCS_ERR_INVALID_ARG; }
+    if (!strcmp(key, "integrator") && value >= 0 && value <= 2) f->opt_integrator = value;
+    else if (!strcmp(key, "sort_seeds") && (value == 0 || value == 1)) f->opt_sort_seeds = value;
+    else if (!strcmp(key, "resort_every") && value >= 0) f->opt_resort_every = value;
+    else if (!strcmp(key, "time_windows") && (value == 0 || value == 1)) { f->opt_time_windows = value; f->win_ev_used = 0; }
+    else if (!strcmp(key, "block") && (value == 0 || (value >= 32 && value <= 1024 && value % 32 == 0))) f->opt_block = value;
+    else { lcs_set_error("unknown option or bad value: %s=%lld", key, (long long)value); return LCS_ERR_INVALID_ARG; }
+    return LCS_OK;
+}
+
+extern "C" lcs_status lcs_field_get_info(const lcs_field *f, const char *key, int64_t *value)
+{
+    if (!f || !key || !value) { lcs_set_error("null argument"); return LCS_ERR_INVALID_ARG; }
+    if (!strcmp(key, "windows")) *value = f->info_windows;
+    else if (!strcmp(key, "h2d_bytes")) *value = f->info_h2d_bytes;
+    else if (!strcmp(key, "n_nodes")) *value = f->nnodes;
+    else if (!strcmp(key, "n_cells")) *value = f->kind == LCS_MESH_SIMPLEX ? f->mesh.nc : 0;
+    else if (!strcmp(key, "n_bins")) *value = f->kind == LCS_MESH_SIMPLEX ? (int64_t)f->mesh.nb[0] * f->mesh.nb[1] * f->mesh.nb[2] : 0;
+    else if (!strcmp(key, "ring")) *value = f->ring;
+    else if (!strcmp(key, "window_launches")) *value = (int64_t)(f->win_ev_used / 2);
+    else if (!strcmp(key, "window_time_ns")) {          // synchronises; sum of the bracketed launch durations
+        double ms = 0.0;
+        for (size_t k = 0; k + 1 < f->win_ev_used; k += 2) {
+            float e = 0.f;
+            if (cudaEventSynchronize(f->win_ev[k + 1]) != cudaSuccess || cudaEventElapsedTime(&e, f->win_ev[k], f->win_ev[k + 1]) != cudaSuccess) {
+                lcs_set_error("window timing events not complete"); return LCS_ERR_CUDA;
+            }
+            ms += e;
+        }
+        *value = (int64_t)(ms * 1e6);
+    }
+    else if (!strcmp(key, "n_boundary_faces")) {
+        *value = 0;
+        if (f->kind == LCS_MESH_SIMPLEX) {
+            std::vector<int32_t> nb((size_t)f->mesh.nc * (f->dim + 1));
+            cudaMemcpy(nb.data(), f->mesh.neigh, nb.size() * 4, cudaMemcpyDeviceToHost);
+            int64_t c = 0;
+            for (int32_t v : nb) c += (v < 0);
+            *value = c;
+        }
+    } else { lcs_set_error("unknown info key %s", key); return LCS_ERR_INVALID_ARG; }
+    return LCS_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+extern "C" lcs_status lcs_locate(lcs_field *f, int64_t n, const double *pos, int32_t *cell, double *bary, void *cuda_stream)
+{
+    if (!f || n < 0 || (n > 0 && (!pos || !cell))) { lcs_set_error("null argument"); return LCS_ERR_INVALID_ARG; }
+    if (n == 0) return LCS_OK;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    return f->kind == LCS_MESH_CARTESIAN ? lcs_cart_locate(f, n, pos, cell, bary, st) : lcs_simplex_locate(f, n, pos, cell, bary, st);
+}
+
+static lcs_status check_interval(const lcs_field *f, double t0, double tf, double h, int64_t *N)
+{
+    if (!(h != 0.0) || !isfinite(h) || !isfinite(t0) || !isfinite(tf)) { lcs_set_error("h must be finite and non-zero"); return LCS_ERR_INVALID_ARG; }
+    double T = tf - t0;
+    if (T == 0.0 || (T > 0) != (h > 0)) { lcs_set_error("sign(h) must equal sign(tf - t0)"); return LCS_ERR_INVALID_ARG; }
+    int64_t n = llround(T / h);
+    if (n < 1 || fabs((double)n * h - T) > 1e-9 * fabs(T)) { lcs_set_error("(tf-t0)/h must be a positive integer (no partial last step)"); return LCS_ERR_INVALID_ARG; }
+    double eps = 1e-9 * f->dt_snap, lo = f->times.front() - eps, hi = f->times.back() + eps;
+    if (t0 < lo || t0 > hi || tf < lo || tf > hi) { lcs_set_error("[t0,tf] = [%g,%g] outside the snapshot times [%g,%g]", t0, tf, f->times.front(), f->times.back()); return LCS_ERR_TIME_RANGE; }
+    *N = n;
+    return LCS_OK;
+}
+
+extern "C" lcs_status lcs_advect(lcs_field *f, int64_t n, const void *seeds, double t0, double tf, double h, void *flowmap,
+                                 uint8_t *exit_flag, int32_t *exit_step, void *cuda_stream)
+{
+    if (!f || n < 0 || (n > 0 && (!seeds || !flowmap))) { lcs_set_error("null argument"); return LCS_ERR_INVALID_ARG; }
+    int64_t N = 0;
+    lcs_status rc = check_interval(f, t0, tf, h, &N);
+    if (rc != LCS_OK) return rc;
+    if (n == 0) return LCS_OK;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    return f->kind == LCS_MESH_CARTESIAN ? lcs_cart_advect(f, n, seeds, t0, h, N, flowmap, exit_flag, exit_step, st)
+                                         : lcs_simplex_advect(f, n, seeds, t0, h, N, flowmap, exit_flag, exit_step, st);
+}
+
+// ---------------------------------------------------------------------------------------------
+extern "C" lcs_status lcs_ftle_host(lcs_field *f, const int32_t ng[3], const double seed_spacing[3], const int32_t seed_periodic[3],
+                                    const double period[3], const void *seeds_host, double t0, double tf, double h,
+                                    void *flowmap_host, uint8_t *exit_flag_host, void *ftle_host)
+{
+    if (!f || !ng || !seeds_host || !ftle_host) { lcs_set_error("null argument"); return LCS_ERR_INVALID_ARG; }
+    int64_t n = (int64_t)ng[0] * ng[1] * (f->dim == 3 ? ng[2] : 1);
+    if (n <= 0) { lcs_set_error("empty seed grid"); return LCS_ERR_INVALID_ARG; }
+    size_t es = lcs_esize(f->compute_dtype);
+    if (f->h_cap < n) {
+        cudaDeviceSynchronize();
+        if (f->h_seeds) cudaFree(f->h_seeds);
+        if (f->h_ftle) cudaFree(f->h_ftle);
+        if (f->h_flag) cudaFree(f->h_flag);
+        f->h_seeds = f->h_ftle = nullptr; f->h_flag = nullptr; f->h_cap = 0;
+        LCS_CUDA_OK(cudaMalloc(&f->h_seeds, (size_t)n * f->dim * es));
+        LCS_CUDA_OK(cudaMalloc(&f->h_ftle, (size_t)n * es));
+        LCS_CUDA_OK(cudaMalloc((void **)&f->h_flag, (size_t)n));
+        f->h_cap = n;
+    }
+    cudaStream_t st = 0;
+    LCS_CUDA_OK(cudaMemcpyAsync(f->h_seeds, seeds_host, (size_t)n * f->dim * es, cudaMemcpyHostToDevice, st));
+    lcs_status rc = lcs_advect(f, n, f->h_seeds, t0, tf, h, f->h_seeds, f->h_flag, nullptr, st);   // flow map in place
+    if (rc != LCS_OK) return rc;
+    rc = lcs_cg_ftle(f->dim, f->compute_dtype, ng, seed_spacing, seed_periodic, period, f->h_seeds, f->h_flag, tf - t0, nullptr,
+                     f->h_ftle, nullptr, st);
+    if (rc != LCS_OK) return rc;
+    LCS_CUDA_OK(cudaMemcpyAsync(ftle_host, f->h_ftle, (size_t)n * es, cudaMemcpyDeviceToHost, st));
+    if (flowmap_host) LCS_CUDA_OK(cudaMemcpyAsync(flowmap_host, f->h_seeds, (size_t)n * f->dim * es, cudaMemcpyDeviceToHost, st));
+    if (exit_flag_host) LCS_CUDA_OK(cudaMemcpyAsync(exit_flag_host, f->h_flag, (size_t)n, cudaMemcpyDeviceToHost, st));
+    LCS_CUDA_OK(cudaStreamSynchronize(st));
+    return LCS_OK;
+}

@@ -1,0 +1,162 @@
+// lcs_internal.cuh -- private declarations of liblcs.so (sm_100a).  Not part of the C-ABI.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <atomic>
+#include <string>
+#include <vector>
+
+#include "../../include/lcs.h"
+
+// ---------------------------------------------------------------------------------------------
+// error plumbing
+void lcs_set_error(const char *fmt, ...);
+extern std::atomic<int64_t> g_lcs_launches;
+
+#define LCS_CUDA_OK(expr)                                                                       \
+    do {                                                                                        \
+        cudaError_t e__ = (expr);                                                               \
+        if (e__ != cudaSuccess) {                                                               \
+            lcs_set_error("%s failed: %s (%s:%d)", #expr, cudaGetErrorString(e__), __FILE__, __LINE__); \
+            return (e__ == cudaErrorMemoryAllocation) ? LCS_ERR_OOM : LCS_ERR_CUDA;             \
+        }                                                                                       \
+    } while (0)
+
+#define LCS_LAUNCH(kernel, grid, block, smem, stream, ...)                                      \
+    do {                                                                                        \
+        kernel<<<(grid), (block), (smem), (stream)>>>(__VA_ARGS__);                             \
+        g_lcs_launches.fetch_add(1, std::memory_order_relaxed);                                 \
+    } while (0)
+
+static inline unsigned lcs_blocks(int64_t n, int block) { return (unsigned)((n + block - 1) / block); }
+
+// ---------------------------------------------------------------------------------------------
+// Velocity "pair record": for one mesh node, the velocity at the earlier snapshot of the current window
+// (a) and the difference to the later one (d = b - a), padded to P = 2 (2D) or 4 (3D) components.
+// u(node, tau) = a + tau*d is one FMA per component, and both time levels of a node share one 32-byte
+// sector for the two hot layouts (3D fp32, 2D fp64).
+template <int DIM> struct PadOf { static constexpr int P = (DIM == 2) ? 2 : 4; };
+
+template <int DIM, typename TV> struct alignas(16) PairRec {
+    TV a[PadOf<DIM>::P];
+    TV d[PadOf<DIM>::P];
+};
+
+// ---------------------------------------------------------------------------------------------
+struct CartGeom {
+    int32_t n[3];          // nodes per axis
+    int32_t periodic[3];
+    int32_t pow2[3];       // n[a] is a power of two (mask wrap)
+    double origin[3];
+    double spacing[3];
+    double inv[3];         // 1.0 / spacing, rounded once (oracle O2)
+};
+
+struct SimplexMesh {
+    int64_t nv = 0, nc = 0;
+    double *verts = nullptr;      // [nv][dim] fp64
+    int32_t *cells = nullptr;     // [nc][dim+1]
+    int32_t *neigh = nullptr;     // [nc][dim+1], -1 = hull face
+    uint8_t *oppside = nullptr;   // [nc] bit j = canonical side of the vertex opposite face j
+    void *cellrec = nullptr;      // [nc] per-cell affine map for the in-advect walk (compute dtype)
+    int32_t *bins = nullptr;      // [nb0*nb1*nb2] start cell per bin
+    int32_t nb[3] = {1, 1, 1};
+    double bin_lo[3] = {0, 0, 0};
+    double bin_inv[3] = {0, 0, 0};
+    int64_t hop_cap = 64;
+};
+
+// tracer scratch owned by the field, grown on demand
+struct TracerScratch {
+    int64_t cap = 0;
+    void *buf = nullptr;          // one allocation, carved by the advect code
+    size_t bytes = 0;
+};
+
+struct lcs_field {
+    int dim = 0, kind = 0;
+    int vel_dtype = 0, compute_dtype = 0;
+    int P = 2;                    // padded components
+    int64_t nnodes = 0;
+    CartGeom cart{};
+    SimplexMesh mesh{};
+    std::vector<double> times;
+    double dt_snap = 0;
+    int ns = 0;
+    // snapshot storage: raw slots hold [node][dim] of vel dtype exactly as supplied
+    int nslots = 0;
+    bool ring = false;
+    std::vector<void *> slot;            // device buffers
+    std::vector<int> slot_snap;          // snapshot held (or being loaded) in slot, -1 = empty
+    std::vector<cudaEvent_t> slot_ready; // recorded on the side stream after the upload
+    std::vector<cudaEvent_t> slot_free;  // recorded on the compute stream after the last reader
+    std::vector<char> slot_free_valid;
+    std::vector<int> snap_slot;          // slot of snapshot s, -1 = not resident
+    std::vector<char> snap_set;
+    std::vector<const void *> host_src;  // ring mode: retained host pointers
+    // pair-record cache (built on the compute stream from two raw slots)
+    static constexpr int kPairCache = 4;
+    void *pair_buf[kPairCache] = {nullptr, nullptr, nullptr, nullptr};
+    int pair_snap[kPairCache] = {-1, -1, -1, -1};
+    int64_t pair_age[kPairCache] = {0, 0, 0, 0};
+    int64_t pair_clock = 0;
+    cudaStream_t side = nullptr;
+    TracerScratch scratch;
+    // host-API scratch
+    void *h_seeds = nullptr, *h_flow = nullptr, *h_ftle = nullptr;
+    uint8_t *h_flag = nullptr;
+    int64_t h_cap = 0;
+    // options
+    int64_t opt_integrator = 0;   // 0 auto, 1 fused, 2 split
+    int64_t opt_sort_seeds = 0;
+    int64_t opt_resort_every = 0;
+    int64_t opt_block = 0;        // threads per block override (0 = default)
+    int64_t opt_time_windows = 0; // record CUDA events around every window (hot) kernel launch
+    // info
+    int64_t info_windows = 0;
+    int64_t info_h2d_bytes = 0;
+    std::vector<cudaEvent_t> win_ev;     // start/stop pairs recorded on the launching stream
+    size_t win_ev_used = 0;
+};
+
+// CUDA-event bracket around the dominant kernel's launches (bench.py's roofline.achieved)
+struct WindowTimer {
+    lcs_field *f; cudaStream_t st; bool on;
+    WindowTimer(lcs_field *f_, cudaStream_t st_) : f(f_), st(st_), on(f_->opt_time_windows != 0) {
+        if (!on) return;
+        while (f->win_ev.size() < f->win_ev_used + 2) { cudaEvent_t e; cudaEventCreate(&e); f->win_ev.push_back(e); }
+        cudaEventRecord(f->win_ev[f->win_ev_used], st);
+    }
+    ~WindowTimer() { if (on) { cudaEventRecord(f->win_ev[f->win_ev_used + 1], st); f->win_ev_used += 2; } }
+};
+
+static inline size_t lcs_esize(int dtype) { return dtype == LCS_F64 ? 8 : 4; }
+
+// field.cu
+lcs_status lcs_field_require_pair(lcs_field *f, int s, cudaStream_t stream, const void **pair);
+lcs_status lcs_field_prefetch(lcs_field *f, int s);
+lcs_status lcs_scratch_reserve(lcs_field *f, size_t bytes);
+
+// simplex.cu
+lcs_status lcs_simplex_build(lcs_field *f, const double *verts_host, const int32_t *cells_host);
+void lcs_simplex_free(lcs_field *f);
+lcs_status lcs_simplex_locate(lcs_field *f, int64_t n, const double *pos, int32_t *cell, double *bary, cudaStream_t st);
+lcs_status lcs_simplex_advect(lcs_field *f, int64_t n, const void *seeds, double t0, double h, int64_t N,
+                              void *flowmap, uint8_t *exit_flag, int32_t *exit_step, cudaStream_t st);
+
+// advect_cart.cu
+lcs_status lcs_cart_locate(lcs_field *f, int64_t n, const double *pos, int32_t *cell, double *w, cudaStream_t st);
+lcs_status lcs_cart_advect(lcs_field *f, int64_t n, const void *seeds, double t0, double h, int64_t N,
+                           void *flowmap, uint8_t *exit_flag, int32_t *exit_step, cudaStream_t st);
+
+// ---------------------------------------------------------------------------------------------
+// Window plan shared by the Cartesian and simplex integrators: consecutive RK4 steps whose three stage
+// times (ta, tb, tc) use the same snapshot pair are run by one launch.
+struct StepWindow {
+    int64_t first = 0;      // first step index
+    int32_t count = 0;      // steps in the window
+    int32_t s[3] = {0, 0, 0};   // snapshot pair index used by the stage times ta, tb, tc
+};
+// tau[3*n + {0,1,2}] = (t - times[s]) / dt for ta, tb, tc of step n (fp64, as the oracle computes them)
+lcs_status lcs_plan_windows(const lcs_field *f, double t0, double h, int64_t N,
+                            std::vector<StepWindow> &windows, std::vector<double> &tau);

@@ -1,0 +1,731 @@
+// simplex.cu -- triangle / tetrahedral meshes: device-built face adjacency and uniform bin grid, cell
+// search by walking (row a2), barycentric space + linear time interpolation (row a3) and the RK4
+// integrator (row a4), for sm_100a.
+//
+// Paper: "an efficient local cell search strategy for unstructured grids [27] ... designed for
+// tetrahedral grids (or triangular grids in 2D)"; the Seed filter "computes which cell in
+// the velocity field mesh each seed point is located in"; the cell search "readily
+// facilitates spatial interpolation" through its natural coordinates; each of the four RK4
+// evaluations needs a preceding cell search.
+//
+// Two predicates are used on purpose:
+//  * lcs_locate and the seeds' initial cells use the CANONICAL fp64 face predicate (face vertices sorted by
+//    id, every product/sum rounded separately, ties as if the point were p + (eps, eps^2, eps^3)), which
+//    makes the owner of a point unique and bit-reproducible;
+//  * the walk inside the integrator uses precomputed per-cell affine maps lambda = M (p - v0) in the compute
+//    dtype with a small tolerance.  P1 interpolation is continuous across faces, so a different-but-adjacent
+//    cell changes the velocity at rounding level only.
+#include <math.h>
+
+#include <algorithm>
+#include <cub/cub.cuh>
+
+#include "lcs_internal.cuh"
+
+namespace {
+
+// ---------------------------------------------------------------------------------------------
+// canonical predicate (must match oracle/lcs_oracle.c face_side bit for bit: no FMA contraction)
+template <int DIM> __device__ __forceinline__ void sort_ids(int32_t *v)
+{
+    if (v[0] > v[1]) { int32_t t = v[0]; v[0] = v[1]; v[1] = t; }
+    if constexpr (DIM == 3) {
+        if (v[1] > v[2]) { int32_t t = v[1]; v[1] = v[2]; v[2] = t; }
+        if (v[0] > v[1]) { int32_t t = v[0]; v[0] = v[1]; v[1] = t; }
+    }
+}
+
+template <int DIM> __device__ __forceinline__ void face_ids(const int32_t *__restrict__ cells, int64_t c, int j, int32_t *fv)
+{
+    int k = 0;
+#pragma unroll
+    for (int i = 0; i <= DIM; ++i)
+        if (i != j) fv[k++] = cells[c * (DIM + 1) + i];
+    sort_ids<DIM>(fv);
+}
+
+template <int DIM>
+__device__ __forceinline__ bool face_side(const double *__restrict__ verts, const int32_t *fv, const double *p)
+{
+    if constexpr (DIM == 2) {
+        const double *a = verts + 2 * (int64_t)fv[0], *b = verts + 2 * (int64_t)fv[1];
+        double ax = a[0], ay = a[1];
+        double ex = __dsub_rn(b[0], ax), ey = __dsub_rn(b[1], ay);
+        double s = __dsub_rn(__dmul_rn(ex, __dsub_rn(p[1], ay)), __dmul_rn(ey, __dsub_rn(p[0], ax)));
+        if (s != 0.0) return s > 0.0;
+        if (ey != 0.0) return -ey > 0.0;
+        return ex > 0.0;
+    } else {
+        const double *a = verts + 3 * (int64_t)fv[0], *b = verts + 3 * (int64_t)fv[1], *c = verts + 3 * (int64_t)fv[2];
+        double ax = a[0], ay = a[1], az = a[2];
+        double ux = __dsub_rn(b[0], ax), uy = __dsub_rn(b[1], ay), uz = __dsub_rn(b[2], az);
+        double vx = __dsub_rn(c[0], ax), vy = __dsub_rn(c[1], ay), vz = __dsub_rn(c[2], az);
+        double nx = __dsub_rn(__dmul_rn(uy, vz), __dmul_rn(uz, vy));
+        double ny = __dsub_rn(__dmul_rn(uz, vx), __dmul_rn(ux, vz));
+        double nz = __dsub_rn(__dmul_rn(ux, vy), __dmul_rn(uy, vx));
+        double wx = __dsub_rn(p[0], ax), wy = __dsub_rn(p[1], ay), wz = __dsub_rn(p[2], az);
+        double s = __dadd_rn(__dadd_rn(__dmul_rn(nx, wx), __dmul_rn(ny, wy)), __dmul_rn(nz, wz));
+        if (s != 0.0) return s > 0.0;
+        if (nx != 0.0) return nx > 0.0;
+        if (ny != 0.0) return ny > 0.0;
+        return nz > 0.0;
+    }
+}
+
+// first face (local order) whose canonical side test fails for p, or -1 if cell c owns p
+template <int DIM>
+__device__ __forceinline__ int first_failing_face(const double *__restrict__ verts, const int32_t *__restrict__ cells,
+                                                  const uint8_t *__restrict__ oppside, int64_t c, const double *p)
+{
+    const unsigned opp = oppside[c];
+#pragma unroll
+    for (int j = 0; j <= DIM; ++j) {
+        int32_t fv[DIM];
+        face_ids<DIM>(cells, c, j, fv);
+        bool sp = face_side<DIM>(verts, fv, p);
+        if (sp != (bool)((opp >> j) & 1u)) return j;
+    }
+    return -1;
+}
+
+// ---------------------------------------------------------------------------------------------
+// create-time kernels
+template <int DIM>
+__global__ void __launch_bounds__(256) face_key_kernel(const int32_t *__restrict__ cells, int64_t nfaces,
+                                                        uint64_t *__restrict__ key_hi, uint32_t *__restrict__ key_lo,
+                                                        int32_t *__restrict__ face_id)
+{
+    int64_t f = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (f >= nfaces) return;
+    int32_t fv[DIM];
+    face_ids<DIM>(cells, f / (DIM + 1), (int)(f % (DIM + 1)), fv);
+    key_hi[f] = ((uint64_t)(uint32_t)fv[0] << 32) | (uint32_t)fv[1];
+    if constexpr (DIM == 3) key_lo[f] = (uint32_t)fv[2];
+    face_id[f] = (int32_t)f;
+}
+
+__global__ void __launch_bounds__(256) gather_u64_kernel(const uint64_t *__restrict__ src, const int32_t *__restrict__ idx,
+                                                          uint64_t *__restrict__ dst, int64_t n)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) dst[i] = src[idx[i]];
+}
+
+// sorted faces: equal neighbours in the sorted order are the two sides of an interior face
+template <int DIM>
+__global__ void __launch_bounds__(256) pair_faces_kernel(const int32_t *__restrict__ cells, const int32_t *__restrict__ sorted_face,
+                                                          int64_t nfaces, int32_t *__restrict__ neigh, int32_t *__restrict__ err)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i + 1 >= nfaces) return;
+    int32_t f0 = sorted_face[i], f1 = sorted_face[i + 1];
+    int32_t a[DIM], b[DIM];
+    face_ids<DIM>(cells, f0 / (DIM + 1), f0 % (DIM + 1), a);
+    face_ids<DIM>(cells, f1 / (DIM + 1), f1 % (DIM + 1), b);
+    bool same = true;
+#pragma unroll
+    for (int k = 0; k < DIM; ++k) same = same && (a[k] == b[k]);
+    if (!same) return;
+    neigh[f0] = f1 / (DIM + 1);
+    neigh[f1] = f0 / (DIM + 1);
+    if (i + 2 < nfaces) {
+        int32_t f2 = sorted_face[i + 2], c[DIM];
+        face_ids<DIM>(cells, f2 / (DIM + 1), f2 % (DIM + 1), c);
+        bool same2 = true;
+#pragma unroll
+        for (int k = 0; k < DIM; ++k) same2 = same2 && (a[k] == c[k]);
+        if (same2) atomicExch(err, 1);       // a face shared by three cells: not a manifold mesh
+    }
+}
+
+template <int DIM>
+__global__ void __launch_bounds__(256) oppside_kernel(const double *__restrict__ verts, const int32_t *__restrict__ cells,
+                                                       int64_t nc, uint8_t *__restrict__ oppside)
+{
+    int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= nc) return;
+    unsigned bits = 0;
+#pragma unroll
+    for (int j = 0; j <= DIM; ++j) {
+        int32_t fv[DIM];
+        face_ids<DIM>(cells, c, j, fv);
+        double p[DIM];
+        const double *v = verts + (int64_t)DIM * cells[c * (DIM + 1) + j];
+#pragma unroll
+        for (int k = 0; k < DIM; ++k) p[k] = v[k];
+        if (face_side<DIM>(verts, fv, p)) bits |= 1u << j;
+    }
+    oppside[c] = (uint8_t)bits;
+}
+
+// per-cell affine map for the integrator's walk: lambda_i = M_i . (p - v0), i = 1..DIM; lambda_0 = 1 - sum
+template <int DIM, typename TC> struct alignas(16) CellRec {
+    TC M[DIM * DIM];
+    TC v0[DIM];
+    int32_t vid[DIM + 1];
+};
+
+template <int DIM, typename TC>
+__global__ void __launch_bounds__(256) cellrec_kernel(const double *__restrict__ verts, const int32_t *__restrict__ cells,
+                                                       int64_t nc, CellRec<DIM, TC> *__restrict__ rec)
+{
+    int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= nc) return;
+    const int32_t *cv = cells + c * (DIM + 1);
+    const double *v0 = verts + (int64_t)DIM * cv[0];
+    CellRec<DIM, TC> r;
+    if constexpr (DIM == 2) {
+        const double *v1 = verts + 2 * (int64_t)cv[1], *v2 = verts + 2 * (int64_t)cv[2];
+        double e1x = v1[0] - v0[0], e1y = v1[1] - v0[1], e2x = v2[0] - v0[0], e2y = v2[1] - v0[1];
+        double idet = 1.0 / (e1x * e2y - e1y * e2x);
+        r.M[0] = (TC)(e2y * idet);  r.M[1] = (TC)(-e2x * idet);      // lambda_1
+        r.M[2] = (TC)(-e1y * idet); r.M[3] = (TC)(e1x * idet);       // lambda_2
+    } else {
+        const double *v1 = verts + 3 * (int64_t)cv[1], *v2 = verts + 3 * (int64_t)cv[2], *v3 = verts + 3 * (int64_t)cv[3];
+        double e1[3], e2[3], e3[3];
+        for (int k = 0; k < 3; ++k) { e1[k] = v1[k] - v0[k]; e2[k] = v2[k] - v0[k]; e3[k] = v3[k] - v0[k]; }
+        double c23[3] = {e2[1] * e3[2] - e2[2] * e3[1], e2[2] * e3[0] - e2[0] * e3[2], e2[0] * e3[1] - e2[1] * e3[0]};
+        double c31[3] = {e3[1] * e1[2] - e3[2] * e1[1], e3[2] * e1[0] - e3[0] * e1[2], e3[0] * e1[1] - e3[1] * e1[0]};
+        double c12[3] = {e1[1] * e2[2] - e1[2] * e2[1], e1[2] * e2[0] - e1[0] * e2[2], e1[0] * e2[1] - e1[1] * e2[0]};
+        double idet = 1.0 / (e1[0] * c23[0] + e1[1] * c23[1] + e1[2] * c23[2]);
+        for (int k = 0; k < 3; ++k) { r.M[k] = (TC)(c23[k] * idet); r.M[3 + k] = (TC)(c31[k] * idet); r.M[6 + k] = (TC)(c12[k] * idet); }
+    }
+    for (int k = 0; k < DIM; ++k) r.v0[k] = (TC)v0[k];
+    for (int k = 0; k <= DIM; ++k) r.vid[k] = cv[k];
+    rec[c] = r;
+}
+
+// ---- bin grid: start cell per bin = the cell with the largest id among those whose centroid falls in the
+// bin; empty bins are filled by jump flooding with the candidate whose centroid is nearest to the bin centre.
+struct BinGrid {
+    int nb[3];
+    double lo[3], inv[3];
+};
+
+template <int DIM> __device__ __forceinline__ void centroid(const double *verts, const int32_t *cells, int64_t c, double *x)
+{
+#pragma unroll
+    for (int k = 0; k < DIM; ++k) x[k] = 0.0;
+    for (int i = 0; i <= DIM; ++i) {
+        const double *v = verts + (int64_t)DIM * cells[c * (DIM + 1) + i];
+#pragma unroll
+        for (int k = 0; k < DIM; ++k) x[k] += v[k];
+    }
+#pragma unroll
+    for (int k = 0; k < DIM; ++k) x[k] *= 1.0 / (DIM + 1);
+}
+
+template <int DIM> __device__ __forceinline__ int64_t bin_of(const BinGrid &b, const double *x)
+{
+    int64_t id = 0, mul = 1;
+#pragma unroll
+    for (int k = 0; k < DIM; ++k) {
+        double q = floor((x[k] - b.lo[k]) * b.inv[k]);
+        int i = q < 0.0 ? 0 : (q > (double)(b.nb[k] - 1) ? b.nb[k] - 1 : (int)q);
+        id += mul * i;
+        mul *= b.nb[k];
+    }
+    return id;
+}
+
+template <int DIM>
+__global__ void __launch_bounds__(256) bin_scatter_kernel(BinGrid b, const double *__restrict__ verts, const int32_t *__restrict__ cells,
+                                                           int64_t nc, int32_t *__restrict__ bins)
+{
+    int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= nc) return;
+    double x[DIM];
+    centroid<DIM>(verts, cells, c, x);
+    atomicMax(bins + bin_of<DIM>(b, x), (int32_t)c);
+}
+
+template <int DIM>
+__global__ void __launch_bounds__(256) bin_flood_kernel(BinGrid b, const double *__restrict__ verts, const int32_t *__restrict__ cells,
+                                                         const int32_t *__restrict__ src, int32_t *__restrict__ dst, int step, int64_t nbins)
+{
+    int64_t id = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (id >= nbins) return;
+    int32_t cur = src[id];
+    if (cur >= 0) { dst[id] = cur; return; }
+    int ijk[3] = {(int)(id % b.nb[0]), (int)((id / b.nb[0]) % b.nb[1]), (int)(id / ((int64_t)b.nb[0] * b.nb[1]))};
+    double ctr[DIM];
+#pragma unroll
+    for (int k = 0; k < DIM; ++k) ctr[k] = b.lo[k] + (ijk[k] + 0.5) / b.inv[k];
+    double best = 1e300;
+    int32_t arg = -1;
+    const int kz0 = DIM == 3 ? -1 : 0, kz1 = DIM == 3 ? 1 : 0;
+    for (int dz = kz0; dz <= kz1; ++dz)
+        for (int dy = -1; dy <= 1; ++dy)
+            for (int dx = -1; dx <= 1; ++dx) {
+                int x = ijk[0] + dx * step, y = ijk[1] + dy * step, z = ijk[2] + dz * step;
+                if (x < 0 || x >= b.nb[0] || y < 0 || y >= b.nb[1] || z < 0 || z >= b.nb[2]) continue;
+                int32_t cand = src[x + (int64_t)b.nb[0] * (y + (int64_t)b.nb[1] * z)];
+                if (cand < 0) continue;
+                double cx[DIM], d2 = 0.0;
+                centroid<DIM>(verts, cells, cand, cx);
+#pragma unroll
+                for (int k = 0; k < DIM; ++k) d2 += (cx[k] - ctr[k]) * (cx[k] - ctr[k]);
+                if (d2 < best || (d2 == best && cand > arg)) { best = d2; arg = cand; }
+            }
+    dst[id] = arg;
+}
+
+// ---------------------------------------------------------------------------------------------
+// canonical location of one point: bin -> start cell -> walk; hop cap -> brute-force scan (never expected)
+template <int DIM>
+__device__ __forceinline__ int32_t locate_canonical(const BinGrid &b, const int32_t *__restrict__ bins, const double *__restrict__ verts,
+                                                    const int32_t *__restrict__ cells, const int32_t *__restrict__ neigh,
+                                                    const uint8_t *__restrict__ oppside, int64_t nc, int64_t hop_cap, const double *p)
+{
+    int64_t c = bins[bin_of<DIM>(b, p)];
+    if (c < 0) c = 0;
+    for (int64_t hop = 0; hop < hop_cap; ++hop) {
+        int j = first_failing_face<DIM>(verts, cells, oppside, c, p);
+        if (j < 0) return (int32_t)c;
+        int32_t nb = neigh[c * (DIM + 1) + j];
+        if (nb < 0) return -1;
+        c = nb;
+    }
+    for (int64_t k = 0; k < nc; ++k)
+        if (first_failing_face<DIM>(verts, cells, oppside, k, p) < 0) return (int32_t)k;
+    return -1;
+}
+
+template <int DIM>
+__global__ void __launch_bounds__(128) simplex_locate_kernel(BinGrid b, const int32_t *__restrict__ bins, const double *__restrict__ verts,
+                                                              const int32_t *__restrict__ cells, const int32_t *__restrict__ neigh,
+                                                              const uint8_t *__restrict__ oppside, int64_t nc, int64_t hop_cap,
+                                                              const double *__restrict__ pos, int64_t n, int32_t *__restrict__ cell,
+                                                              double *__restrict__ bary)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    double p[DIM];
+#pragma unroll
+    for (int k = 0; k < DIM; ++k) p[k] = pos[i * DIM + k];
+    int32_t c = locate_canonical<DIM>(b, bins, verts, cells, neigh, oppside, nc, hop_cap, p);
+    cell[i] = c;
+    if (!bary) return;
+    double lam[DIM + 1];
+    if (c < 0) {
+        for (int k = 0; k <= DIM; ++k) lam[k] = 0.0;
+    } else {
+        // vertex-0-relative signed-volume ratios (oracle rule O3)
+        const int32_t *cv = cells + (int64_t)c * (DIM + 1);
+        const double *v0 = verts + (int64_t)DIM * cv[0];
+        if constexpr (DIM == 2) {
+            const double *v1 = verts + 2 * (int64_t)cv[1], *v2 = verts + 2 * (int64_t)cv[2];
+            double e1x = v1[0] - v0[0], e1y = v1[1] - v0[1], e2x = v2[0] - v0[0], e2y = v2[1] - v0[1];
+            double px = p[0] - v0[0], py = p[1] - v0[1];
+            double tot = e1x * e2y - e1y * e2x;
+            lam[1] = (px * e2y - py * e2x) / tot;
+            lam[2] = (e1x * py - e1y * px) / tot;
+            lam[0] = 1.0 - lam[1] - lam[2];
+        } else {
+            const double *v1 = verts + 3 * (int64_t)cv[1], *v2 = verts + 3 * (int64_t)cv[2], *v3 = verts + 3 * (int64_t)cv[3];
+            double e1[3], e2[3], e3[3], q[3];
+            for (int k = 0; k < 3; ++k) { e1[k] = v1[k] - v0[k]; e2[k] = v2[k] - v0[k]; e3[k] = v3[k] - v0[k]; q[k] = p[k] - v0[k]; }
+            auto det3 = [](const double *a, const double *bb, const double *cc) {
+                return a[0] * (bb[1] * cc[2] - bb[2] * cc[1]) - a[1] * (bb[0] * cc[2] - bb[2] * cc[0]) + a[2] * (bb[0] * cc[1] - bb[1] * cc[0]);
+            };
+            double tot = det3(e1, e2, e3);
+            lam[1] = det3(q, e2, e3) / tot;
+            lam[2] = det3(e1, q, e3) / tot;
+            lam[3] = det3(e1, e2, q) / tot;
+            lam[0] = 1.0 - lam[1] - lam[2] - lam[3];
+        }
+    }
+    for (int k = 0; k <= DIM; ++k) bary[i * (DIM + 1) + k] = lam[k];
+}
+
+// ---------------------------------------------------------------------------------------------
+// integrator
+template <int DIM, typename TC> struct SimplexState {
+    TC *x[3];
+    int32_t *cell;
+    int32_t *steps;
+    uint8_t *flag;
+};
+
+template <int DIM, typename TC>
+__global__ void __launch_bounds__(128) simplex_init_kernel(BinGrid b, const int32_t *__restrict__ bins, const double *__restrict__ verts,
+                                                            const int32_t *__restrict__ cells, const int32_t *__restrict__ neigh,
+                                                            const uint8_t *__restrict__ oppside, int64_t nc, int64_t hop_cap,
+                                                            const TC *__restrict__ seeds, int64_t n, SimplexState<DIM, TC> st)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    double p[DIM];
+#pragma unroll
+    for (int k = 0; k < DIM; ++k) { TC v = seeds[i * DIM + k]; st.x[k][i] = v; p[k] = (double)v; }
+    int32_t c = locate_canonical<DIM>(b, bins, verts, cells, neigh, oppside, nc, hop_cap, p);
+    st.cell[i] = c;
+    st.flag[i] = c < 0 ? 2 : 0;
+    st.steps[i] = 0;
+}
+
+template <typename TC> struct WalkTol {};
+template <> struct WalkTol<float> { static constexpr float eps = 1e-4f; };
+template <> struct WalkTol<double> { static constexpr double eps = 1e-10; };
+
+template <int DIM, typename TV, typename TC>
+__device__ __forceinline__ void vertex_velocity(const PairRec<DIM, TV> *__restrict__ rec, int32_t v, TC tau, TC *out)
+{
+    if constexpr (DIM == 3 && sizeof(TV) == 4) {
+        const float4 *p = reinterpret_cast<const float4 *>(rec + v);
+        float4 a = __ldg(p), d = __ldg(p + 1);
+        out[0] = fma(tau, (TC)d.x, (TC)a.x); out[1] = fma(tau, (TC)d.y, (TC)a.y); out[2] = fma(tau, (TC)d.z, (TC)a.z);
+    } else if constexpr (DIM == 3) {
+        const double2 *p = reinterpret_cast<const double2 *>(rec + v);
+        double2 a0 = __ldg(p), a1 = __ldg(p + 1), d0 = __ldg(p + 2), d1 = __ldg(p + 3);
+        out[0] = fma(tau, (TC)d0.x, (TC)a0.x); out[1] = fma(tau, (TC)d0.y, (TC)a0.y); out[2] = fma(tau, (TC)d1.x, (TC)a1.x);
+    } else if constexpr (sizeof(TV) == 8) {
+        const double2 *p = reinterpret_cast<const double2 *>(rec + v);
+        double2 a = __ldg(p), d = __ldg(p + 1);
+        out[0] = fma(tau, (TC)d.x, (TC)a.x); out[1] = fma(tau, (TC)d.y, (TC)a.y);
+    } else {
+        float4 r = __ldg(reinterpret_cast<const float4 *>(rec + v));
+        out[0] = fma(tau, (TC)r.z, (TC)r.x); out[1] = fma(tau, (TC)r.w, (TC)r.y);
+    }
+}
+
+template <int DIM, typename TC> __device__ __forceinline__ CellRec<DIM, TC> load_cellrec(const CellRec<DIM, TC> *__restrict__ rec, int32_t c)
+{
+    CellRec<DIM, TC> r;
+    constexpr int NQ = sizeof(CellRec<DIM, TC>) / 16;
+    const int4 *src = reinterpret_cast<const int4 *>(rec + c);
+    int4 *dst = reinterpret_cast<int4 *>(&r);
+#pragma unroll
+    for (int k = 0; k < NQ; ++k) dst[k] = __ldg(src + k);
+    return r;
+}
+
+// u(p, tau) with the walk from *cell; false = p left the mesh through a hull face
+template <int DIM, typename TV, typename TC>
+__device__ __forceinline__ bool simplex_velocity(const CellRec<DIM, TC> *__restrict__ crec, const int32_t *__restrict__ neigh,
+                                                 const PairRec<DIM, TV> *__restrict__ vrec, TC tau, const TC *p, int32_t *cell, TC *u)
+{
+    int32_t c = *cell;
+    TC lam[DIM + 1];
+    CellRec<DIM, TC> r;
+    for (int hop = 0;; ++hop) {
+        r = load_cellrec<DIM, TC>(crec, c);
+        TC q[DIM];
+#pragma unroll
+        for (int k = 0; k < DIM; ++k) q[k] = p[k] - r.v0[k];
+        TC sum = TC(0);
+#pragma unroll
+        for (int i = 0; i < DIM; ++i) {
+            TC l = TC(0);
+#pragma unroll
+            for (int k = 0; k < DIM; ++k) l = fma(r.M[i * DIM + k], q[k], l);
+            lam[i + 1] = l;
+            sum += l;
+        }
+        lam[0] = TC(1) - sum;
+        int jmin = 0;
+        TC lmin = lam[0];
+#pragma unroll
+        for (int i = 1; i <= DIM; ++i)
+            if (lam[i] < lmin) { lmin = lam[i]; jmin = i; }
+        if (lmin >= -WalkTol<TC>::eps || hop >= 64) break;
+        int32_t nb = __ldg(neigh + (int64_t)c * (DIM + 1) + jmin);
+        if (nb < 0) return false;
+        c = nb;
+    }
+    *cell = c;
+#pragma unroll
+    for (int k = 0; k < DIM; ++k) u[k] = TC(0);
+#pragma unroll
+    for (int i = 0; i <= DIM; ++i) {
+        TC v[DIM];
+        vertex_velocity<DIM, TV, TC>(vrec, r.vid[i], tau, v);
+#pragma unroll
+        for (int k = 0; k < DIM; ++k) u[k] = fma(lam[i], v[k], u[k]);
+    }
+    return true;
+}
+
+template <int DIM, typename TV, typename TC>
+__global__ void __launch_bounds__(128)
+simplex_window_kernel(const CellRec<DIM, TC> *__restrict__ crec, const int32_t *__restrict__ neigh, const PairRec<DIM, TV> *__restrict__ pa,
+                      const PairRec<DIM, TV> *__restrict__ pb, const PairRec<DIM, TV> *__restrict__ pc, const TC *__restrict__ tau,
+                      int nsteps, int first_step, int64_t n, SimplexState<DIM, TC> st, TC h)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    if (st.flag[i] != 0) return;
+    TC x[DIM];
+#pragma unroll
+    for (int k = 0; k < DIM; ++k) x[k] = st.x[k][i];
+    int32_t cell = st.cell[i];
+    int s = 0;
+    bool ok = true;
+    for (; s < nsteps; ++s) {
+        const TC ta = __ldg(tau + 3 * s), tb = __ldg(tau + 3 * s + 1), tc = __ldg(tau + 3 * s + 2);
+        TC k1[DIM], k2[DIM], k3[DIM], k4[DIM], y[DIM];
+        int32_t c = cell;
+        ok = simplex_velocity<DIM, TV, TC>(crec, neigh, pa, ta, x, &c, k1);
+        if (!ok) break;
+#pragma unroll
+        for (int k = 0; k < DIM; ++k) y[k] = fma(TC(0.5) * h, k1[k], x[k]);
+        ok = simplex_velocity<DIM, TV, TC>(crec, neigh, pb, tb, y, &c, k2);
+        if (!ok) break;
+#pragma unroll
+        for (int k = 0; k < DIM; ++k) y[k] = fma(TC(0.5) * h, k2[k], x[k]);
+        ok = simplex_velocity<DIM, TV, TC>(crec, neigh, pb, tb, y, &c, k3);
+        if (!ok) break;
+#pragma unroll
+        for (int k = 0; k < DIM; ++k) y[k] = fma(h, k3[k], x[k]);
+        ok = simplex_velocity<DIM, TV, TC>(crec, neigh, pc, tc, y, &c, k4);
+        if (!ok) break;
+#pragma unroll
+        for (int k = 0; k < DIM; ++k) x[k] = fma(h * TC(1.0 / 6.0), (k1[k] + k4[k]) + TC(2) * (k2[k] + k3[k]), x[k]);
+        cell = c;
+    }
+#pragma unroll
+    for (int k = 0; k < DIM; ++k) st.x[k][i] = x[k];
+    st.cell[i] = cell;
+    if (!ok) { st.flag[i] = 1; st.steps[i] = first_step + s; }
+}
+
+template <int DIM, typename TC>
+__global__ void __launch_bounds__(256) simplex_final_kernel(int64_t n, SimplexState<DIM, TC> st, int32_t N, TC *__restrict__ flowmap,
+                                                             uint8_t *__restrict__ exit_flag, int32_t *__restrict__ exit_step)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    uint8_t fl = st.flag[i];
+#pragma unroll
+    for (int k = 0; k < DIM; ++k) flowmap[i * DIM + k] = st.x[k][i];
+    if (exit_flag) exit_flag[i] = fl;
+    if (exit_step) exit_step[i] = fl == 0 ? N : (fl == 2 ? 0 : st.steps[i]);
+}
+
+BinGrid make_bins(const lcs_field *f)
+{
+    BinGrid b;
+    for (int k = 0; k < 3; ++k) { b.nb[k] = f->mesh.nb[k]; b.lo[k] = f->mesh.bin_lo[k]; b.inv[k] = f->mesh.bin_inv[k]; }
+    return b;
+}
+
+size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
+
+template <int DIM> lcs_status build_impl(lcs_field *f, const double *vh, const int32_t *ch)
+{
+    SimplexMesh &m = f->mesh;
+    const int64_t nv = m.nv, nc = m.nc, nf = nc * (DIM + 1);
+    // host validation + bounding box
+    for (int64_t i = 0; i < nf; ++i)
+        if (ch[i] < 0 || ch[i] >= nv) { lcs_set_error("cell %lld has vertex index %d out of range", (long long)(i / (DIM + 1)), ch[i]); return LCS_ERR_MESH; }
+    for (int64_t c = 0; c < nc; ++c)
+        for (int a = 0; a <= DIM; ++a)
+            for (int b2 = a + 1; b2 <= DIM; ++b2)
+                if (ch[c * (DIM + 1) + a] == ch[c * (DIM + 1) + b2]) { lcs_set_error("cell %lld repeats a vertex", (long long)c); return LCS_ERR_MESH; }
+    double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
+    for (int64_t v = 0; v < nv; ++v)
+        for (int k = 0; k < DIM; ++k) {
+            double x = vh[v * DIM + k];
+            if (!isfinite(x)) { lcs_set_error("vertex %lld is not finite", (long long)v); return LCS_ERR_MESH; }
+            lo[k] = std::min(lo[k], x); hi[k] = std::max(hi[k], x);
+        }
+    LCS_CUDA_OK(cudaMalloc((void **)&m.verts, (size_t)nv * DIM * 8));
+    LCS_CUDA_OK(cudaMalloc((void **)&m.cells, (size_t)nf * 4));
+    LCS_CUDA_OK(cudaMalloc((void **)&m.neigh, (size_t)nf * 4));
+    LCS_CUDA_OK(cudaMalloc((void **)&m.oppside, (size_t)nc));
+    LCS_CUDA_OK(cudaMemcpy(m.verts, vh, (size_t)nv * DIM * 8, cudaMemcpyHostToDevice));
+    LCS_CUDA_OK(cudaMemcpy(m.cells, ch, (size_t)nf * 4, cudaMemcpyHostToDevice));
+    LCS_CUDA_OK(cudaMemset(m.neigh, 0xff, (size_t)nf * 4));
+    cudaStream_t st = 0;
+
+    // ---- adjacency: sort face keys (CUB radix sort: set-up, not the hot path), pair equal neighbours
+    uint64_t *key_hi = nullptr, *key_hi2 = nullptr;
+    uint32_t *key_lo = nullptr, *key_lo2 = nullptr;
+    int32_t *fid = nullptr, *fid2 = nullptr, *err = nullptr;
+    void *tmp = nullptr;
+    auto cleanup = [&]() {
+        cudaFree(key_hi); cudaFree(key_hi2); cudaFree(key_lo); cudaFree(key_lo2); cudaFree(fid); cudaFree(fid2); cudaFree(err); cudaFree(tmp);
+    };
+#define BUILD_OK(expr) do { cudaError_t e__ = (expr); if (e__ != cudaSuccess) { lcs_set_error("%s: %s", #expr, cudaGetErrorString(e__)); cleanup(); return e__ == cudaErrorMemoryAllocation ? LCS_ERR_OOM : LCS_ERR_CUDA; } } while (0)
+    BUILD_OK(cudaMalloc((void **)&key_hi, (size_t)nf * 8));
+    BUILD_OK(cudaMalloc((void **)&key_hi2, (size_t)nf * 8));
+    BUILD_OK(cudaMalloc((void **)&fid, (size_t)nf * 4));
+    BUILD_OK(cudaMalloc((void **)&fid2, (size_t)nf * 4));
+    BUILD_OK(cudaMalloc((void **)&err, 4));
+    BUILD_OK(cudaMemset(err, 0, 4));
+    if (DIM == 3) { BUILD_OK(cudaMalloc((void **)&key_lo, (size_t)nf * 4)); BUILD_OK(cudaMalloc((void **)&key_lo2, (size_t)nf * 4)); }
+    LCS_LAUNCH((face_key_kernel<DIM>), lcs_blocks(nf, 256), 256, 0, st, m.cells, nf, key_hi, key_lo, fid);
+    size_t tb1 = 0, tb2 = 0;
+    if (DIM == 3) cub::DeviceRadixSort::SortPairs(nullptr, tb1, key_lo, key_lo2, fid, fid2, (int)nf, 0, 32, st);
+    cub::DeviceRadixSort::SortPairs(nullptr, tb2, key_hi, key_hi2, fid, fid2, (int)nf, 0, 64, st);
+    BUILD_OK(cudaMalloc(&tmp, std::max(tb1, tb2)));
+    const int32_t *sorted = nullptr;
+    if (DIM == 3) {
+        // LSD: sort by the third id, then (stable) by the first two
+        BUILD_OK(cub::DeviceRadixSort::SortPairs(tmp, tb1, key_lo, key_lo2, fid, fid2, (int)nf, 0, 32, st));
+        LCS_LAUNCH(gather_u64_kernel, lcs_blocks(nf, 256), 256, 0, st, key_hi, fid2, key_hi2, nf);
+        BUILD_OK(cub::DeviceRadixSort::SortPairs(tmp, tb2, key_hi2, key_hi, fid2, fid, (int)nf, 0, 64, st));
+        sorted = fid;
+    } else {
+        BUILD_OK(cub::DeviceRadixSort::SortPairs(tmp, tb2, key_hi, key_hi2, fid, fid2, (int)nf, 0, 64, st));
+        sorted = fid2;
+    }
+    g_lcs_launches.fetch_add(DIM == 3 ? 2 : 1);
+    LCS_LAUNCH((pair_faces_kernel<DIM>), lcs_blocks(nf, 256), 256, 0, st, m.cells, sorted, nf, m.neigh, err);
+    int32_t herr = 0;
+    BUILD_OK(cudaMemcpy(&herr, err, 4, cudaMemcpyDeviceToHost));
+    cleanup();
+#undef BUILD_OK
+    if (herr) { lcs_set_error("a face is shared by more than two cells"); return LCS_ERR_MESH; }
+
+    LCS_LAUNCH((oppside_kernel<DIM>), lcs_blocks(nc, 256), 256, 0, st, m.verts, m.cells, nc, m.oppside);
+
+    // ---- per-cell affine maps in the compute dtype
+    if (f->compute_dtype == LCS_F64) {
+        LCS_CUDA_OK(cudaMalloc(&m.cellrec, (size_t)nc * sizeof(CellRec<DIM, double>)));
+        LCS_LAUNCH((cellrec_kernel<DIM, double>), lcs_blocks(nc, 256), 256, 0, st, m.verts, m.cells, nc, (CellRec<DIM, double> *)m.cellrec);
+    } else {
+        LCS_CUDA_OK(cudaMalloc(&m.cellrec, (size_t)nc * sizeof(CellRec<DIM, float>)));
+        LCS_LAUNCH((cellrec_kernel<DIM, float>), lcs_blocks(nc, 256), 256, 0, st, m.verts, m.cells, nc, (CellRec<DIM, float> *)m.cellrec);
+    }
+
+    // ---- bin grid: about one bin per cell, cubic bins
+    double ext[3] = {1, 1, 1}, vol = 1.0;
+    for (int k = 0; k < DIM; ++k) { ext[k] = std::max(hi[k] - lo[k], 1e-300); vol *= ext[k]; }
+    double target = std::min((double)nc, (double)(1 << 26));
+    double hb = pow(vol / target, 1.0 / DIM);
+    int64_t nbins = 1;
+    for (int k = 0; k < 3; ++k) {
+        m.nb[k] = k < DIM ? (int)std::max(1.0, std::min(4096.0, ceil(ext[k] / hb))) : 1;
+        m.bin_lo[k] = k < DIM ? lo[k] : 0.0;
+        m.bin_inv[k] = k < DIM ? m.nb[k] / ext[k] : 0.0;
+        nbins *= m.nb[k];
+    }
+    int32_t *bins2 = nullptr;
+    LCS_CUDA_OK(cudaMalloc((void **)&m.bins, (size_t)nbins * 4));
+    LCS_CUDA_OK(cudaMalloc((void **)&bins2, (size_t)nbins * 4));
+    LCS_CUDA_OK(cudaMemset(m.bins, 0xff, (size_t)nbins * 4));
+    BinGrid b = make_bins(f);
+    LCS_LAUNCH((bin_scatter_kernel<DIM>), lcs_blocks(nc, 256), 256, 0, st, b, m.verts, m.cells, nc, m.bins);
+    int maxnb = std::max(m.nb[0], std::max(m.nb[1], m.nb[2]));
+    int step = 1;
+    while (step * 2 < maxnb) step *= 2;
+    int32_t *src = m.bins, *dst = bins2;
+    for (int pass = 0; step >= 1 || pass < 0; ++pass) {
+        LCS_LAUNCH((bin_flood_kernel<DIM>), lcs_blocks(nbins, 256), 256, 0, st, b, m.verts, m.cells, src, dst, step, nbins);
+        std::swap(src, dst);
+        if (step == 1) break;
+        step /= 2;
+    }
+    for (int extra = 0; extra < 2; ++extra) {      // two more unit passes close the remaining gaps
+        LCS_LAUNCH((bin_flood_kernel<DIM>), lcs_blocks(nbins, 256), 256, 0, st, b, m.verts, m.cells, src, dst, 1, nbins);
+        std::swap(src, dst);
+    }
+    LCS_CUDA_OK(cudaDeviceSynchronize());
+    if (src != m.bins) { std::swap(m.bins, bins2); }
+    cudaFree(bins2);
+    m.hop_cap = (int64_t)(4.0 * pow((double)nc, 1.0 / DIM)) + 64;
+    LCS_CUDA_OK(cudaGetLastError());
+    return LCS_OK;
+}
+
+template <int DIM, typename TV, typename TC>
+lcs_status simplex_advect_impl(lcs_field *f, int64_t n, const void *seeds_, double t0, double h, int64_t N, void *flowmap_,
+                               uint8_t *exit_flag, int32_t *exit_step, cudaStream_t st)
+{
+    const TC *seeds = (const TC *)seeds_;
+    TC *flowmap = (TC *)flowmap_;
+    SimplexMesh &m = f->mesh;
+    std::vector<StepWindow> windows;
+    std::vector<double> tau64;
+    lcs_status rc = lcs_plan_windows(f, t0, h, N, windows, tau64);
+    if (rc != LCS_OK) return rc;
+    std::vector<TC> tau(tau64.size());
+    for (size_t k = 0; k < tau.size(); ++k) tau[k] = (TC)tau64[k];
+    size_t off = 0, o_x[3], o_cell, o_steps, o_flag, o_tau;
+    for (int a = 0; a < DIM; ++a) { o_x[a] = off; off = align_up(off + (size_t)n * sizeof(TC)); }
+    o_cell = off; off = align_up(off + (size_t)n * 4);
+    o_steps = off; off = align_up(off + (size_t)n * 4);
+    o_flag = off; off = align_up(off + (size_t)n);
+    o_tau = off; off = align_up(off + tau.size() * sizeof(TC));
+    rc = lcs_scratch_reserve(f, off);
+    if (rc != LCS_OK) return rc;
+    char *base = (char *)f->scratch.buf;
+    SimplexState<DIM, TC> S{};
+    for (int a = 0; a < DIM; ++a) S.x[a] = (TC *)(base + o_x[a]);
+    S.cell = (int32_t *)(base + o_cell);
+    S.steps = (int32_t *)(base + o_steps);
+    S.flag = (uint8_t *)(base + o_flag);
+    TC *d_tau = (TC *)(base + o_tau);
+    LCS_CUDA_OK(cudaMemcpyAsync(d_tau, tau.data(), tau.size() * sizeof(TC), cudaMemcpyHostToDevice, st));
+    BinGrid b = make_bins(f);
+    LCS_LAUNCH((simplex_init_kernel<DIM, TC>), lcs_blocks(n, 128), 128, 0, st, b, m.bins, m.verts, m.cells, m.neigh, m.oppside, m.nc,
+               m.hop_cap, seeds, n, S);
+    const int block = f->opt_block ? (int)f->opt_block : 128;
+    const int dir = h > 0 ? 1 : -1;
+    using VRec = PairRec<DIM, TV>;
+    for (size_t wi = 0; wi < windows.size(); ++wi) {
+        const StepWindow &w = windows[wi];
+        const void *p[3];
+        for (int k = 0; k < 3; ++k) {
+            rc = lcs_field_require_pair(f, w.s[k], st, &p[k]);
+            if (rc != LCS_OK) return rc;
+        }
+        lcs_field_prefetch(f, dir > 0 ? w.s[2] + 2 : w.s[2] - 1);
+        WindowTimer timer(f, st);
+        LCS_LAUNCH((simplex_window_kernel<DIM, TV, TC>), lcs_blocks(n, block), block, 0, st, (const CellRec<DIM, TC> *)m.cellrec, m.neigh,
+                   (const VRec *)p[0], (const VRec *)p[1], (const VRec *)p[2], d_tau + 3 * w.first, w.count, (int)w.first, n, S, (TC)h);
+        f->info_windows++;
+    }
+    LCS_LAUNCH((simplex_final_kernel<DIM, TC>), lcs_blocks(n, 256), 256, 0, st, n, S, (int32_t)N, flowmap, exit_flag, exit_step);
+    LCS_CUDA_OK(cudaGetLastError());
+    return LCS_OK;
+}
+
+}  // namespace
+
+lcs_status lcs_simplex_build(lcs_field *f, const double *verts_host, const int32_t *cells_host)
+{
+    return f->dim == 2 ? build_impl<2>(f, verts_host, cells_host) : build_impl<3>(f, verts_host, cells_host);
+}
+
+void lcs_simplex_free(lcs_field *f)
+{
+    SimplexMesh &m = f->mesh;
+    if (m.verts) cudaFree(m.verts);
+    if (m.cells) cudaFree(m.cells);
+    if (m.neigh) cudaFree(m.neigh);
+    if (m.oppside) cudaFree(m.oppside);
+    if (m.cellrec) cudaFree(m.cellrec);
+    if (m.bins) cudaFree(m.bins);
+    m = SimplexMesh();
+}
+
+lcs_status lcs_simplex_locate(lcs_field *f, int64_t n, const double *pos, int32_t *cell, double *bary, cudaStream_t st)
+{
+    SimplexMesh &m = f->mesh;
+    BinGrid b = make_bins(f);
+    if (f->dim == 2)
+        LCS_LAUNCH((simplex_locate_kernel<2>), lcs_blocks(n, 128), 128, 0, st, b, m.bins, m.verts, m.cells, m.neigh, m.oppside, m.nc, m.hop_cap, pos, n, cell, bary);
+    else
+        LCS_LAUNCH((simplex_locate_kernel<3>), lcs_blocks(n, 128), 128, 0, st, b, m.bins, m.verts, m.cells, m.neigh, m.oppside, m.nc, m.hop_cap, pos, n, cell, bary);
+    LCS_CUDA_OK(cudaGetLastError());
+    return LCS_OK;
+}
+
+lcs_status lcs_simplex_advect(lcs_field *f, int64_t n, const void *seeds, double t0, double h, int64_t N, void *flowmap,
+                              uint8_t *exit_flag, int32_t *exit_step, cudaStream_t st)
+{
+    const bool v64 = f->vel_dtype == LCS_F64, c64 = f->compute_dtype == LCS_F64;
+    if (f->dim == 2) {
+        if (v64 && c64) return simplex_advect_impl<2, double, double>(f, n, seeds, t0, h, N, flowmap, exit_flag, exit_step, st);
+        if (!v64 && c64) return simplex_advect_impl<2, double, double>(f, n, seeds, t0, h, N, flowmap, exit_flag, exit_step, st);
+        if (!v64 && !c64) return simplex_advect_impl<2, float, float>(f, n, seeds, t0, h, N, flowmap, exit_flag, exit_step, st);
+    } else {
+        if (v64 && c64) return simplex_advect_impl<3, double, double>(f, n, seeds, t0, h, N, flowmap, exit_flag, exit_step, st);
+        if (!v64 && c64) return simplex_advect_impl<3, double, double>(f, n, seeds, t0, h, N, flowmap, exit_flag, exit_step, st);
+        if (!v64 && !c64) return simplex_advect_impl<3, float, float>(f, n, seeds, t0, h, N, flowmap, exit_flag, exit_step, st);
+    }
+    lcs_set_error("fp64 velocity with fp32 arithmetic is not supported (compute_dtype must be >= vel_dtype)");
+    return LCS_ERR_INVALID_ARG;
+}

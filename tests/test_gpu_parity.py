@@ -1,0 +1,374 @@
+"""GPU parity tests: the CUDA path (through the C-ABI binding) against the CPU oracle, element by element,
+on the same seeded inputs.  Gates are BASELINE.json's: bit-exact cell indices; fp64 non-chaotic flow maps
+within 1e-10 absolute and FTLE within 1e-8 relative; fp32 / chaotic configs >= 99.9% of seeds within
+1e-3 * domain length and median FTLE relative error <= 1e-3.
+"""
+import numpy as np
+import pytest
+
+from paper_2209_13775_b200 import inputs as I
+from parity_utils import gate_fp64, gate_statistical, gpu_cg, gpu_run, oracle_cg, oracle_run
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def lcs():
+    import torch
+    assert torch.cuda.is_available()
+    from paper_2209_13775_b200 import build, lcs as L
+    build.build()
+    L.lib()
+    return L
+
+
+def cpu(t):
+    return t.detach().cpu().numpy()
+
+
+# -------------------------------------------------------------------------------------------------
+# lcs_locate: bit-exact
+def test_locate_cartesian_bit_exact(lcs, oracle):
+    import torch
+    rng = np.random.default_rng(31)
+    for dim, per in ((2, (0, 0)), (3, (0, 0, 0)), (3, (1, 1, 1)), (3, (1, 0, 1))):
+        n = (11, 7, 5)[:dim]
+        origin, sp = (-1.0, 2.0, 0.5)[:dim], (0.3, 0.25, 0.7)[:dim]
+        w = I.analytic_cartesian(dim, lambda p, t: p, n, origin, sp, (0.0, 1.0), ng=(2,) * dim, seed_lo=(0,) * dim,
+                                 seed_spacing=(1,) * dim, t0=0.0, tf=1.0, h=0.5, periodic=per)
+        lo = np.array(origin)
+        hi = lo + (np.array(n) - 1) * np.array(sp)
+        pts = rng.uniform(lo - 2.0, hi + 2.0, size=(50000, dim))
+        nodes = w.nodes()                                  # points exactly on grid lines / nodes / the closed upper end
+        pts = np.concatenate([pts, nodes, nodes + 1e-16, hi[None, :], lo[None, :]])
+        fo = oracle.OracleField.from_workload(w)
+        co, wo = fo.cart_locate(pts)
+        fg = lcs.Field.from_workload(w)
+        cg_, wg = fg.locate(torch.from_numpy(pts).cuda(), want_bary=True)
+        assert np.array_equal(cpu(cg_), co)
+        assert np.array_equal(cpu(wg)[co >= 0], wo[co >= 0])
+
+
+@pytest.mark.parametrize("dim", [2, 3])
+def test_locate_simplex_exact_ties(lcs, oracle, dim):
+    """Kuhn mesh with integer coordinates: points exactly on faces, edges and vertices (s == 0 ties)."""
+    import torch
+    n = 6 if dim == 2 else 5
+    V, C = I.kuhn_mesh(dim, n)
+    w = I.analytic_simplex(dim, lambda p, t: p, V, C, (0.0, 1.0), ng=(2,) * dim, seed_lo=(0,) * dim,
+                           seed_spacing=(1,) * dim, t0=0.0, tf=1.0, h=0.5)
+    g = np.arange(0, 2 * (n - 1) + 1) * 0.5
+    lattice = np.stack([x.ravel() for x in np.meshgrid(*([g] * dim), indexing="ij")], 1)
+    rng = np.random.default_rng(32)
+    pts = np.concatenate([lattice, rng.uniform(-0.5, n - 0.5, size=(20000, dim)), lattice[:300] * (2.0 / 3.0)])
+    fo = oracle.OracleField.from_workload(w)
+    cb, count = fo.locate_brute(pts)
+    assert count.max() <= 1
+    fg = lcs.Field.from_workload(w)
+    cg_, bary = fg.locate(torch.from_numpy(pts).cuda(), want_bary=True)
+    assert np.array_equal(cpu(cg_), cb)
+    b = cpu(bary)[cb >= 0]
+    assert np.allclose(b.sum(1), 1.0, atol=1e-13) and b.min() > -1e-12
+
+
+@pytest.mark.parametrize("dim", [2, 3])
+def test_locate_simplex_delaunay(lcs, oracle, dim):
+    """Jittered Delaunay meshes (recipe of configs 2 / 4, reduced): all queries vs the oracle's walk, a
+    sample vs brute force; barycentric weights vs the oracle's interpolation of u = x."""
+    import torch
+    rng = np.random.default_rng(33)
+    if dim == 2:
+        w = I.config2(ng=(64, 32), lattice=(80, 40))
+        lo, hi = np.array([0.0, 0.0]), np.array([2.0, 1.0])
+    else:
+        w = I.config4(ng=(8, 8, 8), delta=0.08, n_snap=3, length=3.0)
+        lo, hi = np.array([-1.0, -1.0, 0.0]), np.array([1.0, 1.0, 3.0])
+    fo = oracle.OracleField.from_workload(w)
+    pts = np.concatenate([rng.uniform(lo - 0.05, hi + 0.05, size=(200000, dim)),
+                          w.vertices[w.cells[:2000, 1:]].mean(axis=1)])       # face centroids: near-ties on one face
+    co = fo.locate_walk(pts)
+    fg = lcs.Field.from_workload(w)
+    cg_, bary = fg.locate(torch.from_numpy(pts).cuda(), want_bary=True)
+    cg_ = cpu(cg_)
+    assert np.array_equal(cg_, co)
+    sub = rng.choice(len(pts), 3000, replace=False)
+    cb, count = fo.locate_brute(pts[sub])
+    assert count.max() <= 1 and np.array_equal(cb, cg_[sub])
+    inside = co >= 0
+    assert inside.mean() > 0.5 and (~inside).sum() > 100
+    b = cpu(bary)[inside]
+    rec = np.einsum("ni,nid->nd", b, w.vertices[w.cells[co[inside]]])
+    assert np.max(np.abs(rec - pts[inside])) < 1e-11
+    assert fg.info("n_cells") == len(w.cells)
+    # adjacency: hull faces counted by the library == faces that appear once
+    assert fg.info("n_boundary_faces") == int((fo.neigh < 0).sum())
+
+
+# -------------------------------------------------------------------------------------------------
+# flow map + CG + FTLE parity on the five configs
+def test_config1_full_size_fp64(lcs, oracle):
+    """Config 1 at BASELINE.json's full size: 201x101 grid, 256x128 seeds, 100 steps, fp64."""
+    w = I.config1()
+    fo, Fo, flo, eso = oracle_run(oracle, w)
+    f, sd, F, flag, es = gpu_run(w)
+    cgo, fto, sto = oracle_cg(oracle, w, Fo, flo)
+    cgg, ftg, stg = gpu_cg(w, F, flag)
+    assert np.all(flo == 0) and np.all(eso == 100)                       # closed domain: any exit is a bug
+    err = gate_fp64(cpu(F), Fo, cpu(ftg), fto, w.tf - w.t0, cpu(flag), flo, cpu(es), eso)
+    assert np.array_equal(cpu(stg), sto)
+    assert np.nanmax(np.abs(cpu(cgg) - cgo) / np.maximum(np.abs(cgo), 1.0)) < 1e-7
+    print("config1 max flow-map error %.3e mean %.3e" % (err, np.mean(np.linalg.norm(cpu(F) - Fo, axis=1))))
+
+
+@pytest.mark.parametrize("full", [False, True])
+def test_config2_triangles_fp64(lcs, oracle, full):
+    """Config 2 (reduced and at BASELINE.json's full size: 50 403 vertices, 1024x512 seeds, 300 steps)."""
+    w = I.config2() if full else I.config2(ng=(96, 48), lattice=(60, 30), T=6.0)
+    fo, Fo, flo, eso = oracle_run(oracle, w)
+    f, sd, F, flag, es = gpu_run(w)
+    cgo, fto, sto = oracle_cg(oracle, w, Fo, flo)
+    cgg, ftg, stg = gpu_cg(w, F, flag)
+    assert np.all(flo == 0)
+    err = gate_fp64(cpu(F), Fo, cpu(ftg), fto, w.tf - w.t0, cpu(flag), flo, cpu(es), eso)
+    print("config2 full=%s max flow-map error %.3e" % (full, err))
+
+
+def test_config3_reduced_fp32(lcs, oracle):
+    """Config 3 reduced (ABC, periodic 32^3 grid, 48^3 seeds, fp32 data and arithmetic), full oracle comparison."""
+    w = I.config3(ngrid=48, nn=32, T=5.0, h=0.01, n_snap=21)
+    fo, Fo, flo, eso = oracle_run(oracle, w)
+    f, sd, F, flag, es = gpu_run(w)
+    cgo, fto, sto = oracle_cg(oracle, w, Fo, flo)
+    cgg, ftg, stg = gpu_cg(w, F, flag)
+    assert np.all(cpu(flag) == 0) and np.all(cpu(es) == 500)
+    stats = gate_statistical(cpu(F), Fo, cpu(ftg), fto, w.L, cpu(flag), flo)
+    print("config3 reduced", stats)
+
+
+def test_config3_full_size_sampled_blocks(lcs, oracle):
+    """Config 3 at full size (128^3 grid, 256^3 seeds, 500 steps) in bench.py's launch configuration; the
+    oracle integrates 8 seeded 18^3 blocks (16^3 + halo) and FTLE is compared on their interiors."""
+    import torch
+    w = I.config3()
+    f, sd, F, flag, es = gpu_run(w)
+    cgg, ftg, stg = gpu_cg(w, F, flag)
+    assert int(flag.max()) == 0
+    Fh = cpu(F).reshape(256, 256, 256, 3)
+    fth = cpu(ftg).reshape(256, 256, 256)
+    seeds = w.seeds().reshape(256, 256, 256, 3)
+    fo = oracle.OracleField.from_workload(w)
+    rng = np.random.default_rng(34)
+    B = 18
+    errs, rels = [], []
+    for b in range(8):
+        k0, j0, i0 = rng.integers(0, 256 - B, 3)
+        blk = np.ascontiguousarray(seeds[k0:k0 + B, j0:j0 + B, i0:i0 + B].reshape(-1, 3))
+        Fo, flo, _ = fo.advect(blk.astype(np.float64), w.t0, w.tf, w.h)
+        Fg = Fh[k0:k0 + B, j0:j0 + B, i0:i0 + B].reshape(-1, 3)
+        errs.append(np.linalg.norm(Fg.astype(np.float64) - Fo, axis=1))
+        cgo, fto, sto = oracle.cg_ftle(3, (B, B, B), w.seed_spacing, (0, 0, 0), (0, 0, 0), Fo, flo, w.tf - w.t0)
+        fto = fto.reshape(B, B, B)[1:-1, 1:-1, 1:-1]
+        ftb = fth[k0 + 1:k0 + B - 1, j0 + 1:j0 + B - 1, i0 + 1:i0 + B - 1].astype(np.float64)
+        rels.append((np.abs(ftb - fto) / np.maximum(np.abs(fto), 1e-300)).ravel())
+    err, rel = np.concatenate(errs), np.concatenate(rels)
+    frac = np.mean(err <= 1e-3 * w.L)
+    print("config3 full: frac_ok %.5f median FTLE rel %.3e mean err %.3e max %.3e" % (frac, np.median(rel), err.mean(), err.max()))
+    assert frac >= 0.999 and np.median(rel) <= 1e-3
+
+
+def test_config4_reduced_tets_fp32(lcs, oracle):
+    """Config 4 reduced (pipe, Delaunay tets, fp32 data and arithmetic, bounding-box seeds with flags 0/1/2)."""
+    w = I.config4(ng=(24, 24, 40), delta=0.07, T=2.0, h=0.005, n_snap=12, length=4.0)
+    fo, Fo, flo, eso = oracle_run(oracle, w)
+    f, sd, F, flag, es = gpu_run(w)
+    cgo, fto, sto = oracle_cg(oracle, w, Fo, flo)
+    cgg, ftg, stg = gpu_cg(w, F, flag)
+    fl = cpu(flag)
+    assert (flo == 2).sum() > 100 and (flo == 1).sum() > 100 and (flo == 0).sum() > 100
+    assert np.array_equal(fl == 2, flo == 2)                             # initial location is canonical: exact
+    stats = gate_statistical(cpu(F), Fo, cpu(ftg), fto, w.L, fl, flo)
+    both1 = (fl == 1) & (flo == 1)
+    assert np.mean(np.abs(cpu(es)[both1] - eso[both1]) <= 1) > 0.999
+    print("config4 reduced", stats, "flag mismatches", int((fl != flo).sum()))
+
+
+def test_config5_reduced_backward_streamed(lcs, oracle):
+    """Config 5 reduced: backward-time windows of the ABC field with a ring of 3 device slots fed from pinned
+    host memory on the side stream; results equal the all-resident field bit for bit and pass the gate."""
+    import torch
+    w = I.config5(ngrid=24, nn=32, n_grids=3, T=2.0, h=0.01, n_snap=9)
+    f_ring = lcs.Field.from_workload(w, max_resident_snapshots=3)
+    f_all = lcs.Field.from_workload(w)
+    assert f_ring.info("ring") == 1 and f_all.info("ring") == 0
+    fo = oracle.OracleField.from_workload(w)
+    s = w.seeds()
+    for (t_rel, t_end) in w.meta["windows"]:
+        _, _, Fr, flr, esr = gpu_run(w, field=f_ring, t0=t_rel, tf=t_end, h=w.h)
+        _, _, Fa, fla, esa = gpu_run(w, field=f_all, t0=t_rel, tf=t_end, h=w.h)
+        assert torch.equal(Fr, Fa) and torch.equal(flr, fla)
+        Fo, flo, eso = fo.advect(s.astype(np.float64), t_rel, t_end, w.h)
+        cgo, fto, sto = oracle_cg(oracle, w, Fo, flo, T=t_end - t_rel)
+        cgg, ftg, stg = gpu_cg(w, Fr, flr, T=t_end - t_rel)
+        stats = gate_statistical(cpu(Fr), Fo, cpu(ftg), fto, w.L, cpu(flr), flo)
+    assert f_ring.info("h2d_bytes") > 0
+    print("config5 reduced", stats)
+
+
+# -------------------------------------------------------------------------------------------------
+# closed forms directly on the GPU path, all mesh kinds and dtypes
+@pytest.mark.parametrize("mesh", ["cart2", "cart3", "tri", "tet"])
+@pytest.mark.parametrize("cdt", [np.float64, np.float32])
+def test_linear_flow_closed_form(lcs, oracle, mesh, cdt):
+    """u = A x: x_N = P(hA)^N x0 and C = G^T G with G = P(hA)^N (pin P3), for fp64 and fp32 arithmetic."""
+    import torch
+    from test_oracle_pins import MESHES, P, seedkw
+    mk, d = MESHES[mesh]
+    rng = np.random.default_rng(21)
+    A = rng.normal(size=(d, d)) * 0.25
+    A -= np.eye(d) * np.trace(A) / d
+    h, N = 0.125, 16
+    w = mk(I.linear_flow(A), t0=0.0, tf=h * N, h=h, **seedkw(d))
+    if cdt == np.float32:
+        w.vel = w.vel.astype(np.float32)
+        w.compute_dtype = np.dtype(np.float32)
+    f, sd, F, flag, es = gpu_run(w)
+    M = np.linalg.matrix_power(P(h * A), N)
+    s = w.seeds().astype(np.float64)
+    tol = 2e-12 if cdt == np.float64 else 2e-5
+    assert np.all(cpu(flag) == 0)
+    assert np.max(np.abs(cpu(F) - s @ M.T)) < tol
+    cgg, ftg, stg = gpu_cg(w, F, flag)
+    Cref = (M.T @ M)[np.triu_indices(d)]
+    lam = np.linalg.eigvalsh(M.T @ M)[-1]
+    if cdt == np.float64:
+        assert np.max(np.abs(cpu(cgg) - Cref)) < 1e-9
+        assert np.max(np.abs(cpu(ftg) - np.log(lam) / (2 * h * N))) < 1e-10
+
+
+def test_mixed_precision_f32_data_f64_arithmetic(lcs, oracle):
+    """fp32 velocity storage with fp64 arithmetic: matches the oracle (which widens on read) to the fp64 gate."""
+    w = I.config1(ng=(64, 32))
+    w.vel = w.vel.astype(np.float32)
+    fo, Fo, flo, eso = oracle_run(oracle, w)
+    f, sd, F, flag, es = gpu_run(w)
+    assert np.max(np.abs(cpu(F) - Fo)) < 1e-10
+    w3 = I.config3(ngrid=16, nn=16, T=1.0, n_snap=4)
+    w3.compute_dtype = np.dtype(np.float64)
+    fo, Fo, flo, eso = oracle_run(oracle, w3)
+    f, sd, F, flag, es = gpu_run(w3)
+    assert np.max(np.abs(cpu(F) - Fo)) < 1e-10
+
+
+# -------------------------------------------------------------------------------------------------
+# edge cases
+def test_exit_handling_matches_oracle(lcs, oracle):
+    """Open box with uniform flow: flags 0/1/2, exit_step and frozen positions equal the oracle's."""
+    for dim in (2, 3):
+        c = np.array([1.0, 0.13, -0.07])[:dim]
+        w = I.analytic_cartesian(dim, I.linear_flow(np.zeros((dim, dim)), c), (5,) * dim, (0.0,) * dim, (1.0,) * dim,
+                                 (0.0, 10.0), ng=(16,) * dim, seed_lo=(-0.5,) * dim, seed_spacing=(0.31,) * dim,
+                                 t0=0.0, tf=5.0, h=0.25)
+        fo, Fo, flo, eso = oracle_run(oracle, w)
+        f, sd, F, flag, es = gpu_run(w)
+        assert set(np.unique(flo)) == {0, 1, 2}
+        assert np.array_equal(cpu(flag), flo) and np.array_equal(cpu(es), eso)
+        assert np.max(np.abs(cpu(F) - Fo)) < 1e-12
+        cgo, fto, sto = oracle_cg(oracle, w, Fo, flo)
+        cgg, ftg, stg = gpu_cg(w, F, flag)
+        assert np.array_equal(cpu(stg), sto)
+        ok = np.isfinite(fto)
+        assert np.array_equal(np.isfinite(cpu(ftg)), ok) and np.allclose(cpu(ftg)[ok], fto[ok], atol=1e-9)
+
+
+def test_exit_handling_simplex(lcs, oracle):
+    w = I.config2(ng=(40, 20), lattice=(30, 15), T=3.0)
+    s = I.seed_grid(2, (40, 20, 1), (-0.2, -0.1, 0), (2.4 / 40, 1.2 / 20, 1.0))       # some seeds outside the rectangle
+    w.vel = I.sample_field(I.linear_flow(np.zeros((2, 2)), [0.3, 0.05]), w.vertices, w.times, np.float64)
+    fo, Fo, flo, eso = oracle_run(oracle, w, seeds=s)
+    f, sd, F, flag, es = gpu_run(w, seeds=s)
+    assert set(np.unique(flo)) == {0, 1, 2}
+    assert np.array_equal(cpu(flag) == 2, flo == 2)
+    assert np.mean(cpu(flag) == flo) > 0.995
+    same = cpu(flag) == flo
+    assert np.max(np.abs(cpu(F)[same] - Fo[same])) < 1e-9
+    assert np.mean(np.abs(cpu(es)[same] - eso[same]) <= 1) == 1.0
+
+
+def test_steps_straddling_snapshots(lcs, oracle):
+    """h that does not divide the snapshot spacing: steps straddle snapshot times and each stage time takes
+    its own bracket (single-step windows)."""
+    w = I.config1(ng=(48, 24), T=6.0, h=0.3)
+    fo, Fo, flo, eso = oracle_run(oracle, w, t0=0.35, tf=6.35, h=0.3)
+    f, sd, F, flag, es = gpu_run(w, t0=0.35, tf=6.35, h=0.3)
+    assert np.max(np.abs(cpu(F) - Fo)) < 1e-10
+    assert f.info("windows") > 6
+    # backward, fp64
+    fo, Fo, flo, eso = oracle_run(oracle, w, t0=6.0, tf=0.0, h=-0.1)
+    f, sd, F, flag, es = gpu_run(w, t0=6.0, tf=0.0, h=-0.1)
+    assert np.max(np.abs(cpu(F) - Fo)) < 1e-10
+
+
+def test_argument_errors_and_empty(lcs):
+    import torch
+    w = I.config1(ng=(8, 4))
+    f = lcs.Field.from_workload(w)
+    sd = torch.from_numpy(w.seeds()).cuda()
+    for (t0, tf, h, status) in ((0.0, 1.0, -0.1, 1), (0.0, 1.0, 0.0, 1), (0.0, 1.0, 0.3, 1), (0.0, 11.0, 0.1, 2), (-1.0, 1.0, 0.1, 2)):
+        with pytest.raises(lcs.LcsError) as e:
+            f.advect(sd, t0, tf, h)
+        assert e.value.status == status, (t0, tf, h, str(e.value))
+    F, flag, es = f.advect(sd[:0].contiguous(), 0.0, 1.0, 0.1)
+    assert F.shape[0] == 0
+    with pytest.raises(lcs.LcsError) as e:
+        bad = I.config2(ng=(4, 4), lattice=(6, 5))
+        bad.cells = bad.cells.copy()
+        bad.cells[3, 1] = 10 ** 6
+        lcs.Field.from_workload(bad)
+    assert e.value.status == 3
+    f2 = lcs.Field(2, 0, w.times, np.float64, np.float64, n=w.n, origin=w.origin, spacing=w.spacing)
+    with pytest.raises(lcs.LcsError) as e:
+        f2.advect(sd, 0.0, 1.0, 0.1)                                    # snapshots never set
+    assert e.value.status == 6
+
+
+def test_aliasing_and_host_api(lcs, oracle):
+    """flowmap may alias seeds; lcs_ftle_host (host buffers, copies inside the call) equals the device path."""
+    import torch
+    w = I.config1(ng=(64, 32), T=4.0)
+    f, sd, F, flag, es = gpu_run(w)
+    sd2 = sd.clone()
+    f.advect(sd2, w.t0, w.tf, w.h, flowmap=sd2)
+    torch.cuda.synchronize()
+    assert torch.equal(sd2, F)
+    cgg, ftg, stg = gpu_cg(w, F, flag)
+    Fh = np.empty((w.n_seeds, 2))
+    flh = np.empty(w.n_seeds, np.uint8)
+    ft = f.ftle_host(w.ng, w.seed_spacing, w.seed_periodic, w.period, w.seeds(), w.t0, w.tf, w.h, flowmap=Fh, exit_flag=flh)
+    assert np.array_equal(Fh, cpu(F)) and np.array_equal(ft, cpu(ftg), equal_nan=True) and np.array_equal(flh, cpu(flag))
+
+
+def test_cg_ftle_patterns_vs_oracle(lcs, oracle):
+    """lcs_cg_ftle alone on synthetic flow maps: random exit flags (one-sided / NaN patterns), periodic seams,
+    2D and 3D, fp64 and fp32 storage, ragged grid sizes."""
+    import torch
+    rng = np.random.default_rng(35)
+    for dim, ng, per in ((2, (37, 19), (0, 0)), (2, (16, 16), (1, 0)), (3, (13, 9, 11), (0, 0, 0)), (3, (8, 8, 8), (1, 1, 1)), (2, (5, 1), (0, 0))):
+        n = int(np.prod(ng))
+        dx = tuple(rng.uniform(0.1, 0.5, dim))
+        period = tuple(ng[a] * dx[a] for a in range(dim))
+        s = I.seed_grid(dim, tuple(ng) + (1,) * (3 - dim), (0, 0, 0), dx + (1.0,) * (3 - dim))
+        F = s + 0.3 * np.sin(2 * np.pi * s / np.array(period)) @ rng.normal(size=(dim, dim)) + rng.normal(size=s.shape) * 0.01
+        flag = (rng.uniform(size=n) < 0.15).astype(np.uint8) * rng.integers(1, 3, n).astype(np.uint8)
+        for dt in (np.float64, np.float32):
+            Fd = F.astype(dt)
+            cgo, fto, sto = oracle.cg_ftle(dim, ng, dx, per, period, Fd.astype(np.float64), flag, 3.0)
+            cgg, ftg, stg = lcs.cg_ftle(dim, ng, dx, per, period, torch.from_numpy(Fd).cuda(), torch.from_numpy(flag).cuda(), 3.0)
+            assert np.array_equal(cpu(stg), sto)
+            ok = np.isfinite(fto)
+            assert np.array_equal(np.isfinite(cpu(ftg)), ok)
+            tol = 1e-12 if dt == np.float64 else 2e-6
+            assert np.allclose(cpu(ftg)[ok], fto[ok], rtol=tol, atol=tol)
+            assert np.allclose(cpu(cgg)[ok], cgo[ok], rtol=tol * 10, atol=tol)
+        cgn, ftn, _ = lcs.cg_ftle(dim, ng, dx, per, period, torch.from_numpy(F).cuda(), None, 3.0, want_cg=False, want_status=False)
+        cgo, fto, sto = oracle.cg_ftle(dim, ng, dx, per, period, F, None, 3.0)
+        assert cgn is None and np.allclose(cpu(ftn), fto, rtol=1e-12, atol=1e-12, equal_nan=True)
