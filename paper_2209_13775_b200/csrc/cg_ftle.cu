@@ -80,8 +80,11 @@ __global__ void __launch_bounds__(256) cg_ftle_kernel(const __grid_constant__ Cg
             else if (okm) v = (F0[a] - Fm) * g.inv_dx[b];
             G[a][b] = v;
         }
-        if (!okp && !okm) st |= 1;
-        else if (!(okp && okm)) st |= 2;
+        // status bits accumulate axis by axis until the seed becomes undefined (as the oracle's rule O5 does)
+        if (!(st & 1)) {
+            if (!okp && !okm) st |= 1;
+            else if (!(okp && okm)) st |= 2;
+        }
     }
     double C[NCG], lam;
     if (st & 1) {

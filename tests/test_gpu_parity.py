@@ -264,7 +264,7 @@ def test_mixed_precision_f32_data_f64_arithmetic(lcs, oracle):
 def test_exit_handling_matches_oracle(lcs, oracle):
     """Open box with uniform flow: flags 0/1/2, exit_step and frozen positions equal the oracle's."""
     for dim in (2, 3):
-        c = np.array([1.0, 0.13, -0.07])[:dim]
+        c = np.array([0.3, 0.13, -0.07])[:dim]
         w = I.analytic_cartesian(dim, I.linear_flow(np.zeros((dim, dim)), c), (5,) * dim, (0.0,) * dim, (1.0,) * dim,
                                  (0.0, 10.0), ng=(16,) * dim, seed_lo=(-0.5,) * dim, seed_spacing=(0.31,) * dim,
                                  t0=0.0, tf=5.0, h=0.25)
