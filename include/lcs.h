@@ -85,8 +85,11 @@ void lcs_field_destroy(lcs_field *f);
 
 /* Integer options.  Keys: "integrator" 0 = auto, 1 = fused (one persistent per-seed loop per snapshot
  * window), 2 = split (one short kernel per RK4 stage, tracers advance synchronously: PAPER.md:85);
- * "sort_seeds" 0/1 = process tracers in cell order (results are returned in the caller's order);
- * "resort_every" k = re-bundle tracers by cell every k snapshot windows (0 = never).   */
+ * "bundle" -1 = auto, 0 = off, 1 = on: re-bundle tracers by cell (Morton order of the cell index) so that a
+ * warp gathers from neighbouring cells; results are returned in the caller's order;
+ * "bundle_steps" k = re-bundle every k RK4 steps (0 = once per snapshot window);
+ * "ld256" 0/1 = gather each 32-byte node record with one 256-bit load; "block" = threads per block;
+ * "time_windows" 0/1 = record CUDA events around the integrator launches (read with lcs_field_get_info). */
 lcs_status lcs_field_set_option(lcs_field *f, const char *key, int64_t value);
 lcs_status lcs_field_get_info(const lcs_field *f, const char *key, int64_t *value);
 

@@ -10,7 +10,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liblcs.so")
 SOURCES = ["field.cu", "advect_cart.cu", "cg_ftle.cu", "simplex.cu"]
-HEADERS = [os.path.join(CSRC, "lcs_internal.cuh"), os.path.join(HERE, "..", "include", "lcs.h")]
+HEADERS = [os.path.join(CSRC, "lcs_internal.cuh"), os.path.join(CSRC, "bundle_sort.cuh"), os.path.join(HERE, "..", "include", "lcs.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr", "-Xcudafe", "--diag_suppress=177"]
 
@@ -44,7 +44,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
             for out in ex.map(run, jobs):
                 if verbose and out:
                     print(out, file=sys.stderr)
-    if jobs or not os.path.exists(LIB):
+    if jobs or not os.path.exists(LIB) or os.path.getmtime(LIB) < max(os.path.getmtime(o) for o in objs):
         tmp = LIB + ".tmp.%d" % os.getpid()
         run([_nvcc(), "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", tmp] + objs + ["-lcudart"])
         os.replace(tmp, LIB)

@@ -11,12 +11,19 @@
 //    interpolation weights need, the index is what the gather addresses need, periodic wrap is a mask on
 //    the index and never touches the stored position, and an fp32 offset carries ~1e-7 of a CELL instead
 //    of ~1e-7 of the domain.  Physical positions exist only at the API boundary (fp64 conversion).
-//  * gathers read "pair records" {a, b-a}: both time levels of a node in one 32-byte sector, the time
-//    blend is one FMA per component.
+//  * the tracer state is one 32-byte record (array of structures): one sector in, one sector out per
+//    launch, and re-bundling moves whole sectors.
+//  * gathers read "pair records" {a, b-a}: both time levels of a node in one 32-byte sector (one 256-bit
+//    load), the time blend is one FMA per component.  The record array is padded by one node per axis so
+//    that the 2^d corners of a cell sit at constant offsets from one base address.
+//  * tracers are re-bundled by cell (Morton order) once per snapshot window, so that the 32 tracers of a
+//    warp gather from 2x2x1 neighbouring cells: the kernel is bound by L1 wavefronts, and a wavefront
+//    serves one 128-byte line per instruction (profiles/r1_cfg3_baseline.md).
 //  * fused variant: one thread runs every RK4 step of a snapshot window; split variant (the paper's): one
-//    short kernel per RK4 stage with the tracer state in global memory.
+//    short kernel per RK4 stage with the stage state in global memory.
 #include <math.h>
 
+#include "bundle_sort.cuh"
 #include "lcs_internal.cuh"
 
 namespace {
@@ -25,43 +32,80 @@ struct CartDev {
     int n[3];
     int periodic[3];
     int pow2[3];
+    int np0, np01;         // padded record strides: np0 = n0 + 1, np01 = (n0 + 1) * (n1 + 1)
     double origin[3], spacing[3], inv[3];
 };
 
-template <typename TC> struct CartState {
-    int32_t *ci[3];
-    TC *w[3];
-    int32_t *steps;
-    uint8_t *flag;
+// tracer record.  meta = completed steps at exit (low 30 bits) | exit flag << 30
+template <int DIM, typename TC> struct alignas(16) CartTracer {
+    TC w[DIM];
+    int32_t ci[DIM];
+    int32_t orig;
+    uint32_t meta;
 };
+static_assert(sizeof(CartTracer<3, float>) == 32 && sizeof(CartTracer<2, double>) == 32, "one sector per tracer");
 
-template <typename T> struct Vec2 {};
-template <> struct Vec2<float> { using type = float2; };
-template <> struct Vec2<double> { using type = double2; };
+template <typename REC> __device__ __forceinline__ REC load_record(const REC *p)
+{
+    REC r;
+    constexpr int NQ = sizeof(REC) / 16;
+    const int4 *s = reinterpret_cast<const int4 *>(p);
+    int4 *d = reinterpret_cast<int4 *>(&r);
+#pragma unroll
+    for (int k = 0; k < NQ; ++k) d[k] = s[k];
+    return r;
+}
+template <typename REC> __device__ __forceinline__ void store_record(REC *p, const REC &r)
+{
+    constexpr int NQ = sizeof(REC) / 16;
+    const int4 *s = reinterpret_cast<const int4 *>(&r);
+    int4 *d = reinterpret_cast<int4 *>(p);
+#pragma unroll
+    for (int k = 0; k < NQ; ++k) d[k] = s[k];
+}
 
-// time-blended velocity at one node: out = a + tau * d  (one FMA per component)
-template <int DIM, typename TV, typename TC>
-__device__ __forceinline__ void node_velocity(const PairRec<DIM, TV> *__restrict__ rec, int64_t node, TC tau, TC *out)
+// time-blended velocity at one node: out = a + tau * d  (one FMA per component).  LD256: the 32-byte record is
+// fetched with one 256-bit load (sm_100 ld.global.v8.b32 / v4.b64), i.e. one L1 request per corner.
+template <int DIM, typename TV, typename TC, bool LD256>
+__device__ __forceinline__ void node_velocity(const PairRec<DIM, TV> *__restrict__ p, TC tau, TC *out)
 {
     if constexpr (DIM == 3 && sizeof(TV) == 4) {
-        const float4 *p = reinterpret_cast<const float4 *>(rec + node);
-        float4 a = __ldg(p), d = __ldg(p + 1);
+        float4 a, d;
+        if constexpr (LD256) {
+            asm("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                : "=f"(a.x), "=f"(a.y), "=f"(a.z), "=f"(a.w), "=f"(d.x), "=f"(d.y), "=f"(d.z), "=f"(d.w) : "l"(p));
+        } else {
+            const float4 *q = reinterpret_cast<const float4 *>(p);
+            a = __ldg(q); d = __ldg(q + 1);
+        }
         out[0] = fma(tau, (TC)d.x, (TC)a.x);
         out[1] = fma(tau, (TC)d.y, (TC)a.y);
         out[2] = fma(tau, (TC)d.z, (TC)a.z);
     } else if constexpr (DIM == 3) {
-        const double2 *p = reinterpret_cast<const double2 *>(rec + node);
-        double2 a0 = __ldg(p), a1 = __ldg(p + 1), d0 = __ldg(p + 2), d1 = __ldg(p + 3);
+        double2 a0, a1, d0, d1;
+        if constexpr (LD256) {
+            asm("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(a0.x), "=d"(a0.y), "=d"(a1.x), "=d"(a1.y) : "l"(p));
+            asm("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(d0.x), "=d"(d0.y), "=d"(d1.x), "=d"(d1.y)
+                : "l"(reinterpret_cast<const char *>(p) + 32));
+        } else {
+            const double2 *q = reinterpret_cast<const double2 *>(p);
+            a0 = __ldg(q); a1 = __ldg(q + 1); d0 = __ldg(q + 2); d1 = __ldg(q + 3);
+        }
         out[0] = fma(tau, (TC)d0.x, (TC)a0.x);
         out[1] = fma(tau, (TC)d0.y, (TC)a0.y);
         out[2] = fma(tau, (TC)d1.x, (TC)a1.x);
     } else if constexpr (sizeof(TV) == 8) {
-        const double2 *p = reinterpret_cast<const double2 *>(rec + node);
-        double2 a = __ldg(p), d = __ldg(p + 1);
+        double2 a, d;
+        if constexpr (LD256) {
+            asm("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(a.x), "=d"(a.y), "=d"(d.x), "=d"(d.y) : "l"(p));
+        } else {
+            const double2 *q = reinterpret_cast<const double2 *>(p);
+            a = __ldg(q); d = __ldg(q + 1);
+        }
         out[0] = fma(tau, (TC)d.x, (TC)a.x);
         out[1] = fma(tau, (TC)d.y, (TC)a.y);
     } else {
-        float4 r = __ldg(reinterpret_cast<const float4 *>(rec + node));
+        float4 r = __ldg(reinterpret_cast<const float4 *>(p));
         out[0] = fma(tau, (TC)r.z, (TC)r.x);
         out[1] = fma(tau, (TC)r.w, (TC)r.y);
     }
@@ -74,39 +118,54 @@ __device__ __forceinline__ int wrap_index(int c, int n, int pow2)
     return r < 0 ? r + n : r;
 }
 
+// x -> (floor(x) as int, x - floor(x)).  fp32: floor through an add rounded toward -inf onto 1.5 * 2^23, whose low mantissa
+// bits then hold the integer (exact for |x| < 2^22 cells): three FP32-pipe instructions instead of FRND + F2I on the
+// quarter-rate conversion unit.
+template <typename TC> __device__ __forceinline__ void floor_split(TC x, int &ifl, TC &frac)
+{
+    if constexpr (sizeof(TC) == 4) {
+        const float t = __fadd_rd(x, 12582912.0f);
+        ifl = __float_as_int(t) - 0x4B400000;
+        frac = x - (t - 12582912.0f);
+    } else {
+        const TC f = floor(x);
+        ifl = (int)f;
+        frac = x - f;
+    }
+}
+
 // u(x,t) at the point (ci + xi) in grid units, xi = offset relative to the tracer's cell (any magnitude).
 // Returns false if the point is outside a non-periodic axis (closed upper end, as in oracle rule O2).
-template <int DIM, typename TV, typename TC, bool FASTWRAP>
+// FASTWRAP: every axis periodic with a power-of-two node count (mask wrap, no branches).
+template <int DIM, typename TV, typename TC, bool FASTWRAP, bool LD256>
 __device__ __forceinline__ bool cart_velocity(const CartDev &g, const PairRec<DIM, TV> *__restrict__ rec, TC tau,
                                               const int *ci, const TC *xi, TC *u)
 {
-    int lo[DIM], hi[DIM];
+    int lo[DIM];
     TC wl[DIM];
 #pragma unroll
     for (int a = 0; a < DIM; ++a) {
-        TC fl = floor(xi[a]);
-        wl[a] = xi[a] - fl;
-        int c = ci[a] + (int)fl;
+        int ifl;
+        floor_split<TC>(xi[a], ifl, wl[a]);
+        int c = ci[a] + ifl;
         if constexpr (FASTWRAP) {
             lo[a] = c & (g.n[a] - 1);
-            hi[a] = (c + 1) & (g.n[a] - 1);
         } else if (g.periodic[a]) {
             lo[a] = wrap_index(c, g.n[a], g.pow2[a]);
-            hi[a] = lo[a] + 1 == g.n[a] ? 0 : lo[a] + 1;
         } else {
             if (c == g.n[a] - 1 && wl[a] == TC(0)) { c = g.n[a] - 2; wl[a] = TC(1); }
             if (c < 0 || c > g.n[a] - 2) return false;
             lo[a] = c;
-            hi[a] = c + 1;
         }
     }
+    using Rec = PairRec<DIM, TV>;
     if constexpr (DIM == 2) {
-        int64_t r0 = (int64_t)lo[1] * g.n[0], r1 = (int64_t)hi[1] * g.n[0];
+        const Rec *b = rec + (lo[0] + lo[1] * g.np0);
         TC v00[2], v10[2], v01[2], v11[2];
-        node_velocity<2, TV, TC>(rec, r0 + lo[0], tau, v00);
-        node_velocity<2, TV, TC>(rec, r0 + hi[0], tau, v10);
-        node_velocity<2, TV, TC>(rec, r1 + lo[0], tau, v01);
-        node_velocity<2, TV, TC>(rec, r1 + hi[0], tau, v11);
+        node_velocity<2, TV, TC, LD256>(b, tau, v00);
+        node_velocity<2, TV, TC, LD256>(b + 1, tau, v10);
+        node_velocity<2, TV, TC, LD256>(b + g.np0, tau, v01);
+        node_velocity<2, TV, TC, LD256>(b + g.np0 + 1, tau, v11);
 #pragma unroll
         for (int c = 0; c < 2; ++c) {
             TC a0 = fma(wl[0], v10[c] - v00[c], v00[c]);
@@ -114,18 +173,16 @@ __device__ __forceinline__ bool cart_velocity(const CartDev &g, const PairRec<DI
             u[c] = fma(wl[1], a1 - a0, a0);
         }
     } else {
-        int64_t n0 = g.n[0], n01 = (int64_t)g.n[0] * g.n[1];
-        int64_t r00 = lo[1] * n0 + lo[2] * n01, r10 = hi[1] * n0 + lo[2] * n01;
-        int64_t r01 = lo[1] * n0 + hi[2] * n01, r11 = hi[1] * n0 + hi[2] * n01;
+        const Rec *b = rec + (lo[0] + lo[1] * g.np0 + lo[2] * g.np01);
         TC v[8][3];
-        node_velocity<3, TV, TC>(rec, r00 + lo[0], tau, v[0]);
-        node_velocity<3, TV, TC>(rec, r00 + hi[0], tau, v[1]);
-        node_velocity<3, TV, TC>(rec, r10 + lo[0], tau, v[2]);
-        node_velocity<3, TV, TC>(rec, r10 + hi[0], tau, v[3]);
-        node_velocity<3, TV, TC>(rec, r01 + lo[0], tau, v[4]);
-        node_velocity<3, TV, TC>(rec, r01 + hi[0], tau, v[5]);
-        node_velocity<3, TV, TC>(rec, r11 + lo[0], tau, v[6]);
-        node_velocity<3, TV, TC>(rec, r11 + hi[0], tau, v[7]);
+        node_velocity<3, TV, TC, LD256>(b, tau, v[0]);
+        node_velocity<3, TV, TC, LD256>(b + 1, tau, v[1]);
+        node_velocity<3, TV, TC, LD256>(b + g.np0, tau, v[2]);
+        node_velocity<3, TV, TC, LD256>(b + g.np0 + 1, tau, v[3]);
+        node_velocity<3, TV, TC, LD256>(b + g.np01, tau, v[4]);
+        node_velocity<3, TV, TC, LD256>(b + g.np01 + 1, tau, v[5]);
+        node_velocity<3, TV, TC, LD256>(b + g.np01 + g.np0, tau, v[6]);
+        node_velocity<3, TV, TC, LD256>(b + g.np01 + g.np0 + 1, tau, v[7]);
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
             TC a00 = fma(wl[0], v[1][c] - v[0][c], v[0][c]);
@@ -144,11 +201,13 @@ __device__ __forceinline__ bool cart_velocity(const CartDev &g, const PairRec<DI
 // seeds (physical, compute dtype) -> (cell, offset) state.  fp64 arithmetic, the oracle's O2 formula, so
 // the initial cell agrees with lcs_locate.  flag 2 = seed outside at t0.
 template <int DIM, typename TC>
-__global__ void __launch_bounds__(256) cart_init_kernel(CartDev g, const TC *__restrict__ seeds, int64_t n, CartState<TC> st)
+__global__ void __launch_bounds__(256) cart_init_kernel(CartDev g, const TC *__restrict__ seeds, int64_t n,
+                                                         CartTracer<DIM, TC> *__restrict__ st)
 {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    uint8_t fl = 0;
+    CartTracer<DIM, TC> t;
+    uint32_t fl = 0;
 #pragma unroll
     for (int a = 0; a < DIM; ++a) {
         double xi = ((double)seeds[i * DIM + a] - g.origin[a]) * g.inv[a];
@@ -159,81 +218,152 @@ __global__ void __launch_bounds__(256) cart_init_kernel(CartDev g, const TC *__r
             if (!(xi >= 0.0 && xi <= (double)(g.n[a] - 1))) { fl = 2; c = 0; w = 0; }
             else if (c == g.n[a] - 1) { c = g.n[a] - 2; w = 1.0; }
         }
-        st.ci[a][i] = c;
-        st.w[a][i] = (TC)w;
+        t.ci[a] = c;
+        t.w[a] = (TC)w;
     }
-    st.flag[i] = fl;
-    st.steps[i] = 0;
+    t.orig = (int32_t)i;
+    t.meta = fl << 30;
+    store_record(st + i, t);
 }
 
-// (cell, offset) -> physical flow map + flags
+// (cell, offset) -> physical flow map + flags, scattered back to the caller's seed order
 template <int DIM, typename TC>
-__global__ void __launch_bounds__(256) cart_final_kernel(CartDev g, const TC *__restrict__ seeds, int64_t n, CartState<TC> st,
-                                                          int32_t N, TC *__restrict__ flowmap, uint8_t *__restrict__ exit_flag,
+__global__ void __launch_bounds__(256) cart_final_kernel(CartDev g, const TC *__restrict__ seeds, int64_t n,
+                                                          const CartTracer<DIM, TC> *__restrict__ st, int32_t N,
+                                                          TC *__restrict__ flowmap, uint8_t *__restrict__ exit_flag,
                                                           int32_t *__restrict__ exit_step)
 {
-    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    uint8_t fl = st.flag[i];
+    int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= n) return;
+    const CartTracer<DIM, TC> t = load_record(st + j);
+    const int64_t i = t.orig;
+    const uint32_t fl = t.meta >> 30;
     TC out[DIM];
 #pragma unroll
     for (int a = 0; a < DIM; ++a) {
         if (fl == 2) out[a] = seeds[i * DIM + a];
-        else out[a] = (TC)(g.origin[a] + ((double)st.ci[a][i] + (double)st.w[a][i]) * g.spacing[a]);
+        else out[a] = (TC)(g.origin[a] + ((double)t.ci[a] + (double)t.w[a]) * g.spacing[a]);
     }
 #pragma unroll
     for (int a = 0; a < DIM; ++a) flowmap[i * DIM + a] = out[a];
-    if (exit_flag) exit_flag[i] = fl;
-    if (exit_step) exit_step[i] = fl == 0 ? N : (fl == 2 ? 0 : st.steps[i]);
+    if (exit_flag) exit_flag[i] = (uint8_t)fl;
+    if (exit_step) exit_step[i] = fl == 0 ? N : (fl == 2 ? 0 : (int32_t)(t.meta & 0x3fffffffu));
+}
+
+// sort key of a tracer: Morton code of its (wrapped) cell, coarsened by `shift` bits per axis; finished tracers
+// (flag != 0) go to the last bin so that their warps retire at once
+template <int DIM, typename TC>
+__global__ void __launch_bounds__(256) cart_key_kernel(CartDev g, const CartTracer<DIM, TC> *__restrict__ st, int64_t n, int shift,
+                                                        uint32_t last_bin, uint32_t *__restrict__ key, uint32_t *__restrict__ cnt)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const CartTracer<DIM, TC> t = load_record(st + i);
+    uint32_t k = last_bin;
+    if ((t.meta >> 30) == 0) {
+        int c[DIM];
+#pragma unroll
+        for (int a = 0; a < DIM; ++a) c[a] = (g.periodic[a] ? wrap_index(t.ci[a], g.n[a], g.pow2[a]) : t.ci[a]) >> shift;
+        k = bundle::morton<DIM>(c);
+        if (k > last_bin - 1) k = last_bin - 1;
+    }
+    key[i] = k;
+    atomicAdd(cnt + k, 1u);
 }
 
 // ---------------------------------------------------------------------------------------------
 // Fused variant: one thread = one tracer, every RK4 step of the window.  hs[a] = h / spacing[a] turns a
 // physical velocity into cells per step.  tau: [nsteps][3] time weights of (ta, tb, tc).
-template <int DIM, typename TV, typename TC, bool FASTWRAP>
+template <int DIM, typename TV, typename TC, bool FASTWRAP, bool LD256>
 __global__ void __launch_bounds__(256)
 cart_window_kernel(const __grid_constant__ CartDev g, const PairRec<DIM, TV> *__restrict__ pa,
                    const PairRec<DIM, TV> *__restrict__ pb, const PairRec<DIM, TV> *__restrict__ pc,
-                   const TC *__restrict__ tau, int nsteps, int first_step, int64_t n, CartState<TC> st, TC hs0, TC hs1, TC hs2)
+                   const TC *__restrict__ tau, int nsteps, int first_step, int64_t n, CartTracer<DIM, TC> *__restrict__ st,
+                   TC hs0, TC hs1, TC hs2)
 {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    if (st.flag[i] != 0) return;
+    CartTracer<DIM, TC> t = load_record(st + i);
+    if ((t.meta >> 30) != 0) return;
     const TC hs[3] = {hs0, hs1, hs2};
     int ci[DIM];
     TC w[DIM];
 #pragma unroll
-    for (int a = 0; a < DIM; ++a) { ci[a] = st.ci[a][i]; w[a] = st.w[a][i]; }
+    for (int a = 0; a < DIM; ++a) { ci[a] = t.ci[a]; w[a] = t.w[a]; }
     int s = 0;
     bool ok = true;
     for (; s < nsteps; ++s) {
         const TC ta = __ldg(tau + 3 * s), tb = __ldg(tau + 3 * s + 1), tc = __ldg(tau + 3 * s + 2);
         TC k1[DIM], k2[DIM], k3[DIM], k4[DIM], xi[DIM];
-        ok = cart_velocity<DIM, TV, TC, FASTWRAP>(g, pa, ta, ci, w, k1);
+        ok = cart_velocity<DIM, TV, TC, FASTWRAP, LD256>(g, pa, ta, ci, w, k1);
         if (!ok) break;
 #pragma unroll
         for (int a = 0; a < DIM; ++a) xi[a] = fma(TC(0.5) * hs[a], k1[a], w[a]);
-        ok = cart_velocity<DIM, TV, TC, FASTWRAP>(g, pb, tb, ci, xi, k2);
+        ok = cart_velocity<DIM, TV, TC, FASTWRAP, LD256>(g, pb, tb, ci, xi, k2);
         if (!ok) break;
 #pragma unroll
         for (int a = 0; a < DIM; ++a) xi[a] = fma(TC(0.5) * hs[a], k2[a], w[a]);
-        ok = cart_velocity<DIM, TV, TC, FASTWRAP>(g, pb, tb, ci, xi, k3);
+        ok = cart_velocity<DIM, TV, TC, FASTWRAP, LD256>(g, pb, tb, ci, xi, k3);
         if (!ok) break;
 #pragma unroll
         for (int a = 0; a < DIM; ++a) xi[a] = fma(hs[a], k3[a], w[a]);
-        ok = cart_velocity<DIM, TV, TC, FASTWRAP>(g, pc, tc, ci, xi, k4);
+        ok = cart_velocity<DIM, TV, TC, FASTWRAP, LD256>(g, pc, tc, ci, xi, k4);
         if (!ok) break;
 #pragma unroll
         for (int a = 0; a < DIM; ++a) {
             TC wn = fma(hs[a] * TC(1.0 / 6.0), (k1[a] + k4[a]) + TC(2) * (k2[a] + k3[a]), w[a]);
-            TC fl = floor(wn);
-            ci[a] += (int)fl;
-            w[a] = wn - fl;
+            int ifl;
+            floor_split<TC>(wn, ifl, w[a]);
+            ci[a] += ifl;
         }
     }
 #pragma unroll
-    for (int a = 0; a < DIM; ++a) { st.ci[a][i] = ci[a]; st.w[a][i] = w[a]; }
-    if (!ok) { st.flag[i] = 1; st.steps[i] = first_step + s; }
+    for (int a = 0; a < DIM; ++a) { t.ci[a] = ci[a]; t.w[a] = w[a]; }
+    if (!ok) t.meta = (1u << 30) | (uint32_t)(first_step + s);
+    store_record(st + i, t);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Split variant (the paper's design: "the RK4 computation was divided into several short
+// kernels"; all tracers advance one stage at a time).  One launch per RK4 stage; between the launches the
+// stage point (xi) and the running sum k1 + 2 k2 + 2 k3 (acc) live in global memory as [n][DIM] arrays.
+// A tracer whose stage point leaves the domain gets its flag at once; its record (position at the start of
+// the step) is only rewritten by stage 3 of a step in which all four evaluations succeeded.
+template <int DIM, typename TV, typename TC, bool FASTWRAP, bool LD256, int STAGE>
+__global__ void __launch_bounds__(256)
+cart_stage_kernel(const __grid_constant__ CartDev g, const PairRec<DIM, TV> *__restrict__ rec, TC tau, int step, int64_t n,
+                  CartTracer<DIM, TC> *__restrict__ st, TC *__restrict__ xi_g, TC *__restrict__ acc_g, TC hs0, TC hs1, TC hs2)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    CartTracer<DIM, TC> t = load_record(st + i);
+    if ((t.meta >> 30) != 0) return;
+    const TC hs[3] = {hs0, hs1, hs2};
+    TC xi[DIM], k[DIM];
+#pragma unroll
+    for (int a = 0; a < DIM; ++a) xi[a] = STAGE == 0 ? t.w[a] : xi_g[i * DIM + a];
+    if (!cart_velocity<DIM, TV, TC, FASTWRAP, LD256>(g, rec, tau, t.ci, xi, k)) {
+        t.meta = (1u << 30) | (uint32_t)step;
+        store_record(st + i, t);
+        return;
+    }
+    if constexpr (STAGE < 3) {
+        const TC c = STAGE == 2 ? TC(1) : TC(0.5);
+#pragma unroll
+        for (int a = 0; a < DIM; ++a) {
+            xi_g[i * DIM + a] = fma(c * hs[a], k[a], t.w[a]);
+            acc_g[i * DIM + a] = STAGE == 0 ? k[a] : acc_g[i * DIM + a] + TC(2) * k[a];
+        }
+    } else {
+#pragma unroll
+        for (int a = 0; a < DIM; ++a) {
+            TC wn = fma(hs[a] * TC(1.0 / 6.0), acc_g[i * DIM + a] + k[a], t.w[a]);
+            int ifl;
+            floor_split<TC>(wn, ifl, t.w[a]);
+            t.ci[a] += ifl;
+        }
+        store_record(st + i, t);
+    }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -283,17 +413,43 @@ CartDev make_dev(const lcs_field *f)
         g.n[a] = f->cart.n[a]; g.periodic[a] = f->cart.periodic[a]; g.pow2[a] = f->cart.pow2[a];
         g.origin[a] = f->cart.origin[a]; g.spacing[a] = f->cart.spacing[a]; g.inv[a] = f->cart.inv[a];
     }
+    g.np0 = f->cart.n[0] + 1;
+    g.np01 = (f->cart.n[0] + 1) * (f->cart.n[1] + 1);
     return g;
 }
 
 size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 
+template <int DIM, typename TV, typename TC, bool FASTWRAP, bool LD256>
+void launch_window(const CartDev &g, const void *const p[3], const TC *d_tau, int first, int count, int64_t n, CartTracer<DIM, TC> *S,
+                   const TC *hs, int block, cudaStream_t st)
+{
+    using Rec = PairRec<DIM, TV>;
+    LCS_LAUNCH((cart_window_kernel<DIM, TV, TC, FASTWRAP, LD256>), lcs_blocks(n, block), block, 0, st, g, (const Rec *)p[0], (const Rec *)p[1],
+               (const Rec *)p[2], d_tau + 3 * (size_t)first, count, first, n, S, hs[0], hs[1], hs[2]);
+}
+
+// one RK4 step of the split variant = 4 launches
+template <int DIM, typename TV, typename TC, bool FASTWRAP, bool LD256>
+void launch_split_step(const CartDev &g, const void *const p[3], const TC *tau3, int step, int64_t n, CartTracer<DIM, TC> *S, TC *xi,
+                       TC *acc, const TC *hs, int block, cudaStream_t st)
+{
+    using Rec = PairRec<DIM, TV>;
+    const unsigned grid = lcs_blocks(n, block);
+    LCS_LAUNCH((cart_stage_kernel<DIM, TV, TC, FASTWRAP, LD256, 0>), grid, block, 0, st, g, (const Rec *)p[0], tau3[0], step, n, S, xi, acc, hs[0], hs[1], hs[2]);
+    LCS_LAUNCH((cart_stage_kernel<DIM, TV, TC, FASTWRAP, LD256, 1>), grid, block, 0, st, g, (const Rec *)p[1], tau3[1], step, n, S, xi, acc, hs[0], hs[1], hs[2]);
+    LCS_LAUNCH((cart_stage_kernel<DIM, TV, TC, FASTWRAP, LD256, 2>), grid, block, 0, st, g, (const Rec *)p[1], tau3[1], step, n, S, xi, acc, hs[0], hs[1], hs[2]);
+    LCS_LAUNCH((cart_stage_kernel<DIM, TV, TC, FASTWRAP, LD256, 3>), grid, block, 0, st, g, (const Rec *)p[2], tau3[2], step, n, S, xi, acc, hs[0], hs[1], hs[2]);
+}
+
 template <int DIM, typename TV, typename TC>
 lcs_status cart_advect_impl(lcs_field *f, int64_t n, const void *seeds_, double t0, double h, int64_t N, void *flowmap_,
                             uint8_t *exit_flag, int32_t *exit_step, cudaStream_t st)
 {
+    using Tracer = CartTracer<DIM, TC>;
     const TC *seeds = (const TC *)seeds_;
     TC *flowmap = (TC *)flowmap_;
+    if (n >= (1LL << 31) || N >= (1LL << 30)) { lcs_set_error("too many seeds or steps for 32-bit tracer records"); return LCS_ERR_INVALID_ARG; }
     std::vector<StepWindow> windows;
     std::vector<double> tau64;
     lcs_status rc = lcs_plan_windows(f, t0, h, N, windows, tau64);
@@ -301,31 +457,58 @@ lcs_status cart_advect_impl(lcs_field *f, int64_t n, const void *seeds_, double 
     std::vector<TC> tau(tau64.size());
     for (size_t k = 0; k < tau.size(); ++k) tau[k] = (TC)tau64[k];
 
+    const bool split = f->opt_integrator == 2;
+    const bool do_bundle = f->opt_bundle == 1 || (f->opt_bundle < 0 && n >= (1 << 20));
+    // sort bins: Morton code of the cell index, coarsened so that the histogram stays <= 2^24 bins
+    int shift = 0, bits = 0;
+    for (;; ++shift) {
+        bits = 0;
+        for (int a = 0; a < DIM; ++a) {
+            int cells = ((f->cart.n[a] - 1) >> shift) + 1, b = 0;
+            while ((1 << b) < cells) ++b;
+            bits = b > bits ? b : bits;
+        }
+        if (bits * DIM <= 24) break;
+    }
+    const int64_t nbins = do_bundle ? ((int64_t)1 << (bits * DIM)) + 1 : 0;
+
     // carve the tracer scratch
-    size_t off = 0, o_ci[3], o_w[3], o_steps, o_flag, o_tau;
-    for (int a = 0; a < DIM; ++a) { o_ci[a] = off; off = align_up(off + (size_t)n * 4); }
-    for (int a = 0; a < DIM; ++a) { o_w[a] = off; off = align_up(off + (size_t)n * sizeof(TC)); }
-    o_steps = off; off = align_up(off + (size_t)n * 4);
-    o_flag = off; off = align_up(off + (size_t)n);
-    o_tau = off; off = align_up(off + tau.size() * sizeof(TC));
+    size_t off = 0;
+    const size_t o_a = off; off = align_up(off + (size_t)n * sizeof(Tracer));
+    const size_t o_b = off; if (do_bundle) off = align_up(off + (size_t)n * sizeof(Tracer));
+    const size_t o_xi = off; if (split) off = align_up(off + (size_t)n * DIM * sizeof(TC));
+    const size_t o_acc = off; if (split) off = align_up(off + (size_t)n * DIM * sizeof(TC));
+    const size_t o_tau = off; off = align_up(off + tau.size() * sizeof(TC));
+    const int64_t ntiles = (nbins + bundle::kScanTile - 1) / bundle::kScanTile;
+    const size_t o_key = off; if (do_bundle) off = align_up(off + (size_t)n * 4);
+    const size_t o_cnt = off; if (do_bundle) off = align_up(off + (size_t)nbins * 4);
+    const size_t o_tile = off; if (do_bundle) off = align_up(off + (size_t)ntiles * 4);
     rc = lcs_scratch_reserve(f, off);
     if (rc != LCS_OK) return rc;
     char *base = (char *)f->scratch.buf;
-    CartState<TC> S{};
-    for (int a = 0; a < DIM; ++a) { S.ci[a] = (int32_t *)(base + o_ci[a]); S.w[a] = (TC *)(base + o_w[a]); }
-    S.steps = (int32_t *)(base + o_steps);
-    S.flag = (uint8_t *)(base + o_flag);
-    TC *d_tau = (TC *)(base + o_tau);
+    Tracer *cur = (Tracer *)(base + o_a), *alt = (Tracer *)(base + o_b);
+    TC *d_xi = (TC *)(base + o_xi), *d_acc = (TC *)(base + o_acc), *d_tau = (TC *)(base + o_tau);
+    uint32_t *d_key = (uint32_t *)(base + o_key), *d_cnt = (uint32_t *)(base + o_cnt), *d_tile = (uint32_t *)(base + o_tile);
     LCS_CUDA_OK(cudaMemcpyAsync(d_tau, tau.data(), tau.size() * sizeof(TC), cudaMemcpyHostToDevice, st));
 
     CartDev g = make_dev(f);
-    const int block = f->opt_block ? (int)f->opt_block : 256;
-    LCS_LAUNCH((cart_init_kernel<DIM, TC>), lcs_blocks(n, 256), 256, 0, st, g, seeds, n, S);
+    const int block = f->opt_block ? (int)(f->opt_block > 256 ? 256 : f->opt_block) : 256;
+    LCS_LAUNCH((cart_init_kernel<DIM, TC>), lcs_blocks(n, 256), 256, 0, st, g, seeds, n, cur);
     bool fast = true;
     for (int a = 0; a < DIM; ++a) fast = fast && g.periodic[a] && g.pow2[a];
+    const bool ld256 = f->opt_ld256 != 0;
     TC hs[3] = {TC(1), TC(1), TC(1)};
     for (int a = 0; a < DIM; ++a) hs[a] = (TC)(h * f->cart.inv[a]);
     const int dir = h > 0 ? 1 : -1;
+
+    auto rebundle = [&]() -> lcs_status {
+        LCS_CUDA_OK(cudaMemsetAsync(d_cnt, 0, (size_t)nbins * 4, st));
+        LCS_LAUNCH((cart_key_kernel<DIM, TC>), lcs_blocks(n, 256), 256, 0, st, g, cur, n, shift, (uint32_t)(nbins - 1), d_key, d_cnt);
+        bundle::sort_records<Tracer>(cur, alt, d_key, d_cnt, d_tile, n, nbins, st);
+        std::swap(cur, alt);
+        return LCS_OK;
+    };
+
     for (size_t wi = 0; wi < windows.size(); ++wi) {
         const StepWindow &w = windows[wi];
         const void *p[3];
@@ -335,17 +518,30 @@ lcs_status cart_advect_impl(lcs_field *f, int64_t n, const void *seeds_, double 
         }
         // stream the snapshot the NEXT window will need while this one computes (side stream)
         lcs_field_prefetch(f, dir > 0 ? w.s[2] + 2 : w.s[2] - 1);
-        using Rec = PairRec<DIM, TV>;
-        WindowTimer timer(f, st);
-        if (fast)
-            LCS_LAUNCH((cart_window_kernel<DIM, TV, TC, true>), lcs_blocks(n, block), block, 0, st, g, (const Rec *)p[0], (const Rec *)p[1],
-                       (const Rec *)p[2], d_tau + 3 * w.first, w.count, (int)w.first, n, S, hs[0], hs[1], hs[2]);
-        else
-            LCS_LAUNCH((cart_window_kernel<DIM, TV, TC, false>), lcs_blocks(n, block), block, 0, st, g, (const Rec *)p[0], (const Rec *)p[1],
-                       (const Rec *)p[2], d_tau + 3 * w.first, w.count, (int)w.first, n, S, hs[0], hs[1], hs[2]);
+        const int chunk = (do_bundle && f->opt_bundle_steps > 0 && f->opt_bundle_steps < w.count) ? (int)f->opt_bundle_steps : w.count;
+        for (int done = 0; done < w.count; done += chunk) {
+            const int cnt = w.count - done < chunk ? w.count - done : chunk;
+            const int first = (int)w.first + done;
+            if (do_bundle) { rc = rebundle(); if (rc != LCS_OK) return rc; }
+            WindowTimer timer(f, st);
+            if (!split) {
+                if (fast && ld256) launch_window<DIM, TV, TC, true, true>(g, p, d_tau, first, cnt, n, cur, hs, block, st);
+                else if (fast) launch_window<DIM, TV, TC, true, false>(g, p, d_tau, first, cnt, n, cur, hs, block, st);
+                else if (ld256) launch_window<DIM, TV, TC, false, true>(g, p, d_tau, first, cnt, n, cur, hs, block, st);
+                else launch_window<DIM, TV, TC, false, false>(g, p, d_tau, first, cnt, n, cur, hs, block, st);
+            } else {
+                for (int s = first; s < first + cnt; ++s) {
+                    const TC *t3 = tau.data() + 3 * (size_t)s;
+                    if (fast && ld256) launch_split_step<DIM, TV, TC, true, true>(g, p, t3, s, n, cur, d_xi, d_acc, hs, block, st);
+                    else if (fast) launch_split_step<DIM, TV, TC, true, false>(g, p, t3, s, n, cur, d_xi, d_acc, hs, block, st);
+                    else if (ld256) launch_split_step<DIM, TV, TC, false, true>(g, p, t3, s, n, cur, d_xi, d_acc, hs, block, st);
+                    else launch_split_step<DIM, TV, TC, false, false>(g, p, t3, s, n, cur, d_xi, d_acc, hs, block, st);
+                }
+            }
+        }
         f->info_windows++;
     }
-    LCS_LAUNCH((cart_final_kernel<DIM, TC>), lcs_blocks(n, 256), 256, 0, st, g, seeds, n, S, (int32_t)N, flowmap, exit_flag, exit_step);
+    LCS_LAUNCH((cart_final_kernel<DIM, TC>), lcs_blocks(n, 256), 256, 0, st, g, seeds, n, cur, (int32_t)N, flowmap, exit_flag, exit_step);
     LCS_CUDA_OK(cudaGetLastError());
     return LCS_OK;
 }
@@ -366,13 +562,11 @@ lcs_status lcs_cart_advect(lcs_field *f, int64_t n, const void *seeds, double t0
 {
     const bool v64 = f->vel_dtype == LCS_F64, c64 = f->compute_dtype == LCS_F64;
     if (f->dim == 2) {
-        if (v64 && c64) return cart_advect_impl<2, double, double>(f, n, seeds, t0, h, N, flowmap, exit_flag, exit_step, st);
-        if (!v64 && c64) return cart_advect_impl<2, double, double>(f, n, seeds, t0, h, N, flowmap, exit_flag, exit_step, st);
-        if (!v64 && !c64) return cart_advect_impl<2, float, float>(f, n, seeds, t0, h, N, flowmap, exit_flag, exit_step, st);
+        if (c64) return cart_advect_impl<2, double, double>(f, n, seeds, t0, h, N, flowmap, exit_flag, exit_step, st);
+        if (!v64) return cart_advect_impl<2, float, float>(f, n, seeds, t0, h, N, flowmap, exit_flag, exit_step, st);
     } else {
-        if (v64 && c64) return cart_advect_impl<3, double, double>(f, n, seeds, t0, h, N, flowmap, exit_flag, exit_step, st);
-        if (!v64 && c64) return cart_advect_impl<3, double, double>(f, n, seeds, t0, h, N, flowmap, exit_flag, exit_step, st);
-        if (!v64 && !c64) return cart_advect_impl<3, float, float>(f, n, seeds, t0, h, N, flowmap, exit_flag, exit_step, st);
+        if (c64) return cart_advect_impl<3, double, double>(f, n, seeds, t0, h, N, flowmap, exit_flag, exit_step, st);
+        if (!v64) return cart_advect_impl<3, float, float>(f, n, seeds, t0, h, N, flowmap, exit_flag, exit_step, st);
     }
     lcs_set_error("fp64 velocity with fp32 arithmetic is not supported (compute_dtype must be >= vel_dtype)");
     return LCS_ERR_INVALID_ARG;

@@ -48,8 +48,34 @@ __global__ void __launch_bounds__(256) build_pair_kernel(const TV *__restrict__ 
     rec[i] = r;
 }
 
+// Cartesian grids: the record array is padded by one node per axis (np = n + 1), record (i0,i1,i2) holding node
+// (i0 mod n0, i1 mod n1, i2 mod n2).  The upper corner of any cell, periodic seam included, is then at a constant
+// offset from the lower one: one base address and 2^DIM constant offsets per interpolation.
+template <int DIM, typename TV, typename TR>
+__global__ void __launch_bounds__(256) build_pair_padded_kernel(const TV *__restrict__ a, const TV *__restrict__ b,
+                                                                 PairRec<DIM, TR> *__restrict__ rec, int n0, int n1, int n2)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t p0 = n0 + 1, p1 = n1 + 1, p2 = DIM == 3 ? n2 + 1 : 1;
+    if (i >= p0 * p1 * p2) return;
+    int i0 = (int)(i % p0), i1 = (int)((i / p0) % p1), i2 = (int)(i / (p0 * p1));
+    if (i0 == n0) i0 = 0;
+    if (i1 == n1) i1 = 0;
+    if (DIM == 3 && i2 == n2) i2 = 0;
+    const int64_t node = i0 + (int64_t)n0 * (i1 + (int64_t)n1 * i2);
+    PairRec<DIM, TR> r;
+#pragma unroll
+    for (int c = 0; c < PadOf<DIM>::P; ++c) {
+        TR va = (c < DIM) ? (TR)a[node * DIM + c] : TR(0);
+        TR vb = (c < DIM) ? (TR)b[node * DIM + c] : TR(0);
+        r.a[c] = va;
+        r.d[c] = vb - va;
+    }
+    rec[i] = r;
+}
+
 static int rec_dtype(const lcs_field *f) { return (f->vel_dtype == LCS_F64 || f->compute_dtype == LCS_F64) ? LCS_F64 : LCS_F32; }
-static size_t pair_bytes(const lcs_field *f) { return (size_t)f->nnodes * 2 * f->P * lcs_esize(rec_dtype(f)); }
+static size_t pair_bytes(const lcs_field *f) { return (size_t)f->nrec * 2 * f->P * lcs_esize(rec_dtype(f)); }
 static size_t raw_bytes(const lcs_field *f) { return (size_t)f->nnodes * f->dim * lcs_esize(f->vel_dtype); }
 
 // Makes snapshot s resident in some raw slot (enqueueing the upload on the side stream if needed) and
@@ -91,10 +117,14 @@ lcs_status lcs_field_prefetch(lcs_field *f, int s)
 }
 
 template <int DIM, typename TV, typename TR>
-static void launch_build_pair(const void *a, const void *b, void *rec, int64_t nnodes, cudaStream_t st)
+static void launch_build_pair(const lcs_field *f, const void *a, const void *b, void *rec, cudaStream_t st)
 {
-    LCS_LAUNCH((build_pair_kernel<DIM, TV, TR>), lcs_blocks(nnodes, 256), 256, 0, st, (const TV *)a, (const TV *)b,
-               (PairRec<DIM, TR> *)rec, nnodes);
+    if (f->kind == LCS_MESH_CARTESIAN)
+        LCS_LAUNCH((build_pair_padded_kernel<DIM, TV, TR>), lcs_blocks(f->nrec, 256), 256, 0, st, (const TV *)a, (const TV *)b,
+                   (PairRec<DIM, TR> *)rec, f->cart.n[0], f->cart.n[1], f->cart.n[2]);
+    else
+        LCS_LAUNCH((build_pair_kernel<DIM, TV, TR>), lcs_blocks(f->nnodes, 256), 256, 0, st, (const TV *)a, (const TV *)b,
+                   (PairRec<DIM, TR> *)rec, f->nnodes);
 }
 
 lcs_status lcs_field_require_pair(lcs_field *f, int s, cudaStream_t st, const void **pair)
@@ -118,13 +148,13 @@ lcs_status lcs_field_require_pair(lcs_field *f, int s, cudaStream_t st, const vo
     const void *A = f->slot[s0], *B = f->slot[s1];
     void *R = f->pair_buf[k];
     if (f->dim == 2) {
-        if (v64) launch_build_pair<2, double, double>(A, B, R, f->nnodes, st);
-        else if (r64) launch_build_pair<2, float, double>(A, B, R, f->nnodes, st);
-        else launch_build_pair<2, float, float>(A, B, R, f->nnodes, st);
+        if (v64) launch_build_pair<2, double, double>(f, A, B, R, st);
+        else if (r64) launch_build_pair<2, float, double>(f, A, B, R, st);
+        else launch_build_pair<2, float, float>(f, A, B, R, st);
     } else {
-        if (v64) launch_build_pair<3, double, double>(A, B, R, f->nnodes, st);
-        else if (r64) launch_build_pair<3, float, double>(A, B, R, f->nnodes, st);
-        else launch_build_pair<3, float, float>(A, B, R, f->nnodes, st);
+        if (v64) launch_build_pair<3, double, double>(f, A, B, R, st);
+        else if (r64) launch_build_pair<3, float, double>(f, A, B, R, st);
+        else launch_build_pair<3, float, float>(f, A, B, R, st);
     }
     LCS_CUDA_OK(cudaGetLastError());
     if (f->ring) {
@@ -230,12 +260,16 @@ extern "C" lcs_status lcs_field_create(const lcs_field_desc *d, lcs_field **out)
         }
         if (nn >= (1LL << 31)) { lcs_set_error("grid too large for int32 node ids"); delete f; return LCS_ERR_INVALID_ARG; }
         f->nnodes = nn;
+        f->nrec = 1;
+        for (int a = 0; a < d->dim; ++a) f->nrec *= (int64_t)d->n[a] + 1;
+        if (f->nrec >= (1LL << 31)) { lcs_set_error("grid too large for int32 node ids"); delete f; return LCS_ERR_INVALID_ARG; }
     } else {
         if (d->n_vertices < d->dim + 1 || d->n_cells < 1 || !d->vertices || !d->cells || d->n_vertices >= (1LL << 31) ||
             d->n_cells >= (1LL << 31) / (d->dim + 1)) {
             lcs_set_error("bad simplex mesh sizes / null pointers"); delete f; return LCS_ERR_INVALID_ARG;
         }
         f->nnodes = d->n_vertices;
+        f->nrec = d->n_vertices;
         f->mesh.nv = d->n_vertices; f->mesh.nc = d->n_cells;
         rc = lcs_simplex_build(f, d->vertices, d->cells);
         if (rc != LCS_OK) { lcs_field_destroy(f); return rc; }
@@ -314,8 +348,9 @@ extern "C" lcs_status lcs_field_set_option(lcs_field *f, const char *key, int64_
 {
     if (!f || !key) { lcs_set_error("null argument"); return LCS_ERR_INVALID_ARG; }
     if (!strcmp(key, "integrator") && value >= 0 && value <= 2) f->opt_integrator = value;
-    else if (!strcmp(key, "sort_seeds") && (value == 0 || value == 1)) f->opt_sort_seeds = value;
-    else if (!strcmp(key, "resort_every") && value >= 0) f->opt_resort_every = value;
+    else if (!strcmp(key, "bundle") && value >= -1 && value <= 1) f->opt_bundle = value;
+    else if (!strcmp(key, "bundle_steps") && value >= 0) f->opt_bundle_steps = value;
+    else if (!strcmp(key, "ld256") && (value == 0 || value == 1)) f->opt_ld256 = value;
     else if (!strcmp(key, "time_windows") && (value == 0 || value == 1)) { f->opt_time_windows = value; f->win_ev_used = 0; }
     else if (!strcmp(key, "block") && (value == 0 || (value >= 32 && value <= 1024 && value % 32 == 0))) f->opt_block = value;
     else { lcs_set_error("unknown option or bad value: %s=%lld", key, (long long)value); return LCS_ERR_INVALID_ARG; }

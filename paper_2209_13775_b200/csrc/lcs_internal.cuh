@@ -44,7 +44,7 @@ template <int DIM, typename TV> struct alignas(16) PairRec {
 
 // ---------------------------------------------------------------------------------------------
 struct CartGeom {
-    int32_t n[3];          // nodes per axis
+    int32_t n[3];          // nodes per axis (pair records are padded to n + 1 per axis)
     int32_t periodic[3];
     int32_t pow2[3];       // n[a] is a power of two (mask wrap)
     double origin[3];
@@ -78,6 +78,7 @@ struct lcs_field {
     int vel_dtype = 0, compute_dtype = 0;
     int P = 2;                    // padded components
     int64_t nnodes = 0;
+    int64_t nrec = 0;             // pair records per window buffer (Cartesian: padded by one node per axis)
     CartGeom cart{};
     SimplexMesh mesh{};
     std::vector<double> times;
@@ -108,8 +109,9 @@ struct lcs_field {
     int64_t h_cap = 0;
     // options
     int64_t opt_integrator = 0;   // 0 auto, 1 fused, 2 split
-    int64_t opt_sort_seeds = 0;
-    int64_t opt_resort_every = 0;
+    int64_t opt_bundle = -1;      // re-bundle tracers by cell: -1 auto (large seed sets), 0 off, 1 on
+    int64_t opt_bundle_steps = 0; // RK4 steps between re-bundlings (0 = once per snapshot window)
+    int64_t opt_ld256 = 1;        // gather pair records with one 256-bit load instead of two 128-bit loads
     int64_t opt_block = 0;        // threads per block override (0 = default)
     int64_t opt_time_windows = 0; // record CUDA events around every window (hot) kernel launch
     // info

@@ -372,3 +372,48 @@ def test_cg_ftle_patterns_vs_oracle(lcs, oracle):
         cgn, ftn, _ = lcs.cg_ftle(dim, ng, dx, per, period, torch.from_numpy(F).cuda(), None, 3.0, want_cg=False, want_status=False)
         cgo, fto, sto = oracle.cg_ftle(dim, ng, dx, per, period, F, None, 3.0)
         assert cgn is None and np.allclose(cpu(ftn), fto, rtol=1e-12, atol=1e-12, equal_nan=True)
+
+
+# -------------------------------------------------------------------------------------------------
+# integrator variants: re-bundled tracers and the paper's split (one kernel per RK4 stage) design
+@pytest.mark.parametrize("options", [dict(bundle=1), dict(bundle=1, bundle_steps=7), dict(bundle=1, ld256=0),
+                                     dict(integrator=2, bundle=0), dict(integrator=2, bundle=1, bundle_steps=13)])
+def test_cartesian_variants_fp64_identical_to_default(lcs, oracle, options):
+    """Config 1 reduced in fp64: every variant (bundling on, odd re-bundling period, 128-bit loads, split stages)
+    passes the fp64 gate against the oracle, and results come back in the caller's seed order."""
+    w = I.config1(ng=(96, 48), T=10.0)
+    fo, Fo, flo, eso = oracle_run(oracle, w)
+    f, sd, F, flag, es = gpu_run(w, options=options)
+    cgo, fto, sto = oracle_cg(oracle, w, Fo, flo)
+    cgg, ftg, stg = gpu_cg(w, F, flag)
+    gate_fp64(cpu(F), Fo, cpu(ftg), fto, w.tf - w.t0, cpu(flag), flo, cpu(es), eso)
+
+
+@pytest.mark.parametrize("options", [dict(bundle=1, bundle_steps=20), dict(integrator=2, bundle=1), dict(bundle=0, ld256=0)])
+def test_config3_variants_fp32(lcs, oracle, options):
+    """Config 3 reduced (periodic, fp32) with bundling / split stages: statistical gate; fused variants that differ
+    only in tracer order are bit-identical to the default path (a tracer's arithmetic does not depend on its slot)."""
+    w = I.config3(ngrid=40, nn=32, T=2.0, h=0.01, n_snap=9)
+    fo, Fo, flo, eso = oracle_run(oracle, w)
+    f0, sd0, F0, flag0, es0 = gpu_run(w, options=dict(bundle=0))
+    f, sd, F, flag, es = gpu_run(w, options=options)
+    cgo, fto, sto = oracle_cg(oracle, w, Fo, flo)
+    cgg, ftg, stg = gpu_cg(w, F, flag)
+    gate_statistical(cpu(F), Fo, cpu(ftg), fto, w.L, cpu(flag), flo)
+    if options.get("integrator", 0) != 2:
+        assert np.array_equal(cpu(F), cpu(F0))
+
+
+@pytest.mark.parametrize("options", [dict(bundle=1, bundle_steps=5), dict(integrator=2, bundle=1)])
+def test_exit_handling_variants(lcs, oracle, options):
+    """Exits (flags 0/1/2, exit_step) with re-bundling (finished tracers are parked in the last bin) and with the
+    split stages (flag raised by the failing stage, record frozen at the start of the step)."""
+    A = np.array([[0.03, 0.05], [-0.02, 0.04]])
+    w = I.analytic_cartesian(2, I.linear_flow(A, np.array([0.25, -0.1])), (41, 31), (0.0, 0.0), (0.05, 0.05),
+                             (0.0, 2.0, 4.0), ng=(64, 48), seed_lo=(-0.2, -0.1), seed_spacing=(2.4 / 64, 1.7 / 48),
+                             t0=0.0, tf=4.0, h=0.05)
+    fo, Fo, flo, eso = oracle_run(oracle, w)
+    f, sd, F, flag, es = gpu_run(w, options=options)
+    assert (flo == 0).sum() > 20 and (flo == 1).sum() > 100 and (flo == 2).sum() > 20
+    assert np.array_equal(cpu(flag), flo) and np.array_equal(cpu(es), eso)
+    assert np.max(np.abs(cpu(F) - Fo)) <= 1e-10
