@@ -324,6 +324,149 @@ cart_window_kernel(const __grid_constant__ CartDev g, const PairRec<DIM, TV> *__
 }
 
 // ---------------------------------------------------------------------------------------------
+// Pre-blended variant (3D, fp32): the time blend u(node, t) = a + tau (b - a) does not depend on the tracer, and the
+// integrator is bound by the bytes the L1 delivers into registers (128 B per cycle per SM), so the blend is hoisted
+// out of the gather: for a chunk of k RK4 steps the 2k+1 distinct stage times are blended once per node into
+// "x-pair" records {u(i0,i1,i2), u(i0+1,i1,i2)} (2 x float4 = one 32-byte sector, one 256-bit load), and a stage
+// gathers 4 records = 128 B per tracer instead of 8 pair records = 256 B.  The arithmetic per tracer is unchanged
+// (fma(tau, b - a, a) per node, then the nested lerps), so results are bit-identical to the pair-record path.
+struct alignas(32) XPair {
+    float lo[4];
+    float hi[4];
+};
+
+constexpr int kMaxBlendFields = 2 * 256 + 1;
+
+// one thread per padded record; raw snapshots a, b are [node][3] fp32; field f of the chunk gets tau[f]
+__global__ void __launch_bounds__(256) blend_xpair_kernel(const float *__restrict__ a, const float *__restrict__ b, int n0, int n1, int n2,
+                                                           const float *__restrict__ tau, int nfields, XPair *__restrict__ fields,
+                                                           int64_t field_stride)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t p0 = n0 + 1, p1 = n1 + 1, p2 = n2 + 1;
+    if (i >= p0 * p1 * p2) return;
+    int i0 = (int)(i % p0), i1 = (int)((i / p0) % p1), i2 = (int)(i / (p0 * p1));
+    if (i0 == n0) i0 = 0;
+    if (i1 == n1) i1 = 0;
+    if (i2 == n2) i2 = 0;
+    const int j0 = i0 + 1 == n0 ? 0 : i0 + 1;
+    const int64_t row = (int64_t)n0 * (i1 + (int64_t)n1 * i2);
+    const float *al = a + 3 * (row + i0), *bl = b + 3 * (row + i0), *ah = a + 3 * (row + j0), *bh = b + 3 * (row + j0);
+    float va[6], vd[6];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        va[c] = al[c]; vd[c] = bl[c] - al[c];
+        va[3 + c] = ah[c]; vd[3 + c] = bh[c] - ah[c];
+    }
+    for (int f = 0; f < nfields; ++f) {
+        const float t = __ldg(tau + f);
+        float4 lo, hi;
+        lo.x = fmaf(t, vd[0], va[0]); lo.y = fmaf(t, vd[1], va[1]); lo.z = fmaf(t, vd[2], va[2]); lo.w = 0.f;
+        hi.x = fmaf(t, vd[3], va[3]); hi.y = fmaf(t, vd[4], va[4]); hi.z = fmaf(t, vd[5], va[5]); hi.w = 0.f;
+        float4 *dst = reinterpret_cast<float4 *>(fields + (int64_t)f * field_stride + i);
+        __stcs(dst, lo);
+        __stcs(dst + 1, hi);
+    }
+}
+
+__device__ __forceinline__ void load_xpair(const XPair *p, float4 &lo, float4 &hi)
+{
+    asm("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+        : "=f"(lo.x), "=f"(lo.y), "=f"(lo.z), "=f"(lo.w), "=f"(hi.x), "=f"(hi.y), "=f"(hi.z), "=f"(hi.w) : "l"(p));
+}
+
+template <bool FASTWRAP>
+__device__ __forceinline__ bool cart_velocity_xpair(const CartDev &g, const XPair *__restrict__ field, const int *ci, const float *xi, float *u)
+{
+    int lo[3];
+    float wl[3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        int ifl;
+        floor_split<float>(xi[a], ifl, wl[a]);
+        int c = ci[a] + ifl;
+        if constexpr (FASTWRAP) {
+            lo[a] = c & (g.n[a] - 1);
+        } else if (g.periodic[a]) {
+            lo[a] = wrap_index(c, g.n[a], g.pow2[a]);
+        } else {
+            if (c == g.n[a] - 1 && wl[a] == 0.f) { c = g.n[a] - 2; wl[a] = 1.f; }
+            if (c < 0 || c > g.n[a] - 2) return false;
+            lo[a] = c;
+        }
+    }
+    const XPair *b = field + (lo[0] + lo[1] * g.np0 + lo[2] * g.np01);
+    float4 l00, h00, l10, h10, l01, h01, l11, h11;
+    load_xpair(b, l00, h00);
+    load_xpair(b + g.np0, l10, h10);
+    load_xpair(b + g.np01, l01, h01);
+    load_xpair(b + g.np01 + g.np0, l11, h11);
+    const float v[8][3] = {{l00.x, l00.y, l00.z}, {h00.x, h00.y, h00.z}, {l10.x, l10.y, l10.z}, {h10.x, h10.y, h10.z},
+                           {l01.x, l01.y, l01.z}, {h01.x, h01.y, h01.z}, {l11.x, l11.y, l11.z}, {h11.x, h11.y, h11.z}};
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        float a00 = fmaf(wl[0], v[1][c] - v[0][c], v[0][c]);
+        float a10 = fmaf(wl[0], v[3][c] - v[2][c], v[2][c]);
+        float a01 = fmaf(wl[0], v[5][c] - v[4][c], v[4][c]);
+        float a11 = fmaf(wl[0], v[7][c] - v[6][c], v[6][c]);
+        float b0 = fmaf(wl[1], a10 - a00, a00);
+        float b1 = fmaf(wl[1], a11 - a01, a01);
+        u[c] = fmaf(wl[2], b1 - b0, b0);
+    }
+    return true;
+}
+
+// fidx: [nsteps][3] index of the blended field of (ta, tb, tc) within `fields`
+template <bool FASTWRAP>
+__global__ void __launch_bounds__(256)
+cart_xpair_kernel(const __grid_constant__ CartDev g, const XPair *__restrict__ fields, int64_t field_stride, const int *__restrict__ fidx,
+                  int nsteps, int first_step, int64_t n, CartTracer<3, float> *__restrict__ st, float hs0, float hs1, float hs2)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    CartTracer<3, float> t = load_record(st + i);
+    if ((t.meta >> 30) != 0) return;
+    const float hs[3] = {hs0, hs1, hs2};
+    int ci[3];
+    float w[3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) { ci[a] = t.ci[a]; w[a] = t.w[a]; }
+    int s = 0;
+    bool ok = true;
+    for (; s < nsteps; ++s) {
+        const XPair *fa = fields + (int64_t)__ldg(fidx + 3 * s) * field_stride;
+        const XPair *fb = fields + (int64_t)__ldg(fidx + 3 * s + 1) * field_stride;
+        const XPair *fc = fields + (int64_t)__ldg(fidx + 3 * s + 2) * field_stride;
+        float k1[3], k2[3], k3[3], k4[3], xi[3];
+        ok = cart_velocity_xpair<FASTWRAP>(g, fa, ci, w, k1);
+        if (!ok) break;
+#pragma unroll
+        for (int a = 0; a < 3; ++a) xi[a] = fmaf(0.5f * hs[a], k1[a], w[a]);
+        ok = cart_velocity_xpair<FASTWRAP>(g, fb, ci, xi, k2);
+        if (!ok) break;
+#pragma unroll
+        for (int a = 0; a < 3; ++a) xi[a] = fmaf(0.5f * hs[a], k2[a], w[a]);
+        ok = cart_velocity_xpair<FASTWRAP>(g, fb, ci, xi, k3);
+        if (!ok) break;
+#pragma unroll
+        for (int a = 0; a < 3; ++a) xi[a] = fmaf(hs[a], k3[a], w[a]);
+        ok = cart_velocity_xpair<FASTWRAP>(g, fc, ci, xi, k4);
+        if (!ok) break;
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            float wn = fmaf(hs[a] * (1.0f / 6.0f), (k1[a] + k4[a]) + 2.0f * (k2[a] + k3[a]), w[a]);
+            int ifl;
+            floor_split<float>(wn, ifl, w[a]);
+            ci[a] += ifl;
+        }
+    }
+#pragma unroll
+    for (int a = 0; a < 3; ++a) { t.ci[a] = ci[a]; t.w[a] = w[a]; }
+    if (!ok) t.meta = (1u << 30) | (uint32_t)(first_step + s);
+    store_record(st + i, t);
+}
+
+// ---------------------------------------------------------------------------------------------
 // Split variant (the paper's design: "the RK4 computation was divided into several short
 // kernels"; all tracers advance one stage at a time).  One launch per RK4 stage; between the launches the
 // stage point (xi) and the running sum k1 + 2 k2 + 2 k3 (acc) live in global memory as [n][DIM] arrays.
@@ -472,6 +615,36 @@ lcs_status cart_advect_impl(lcs_field *f, int64_t n, const void *seeds_, double 
     }
     const int64_t nbins = do_bundle ? ((int64_t)1 << (bits * DIM)) + 1 : 0;
 
+    // launch units: a snapshot window is cut into chunks (pre-blended variant: <= preblend_steps steps, whose
+    // distinct stage times are blended once per node; otherwise <= bundle_steps steps between re-bundlings)
+    constexpr bool kCanBlend = DIM == 3 && sizeof(TC) == 4 && sizeof(TV) == 4;
+    const bool preblend = kCanBlend && !split && (f->opt_preblend == 1 || (f->opt_preblend < 0 && n >= (1 << 20)));
+    struct Unit { int win, first, count, blend, ftau_off, nfields; };
+    std::vector<Unit> units;
+    std::vector<float> ftau;
+    std::vector<int> fidx((size_t)3 * N, 0);
+    int max_fields = 0;
+    for (size_t wi = 0; wi < windows.size(); ++wi) {
+        const StepWindow &w = windows[wi];
+        const bool blend = preblend && w.s[0] == w.s[1] && w.s[1] == w.s[2];
+        int chunk = w.count;
+        if (blend) chunk = (int)f->opt_preblend_steps;
+        else if (do_bundle && f->opt_bundle_steps > 0) chunk = (int)f->opt_bundle_steps;
+        for (int done = 0; done < w.count; done += chunk) {
+            Unit u{(int)wi, (int)w.first + done, w.count - done < chunk ? w.count - done : chunk, blend ? 1 : 0, (int)ftau.size(), 0};
+            if (blend) {
+                for (int s = u.first; s < u.first + u.count; ++s)
+                    for (int k = 0; k < 3; ++k) {
+                        const float t = (float)tau64[3 * (size_t)s + k];
+                        if (u.nfields == 0 || ftau.back() != t) { ftau.push_back(t); u.nfields++; }
+                        fidx[3 * (size_t)s + k] = u.nfields - 1;
+                    }
+                max_fields = u.nfields > max_fields ? u.nfields : max_fields;
+            }
+            units.push_back(u);
+        }
+    }
+
     // carve the tracer scratch
     size_t off = 0;
     const size_t o_a = off; off = align_up(off + (size_t)n * sizeof(Tracer));
@@ -483,13 +656,22 @@ lcs_status cart_advect_impl(lcs_field *f, int64_t n, const void *seeds_, double 
     const size_t o_key = off; if (do_bundle) off = align_up(off + (size_t)n * 4);
     const size_t o_cnt = off; if (do_bundle) off = align_up(off + (size_t)nbins * 4);
     const size_t o_tile = off; if (do_bundle) off = align_up(off + (size_t)ntiles * 4);
+    const size_t o_ftau = off; off = align_up(off + ftau.size() * 4 + 4);
+    const size_t o_fidx = off; if (max_fields) off = align_up(off + fidx.size() * 4);
+    const size_t o_fields = off; off = align_up(off + (size_t)max_fields * (size_t)f->nrec * 32);
     rc = lcs_scratch_reserve(f, off);
     if (rc != LCS_OK) return rc;
     char *base = (char *)f->scratch.buf;
     Tracer *cur = (Tracer *)(base + o_a), *alt = (Tracer *)(base + o_b);
     TC *d_xi = (TC *)(base + o_xi), *d_acc = (TC *)(base + o_acc), *d_tau = (TC *)(base + o_tau);
     uint32_t *d_key = (uint32_t *)(base + o_key), *d_cnt = (uint32_t *)(base + o_cnt), *d_tile = (uint32_t *)(base + o_tile);
+    float *d_ftau = (float *)(base + o_ftau);
+    int *d_fidx = (int *)(base + o_fidx);
     LCS_CUDA_OK(cudaMemcpyAsync(d_tau, tau.data(), tau.size() * sizeof(TC), cudaMemcpyHostToDevice, st));
+    if (max_fields) {
+        LCS_CUDA_OK(cudaMemcpyAsync(d_ftau, ftau.data(), ftau.size() * 4, cudaMemcpyHostToDevice, st));
+        LCS_CUDA_OK(cudaMemcpyAsync(d_fidx, fidx.data(), fidx.size() * 4, cudaMemcpyHostToDevice, st));
+    }
 
     CartDev g = make_dev(f);
     const int block = f->opt_block ? (int)(f->opt_block > 256 ? 256 : f->opt_block) : 256;
@@ -509,37 +691,67 @@ lcs_status cart_advect_impl(lcs_field *f, int64_t n, const void *seeds_, double 
         return LCS_OK;
     };
 
-    for (size_t wi = 0; wi < windows.size(); ++wi) {
-        const StepWindow &w = windows[wi];
-        const void *p[3];
-        for (int k = 0; k < 3; ++k) {
-            rc = lcs_field_require_pair(f, w.s[k], st, &p[k]);
-            if (rc != LCS_OK) return rc;
-        }
-        // stream the snapshot the NEXT window will need while this one computes (side stream)
-        lcs_field_prefetch(f, dir > 0 ? w.s[2] + 2 : w.s[2] - 1);
-        const int chunk = (do_bundle && f->opt_bundle_steps > 0 && f->opt_bundle_steps < w.count) ? (int)f->opt_bundle_steps : w.count;
-        for (int done = 0; done < w.count; done += chunk) {
-            const int cnt = w.count - done < chunk ? w.count - done : chunk;
-            const int first = (int)w.first + done;
-            if (do_bundle) { rc = rebundle(); if (rc != LCS_OK) return rc; }
-            WindowTimer timer(f, st);
-            if (!split) {
-                if (fast && ld256) launch_window<DIM, TV, TC, true, true>(g, p, d_tau, first, cnt, n, cur, hs, block, st);
-                else if (fast) launch_window<DIM, TV, TC, true, false>(g, p, d_tau, first, cnt, n, cur, hs, block, st);
-                else if (ld256) launch_window<DIM, TV, TC, false, true>(g, p, d_tau, first, cnt, n, cur, hs, block, st);
-                else launch_window<DIM, TV, TC, false, false>(g, p, d_tau, first, cnt, n, cur, hs, block, st);
+    int cur_win = -1, since_bundle = 0;
+    const void *p[3] = {nullptr, nullptr, nullptr}, *raw_a = nullptr, *raw_b = nullptr;
+    for (size_t ui = 0; ui < units.size(); ++ui) {
+        const Unit &u = units[ui];
+        const StepWindow &w = windows[u.win];
+        const bool new_win = u.win != cur_win;
+        if (new_win) {
+            if (u.blend) {
+                rc = lcs_field_acquire_raw(f, w.s[0], st, &raw_a, &raw_b);
+                if (rc != LCS_OK) return rc;
             } else {
-                for (int s = first; s < first + cnt; ++s) {
-                    const TC *t3 = tau.data() + 3 * (size_t)s;
-                    if (fast && ld256) launch_split_step<DIM, TV, TC, true, true>(g, p, t3, s, n, cur, d_xi, d_acc, hs, block, st);
-                    else if (fast) launch_split_step<DIM, TV, TC, true, false>(g, p, t3, s, n, cur, d_xi, d_acc, hs, block, st);
-                    else if (ld256) launch_split_step<DIM, TV, TC, false, true>(g, p, t3, s, n, cur, d_xi, d_acc, hs, block, st);
-                    else launch_split_step<DIM, TV, TC, false, false>(g, p, t3, s, n, cur, d_xi, d_acc, hs, block, st);
+                for (int k = 0; k < 3; ++k) {
+                    rc = lcs_field_require_pair(f, w.s[k], st, &p[k]);
+                    if (rc != LCS_OK) return rc;
                 }
             }
+            // stream the snapshot the NEXT window will need while this one computes (side stream)
+            lcs_field_prefetch(f, dir > 0 ? w.s[2] + 2 : w.s[2] - 1, w.s[2], w.s[2] + 1);
+            cur_win = u.win;
+            f->info_windows++;
         }
-        f->info_windows++;
+        if (do_bundle && (new_win || (f->opt_bundle_steps > 0 && since_bundle >= f->opt_bundle_steps))) {
+            rc = rebundle();
+            if (rc != LCS_OK) return rc;
+            since_bundle = 0;
+        }
+        since_bundle += u.count;
+        if constexpr (kCanBlend) {
+            if (u.blend) {
+                XPair *fields = (XPair *)(base + o_fields);
+                LCS_LAUNCH(blend_xpair_kernel, lcs_blocks(f->nrec, 256), 256, 0, st, (const float *)raw_a, (const float *)raw_b, g.n[0], g.n[1],
+                           g.n[2], d_ftau + u.ftau_off, u.nfields, fields, f->nrec);
+                {
+                    WindowTimer timer(f, st);
+                    if (fast)
+                        LCS_LAUNCH((cart_xpair_kernel<true>), lcs_blocks(n, block), block, 0, st, g, (const XPair *)fields, f->nrec,
+                                   d_fidx + 3 * (size_t)u.first, u.count, u.first, n, cur, hs[0], hs[1], hs[2]);
+                    else
+                        LCS_LAUNCH((cart_xpair_kernel<false>), lcs_blocks(n, block), block, 0, st, g, (const XPair *)fields, f->nrec,
+                                   d_fidx + 3 * (size_t)u.first, u.count, u.first, n, cur, hs[0], hs[1], hs[2]);
+                }
+                const bool last_of_win = ui + 1 == units.size() || units[ui + 1].win != u.win;
+                if (last_of_win) { rc = lcs_field_release_raw(f, w.s[0], st); if (rc != LCS_OK) return rc; }
+                continue;
+            }
+        }
+        WindowTimer timer(f, st);
+        if (!split) {
+            if (fast && ld256) launch_window<DIM, TV, TC, true, true>(g, p, d_tau, u.first, u.count, n, cur, hs, block, st);
+            else if (fast) launch_window<DIM, TV, TC, true, false>(g, p, d_tau, u.first, u.count, n, cur, hs, block, st);
+            else if (ld256) launch_window<DIM, TV, TC, false, true>(g, p, d_tau, u.first, u.count, n, cur, hs, block, st);
+            else launch_window<DIM, TV, TC, false, false>(g, p, d_tau, u.first, u.count, n, cur, hs, block, st);
+        } else {
+            for (int s = u.first; s < u.first + u.count; ++s) {
+                const TC *t3 = tau.data() + 3 * (size_t)s;
+                if (fast && ld256) launch_split_step<DIM, TV, TC, true, true>(g, p, t3, s, n, cur, d_xi, d_acc, hs, block, st);
+                else if (fast) launch_split_step<DIM, TV, TC, true, false>(g, p, t3, s, n, cur, d_xi, d_acc, hs, block, st);
+                else if (ld256) launch_split_step<DIM, TV, TC, false, true>(g, p, t3, s, n, cur, d_xi, d_acc, hs, block, st);
+                else launch_split_step<DIM, TV, TC, false, false>(g, p, t3, s, n, cur, d_xi, d_acc, hs, block, st);
+            }
+        }
     }
     LCS_LAUNCH((cart_final_kernel<DIM, TC>), lcs_blocks(n, 256), 256, 0, st, g, seeds, n, cur, (int32_t)N, flowmap, exit_flag, exit_step);
     LCS_CUDA_OK(cudaGetLastError());

@@ -108,12 +108,14 @@ static lcs_status ensure_slot(lcs_field *f, int s, int keep0, int keep1, int *sl
     return LCS_OK;
 }
 
-lcs_status lcs_field_prefetch(lcs_field *f, int s)
+lcs_status lcs_field_prefetch(lcs_field *f, int s, int keep0, int keep1)
 {
-    if (!f->ring || s < 0 || s >= f->ns || !f->snap_set[s]) return LCS_OK;
+    if (!f->ring || s < 0 || s >= f->ns || !f->snap_set[s] || f->snap_slot[s] >= 0) return LCS_OK;
+    // never evict the snapshots of the window that is being integrated (keep0, keep1): the pre-blended integrator
+    // reads their raw slots until the end of the window.  No other slot free => no prefetch (loaded on demand).
     int slot;
-    // keep the neighbours of s (the pair that is most likely in use)
-    return ensure_slot(f, s, s - 1, s + 1, &slot);
+    lcs_status rc = ensure_slot(f, s, keep0, keep1, &slot);
+    return rc == LCS_ERR_INVALID_ARG ? LCS_OK : rc;
 }
 
 template <int DIM, typename TV, typename TR>
@@ -165,6 +167,35 @@ lcs_status lcs_field_require_pair(lcs_field *f, int s, cudaStream_t st, const vo
     f->pair_snap[k] = s;
     f->pair_age[k] = f->pair_clock;
     *pair = f->pair_buf[k];
+    return LCS_OK;
+}
+
+// Raw snapshots s and s + 1 for kernels that read the [node][dim] slots directly (the per-stage-time blend of the
+// pre-blended integrator).  release_raw marks the end of the last reader on `st` so that the ring may reuse the slots.
+lcs_status lcs_field_acquire_raw(lcs_field *f, int s, cudaStream_t st, const void **a, const void **b)
+{
+    if (s < 0 || s + 1 >= f->ns) { lcs_set_error("pair %d out of range", s); return LCS_ERR_INVALID_ARG; }
+    int s0, s1;
+    lcs_status rc = ensure_slot(f, s, s, s + 1, &s0);
+    if (rc != LCS_OK) return rc;
+    rc = ensure_slot(f, s + 1, s, s + 1, &s1);
+    if (rc != LCS_OK) return rc;
+    LCS_CUDA_OK(cudaStreamWaitEvent(st, f->slot_ready[s0], 0));
+    LCS_CUDA_OK(cudaStreamWaitEvent(st, f->slot_ready[s1], 0));
+    *a = f->slot[s0];
+    *b = f->slot[s1];
+    return LCS_OK;
+}
+
+lcs_status lcs_field_release_raw(lcs_field *f, int s, cudaStream_t st)
+{
+    if (!f->ring) return LCS_OK;
+    for (int k = s; k <= s + 1; ++k) {
+        int sl = f->snap_slot[k];
+        if (sl < 0) continue;
+        LCS_CUDA_OK(cudaEventRecord(f->slot_free[sl], st));
+        f->slot_free_valid[sl] = 1;
+    }
     return LCS_OK;
 }
 
@@ -351,6 +382,8 @@ extern "C" lcs_status lcs_field_set_option(lcs_field *f, const char *key, int64_
     else if (!strcmp(key, "bundle") && value >= -1 && value <= 1) f->opt_bundle = value;
     else if (!strcmp(key, "bundle_steps") && value >= 0) f->opt_bundle_steps = value;
     else if (!strcmp(key, "ld256") && (value == 0 || value == 1)) f->opt_ld256 = value;
+    else if (!strcmp(key, "preblend") && value >= -1 && value <= 1) f->opt_preblend = value;
+    else if (!strcmp(key, "preblend_steps") && value >= 1 && value <= 256) f->opt_preblend_steps = value;
     else if (!strcmp(key, "time_windows") && (value == 0 || value == 1)) { f->opt_time_windows = value; f->win_ev_used = 0; }
     else if (!strcmp(key, "block") && (value == 0 || (value >= 32 && value <= 1024 && value % 32 == 0))) f->opt_block = value;
     else { lcs_set_error("unknown option or bad value: %s=%lld", key, (long long)value); return LCS_ERR_INVALID_ARG; }

@@ -111,6 +111,8 @@ struct lcs_field {
     int64_t opt_integrator = 0;   // 0 auto, 1 fused, 2 split
     int64_t opt_bundle = -1;      // re-bundle tracers by cell: -1 auto (large seed sets), 0 off, 1 on
     int64_t opt_bundle_steps = 0; // RK4 steps between re-bundlings (0 = once per snapshot window)
+    int64_t opt_preblend = -1;    // 3D fp32 Cartesian: gather from per-stage-time blended fields (-1 auto, 0 off, 1 on)
+    int64_t opt_preblend_steps = 10; // RK4 steps per launch of the pre-blended integrator (2k+1 blended fields resident)
     int64_t opt_ld256 = 1;        // gather pair records with one 256-bit load instead of two 128-bit loads
     int64_t opt_block = 0;        // threads per block override (0 = default)
     int64_t opt_time_windows = 0; // record CUDA events around every window (hot) kernel launch
@@ -136,7 +138,9 @@ static inline size_t lcs_esize(int dtype) { return dtype == LCS_F64 ? 8 : 4; }
 
 // field.cu
 lcs_status lcs_field_require_pair(lcs_field *f, int s, cudaStream_t stream, const void **pair);
-lcs_status lcs_field_prefetch(lcs_field *f, int s);
+lcs_status lcs_field_prefetch(lcs_field *f, int s, int keep0, int keep1);
+lcs_status lcs_field_acquire_raw(lcs_field *f, int s, cudaStream_t stream, const void **a, const void **b);
+lcs_status lcs_field_release_raw(lcs_field *f, int s, cudaStream_t stream);
 lcs_status lcs_scratch_reserve(lcs_field *f, size_t bytes);
 
 // simplex.cu

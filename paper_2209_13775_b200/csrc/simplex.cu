@@ -671,7 +671,7 @@ lcs_status simplex_advect_impl(lcs_field *f, int64_t n, const void *seeds_, doub
             rc = lcs_field_require_pair(f, w.s[k], st, &p[k]);
             if (rc != LCS_OK) return rc;
         }
-        lcs_field_prefetch(f, dir > 0 ? w.s[2] + 2 : w.s[2] - 1);
+        lcs_field_prefetch(f, dir > 0 ? w.s[2] + 2 : w.s[2] - 1, w.s[2], w.s[2] + 1);
         WindowTimer timer(f, st);
         LCS_LAUNCH((simplex_window_kernel<DIM, TV, TC>), lcs_blocks(n, block), block, 0, st, (const CellRec<DIM, TC> *)m.cellrec, m.neigh,
                    (const VRec *)p[0], (const VRec *)p[1], (const VRec *)p[2], d_tau + 3 * w.first, w.count, (int)w.first, n, S, (TC)h);

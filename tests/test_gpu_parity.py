@@ -192,13 +192,16 @@ def test_config4_reduced_tets_fp32(lcs, oracle):
     print("config4 reduced", stats, "flag mismatches", int((fl != flo).sum()))
 
 
-def test_config5_reduced_backward_streamed(lcs, oracle):
+@pytest.mark.parametrize("options", [dict(), dict(preblend=1, bundle=1, preblend_steps=9)])
+def test_config5_reduced_backward_streamed(lcs, oracle, options):
     """Config 5 reduced: backward-time windows of the ABC field with a ring of 3 device slots fed from pinned
     host memory on the side stream; results equal the all-resident field bit for bit and pass the gate."""
     import torch
     w = I.config5(ngrid=24, nn=32, n_grids=3, T=2.0, h=0.01, n_snap=9)
     f_ring = lcs.Field.from_workload(w, max_resident_snapshots=3)
     f_all = lcs.Field.from_workload(w)
+    for k, v in options.items():
+        f_ring.set_option(k, v)
     assert f_ring.info("ring") == 1 and f_all.info("ring") == 0
     fo = oracle.OracleField.from_workload(w)
     s = w.seeds()
@@ -389,7 +392,8 @@ def test_cartesian_variants_fp64_identical_to_default(lcs, oracle, options):
     gate_fp64(cpu(F), Fo, cpu(ftg), fto, w.tf - w.t0, cpu(flag), flo, cpu(es), eso)
 
 
-@pytest.mark.parametrize("options", [dict(bundle=1, bundle_steps=20), dict(integrator=2, bundle=1), dict(bundle=0, ld256=0)])
+@pytest.mark.parametrize("options", [dict(bundle=1, bundle_steps=20), dict(integrator=2, bundle=1), dict(bundle=0, ld256=0),
+                                     dict(preblend=1, preblend_steps=7), dict(preblend=1, bundle=1, bundle_steps=20)])
 def test_config3_variants_fp32(lcs, oracle, options):
     """Config 3 reduced (periodic, fp32) with bundling / split stages: statistical gate; fused variants that differ
     only in tracer order are bit-identical to the default path (a tracer's arithmetic does not depend on its slot)."""
@@ -417,3 +421,20 @@ def test_exit_handling_variants(lcs, oracle, options):
     assert (flo == 0).sum() > 20 and (flo == 1).sum() > 100 and (flo == 2).sum() > 20
     assert np.array_equal(cpu(flag), flo) and np.array_equal(cpu(es), eso)
     assert np.max(np.abs(cpu(F) - Fo)) <= 1e-10
+
+
+def test_preblend_nonperiodic_3d_fp32_with_exits(lcs, oracle):
+    """Pre-blended x-pair gathers on a non-periodic 3D fp32 grid with exits (flags 0/1/2) and a step size that makes
+    some steps straddle snapshots (those windows fall back to pair records): bit-identical to the pair-record path."""
+    A = np.array([[0.05, 0.3, 0.0], [-0.3, 0.02, 0.1], [0.0, -0.1, 0.04]])
+    w = I.analytic_cartesian(3, I.linear_flow(A, np.array([0.2, -0.05, 0.1])), (21, 17, 13), (0.0, 0.0, 0.0), (0.1, 0.1, 0.1),
+                             (0.0, 1.0, 2.0, 3.0), ng=(40, 32, 24), seed_lo=(-0.1, -0.1, -0.1), seed_spacing=(2.2 / 40, 1.8 / 32, 1.4 / 24),
+                             t0=0.0, tf=3.0, h=0.04, vel_dtype=np.float32, compute_dtype=np.float32)
+    fo, Fo, flo, eso = oracle_run(oracle, w)
+    f0, sd0, F0, flag0, es0 = gpu_run(w, options=dict(preblend=0, bundle=0))
+    f1, sd1, F1, flag1, es1 = gpu_run(w, options=dict(preblend=1, bundle=1, preblend_steps=6))
+    assert set(np.unique(flo)) == {0, 1, 2}
+    assert np.array_equal(cpu(F0), cpu(F1)) and np.array_equal(cpu(flag0), cpu(flag1)) and np.array_equal(cpu(es0), cpu(es1))
+    assert np.mean(cpu(flag1) == flo) > 0.995
+    same = cpu(flag1) == flo
+    assert np.max(np.linalg.norm(cpu(F1)[same].astype(np.float64) - Fo[same], axis=1)) < 1e-3 * w.L
