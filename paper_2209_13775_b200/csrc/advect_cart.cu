@@ -375,8 +375,17 @@ __device__ __forceinline__ void load_xpair(const XPair *p, float4 &lo, float4 &h
         : "=f"(lo.x), "=f"(lo.y), "=f"(lo.z), "=f"(lo.w), "=f"(hi.x), "=f"(hi.y), "=f"(hi.z), "=f"(hi.w) : "l"(p));
 }
 
-template <bool FASTWRAP>
-__device__ __forceinline__ bool cart_velocity_xpair(const CartDev &g, const XPair *__restrict__ field, const int *ci, const float *xi, float *u)
+// Corner values of the cell a tracer last gathered from, kept in registers: stages 2 and 3 of a step read the same
+// blended field, and so do stage 4 and stage 1 of the next step, at points that are O(h^2) apart -- almost always the
+// same cell.  A lane reloads (predicated, per lane) only when its cell changed, which halves the L1 traffic per step.
+struct HeldCell {
+    int idx;               // record index of the held cell, -1 = nothing held
+    float v[8][3];
+};
+
+template <bool FASTWRAP, bool REUSE>
+__device__ __forceinline__ bool cart_velocity_xpair(const CartDev &g, const XPair *__restrict__ field, const int *ci, const float *xi,
+                                                    HeldCell &hc, float *u)
 {
     int lo[3];
     float wl[3];
@@ -395,20 +404,30 @@ __device__ __forceinline__ bool cart_velocity_xpair(const CartDev &g, const XPai
             lo[a] = c;
         }
     }
-    const XPair *b = field + (lo[0] + lo[1] * g.np0 + lo[2] * g.np01);
-    float4 l00, h00, l10, h10, l01, h01, l11, h11;
-    load_xpair(b, l00, h00);
-    load_xpair(b + g.np0, l10, h10);
-    load_xpair(b + g.np01, l01, h01);
-    load_xpair(b + g.np01 + g.np0, l11, h11);
-    const float v[8][3] = {{l00.x, l00.y, l00.z}, {h00.x, h00.y, h00.z}, {l10.x, l10.y, l10.z}, {h10.x, h10.y, h10.z},
-                           {l01.x, l01.y, l01.z}, {h01.x, h01.y, h01.z}, {l11.x, l11.y, l11.z}, {h11.x, h11.y, h11.z}};
+    const int idx = lo[0] + lo[1] * g.np0 + lo[2] * g.np01;
+    if (!REUSE || idx != hc.idx) {
+        const XPair *b = field + idx;
+        float4 l00, h00, l10, h10, l01, h01, l11, h11;
+        load_xpair(b, l00, h00);
+        load_xpair(b + g.np0, l10, h10);
+        load_xpair(b + g.np01, l01, h01);
+        load_xpair(b + g.np01 + g.np0, l11, h11);
+        hc.v[0][0] = l00.x; hc.v[0][1] = l00.y; hc.v[0][2] = l00.z;
+        hc.v[1][0] = h00.x; hc.v[1][1] = h00.y; hc.v[1][2] = h00.z;
+        hc.v[2][0] = l10.x; hc.v[2][1] = l10.y; hc.v[2][2] = l10.z;
+        hc.v[3][0] = h10.x; hc.v[3][1] = h10.y; hc.v[3][2] = h10.z;
+        hc.v[4][0] = l01.x; hc.v[4][1] = l01.y; hc.v[4][2] = l01.z;
+        hc.v[5][0] = h01.x; hc.v[5][1] = h01.y; hc.v[5][2] = h01.z;
+        hc.v[6][0] = l11.x; hc.v[6][1] = l11.y; hc.v[6][2] = l11.z;
+        hc.v[7][0] = h11.x; hc.v[7][1] = h11.y; hc.v[7][2] = h11.z;
+        hc.idx = idx;
+    }
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-        float a00 = fmaf(wl[0], v[1][c] - v[0][c], v[0][c]);
-        float a10 = fmaf(wl[0], v[3][c] - v[2][c], v[2][c]);
-        float a01 = fmaf(wl[0], v[5][c] - v[4][c], v[4][c]);
-        float a11 = fmaf(wl[0], v[7][c] - v[6][c], v[6][c]);
+        float a00 = fmaf(wl[0], hc.v[1][c] - hc.v[0][c], hc.v[0][c]);
+        float a10 = fmaf(wl[0], hc.v[3][c] - hc.v[2][c], hc.v[2][c]);
+        float a01 = fmaf(wl[0], hc.v[5][c] - hc.v[4][c], hc.v[4][c]);
+        float a11 = fmaf(wl[0], hc.v[7][c] - hc.v[6][c], hc.v[6][c]);
         float b0 = fmaf(wl[1], a10 - a00, a00);
         float b1 = fmaf(wl[1], a11 - a01, a01);
         u[c] = fmaf(wl[2], b1 - b0, b0);
@@ -433,24 +452,29 @@ cart_xpair_kernel(const __grid_constant__ CartDev g, const XPair *__restrict__ f
     for (int a = 0; a < 3; ++a) { ci[a] = t.ci[a]; w[a] = t.w[a]; }
     int s = 0;
     bool ok = true;
+    HeldCell hc;
+    hc.idx = -1;
+    const XPair *held_field = nullptr;
     for (; s < nsteps; ++s) {
         const XPair *fa = fields + (int64_t)__ldg(fidx + 3 * s) * field_stride;
         const XPair *fb = fields + (int64_t)__ldg(fidx + 3 * s + 1) * field_stride;
         const XPair *fc = fields + (int64_t)__ldg(fidx + 3 * s + 2) * field_stride;
         float k1[3], k2[3], k3[3], k4[3], xi[3];
-        ok = cart_velocity_xpair<FASTWRAP>(g, fa, ci, w, k1);
+        if (fa != held_field) hc.idx = -1;                     // uniform: tc of the previous step is ta of this one
+        ok = cart_velocity_xpair<FASTWRAP, true>(g, fa, ci, w, hc, k1);
         if (!ok) break;
 #pragma unroll
         for (int a = 0; a < 3; ++a) xi[a] = fmaf(0.5f * hs[a], k1[a], w[a]);
-        ok = cart_velocity_xpair<FASTWRAP>(g, fb, ci, xi, k2);
+        ok = cart_velocity_xpair<FASTWRAP, false>(g, fb, ci, xi, hc, k2);
         if (!ok) break;
 #pragma unroll
         for (int a = 0; a < 3; ++a) xi[a] = fmaf(0.5f * hs[a], k2[a], w[a]);
-        ok = cart_velocity_xpair<FASTWRAP>(g, fb, ci, xi, k3);
+        ok = cart_velocity_xpair<FASTWRAP, true>(g, fb, ci, xi, hc, k3);
         if (!ok) break;
 #pragma unroll
         for (int a = 0; a < 3; ++a) xi[a] = fmaf(hs[a], k3[a], w[a]);
-        ok = cart_velocity_xpair<FASTWRAP>(g, fc, ci, xi, k4);
+        ok = cart_velocity_xpair<FASTWRAP, false>(g, fc, ci, xi, hc, k4);
+        held_field = fc;
         if (!ok) break;
 #pragma unroll
         for (int a = 0; a < 3; ++a) {
