@@ -411,6 +411,14 @@ extern "C" lcs_status lcs_field_get_info(const lcs_field *f, const char *key, in
         }
         *value = (int64_t)(ms * 1e6);
     }
+    else if (!strcmp(key, "locate_fallbacks") || !strcmp(key, "locate_hops") || !strcmp(key, "locate_max_hops") || !strcmp(key, "locate_random_walks")) {
+        *value = 0;
+        if (f->kind == LCS_MESH_SIMPLEX) {
+            unsigned long long h[4] = {0, 0, 0, 0};
+            cudaMemcpy(h, f->mesh.stats, sizeof h, cudaMemcpyDeviceToHost);
+            *value = (int64_t)h[!strcmp(key, "locate_fallbacks") ? 0 : (!strcmp(key, "locate_hops") ? 1 : (!strcmp(key, "locate_max_hops") ? 2 : 3))];
+        }
+    }
     else if (!strcmp(key, "n_boundary_faces")) {
         *value = 0;
         if (f->kind == LCS_MESH_SIMPLEX) {

@@ -64,6 +64,7 @@ struct SimplexMesh {
     double bin_lo[3] = {0, 0, 0};
     double bin_inv[3] = {0, 0, 0};
     int64_t hop_cap = 64;
+    unsigned long long *stats = nullptr;   // [0] brute-force fallbacks, [1] walk hops, [2] max hops of one walk (lcs_locate + seeds)
 };
 
 // tracer scratch owned by the field, grown on demand

@@ -45,13 +45,14 @@ template <int DIM> __device__ __forceinline__ void face_ids(const int32_t *__res
 }
 
 template <int DIM>
-__device__ __forceinline__ bool face_side(const double *__restrict__ verts, const int32_t *fv, const double *p)
+__device__ __forceinline__ bool face_side(const double *__restrict__ verts, const int32_t *fv, const double *p, bool *strict = nullptr)
 {
     if constexpr (DIM == 2) {
         const double *a = verts + 2 * (int64_t)fv[0], *b = verts + 2 * (int64_t)fv[1];
         double ax = a[0], ay = a[1];
         double ex = __dsub_rn(b[0], ax), ey = __dsub_rn(b[1], ay);
         double s = __dsub_rn(__dmul_rn(ex, __dsub_rn(p[1], ay)), __dmul_rn(ey, __dsub_rn(p[0], ax)));
+        if (strict) *strict = s != 0.0;
         if (s != 0.0) return s > 0.0;
         if (ey != 0.0) return -ey > 0.0;
         return ex > 0.0;
@@ -65,6 +66,7 @@ __device__ __forceinline__ bool face_side(const double *__restrict__ verts, cons
         double nz = __dsub_rn(__dmul_rn(ux, vy), __dmul_rn(uy, vx));
         double wx = __dsub_rn(p[0], ax), wy = __dsub_rn(p[1], ay), wz = __dsub_rn(p[2], az);
         double s = __dadd_rn(__dadd_rn(__dmul_rn(nx, wx), __dmul_rn(ny, wy)), __dmul_rn(nz, wz));
+        if (strict) *strict = s != 0.0;
         if (s != 0.0) return s > 0.0;
         if (nx != 0.0) return nx > 0.0;
         if (ny != 0.0) return ny > 0.0;
@@ -86,6 +88,34 @@ __device__ __forceinline__ int first_failing_face(const double *__restrict__ ver
         if (sp != (bool)((opp >> j) & 1u)) return j;
     }
     return -1;
+}
+
+// The walk's view of cell c: first failing face (local order, -1 = c owns p) and whether p lies STRICTLY beyond a hull
+// face of c.  The meshes are triangulations of convex hulls (Delaunay), so a point strictly beyond a hull face is in
+// no cell: the walk stops there instead of circling along the hull, where Qhull's near-flat boundary slivers are not
+// numerically Delaunay and the visibility walk can cycle.  (A point exactly ON a hull plane is left to the
+// first-failing-face rule, so ties resolve exactly as in the oracle.)
+template <int DIM>
+__device__ __forceinline__ int walk_probe(const double *__restrict__ verts, const int32_t *__restrict__ cells,
+                                          const int32_t *__restrict__ neigh, const uint8_t *__restrict__ oppside, int64_t c,
+                                          const double *p, bool *beyond_hull)
+{
+    const unsigned opp = oppside[c];
+    int first = -1;
+    bool out = false;
+#pragma unroll
+    for (int j = 0; j <= DIM; ++j) {
+        int32_t fv[DIM];
+        face_ids<DIM>(cells, c, j, fv);
+        bool strict;
+        bool sp = face_side<DIM>(verts, fv, p, &strict);
+        if (sp != (bool)((opp >> j) & 1u)) {
+            if (first < 0) first = j;
+            if (strict && neigh[c * (DIM + 1) + j] < 0) out = true;
+        }
+    }
+    *beyond_hull = out;
+    return first;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -239,14 +269,16 @@ __global__ void __launch_bounds__(256) bin_scatter_kernel(BinGrid b, const doubl
     atomicMax(bins + bin_of<DIM>(b, x), (int32_t)c);
 }
 
+// One jump-flooding pass.  own[id] >= 0: the bin has a cell of its own (never replaced).  Otherwise the bin keeps the
+// nearest (centroid to bin centre) of its current candidate and the candidates of the 26 (8) bins at distance `step`.
 template <int DIM>
 __global__ void __launch_bounds__(256) bin_flood_kernel(BinGrid b, const double *__restrict__ verts, const int32_t *__restrict__ cells,
-                                                         const int32_t *__restrict__ src, int32_t *__restrict__ dst, int step, int64_t nbins)
+                                                         const int32_t *__restrict__ own, const int32_t *__restrict__ src,
+                                                         int32_t *__restrict__ dst, int step, int64_t nbins)
 {
     int64_t id = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (id >= nbins) return;
-    int32_t cur = src[id];
-    if (cur >= 0) { dst[id] = cur; return; }
+    if (own[id] >= 0) { dst[id] = own[id]; return; }
     int ijk[3] = {(int)(id % b.nb[0]), (int)((id / b.nb[0]) % b.nb[1]), (int)(id / ((int64_t)b.nb[0] * b.nb[1]))};
     double ctr[DIM];
 #pragma unroll
@@ -275,17 +307,48 @@ __global__ void __launch_bounds__(256) bin_flood_kernel(BinGrid b, const double 
 template <int DIM>
 __device__ __forceinline__ int32_t locate_canonical(const BinGrid &b, const int32_t *__restrict__ bins, const double *__restrict__ verts,
                                                     const int32_t *__restrict__ cells, const int32_t *__restrict__ neigh,
-                                                    const uint8_t *__restrict__ oppside, int64_t nc, int64_t hop_cap, const double *p)
+                                                    const uint8_t *__restrict__ oppside, int64_t nc, int64_t hop_cap, const double *p,
+                                                    unsigned long long *__restrict__ stats)
 {
     int64_t c = bins[bin_of<DIM>(b, p)];
     if (c < 0) c = 0;
     for (int64_t hop = 0; hop < hop_cap; ++hop) {
-        int j = first_failing_face<DIM>(verts, cells, oppside, c, p);
-        if (j < 0) return (int32_t)c;
-        int32_t nb = neigh[c * (DIM + 1) + j];
-        if (nb < 0) return -1;
+        bool beyond;
+        int j = walk_probe<DIM>(verts, cells, neigh, oppside, c, p, &beyond);
+        int32_t nb = j < 0 ? 0 : (beyond ? -1 : neigh[c * (DIM + 1) + j]);
+        if (j < 0 || nb < 0) {
+            atomicAdd(stats + 1, (unsigned long long)hop);
+            if ((unsigned long long)hop > stats[2]) atomicMax(stats + 2, (unsigned long long)hop);
+            return j < 0 ? (int32_t)c : -1;
+        }
         c = nb;
     }
+    // The deterministic walk hit its cap: it is circling among slivers that are not numerically Delaunay.  A walk that
+    // picks a pseudo-random failing face cannot stay in a cycle; the owner it finds is the same unique owner.
+    uint32_t rs = (uint32_t)(c * 2654435761u) ^ (uint32_t)__double2loint(p[0]) ^ 0x9e3779b9u;
+    for (int64_t hop = 0; hop < 8 * hop_cap; ++hop) {
+        const unsigned opp = oppside[c];
+        int failing[DIM + 1], nf = 0;
+        bool out = false;
+#pragma unroll
+        for (int j = 0; j <= DIM; ++j) {
+            int32_t fv[DIM];
+            face_ids<DIM>(cells, c, j, fv);
+            bool strict;
+            bool sp = face_side<DIM>(verts, fv, p, &strict);
+            if (sp != (bool)((opp >> j) & 1u)) {
+                failing[nf++] = j;
+                if (strict && neigh[c * (DIM + 1) + j] < 0) out = true;
+            }
+        }
+        if (nf == 0 || out) { atomicAdd(stats + 3, 1ull); return nf == 0 ? (int32_t)c : -1; }
+        rs = rs * 1664525u + 1013904223u;
+        int j = failing[(rs >> 16) % (unsigned)nf];
+        int32_t nb = neigh[c * (DIM + 1) + j];
+        if (nb < 0) { atomicAdd(stats + 3, 1ull); return -1; }
+        c = nb;
+    }
+    atomicAdd(stats, 1ull);
     for (int64_t k = 0; k < nc; ++k)
         if (first_failing_face<DIM>(verts, cells, oppside, k, p) < 0) return (int32_t)k;
     return -1;
@@ -296,14 +359,14 @@ __global__ void __launch_bounds__(128) simplex_locate_kernel(BinGrid b, const in
                                                               const int32_t *__restrict__ cells, const int32_t *__restrict__ neigh,
                                                               const uint8_t *__restrict__ oppside, int64_t nc, int64_t hop_cap,
                                                               const double *__restrict__ pos, int64_t n, int32_t *__restrict__ cell,
-                                                              double *__restrict__ bary)
+                                                              double *__restrict__ bary, unsigned long long *__restrict__ stats)
 {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     double p[DIM];
 #pragma unroll
     for (int k = 0; k < DIM; ++k) p[k] = pos[i * DIM + k];
-    int32_t c = locate_canonical<DIM>(b, bins, verts, cells, neigh, oppside, nc, hop_cap, p);
+    int32_t c = locate_canonical<DIM>(b, bins, verts, cells, neigh, oppside, nc, hop_cap, p, stats);
     cell[i] = c;
     if (!bary) return;
     double lam[DIM + 1];
@@ -351,14 +414,15 @@ template <int DIM, typename TC>
 __global__ void __launch_bounds__(128) simplex_init_kernel(BinGrid b, const int32_t *__restrict__ bins, const double *__restrict__ verts,
                                                             const int32_t *__restrict__ cells, const int32_t *__restrict__ neigh,
                                                             const uint8_t *__restrict__ oppside, int64_t nc, int64_t hop_cap,
-                                                            const TC *__restrict__ seeds, int64_t n, SimplexState<DIM, TC> st)
+                                                            const TC *__restrict__ seeds, int64_t n, SimplexState<DIM, TC> st,
+                                                            unsigned long long *__restrict__ stats)
 {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     double p[DIM];
 #pragma unroll
     for (int k = 0; k < DIM; ++k) { TC v = seeds[i * DIM + k]; st.x[k][i] = v; p[k] = (double)v; }
-    int32_t c = locate_canonical<DIM>(b, bins, verts, cells, neigh, oppside, nc, hop_cap, p);
+    int32_t c = locate_canonical<DIM>(b, bins, verts, cells, neigh, oppside, nc, hop_cap, p, stats);
     st.cell[i] = c;
     st.flag[i] = c < 0 ? 2 : 0;
     st.steps[i] = 0;
@@ -533,6 +597,8 @@ template <int DIM> lcs_status build_impl(lcs_field *f, const double *vh, const i
     LCS_CUDA_OK(cudaMalloc((void **)&m.cells, (size_t)nf * 4));
     LCS_CUDA_OK(cudaMalloc((void **)&m.neigh, (size_t)nf * 4));
     LCS_CUDA_OK(cudaMalloc((void **)&m.oppside, (size_t)nc));
+    LCS_CUDA_OK(cudaMalloc((void **)&m.stats, 4 * sizeof(unsigned long long)));
+    LCS_CUDA_OK(cudaMemset(m.stats, 0, 4 * sizeof(unsigned long long)));
     LCS_CUDA_OK(cudaMemcpy(m.verts, vh, (size_t)nv * DIM * 8, cudaMemcpyHostToDevice));
     LCS_CUDA_OK(cudaMemcpy(m.cells, ch, (size_t)nf * 4, cudaMemcpyHostToDevice));
     LCS_CUDA_OK(cudaMemset(m.neigh, 0xff, (size_t)nf * 4));
@@ -601,29 +667,29 @@ template <int DIM> lcs_status build_impl(lcs_field *f, const double *vh, const i
         m.bin_inv[k] = k < DIM ? m.nb[k] / ext[k] : 0.0;
         nbins *= m.nb[k];
     }
-    int32_t *bins2 = nullptr;
-    LCS_CUDA_OK(cudaMalloc((void **)&m.bins, (size_t)nbins * 4));
-    LCS_CUDA_OK(cudaMalloc((void **)&bins2, (size_t)nbins * 4));
-    LCS_CUDA_OK(cudaMemset(m.bins, 0xff, (size_t)nbins * 4));
+    int32_t *own = nullptr, *ping = nullptr, *pong = nullptr;
+    LCS_CUDA_OK(cudaMalloc((void **)&own, (size_t)nbins * 4));
+    LCS_CUDA_OK(cudaMalloc((void **)&ping, (size_t)nbins * 4));
+    LCS_CUDA_OK(cudaMalloc((void **)&pong, (size_t)nbins * 4));
+    LCS_CUDA_OK(cudaMemset(own, 0xff, (size_t)nbins * 4));
     BinGrid b = make_bins(f);
-    LCS_LAUNCH((bin_scatter_kernel<DIM>), lcs_blocks(nc, 256), 256, 0, st, b, m.verts, m.cells, nc, m.bins);
+    LCS_LAUNCH((bin_scatter_kernel<DIM>), lcs_blocks(nc, 256), 256, 0, st, b, m.verts, m.cells, nc, own);
+    LCS_CUDA_OK(cudaMemcpyAsync(ping, own, (size_t)nbins * 4, cudaMemcpyDeviceToDevice, st));
     int maxnb = std::max(m.nb[0], std::max(m.nb[1], m.nb[2]));
     int step = 1;
     while (step * 2 < maxnb) step *= 2;
-    int32_t *src = m.bins, *dst = bins2;
-    for (int pass = 0; step >= 1 || pass < 0; ++pass) {
-        LCS_LAUNCH((bin_flood_kernel<DIM>), lcs_blocks(nbins, 256), 256, 0, st, b, m.verts, m.cells, src, dst, step, nbins);
-        std::swap(src, dst);
-        if (step == 1) break;
-        step /= 2;
+    for (; step >= 1; step /= 2) {                 // jump flooding, then two more unit passes
+        LCS_LAUNCH((bin_flood_kernel<DIM>), lcs_blocks(nbins, 256), 256, 0, st, b, m.verts, m.cells, own, ping, pong, step, nbins);
+        std::swap(ping, pong);
     }
-    for (int extra = 0; extra < 2; ++extra) {      // two more unit passes close the remaining gaps
-        LCS_LAUNCH((bin_flood_kernel<DIM>), lcs_blocks(nbins, 256), 256, 0, st, b, m.verts, m.cells, src, dst, 1, nbins);
-        std::swap(src, dst);
+    for (int extra = 0; extra < 2; ++extra) {
+        LCS_LAUNCH((bin_flood_kernel<DIM>), lcs_blocks(nbins, 256), 256, 0, st, b, m.verts, m.cells, own, ping, pong, 1, nbins);
+        std::swap(ping, pong);
     }
     LCS_CUDA_OK(cudaDeviceSynchronize());
-    if (src != m.bins) { std::swap(m.bins, bins2); }
-    cudaFree(bins2);
+    m.bins = ping;
+    cudaFree(pong);
+    cudaFree(own);
     m.hop_cap = (int64_t)(4.0 * pow((double)nc, 1.0 / DIM)) + 64;
     LCS_CUDA_OK(cudaGetLastError());
     return LCS_OK;
@@ -660,7 +726,7 @@ lcs_status simplex_advect_impl(lcs_field *f, int64_t n, const void *seeds_, doub
     LCS_CUDA_OK(cudaMemcpyAsync(d_tau, tau.data(), tau.size() * sizeof(TC), cudaMemcpyHostToDevice, st));
     BinGrid b = make_bins(f);
     LCS_LAUNCH((simplex_init_kernel<DIM, TC>), lcs_blocks(n, 128), 128, 0, st, b, m.bins, m.verts, m.cells, m.neigh, m.oppside, m.nc,
-               m.hop_cap, seeds, n, S);
+               m.hop_cap, seeds, n, S, m.stats);
     const int block = f->opt_block ? (int)f->opt_block : 128;
     const int dir = h > 0 ? 1 : -1;
     using VRec = PairRec<DIM, TV>;
@@ -698,6 +764,7 @@ void lcs_simplex_free(lcs_field *f)
     if (m.oppside) cudaFree(m.oppside);
     if (m.cellrec) cudaFree(m.cellrec);
     if (m.bins) cudaFree(m.bins);
+    if (m.stats) cudaFree(m.stats);
     m = SimplexMesh();
 }
 
@@ -706,9 +773,9 @@ lcs_status lcs_simplex_locate(lcs_field *f, int64_t n, const double *pos, int32_
     SimplexMesh &m = f->mesh;
     BinGrid b = make_bins(f);
     if (f->dim == 2)
-        LCS_LAUNCH((simplex_locate_kernel<2>), lcs_blocks(n, 128), 128, 0, st, b, m.bins, m.verts, m.cells, m.neigh, m.oppside, m.nc, m.hop_cap, pos, n, cell, bary);
+        LCS_LAUNCH((simplex_locate_kernel<2>), lcs_blocks(n, 128), 128, 0, st, b, m.bins, m.verts, m.cells, m.neigh, m.oppside, m.nc, m.hop_cap, pos, n, cell, bary, m.stats);
     else
-        LCS_LAUNCH((simplex_locate_kernel<3>), lcs_blocks(n, 128), 128, 0, st, b, m.bins, m.verts, m.cells, m.neigh, m.oppside, m.nc, m.hop_cap, pos, n, cell, bary);
+        LCS_LAUNCH((simplex_locate_kernel<3>), lcs_blocks(n, 128), 128, 0, st, b, m.bins, m.verts, m.cells, m.neigh, m.oppside, m.nc, m.hop_cap, pos, n, cell, bary, m.stats);
     LCS_CUDA_OK(cudaGetLastError());
     return LCS_OK;
 }
