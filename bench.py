@@ -314,13 +314,29 @@ def main():
         bytes_unit = algorithmic_bytes_per_seed_step(w)
         units_per_launch = steps_per_pass * args.steps / max(win_launches, 1)
         achieved = bytes_unit * units_per_launch / max(kernel_s, 1e-12) / 1e9
-        roofline = {"bound": "hbm", "kernel": "cart_window_kernel" if w.kind == 0 else "simplex_window_kernel",
-                    "achieved": achieved, "peak": hbm_gbs, "unit": "GB/s", "frac": achieved / hbm_gbs, "traffic": None,
-                    "peak_source": peak_src, "algorithmic_bytes_per_seed_step": bytes_unit,
-                    "seed_steps_per_launch": units_per_launch, "avg_launch_ms": kernel_s * 1e3,
-                    "kernel_share_of_step": (win_ns * 1e-9) / (elapsed_ms * 1e-3) if world == 1 else None,
-                    "note": "gathers are served by L1/L2 (two snapshots fit in L2), so achieved gather bandwidth may exceed the "
-                            "HBM copy peak; see DESIGN.md for the L2 / issue-slot ceilings"}
+        share = (win_ns * 1e-9) / (elapsed_ms * 1e-3) if world == 1 else None
+        common = {"traffic": None, "seed_steps_per_launch": units_per_launch, "avg_launch_ms": kernel_s * 1e3,
+                  "kernel_share_of_step": share, "algorithmic_bytes_per_seed_step": bytes_unit}
+        if w.kind == 0 and w.dim == 3 and w.compute_dtype == np.float32:
+            # the 3D fp32 Cartesian integrator gathers from L1 (DRAM < 20% of peak) and is bound by
+            # FP32 issue slots + L1 wavefronts.  ALU roofline: SURVEY.md 8.3's 720 flop per seed-step against
+            # 148 SMs x 128 FP32 lanes x 2 flop x max SM clock.
+            flop_unit = 720.0
+            peak_tf = 148 * 128 * 2 * sm_max_mhz * 1e6 / 1e12
+            ach_tf = flop_unit * units_per_launch / max(kernel_s, 1e-12) / 1e12
+            l1_peak = 148 * 128 * sm_max_mhz * 1e6 / 1e9
+            roofline = {"bound": "alu", "kernel": "cart_xpair_kernel", "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s",
+                        "frac": ach_tf / peak_tf, "peak_source": "derived: 148 SMs x 128 FP32 lanes x 2 x %.0f MHz (DESIGN.md)" % sm_max_mhz,
+                        "algorithmic_flop_per_seed_step": flop_unit,
+                        "l1_gather": {"achieved": achieved, "peak": l1_peak, "unit": "GB/s", "frac": achieved / l1_peak,
+                                      "note": "768 B per seed-step of the straightforward 4-stage scheme against 148 SMs x 128 B/clk; "
+                                              "above 1 because the kernel gathers pre-blended fields and reuses corners in registers"},
+                        **common}
+        else:
+            roofline = {"bound": "hbm", "kernel": "cart_window_kernel" if w.kind == 0 else "simplex_window_kernel",
+                        "achieved": achieved, "peak": hbm_gbs, "unit": "GB/s", "frac": achieved / hbm_gbs, "peak_source": peak_src,
+                        "note": "algorithmic gather bytes; small fields are served by L1/L2, so this can exceed the HBM copy peak "
+                                "(DESIGN.md section 6)", **common}
         tr = os.path.join(ROOT, "profiles", "traffic_cfg%d.json" % args.config)
         if os.path.exists(tr):
             roofline["traffic"] = json.load(open(tr)).get("dram_bytes_per_launch")
