@@ -189,7 +189,7 @@ __global__ void __launch_bounds__(256) oppside_kernel(const double *__restrict__
 }
 
 // per-cell affine map for the integrator's walk: lambda_i = M_i . (p - v0), i = 1..DIM; lambda_0 = 1 - sum
-template <int DIM, typename TC> struct alignas(16) CellRec {
+template <int DIM, typename TC> struct alignas(32) CellRec {
     TC M[DIM * DIM];
     TC v0[DIM];
     int32_t vid[DIM + 1];
@@ -432,57 +432,88 @@ template <typename TC> struct WalkTol {};
 template <> struct WalkTol<float> { static constexpr float eps = 1e-4f; };
 template <> struct WalkTol<double> { static constexpr double eps = 1e-10; };
 
-template <int DIM, typename TV, typename TC>
-__device__ __forceinline__ void vertex_velocity(const PairRec<DIM, TV> *__restrict__ rec, int32_t v, TC tau, TC *out)
+// NBYTES (multiple of 16) from a 32-byte-aligned read-only record into registers: 256-bit loads (sm_100
+// ld.global.nc.v8.b32), one L1 request per 32 bytes per lane, plus one 128-bit load for a 16-byte tail.
+template <int NBYTES> __device__ __forceinline__ void load_words(const void *src, uint32_t *w)
 {
-    if constexpr (DIM == 3 && sizeof(TV) == 4) {
-        const float4 *p = reinterpret_cast<const float4 *>(rec + v);
-        float4 a = __ldg(p), d = __ldg(p + 1);
-        out[0] = fma(tau, (TC)d.x, (TC)a.x); out[1] = fma(tau, (TC)d.y, (TC)a.y); out[2] = fma(tau, (TC)d.z, (TC)a.z);
-    } else if constexpr (DIM == 3) {
-        const double2 *p = reinterpret_cast<const double2 *>(rec + v);
-        double2 a0 = __ldg(p), a1 = __ldg(p + 1), d0 = __ldg(p + 2), d1 = __ldg(p + 3);
-        out[0] = fma(tau, (TC)d0.x, (TC)a0.x); out[1] = fma(tau, (TC)d0.y, (TC)a0.y); out[2] = fma(tau, (TC)d1.x, (TC)a1.x);
-    } else if constexpr (sizeof(TV) == 8) {
-        const double2 *p = reinterpret_cast<const double2 *>(rec + v);
-        double2 a = __ldg(p), d = __ldg(p + 1);
-        out[0] = fma(tau, (TC)d.x, (TC)a.x); out[1] = fma(tau, (TC)d.y, (TC)a.y);
-    } else {
-        float4 r = __ldg(reinterpret_cast<const float4 *>(rec + v));
-        out[0] = fma(tau, (TC)r.z, (TC)r.x); out[1] = fma(tau, (TC)r.w, (TC)r.y);
+    static_assert(NBYTES % 16 == 0, "records are multiples of 16 bytes");
+    const char *p = reinterpret_cast<const char *>(src);
+#pragma unroll
+    for (int k = 0; k < NBYTES / 32; ++k)
+        asm("ld.global.nc.v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+            : "=r"(w[8 * k]), "=r"(w[8 * k + 1]), "=r"(w[8 * k + 2]), "=r"(w[8 * k + 3]), "=r"(w[8 * k + 4]), "=r"(w[8 * k + 5]),
+              "=r"(w[8 * k + 6]), "=r"(w[8 * k + 7]) : "l"(p + 32 * k));
+    if constexpr (NBYTES % 32 != 0) {
+        constexpr int o = NBYTES / 32 * 8;
+        asm("ld.global.nc.v4.b32 {%0,%1,%2,%3}, [%4];" : "=r"(w[o]), "=r"(w[o + 1]), "=r"(w[o + 2]), "=r"(w[o + 3]) : "l"(p + 4 * o));
     }
 }
 
-template <int DIM, typename TC> __device__ __forceinline__ CellRec<DIM, TC> load_cellrec(const CellRec<DIM, TC> *__restrict__ rec, int32_t c)
+template <typename T> __device__ __forceinline__ T word_value(const uint32_t *w, int i)
 {
+    if constexpr (sizeof(T) == 4) return __uint_as_float(w[i]);
+    else return __hiloint2double((int)w[2 * i + 1], (int)w[2 * i]);
+}
+
+// The tet/triangle a tracer last evaluated in, kept in registers: its affine map (CellRec) and the two time levels
+// {a, b - a} of its vertices.  Consecutive RK4 stage points are a fraction of a cell apart (h |u| ~ 0.4 cells in
+// config 4), so most stages find the point still inside the held cell and issue no load at all; a lane that crossed a
+// face walks and reloads alone (predicated), which costs L1 wavefronts only for the lines that lane touches.
+template <int DIM, typename TV, typename TC> struct HeldSimplex {
+    int32_t cell = -1;              // cell whose CellRec is held
+    bool vel = false;               // vertex records of `cell` from `pair` are held
+    const void *pair = nullptr;
     CellRec<DIM, TC> r;
-    constexpr int NQ = sizeof(CellRec<DIM, TC>) / 16;
-    const int4 *src = reinterpret_cast<const int4 *>(rec + c);
-    int4 *dst = reinterpret_cast<int4 *>(&r);
+    TC a[DIM + 1][DIM], d[DIM + 1][DIM];
+};
+
+template <int DIM, typename TC> __device__ __forceinline__ void load_cellrec(const CellRec<DIM, TC> *__restrict__ rec, int32_t c,
+                                                                            CellRec<DIM, TC> &r)
+{
+    constexpr int NB = sizeof(CellRec<DIM, TC>);
+    uint32_t w[NB / 4];
+    load_words<NB>(rec + c, w);
+    constexpr int E = sizeof(TC) / 4;
 #pragma unroll
-    for (int k = 0; k < NQ; ++k) dst[k] = __ldg(src + k);
-    return r;
+    for (int k = 0; k < DIM * DIM; ++k) r.M[k] = word_value<TC>(w, k);
+#pragma unroll
+    for (int k = 0; k < DIM; ++k) r.v0[k] = word_value<TC>(w, DIM * DIM + k);
+#pragma unroll
+    for (int k = 0; k <= DIM; ++k) r.vid[k] = (int32_t)w[(DIM * DIM + DIM) * E + k];
+}
+
+// both time levels of vertex v: a[0..DIM), d[0..DIM) widened to the compute type
+template <int DIM, typename TV, typename TC>
+__device__ __forceinline__ void load_vertex(const PairRec<DIM, TV> *__restrict__ rec, int32_t v, TC *a, TC *d)
+{
+    constexpr int NB = sizeof(PairRec<DIM, TV>);
+    constexpr int P = PadOf<DIM>::P;
+    uint32_t w[NB / 4];
+    load_words<NB>(rec + v, w);
+#pragma unroll
+    for (int k = 0; k < DIM; ++k) { a[k] = (TC)word_value<TV>(w, k); d[k] = (TC)word_value<TV>(w, P + k); }
 }
 
 // u(p, tau) with the walk from *cell; false = p left the mesh through a hull face
 template <int DIM, typename TV, typename TC>
 __device__ __forceinline__ bool simplex_velocity(const CellRec<DIM, TC> *__restrict__ crec, const int32_t *__restrict__ neigh,
-                                                 const PairRec<DIM, TV> *__restrict__ vrec, TC tau, const TC *p, int32_t *cell, TC *u)
+                                                 const PairRec<DIM, TV> *__restrict__ vrec, TC tau, const TC *p, int32_t *cell,
+                                                 HeldSimplex<DIM, TV, TC> &h, TC *u)
 {
     int32_t c = *cell;
     TC lam[DIM + 1];
-    CellRec<DIM, TC> r;
+    if (h.pair != (const void *)vrec) { h.vel = false; h.pair = vrec; }        // uniform: another snapshot pair
     for (int hop = 0;; ++hop) {
-        r = load_cellrec<DIM, TC>(crec, c);
+        if (h.cell != c) { load_cellrec<DIM, TC>(crec, c, h.r); h.cell = c; h.vel = false; }
         TC q[DIM];
 #pragma unroll
-        for (int k = 0; k < DIM; ++k) q[k] = p[k] - r.v0[k];
+        for (int k = 0; k < DIM; ++k) q[k] = p[k] - h.r.v0[k];
         TC sum = TC(0);
 #pragma unroll
         for (int i = 0; i < DIM; ++i) {
             TC l = TC(0);
 #pragma unroll
-            for (int k = 0; k < DIM; ++k) l = fma(r.M[i * DIM + k], q[k], l);
+            for (int k = 0; k < DIM; ++k) l = fma(h.r.M[i * DIM + k], q[k], l);
             lam[i + 1] = l;
             sum += l;
         }
@@ -498,14 +529,17 @@ __device__ __forceinline__ bool simplex_velocity(const CellRec<DIM, TC> *__restr
         c = nb;
     }
     *cell = c;
+    if (!h.vel) {
+#pragma unroll
+        for (int i = 0; i <= DIM; ++i) load_vertex<DIM, TV, TC>(vrec, h.r.vid[i], h.a[i], h.d[i]);
+        h.vel = true;
+    }
 #pragma unroll
     for (int k = 0; k < DIM; ++k) u[k] = TC(0);
 #pragma unroll
     for (int i = 0; i <= DIM; ++i) {
-        TC v[DIM];
-        vertex_velocity<DIM, TV, TC>(vrec, r.vid[i], tau, v);
 #pragma unroll
-        for (int k = 0; k < DIM; ++k) u[k] = fma(lam[i], v[k], u[k]);
+        for (int k = 0; k < DIM; ++k) u[k] = fma(lam[i], fma(tau, h.d[i][k], h.a[i][k]), u[k]);
     }
     return true;
 }
@@ -525,23 +559,24 @@ simplex_window_kernel(const CellRec<DIM, TC> *__restrict__ crec, const int32_t *
     int32_t cell = st.cell[i];
     int s = 0;
     bool ok = true;
+    HeldSimplex<DIM, TV, TC> held;
     for (; s < nsteps; ++s) {
         const TC ta = __ldg(tau + 3 * s), tb = __ldg(tau + 3 * s + 1), tc = __ldg(tau + 3 * s + 2);
         TC k1[DIM], k2[DIM], k3[DIM], k4[DIM], y[DIM];
         int32_t c = cell;
-        ok = simplex_velocity<DIM, TV, TC>(crec, neigh, pa, ta, x, &c, k1);
+        ok = simplex_velocity<DIM, TV, TC>(crec, neigh, pa, ta, x, &c, held, k1);
         if (!ok) break;
 #pragma unroll
         for (int k = 0; k < DIM; ++k) y[k] = fma(TC(0.5) * h, k1[k], x[k]);
-        ok = simplex_velocity<DIM, TV, TC>(crec, neigh, pb, tb, y, &c, k2);
+        ok = simplex_velocity<DIM, TV, TC>(crec, neigh, pb, tb, y, &c, held, k2);
         if (!ok) break;
 #pragma unroll
         for (int k = 0; k < DIM; ++k) y[k] = fma(TC(0.5) * h, k2[k], x[k]);
-        ok = simplex_velocity<DIM, TV, TC>(crec, neigh, pb, tb, y, &c, k3);
+        ok = simplex_velocity<DIM, TV, TC>(crec, neigh, pb, tb, y, &c, held, k3);
         if (!ok) break;
 #pragma unroll
         for (int k = 0; k < DIM; ++k) y[k] = fma(h, k3[k], x[k]);
-        ok = simplex_velocity<DIM, TV, TC>(crec, neigh, pc, tc, y, &c, k4);
+        ok = simplex_velocity<DIM, TV, TC>(crec, neigh, pc, tc, y, &c, held, k4);
         if (!ok) break;
 #pragma unroll
         for (int k = 0; k < DIM; ++k) x[k] = fma(h * TC(1.0 / 6.0), (k1[k] + k4[k]) + TC(2) * (k2[k] + k3[k]), x[k]);
