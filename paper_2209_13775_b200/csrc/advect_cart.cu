@@ -268,7 +268,7 @@ __global__ void __launch_bounds__(256) cart_key_kernel(CartDev g, const CartTrac
         if (k > last_bin - 1) k = last_bin - 1;
     }
     key[i] = k;
-    atomicAdd(cnt + k, 1u);
+    bundle::count_key(cnt, k, last_bin);
 }
 
 // ---------------------------------------------------------------------------------------------

@@ -122,10 +122,21 @@ static __global__ void __launch_bounds__(kScanBlock) scan_apply_kernel(uint32_t 
     }
 }
 
-// scatter: record i goes to the next free slot of its key
+// histogram increment; the last bin (finished tracers, possibly most of the set) is aggregated per warp so that its
+// single counter is hit once per warp instead of once per tracer
+__device__ __forceinline__ void count_key(uint32_t *__restrict__ cnt, uint32_t k, uint32_t last_bin)
+{
+    const unsigned active = __activemask();
+    const unsigned parked = __ballot_sync(active, k == last_bin);
+    if (k != last_bin) atomicAdd(cnt + k, 1u);
+    else if ((threadIdx.x & 31) == __ffs(parked) - 1) atomicAdd(cnt + last_bin, (uint32_t)__popc(parked));
+}
+
+// scatter: record i goes to the next free slot of its key (warp-aggregated for the last bin)
 template <typename REC>
 static __global__ void __launch_bounds__(256) scatter_kernel(const REC *__restrict__ src, const uint32_t *__restrict__ key,
-                                                             uint32_t *__restrict__ offset, int64_t n, REC *__restrict__ dst)
+                                                             uint32_t *__restrict__ offset, int64_t n, uint32_t last_bin,
+                                                             REC *__restrict__ dst)
 {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
@@ -135,10 +146,22 @@ static __global__ void __launch_bounds__(256) scatter_kernel(const REC *__restri
     const int4 *s = reinterpret_cast<const int4 *>(src + i);
 #pragma unroll
     for (int k = 0; k < NQ; ++k) q[k] = s[k];
-    uint32_t pos = atomicAdd(offset + key[i], 1u);
+    const uint32_t k = key[i];
+    const unsigned active = __activemask();
+    const unsigned parked = __ballot_sync(active, k == last_bin);
+    uint32_t pos;
+    if (k != last_bin) {
+        pos = atomicAdd(offset + k, 1u);
+    } else {
+        const int lane = threadIdx.x & 31, leader = __ffs(parked) - 1;
+        uint32_t base = 0;
+        if (lane == leader) base = atomicAdd(offset + last_bin, (uint32_t)__popc(parked));
+        base = __shfl_sync(parked, base, leader);
+        pos = base + (uint32_t)__popc(parked & ((1u << lane) - 1u));
+    }
     int4 *d = reinterpret_cast<int4 *>(dst + pos);
 #pragma unroll
-    for (int k = 0; k < NQ; ++k) d[k] = q[k];
+    for (int k2 = 0; k2 < NQ; ++k2) d[k2] = q[k2];
 }
 
 static inline size_t scratch_bytes(int64_t n, int64_t nbins)
@@ -157,7 +180,7 @@ static inline void sort_records(const REC *src, REC *dst, const uint32_t *key, u
     LCS_LAUNCH(scan_tile_sums_kernel, (unsigned)ntiles, kScanBlock, 0, st, cnt, nbins, tile);
     LCS_LAUNCH(scan_tile_offsets_kernel, 1, kScanBlock, 0, st, tile, ntiles);
     LCS_LAUNCH(scan_apply_kernel, (unsigned)ntiles, kScanBlock, 0, st, cnt, nbins, tile);
-    LCS_LAUNCH((scatter_kernel<REC>), lcs_blocks(n, 256), 256, 0, st, src, key, cnt, n, dst);
+    LCS_LAUNCH((scatter_kernel<REC>), lcs_blocks(n, 256), 256, 0, st, src, key, cnt, n, (uint32_t)(nbins - 1), dst);
 }
 
 }  // namespace bundle

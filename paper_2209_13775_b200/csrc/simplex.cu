@@ -20,6 +20,7 @@
 #include <algorithm>
 #include <cub/cub.cuh>
 
+#include "bundle_sort.cuh"
 #include "lcs_internal.cuh"
 
 namespace {
@@ -403,29 +404,77 @@ __global__ void __launch_bounds__(128) simplex_locate_kernel(BinGrid b, const in
 
 // ---------------------------------------------------------------------------------------------
 // integrator
-template <int DIM, typename TC> struct SimplexState {
-    TC *x[3];
-    int32_t *cell;
-    int32_t *steps;
-    uint8_t *flag;
+// tracer record (array of structures, whole 32-byte sectors: one sector for 3D fp32 and 2D fp64).
+// meta = completed steps at exit (low 30 bits) | exit flag << 30
+template <int DIM, typename TC> struct alignas(16) SimplexTracer {
+    TC x[DIM];
+    int32_t cell;
+    int32_t orig;
+    uint32_t meta;
 };
+
+template <typename REC> __device__ __forceinline__ REC load_tracer(const REC *p)
+{
+    REC r;
+    constexpr int NQ = sizeof(REC) / 16;
+    const int4 *s = reinterpret_cast<const int4 *>(p);
+    int4 *d = reinterpret_cast<int4 *>(&r);
+#pragma unroll
+    for (int k = 0; k < NQ; ++k) d[k] = s[k];
+    return r;
+}
+template <typename REC> __device__ __forceinline__ void store_tracer(REC *p, const REC &r)
+{
+    constexpr int NQ = sizeof(REC) / 16;
+    const int4 *s = reinterpret_cast<const int4 *>(&r);
+    int4 *d = reinterpret_cast<int4 *>(p);
+#pragma unroll
+    for (int k = 0; k < NQ; ++k) d[k] = s[k];
+}
 
 template <int DIM, typename TC>
 __global__ void __launch_bounds__(128) simplex_init_kernel(BinGrid b, const int32_t *__restrict__ bins, const double *__restrict__ verts,
                                                             const int32_t *__restrict__ cells, const int32_t *__restrict__ neigh,
                                                             const uint8_t *__restrict__ oppside, int64_t nc, int64_t hop_cap,
-                                                            const TC *__restrict__ seeds, int64_t n, SimplexState<DIM, TC> st,
+                                                            const TC *__restrict__ seeds, int64_t n, SimplexTracer<DIM, TC> *__restrict__ st,
                                                             unsigned long long *__restrict__ stats)
 {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
+    SimplexTracer<DIM, TC> t;
     double p[DIM];
 #pragma unroll
-    for (int k = 0; k < DIM; ++k) { TC v = seeds[i * DIM + k]; st.x[k][i] = v; p[k] = (double)v; }
+    for (int k = 0; k < DIM; ++k) { TC v = seeds[i * DIM + k]; t.x[k] = v; p[k] = (double)v; }
     int32_t c = locate_canonical<DIM>(b, bins, verts, cells, neigh, oppside, nc, hop_cap, p, stats);
-    st.cell[i] = c;
-    st.flag[i] = c < 0 ? 2 : 0;
-    st.steps[i] = 0;
+    t.cell = c;
+    t.orig = (int32_t)i;
+    t.meta = c < 0 ? (2u << 30) : 0u;
+    store_tracer(st + i, t);
+}
+
+// sort key: Morton code of the tracer's bin (bin grid coarsened by `shift`); finished tracers go to the last bin so
+// that live tracers stay compacted at the front and whole warps of finished ones retire at once
+template <int DIM, typename TC>
+__global__ void __launch_bounds__(256) simplex_key_kernel(BinGrid b, const SimplexTracer<DIM, TC> *__restrict__ st, int64_t n, int shift,
+                                                           uint32_t last_bin, uint32_t *__restrict__ key, uint32_t *__restrict__ cnt)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const SimplexTracer<DIM, TC> t = load_tracer(st + i);
+    uint32_t k = last_bin;
+    if ((t.meta >> 30) == 0) {
+        int c[DIM];
+#pragma unroll
+        for (int a = 0; a < DIM; ++a) {
+            double q = floor(((double)t.x[a] - b.lo[a]) * b.inv[a]);
+            int ia = q < 0.0 ? 0 : (q > (double)(b.nb[a] - 1) ? b.nb[a] - 1 : (int)q);
+            c[a] = ia >> shift;
+        }
+        k = bundle::morton<DIM>(c);
+        if (k > last_bin - 1) k = last_bin - 1;
+    }
+    key[i] = k;
+    bundle::count_key(cnt, k, last_bin);
 }
 
 template <typename TC> struct WalkTol {};
@@ -548,15 +597,16 @@ template <int DIM, typename TV, typename TC>
 __global__ void __launch_bounds__(128)
 simplex_window_kernel(const CellRec<DIM, TC> *__restrict__ crec, const int32_t *__restrict__ neigh, const PairRec<DIM, TV> *__restrict__ pa,
                       const PairRec<DIM, TV> *__restrict__ pb, const PairRec<DIM, TV> *__restrict__ pc, const TC *__restrict__ tau,
-                      int nsteps, int first_step, int64_t n, SimplexState<DIM, TC> st, TC h)
+                      int nsteps, int first_step, int64_t n, SimplexTracer<DIM, TC> *__restrict__ st, TC h)
 {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    if (st.flag[i] != 0) return;
+    SimplexTracer<DIM, TC> t = load_tracer(st + i);
+    if ((t.meta >> 30) != 0) return;
     TC x[DIM];
 #pragma unroll
-    for (int k = 0; k < DIM; ++k) x[k] = st.x[k][i];
-    int32_t cell = st.cell[i];
+    for (int k = 0; k < DIM; ++k) x[k] = t.x[k];
+    int32_t cell = t.cell;
     int s = 0;
     bool ok = true;
     HeldSimplex<DIM, TV, TC> held;
@@ -583,22 +633,26 @@ simplex_window_kernel(const CellRec<DIM, TC> *__restrict__ crec, const int32_t *
         cell = c;
     }
 #pragma unroll
-    for (int k = 0; k < DIM; ++k) st.x[k][i] = x[k];
-    st.cell[i] = cell;
-    if (!ok) { st.flag[i] = 1; st.steps[i] = first_step + s; }
+    for (int k = 0; k < DIM; ++k) t.x[k] = x[k];
+    t.cell = cell;
+    if (!ok) t.meta = (1u << 30) | (uint32_t)(first_step + s);
+    store_tracer(st + i, t);
 }
 
 template <int DIM, typename TC>
-__global__ void __launch_bounds__(256) simplex_final_kernel(int64_t n, SimplexState<DIM, TC> st, int32_t N, TC *__restrict__ flowmap,
-                                                             uint8_t *__restrict__ exit_flag, int32_t *__restrict__ exit_step)
+__global__ void __launch_bounds__(256) simplex_final_kernel(int64_t n, const SimplexTracer<DIM, TC> *__restrict__ st, int32_t N,
+                                                             TC *__restrict__ flowmap, uint8_t *__restrict__ exit_flag,
+                                                             int32_t *__restrict__ exit_step)
 {
-    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    uint8_t fl = st.flag[i];
+    int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= n) return;
+    const SimplexTracer<DIM, TC> t = load_tracer(st + j);
+    const int64_t i = t.orig;
+    const uint32_t fl = t.meta >> 30;
 #pragma unroll
-    for (int k = 0; k < DIM; ++k) flowmap[i * DIM + k] = st.x[k][i];
-    if (exit_flag) exit_flag[i] = fl;
-    if (exit_step) exit_step[i] = fl == 0 ? N : (fl == 2 ? 0 : st.steps[i]);
+    for (int k = 0; k < DIM; ++k) flowmap[i * DIM + k] = t.x[k];
+    if (exit_flag) exit_flag[i] = (uint8_t)fl;
+    if (exit_step) exit_step[i] = fl == 0 ? N : (fl == 2 ? 0 : (int32_t)(t.meta & 0x3fffffffu));
 }
 
 BinGrid make_bins(const lcs_field *f)
@@ -734,37 +788,57 @@ template <int DIM, typename TV, typename TC>
 lcs_status simplex_advect_impl(lcs_field *f, int64_t n, const void *seeds_, double t0, double h, int64_t N, void *flowmap_,
                                uint8_t *exit_flag, int32_t *exit_step, cudaStream_t st)
 {
+    using Tracer = SimplexTracer<DIM, TC>;
     const TC *seeds = (const TC *)seeds_;
     TC *flowmap = (TC *)flowmap_;
     SimplexMesh &m = f->mesh;
+    if (n >= (1LL << 31) || N >= (1LL << 30)) { lcs_set_error("too many seeds or steps for 32-bit tracer records"); return LCS_ERR_INVALID_ARG; }
     std::vector<StepWindow> windows;
     std::vector<double> tau64;
     lcs_status rc = lcs_plan_windows(f, t0, h, N, windows, tau64);
     if (rc != LCS_OK) return rc;
     std::vector<TC> tau(tau64.size());
     for (size_t k = 0; k < tau.size(); ++k) tau[k] = (TC)tau64[k];
-    size_t off = 0, o_x[3], o_cell, o_steps, o_flag, o_tau;
-    for (int a = 0; a < DIM; ++a) { o_x[a] = off; off = align_up(off + (size_t)n * sizeof(TC)); }
-    o_cell = off; off = align_up(off + (size_t)n * 4);
-    o_steps = off; off = align_up(off + (size_t)n * 4);
-    o_flag = off; off = align_up(off + (size_t)n);
-    o_tau = off; off = align_up(off + tau.size() * sizeof(TC));
+
+    // re-bundling by bin (Morton order of the coarsened bin grid), histogram <= 2^24 bins
+    const bool do_bundle = f->opt_bundle == 1 || (f->opt_bundle < 0 && n >= (1 << 20));
+    int shift = 0, bits = 0;
+    for (;; ++shift) {
+        bits = 0;
+        for (int a = 0; a < DIM; ++a) {
+            int cells = ((m.nb[a] - 1) >> shift) + 1, b = 0;
+            while ((1 << b) < cells) ++b;
+            bits = b > bits ? b : bits;
+        }
+        if (bits * DIM <= 24) break;
+    }
+    const int64_t nbins = do_bundle ? ((int64_t)1 << (bits * DIM)) + 1 : 0;
+    const int64_t ntiles = (nbins + bundle::kScanTile - 1) / bundle::kScanTile;
+
+    size_t off = 0;
+    const size_t o_a = off; off = align_up(off + (size_t)n * sizeof(Tracer));
+    const size_t o_b = off; if (do_bundle) off = align_up(off + (size_t)n * sizeof(Tracer));
+    const size_t o_tau = off; off = align_up(off + tau.size() * sizeof(TC));
+    const size_t o_key = off; if (do_bundle) off = align_up(off + (size_t)n * 4);
+    const size_t o_cnt = off; if (do_bundle) off = align_up(off + (size_t)nbins * 4);
+    const size_t o_tile = off; if (do_bundle) off = align_up(off + (size_t)ntiles * 4);
     rc = lcs_scratch_reserve(f, off);
     if (rc != LCS_OK) return rc;
     char *base = (char *)f->scratch.buf;
-    SimplexState<DIM, TC> S{};
-    for (int a = 0; a < DIM; ++a) S.x[a] = (TC *)(base + o_x[a]);
-    S.cell = (int32_t *)(base + o_cell);
-    S.steps = (int32_t *)(base + o_steps);
-    S.flag = (uint8_t *)(base + o_flag);
+    Tracer *cur = (Tracer *)(base + o_a), *alt = (Tracer *)(base + o_b);
     TC *d_tau = (TC *)(base + o_tau);
+    uint32_t *d_key = (uint32_t *)(base + o_key), *d_cnt = (uint32_t *)(base + o_cnt), *d_tile = (uint32_t *)(base + o_tile);
     LCS_CUDA_OK(cudaMemcpyAsync(d_tau, tau.data(), tau.size() * sizeof(TC), cudaMemcpyHostToDevice, st));
     BinGrid b = make_bins(f);
     LCS_LAUNCH((simplex_init_kernel<DIM, TC>), lcs_blocks(n, 128), 128, 0, st, b, m.bins, m.verts, m.cells, m.neigh, m.oppside, m.nc,
-               m.hop_cap, seeds, n, S, m.stats);
-    const int block = f->opt_block ? (int)f->opt_block : 128;
+               m.hop_cap, seeds, n, cur, m.stats);
+    const int block = f->opt_block ? (int)(f->opt_block > 128 ? 128 : f->opt_block) : 128;
     const int dir = h > 0 ? 1 : -1;
     using VRec = PairRec<DIM, TV>;
+    int64_t since_bundle = -1;                       // -1: not bundled yet
+    // unstructured meshes: tracers cross a cell in ~2.5 steps but stay spatially coherent much longer, and a sort moves
+    // every record: re-bundle every 160 steps unless told otherwise (measured on config 4: 160 > per window > once)
+    const int64_t bundle_every = f->opt_bundle_steps > 0 ? f->opt_bundle_steps : 160;
     for (size_t wi = 0; wi < windows.size(); ++wi) {
         const StepWindow &w = windows[wi];
         const void *p[3];
@@ -773,12 +847,25 @@ lcs_status simplex_advect_impl(lcs_field *f, int64_t n, const void *seeds_, doub
             if (rc != LCS_OK) return rc;
         }
         lcs_field_prefetch(f, dir > 0 ? w.s[2] + 2 : w.s[2] - 1, w.s[2], w.s[2] + 1);
-        WindowTimer timer(f, st);
-        LCS_LAUNCH((simplex_window_kernel<DIM, TV, TC>), lcs_blocks(n, block), block, 0, st, (const CellRec<DIM, TC> *)m.cellrec, m.neigh,
-                   (const VRec *)p[0], (const VRec *)p[1], (const VRec *)p[2], d_tau + 3 * w.first, w.count, (int)w.first, n, S, (TC)h);
+        const int chunk = (do_bundle && f->opt_bundle_steps > 0 && f->opt_bundle_steps < w.count) ? (int)f->opt_bundle_steps : w.count;
+        for (int done = 0; done < w.count; done += chunk) {
+            const int cnt = w.count - done < chunk ? w.count - done : chunk;
+            const int first = (int)w.first + done;
+            if (do_bundle && (since_bundle < 0 || since_bundle >= bundle_every)) {
+                LCS_CUDA_OK(cudaMemsetAsync(d_cnt, 0, (size_t)nbins * 4, st));
+                LCS_LAUNCH((simplex_key_kernel<DIM, TC>), lcs_blocks(n, 256), 256, 0, st, b, cur, n, shift, (uint32_t)(nbins - 1), d_key, d_cnt);
+                bundle::sort_records<Tracer>(cur, alt, d_key, d_cnt, d_tile, n, nbins, st);
+                std::swap(cur, alt);
+                since_bundle = 0;
+            }
+            since_bundle += cnt;
+            WindowTimer timer(f, st);
+            LCS_LAUNCH((simplex_window_kernel<DIM, TV, TC>), lcs_blocks(n, block), block, 0, st, (const CellRec<DIM, TC> *)m.cellrec, m.neigh,
+                       (const VRec *)p[0], (const VRec *)p[1], (const VRec *)p[2], d_tau + 3 * (size_t)first, cnt, first, n, cur, (TC)h);
+        }
         f->info_windows++;
     }
-    LCS_LAUNCH((simplex_final_kernel<DIM, TC>), lcs_blocks(n, 256), 256, 0, st, n, S, (int32_t)N, flowmap, exit_flag, exit_step);
+    LCS_LAUNCH((simplex_final_kernel<DIM, TC>), lcs_blocks(n, 256), 256, 0, st, n, cur, (int32_t)N, flowmap, exit_flag, exit_step);
     LCS_CUDA_OK(cudaGetLastError());
     return LCS_OK;
 }

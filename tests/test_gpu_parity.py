@@ -438,3 +438,15 @@ def test_preblend_nonperiodic_3d_fp32_with_exits(lcs, oracle):
     assert np.mean(cpu(flag1) == flo) > 0.995
     same = cpu(flag1) == flo
     assert np.max(np.linalg.norm(cpu(F1)[same].astype(np.float64) - Fo[same], axis=1)) < 1e-3 * w.L
+
+
+@pytest.mark.parametrize("options", [dict(bundle=1), dict(bundle=1, bundle_steps=7)])
+def test_simplex_bundled_identical_to_unbundled(lcs, oracle, options):
+    """Re-bundling tracers by bin (triangles fp64, tets fp32 with flags 0/1/2): a tracer's arithmetic does not depend on
+    its slot, so results are bit-identical to the unbundled run and come back in the caller's order."""
+    import torch
+    for w in (I.config2(ng=(96, 48), lattice=(40, 20), T=4.0), I.config4(ng=(20, 20, 36), delta=0.08, T=1.5, h=0.005, n_snap=10, length=4.0)):
+        f0, sd0, F0, flag0, es0 = gpu_run(w, options=dict(bundle=0))
+        f1, sd1, F1, flag1, es1 = gpu_run(w, options=options)
+        assert torch.equal(F0, F1) and torch.equal(flag0, flag1) and torch.equal(es0, es1)
+        assert f1.info("locate_fallbacks") == 0
