@@ -185,6 +185,20 @@ def reference_arm(args):
     return 0
 
 
+def reduce_over_ranks(elapsed_ms, seed_steps, seeds, device, world):
+    """Whole-job figures: the time is the MAX over ranks, the work is the SUM (every rank integrates its own FTLE volume;
+    there is no data-path collective).  Backend-agnostic (nccl on GPUs, gloo in the CPU test)."""
+    if world <= 1:
+        return float(elapsed_ms), float(seed_steps), float(seeds)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([elapsed_ms], dtype=torch.float64, device=device)
+    tot = torch.tensor([seed_steps, seeds], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(tot, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(tot[0].item()), float(tot[1].item())
+
+
 # ------------------------------------------------------------------------------------------------
 def main():
     ap = argparse.ArgumentParser()
@@ -272,13 +286,7 @@ def main():
     win_ns = field.info("window_time_ns")
     win_launches = field.info("window_launches")
     field.set_option("time_windows", 0)
-    t = torch.tensor([elapsed_ms], dtype=torch.float64, device="cuda")
-    tot = torch.tensor([steps_per_pass, float(n * len(runs))], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
-    elapsed_ms = float(t.item())
-    steps_all, seeds_all = float(tot[0].item()), float(tot[1].item())
+    elapsed_ms, steps_all, seeds_all = reduce_over_ranks(elapsed_ms, steps_per_pass, float(n * len(runs)), "cuda", world)
     sec_per_step = elapsed_ms * 1e-3 / args.steps
     value = steps_all / sec_per_step
 

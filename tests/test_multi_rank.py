@@ -1,0 +1,58 @@
+"""N > 1 path of bench.py on CPU (gloo, world_size 2): the path shards with no data-path collective -- every rank
+integrates its own FTLE volume -- so what ranks share is only the reduction of the timing
+(MAX over ranks) and of the work (SUM).  The kernels themselves need a GPU and are covered by the -m gpu tests."""
+import os
+import sys
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _worker(rank, world, port, out):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    sys.path.insert(0, ROOT)
+    import torch.distributed as dist
+    import bench
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        ms, steps, seeds = bench.reduce_over_ranks(100.0 + 25.0 * rank, 1000.0 * (rank + 1), 64.0, "cpu", world)
+        out.put((rank, ms, steps, seeds))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_reduce_over_ranks_gloo_world2():
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 29500 + os.getpid() % 2000
+    procs = [ctx.Process(target=_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = sorted(q.get(timeout=120) for _ in procs)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    for rank, ms, steps, seeds in res:
+        assert ms == 125.0 and steps == 3000.0 and seeds == 128.0      # max time, summed work, on every rank
+
+
+def test_reduce_single_rank_is_identity():
+    sys.path.insert(0, ROOT)
+    import bench
+    assert bench.reduce_over_ranks(12.5, 7.0, 3.0, "cpu", 1) == (12.5, 7.0, 3.0)
+
+
+def test_rank_shards_are_independent_volumes_of_equal_size():
+    """Weak scaling: rank r integrates the seed grid released at t0 = 0.5 r over the same T; every window stays inside the
+    snapshot times for the 8 ranks of one node, and all ranks do the same amount of work."""
+    sys.path.insert(0, ROOT)
+    from paper_2209_13775_b200 import inputs as I
+    w = I.config3(ngrid=8, nn=8)
+    for rank in range(8):
+        t0 = 0.5 * rank
+        assert w.times[0] <= t0 and t0 + 5.0 <= w.times[-1] + 1e-12
+    src = open(os.path.join(ROOT, "bench.py")).read()
+    assert "t0 = 0.5 * rank" in src and "\"scaling\": \"weak\"" in src
