@@ -113,7 +113,7 @@ struct lcs_field {
     int64_t opt_bundle = -1;      // re-bundle tracers by cell: -1 auto (large seed sets), 0 off, 1 on
     int64_t opt_bundle_steps = 0; // RK4 steps between re-bundlings (0 = once per snapshot window)
     int64_t opt_preblend = -1;    // 3D fp32 Cartesian: gather from per-stage-time blended fields (-1 auto, 0 off, 1 on)
-    int64_t opt_preblend_steps = 10; // RK4 steps per launch of the pre-blended integrator (2k+1 blended fields resident)
+    int64_t opt_preblend_steps = 25; // RK4 steps per launch of the pre-blended integrator (2k+1 blended fields resident)
     int64_t opt_ld256 = 1;        // gather pair records with one 256-bit load instead of two 128-bit loads
     int64_t opt_block = 0;        // threads per block override (0 = default)
     int64_t opt_time_windows = 0; // record CUDA events around every window (hot) kernel launch
