@@ -450,3 +450,92 @@ def test_simplex_bundled_identical_to_unbundled(lcs, oracle, options):
         f1, sd1, F1, flag1, es1 = gpu_run(w, options=options)
         assert torch.equal(F0, F1) and torch.equal(flag0, flag1) and torch.equal(es0, es1)
         assert f1.info("locate_fallbacks") == 0
+
+
+@pytest.mark.slow
+def test_config4_full_size_sampled(lcs, oracle):
+    """Config 4 at full size (2.01 M vertices / 13.4 M tets, 256x256x512 box seeds, 1600 steps) in bench.py's launch
+    configuration (bundling on by default at this size).  lcs_locate: bit-exact against the oracle's walk on 2e5 sampled
+    seeds and against brute force over all cells on 64 of them, with no fallback.  Flow map / FTLE: the oracle integrates
+    6 seeded 12^3 blocks; statistical gate of BASELINE.json."""
+    import torch
+    w = I.config4()
+    f = lcs.Field.from_workload(w)
+    fo = oracle.OracleField.from_workload(w)
+    seeds = w.seeds()
+    rng = np.random.default_rng(44)
+    pick = rng.choice(seeds.shape[0], 200000, replace=False)
+    pts = np.ascontiguousarray(seeds[pick].astype(np.float64))
+    cg_ = cpu(f.locate(torch.from_numpy(pts).cuda()))
+    assert np.array_equal(cg_, fo.locate_walk(pts))
+    cb, count = fo.locate_brute(pts[:64])
+    assert np.array_equal(cg_[:64], cb) and np.all(count <= 1)
+    assert f.info("locate_fallbacks") == 0
+    sd = torch.from_numpy(seeds).cuda()
+    F, flag, es = f.advect(sd, w.t0, w.tf, w.h)
+    cgg, ftg, stg = gpu_cg(w, F, flag)
+    torch.cuda.synchronize()
+    assert f.info("locate_fallbacks") == 0
+    nx, ny, nz = w.ng
+    Fh = cpu(F).reshape(nz, ny, nx, 3); fth = cpu(ftg).reshape(nz, ny, nx); flh = cpu(flag).reshape(nz, ny, nx)
+    S = seeds.reshape(nz, ny, nx, 3)
+    B = 12
+    errs, rels, mism, tot = [], [], 0, 0
+    for b in range(6):
+        if b < 3:      # slow tracers near the wall (r ~ 0.8, u_z ~ 0.7): stay inside for all 1600 steps, FTLE is defined
+            k0, j0, i0 = int(rng.integers(10, 150)), int(rng.integers(110, 134)), 228
+        else:          # core of the pipe: leave through the outlet (flag 1), early or late
+            k0 = int(rng.integers(0, nz // 3)) if b < 5 else int(rng.integers(nz // 2, nz - B))
+            j0, i0 = (int(v) for v in rng.integers(ny // 4, 3 * ny // 4 - B, 2))
+        blk = np.ascontiguousarray(S[k0:k0 + B, j0:j0 + B, i0:i0 + B].reshape(-1, 3))
+        Fo, flo, eso = fo.advect(blk.astype(np.float64), w.t0, w.tf, w.h)
+        Fg = Fh[k0:k0 + B, j0:j0 + B, i0:i0 + B].reshape(-1, 3).astype(np.float64)
+        fg = flh[k0:k0 + B, j0:j0 + B, i0:i0 + B].ravel()
+        bad = (np.linalg.norm(Fg - Fo, axis=1) > 1e-3 * w.L) | (fg != flo)
+        mism += int(bad.sum()); tot += bad.size
+        errs.append(np.linalg.norm(Fg - Fo, axis=1)[fg == flo])
+        cgo, fto, sto = oracle.cg_ftle(3, (B, B, B), w.seed_spacing, (0, 0, 0), (0, 0, 0), Fo, flo, w.tf - w.t0)
+        fto = fto.reshape(B, B, B)[1:-1, 1:-1, 1:-1]
+        ftb = fth[k0 + 1:k0 + B - 1, j0 + 1:j0 + B - 1, i0 + 1:i0 + B - 1].astype(np.float64)
+        ok = np.isfinite(fto) & np.isfinite(ftb)
+        rels.append((np.abs(ftb[ok] - fto[ok]) / np.maximum(np.abs(fto[ok]), 1e-300)).ravel())
+    err = np.concatenate(errs); rel = np.concatenate(rels)
+    print("config4 full: frac_ok %.5f (n=%d) median FTLE rel %.3e (n=%d) mean err %.3e max %.3e" %
+          (1 - mism / tot, tot, np.median(rel) if rel.size else 0.0, rel.size, err.mean(), err.max()))
+    assert 1 - mism / tot >= 0.999
+    assert rel.size > 1000 and np.median(rel) <= 1e-3
+
+
+@pytest.mark.slow
+def test_config5_full_size_one_volume_streamed(lcs, oracle):
+    """Config 5 at full size for one of its 16 volumes (192^3 seeds, backward 500 steps, ring of 4 slots fed from pinned
+    host memory, pre-blended integrator): the oracle integrates 6 seeded 14^3 blocks; statistical gate."""
+    import torch
+    w = I.config5()
+    f = lcs.Field.from_workload(w, max_resident_snapshots=4, pinned=True)
+    t_rel, t_end = w.meta["windows"][7]
+    sd = torch.from_numpy(w.seeds()).cuda()
+    F, flag, es = f.advect(sd, t_rel, t_end, w.h)
+    cgg, ftg, stg = gpu_cg(w, F, flag, T=t_end - t_rel)
+    torch.cuda.synchronize()
+    assert int(flag.max()) == 0 and f.info("ring") == 1 and f.info("h2d_bytes") > 0
+    n = w.ng[0]
+    Fh = cpu(F).reshape(n, n, n, 3); fth = cpu(ftg).reshape(n, n, n); S = w.seeds().reshape(n, n, n, 3)
+    fo = oracle.OracleField.from_workload(w)
+    rng = np.random.default_rng(55)
+    B = 14
+    errs, rels = [], []
+    for b in range(6):
+        k0, j0, i0 = (int(v) for v in rng.integers(0, n - B, 3))
+        blk = np.ascontiguousarray(S[k0:k0 + B, j0:j0 + B, i0:i0 + B].reshape(-1, 3))
+        Fo, flo, _ = fo.advect(blk.astype(np.float64), t_rel, t_end, w.h)
+        Fg = Fh[k0:k0 + B, j0:j0 + B, i0:i0 + B].reshape(-1, 3)
+        errs.append(np.linalg.norm(Fg.astype(np.float64) - Fo, axis=1))
+        cgo, fto, sto = oracle.cg_ftle(3, (B, B, B), w.seed_spacing, (0, 0, 0), (0, 0, 0), Fo, flo, t_end - t_rel)
+        fto = fto.reshape(B, B, B)[1:-1, 1:-1, 1:-1]
+        ftb = fth[k0 + 1:k0 + B - 1, j0 + 1:j0 + B - 1, i0 + 1:i0 + B - 1].astype(np.float64)
+        rels.append((np.abs(ftb - fto) / np.maximum(np.abs(fto), 1e-300)).ravel())
+    err, rel = np.concatenate(errs), np.concatenate(rels)
+    frac = np.mean(err <= 1e-3 * w.L)
+    print("config5 full (volume 7): frac_ok %.5f median FTLE rel %.3e mean err %.3e max %.3e" % (frac, np.median(rel), err.mean(), err.max()))
+    assert frac >= 0.999 and np.median(rel) <= 1e-3
