@@ -522,6 +522,82 @@ void orc_cg_ftle(int32_t dim, const int32_t *ng, const double *dx, const int32_t
     }
 }
 
+/* ---- O8 (row f2): full eigen-decomposition of the Cauchy-Green tensor ---------------------------------------
+ * The Cauchy-Green filter attaches "eigenvalues and eigenvectors" of C to the seed points; the
+ * eigenvectors are what hyperbolic-LCS criteria (strainlines) need.  The paper gives no algorithm.
+ * Reading (#27): classical cyclic Jacobi on the symmetric d x d matrix in fp64 (the closed forms are
+ * ill-conditioned for the small eigenvalues): sweep the pairs (0,1), (0,2), (1,2), rotate away each off-diagonal
+ * entry with the stable tangent formula t = sgn(theta) / (|theta| + sqrt(theta^2 + 1)), theta = (a_qq - a_pp) / (2 a_pq);
+ * stop when every off-diagonal entry is exactly zero or after 50 sweeps.  Eigenvalues ascending; row i of evec is
+ * the unit eigenvector of eval[i], sign fixed so that its component of largest magnitude (first on ties) is positive.
+ * Any non-finite input gives NaN everywhere.  cg: [n][3] (C11,C12,C22) or [n][6] (C11,C12,C13,C22,C23,C33).           */
+static void jacobi_sym(int d, double a[3][3], double v[3][3])
+{
+    for (int i = 0; i < d; ++i)
+        for (int j = 0; j < d; ++j) v[i][j] = (i == j) ? 1.0 : 0.0;
+    for (int sweep = 0; sweep < 50; ++sweep) {
+        double off = 0.0;
+        for (int p = 0; p < d; ++p)
+            for (int q = p + 1; q < d; ++q) off += fabs(a[p][q]);
+        if (off == 0.0) break;
+        for (int p = 0; p < d; ++p)
+            for (int q = p + 1; q < d; ++q) {
+                double apq = a[p][q];
+                if (apq == 0.0) continue;
+                double theta = (a[q][q] - a[p][p]) / (2.0 * apq);
+                double t = (theta >= 0.0 ? 1.0 : -1.0) / (fabs(theta) + sqrt(theta * theta + 1.0));
+                if (!isfinite(theta)) t = 0.0;          /* a_pq negligible against the diagonal gap */
+                double c = 1.0 / sqrt(t * t + 1.0), s = t * c;
+                a[p][p] -= t * apq;
+                a[q][q] += t * apq;
+                a[p][q] = a[q][p] = 0.0;
+                for (int r = 0; r < d; ++r) {
+                    if (r != p && r != q) {
+                        double arp = a[r][p], arq = a[r][q];
+                        a[r][p] = a[p][r] = c * arp - s * arq;
+                        a[r][q] = a[q][r] = s * arp + c * arq;
+                    }
+                    double vrp = v[r][p], vrq = v[r][q];   /* columns of v are the eigenvectors */
+                    v[r][p] = c * vrp - s * vrq;
+                    v[r][q] = s * vrp + c * vrq;
+                }
+            }
+    }
+}
+
+void orc_cg_eigen(int32_t dim, int64_t n, const double *cg, double *evals, double *evecs)
+{
+    const int d = dim, ncg = dim == 2 ? 3 : 6;
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n; ++i) {
+        const double *c = cg + i * ncg;
+        double *ev = evals + i * d, *vv = evecs + i * d * d;
+        int finite = 1;
+        for (int k = 0; k < ncg; ++k) finite = finite && isfinite(c[k]);
+        if (!finite) {
+            for (int k = 0; k < d; ++k) ev[k] = NAN;
+            for (int k = 0; k < d * d; ++k) vv[k] = NAN;
+            continue;
+        }
+        double a[3][3], v[3][3];
+        if (d == 2) { a[0][0] = c[0]; a[0][1] = a[1][0] = c[1]; a[1][1] = c[2]; }
+        else { a[0][0] = c[0]; a[0][1] = a[1][0] = c[1]; a[0][2] = a[2][0] = c[2]; a[1][1] = c[3]; a[1][2] = a[2][1] = c[4]; a[2][2] = c[5]; }
+        jacobi_sym(d, a, v);
+        int order[3] = {0, 1, 2};
+        for (int x = 0; x < d; ++x)                      /* ascending, stable */
+            for (int y = x + 1; y < d; ++y)
+                if (a[order[y]][order[y]] < a[order[x]][order[x]]) { int t = order[x]; order[x] = order[y]; order[y] = t; }
+        for (int k = 0; k < d; ++k) {
+            int col = order[k], big = 0;
+            ev[k] = a[col][col];
+            for (int r = 1; r < d; ++r)
+                if (fabs(v[r][col]) > fabs(v[big][col])) big = r;
+            double sg = v[big][col] < 0.0 ? -1.0 : 1.0;
+            for (int r = 0; r < d; ++r) vv[k * d + r] = sg * v[r][col];
+        }
+    }
+}
+
 int orc_max_threads(void)
 {
 #ifdef _OPENMP

@@ -201,6 +201,17 @@ def cg_ftle(dim, ng, seed_spacing, seed_periodic, period, flowmap, exit_flag, T)
     return cg, ftle, status
 
 
+def cg_eigen(dim, cg):
+    """All eigenvalues (ascending) and unit eigenvectors (row i belongs to eigenvalue i) of C: rule O8."""
+    c = np.ascontiguousarray(cg, dtype=np.float64)
+    n = c.shape[0]
+    assert c.shape[1] == (3 if dim == 2 else 6)
+    evals = np.empty((n, dim), dtype=np.float64)
+    evecs = np.empty((n, dim, dim), dtype=np.float64)
+    lib().orc_cg_eigen(C.c_int32(dim), C.c_int64(n), _p(c), _p(evals), _p(evecs))
+    return evals, evecs
+
+
 def eigmax_sym2(c11, c12, c22):
     return lib().orc_eigmax_sym2(c11, c12, c22)
 

@@ -558,3 +558,70 @@ def test_trajectory_recording(oracle):
     f = oracle.OracleField.from_workload(w)
     F, flag, es, traj = f.advect(w.seeds(), 0.0, 2.0, 0.1, rec_every=5)
     assert traj.shape == (4, 32, 2) and np.array_equal(traj[-1], F)
+
+
+# -------------------------------------------------------------------------------------------------
+# O8 (row f2): full eigen-decomposition of C
+def _sym_from_upper(dim, c):
+    if dim == 2:
+        return np.array([[c[0], c[1]], [c[1], c[2]]])
+    return np.array([[c[0], c[1], c[2]], [c[1], c[3], c[4]], [c[2], c[4], c[5]]])
+
+
+def _random_spd(rng, dim, n, max_cond_log10):
+    """Q diag(lambda) Q^T with log-uniform condition numbers up to 10^max_cond_log10, as upper triangles."""
+    out = np.empty((n, 3 if dim == 2 else 6))
+    for i in range(n):
+        q, _ = np.linalg.qr(rng.standard_normal((dim, dim)))
+        lam = 10.0 ** rng.uniform(-max_cond_log10 / 2, max_cond_log10 / 2, dim)
+        a = (q * lam) @ q.T
+        a = 0.5 * (a + a.T)
+        out[i] = a[np.triu_indices(dim)]
+    return out
+
+
+@pytest.mark.parametrize("dim", [2, 3])
+def test_P15_eigen_decomposition_vs_lapack(oracle, dim):
+    """Pin for O8: eigenvalues against LAPACK (numpy.linalg.eigh) to 1e-13 of lambda_max on SPD matrices with condition
+    numbers up to 1e12; residual |C v - lambda v| <= 1e-13 |C|; V orthonormal; eigenvectors equal LAPACK's up to sign
+    where the spectrum is well separated; sign convention (largest component positive); ascending order."""
+    rng = np.random.default_rng(150 + dim)
+    cg = _random_spd(rng, dim, 2000, 12)
+    ev, vec = oracle.cg_eigen(dim, cg)
+    assert np.all(np.diff(ev, axis=1) >= 0)
+    for i in range(cg.shape[0]):
+        a = _sym_from_upper(dim, cg[i])
+        wl, vl = np.linalg.eigh(a)
+        scale = np.abs(wl).max()
+        assert np.max(np.abs(ev[i] - wl)) <= 1e-13 * scale
+        assert np.max(np.abs(vec[i] @ vec[i].T - np.eye(dim))) <= 1e-13
+        for k in range(dim):
+            assert np.linalg.norm(a @ vec[i, k] - ev[i, k] * vec[i, k]) <= 1e-13 * scale
+            j = int(np.argmax(np.abs(vec[i, k])))
+            assert vec[i, k, j] > 0
+            gap = min(abs(wl[k] - wl[m]) for m in range(dim) if m != k)
+            if gap > 1e-3 * scale:
+                assert abs(abs(vec[i, k] @ vl[:, k]) - 1.0) <= 1e-9
+
+
+def test_P15_eigen_closed_forms(oracle):
+    """Closed forms: simple shear (pin P5) C = [[1, k], [k, 1 + k^2]] has lambda = 1 + k^2/2 +- k sqrt(1 + k^2/4), product 1,
+    and eigenvector (k, lambda - 1) / norm; diagonal matrices return the sorted diagonal and unit axes; a matrix with NaN
+    returns NaN; the largest eigenvalue equals the closed form of rule O7."""
+    k = 5.0
+    ev, vec = oracle.cg_eigen(2, np.array([[1.0, k, 1.0 + k * k]]))
+    lp = 1 + k * k / 2 + k * np.sqrt(1 + k * k / 4)
+    assert abs(ev[0, 1] - lp) <= 1e-13 * lp and abs(ev[0, 0] * ev[0, 1] - 1.0) <= 1e-12
+    assert abs(ev[0, 1] - 26.96291201783626) <= 1e-12                       # tests/golden pin P5, gamma T = 5
+    v = np.array([k, lp - 1.0]); v /= np.linalg.norm(v)
+    assert np.max(np.abs(vec[0, 1] - v)) <= 1e-14
+    ev, vec = oracle.cg_eigen(3, np.array([[3.0, 0.0, 0.0, 1.0, 0.0, 2.0]]))
+    assert np.array_equal(ev[0], [1.0, 2.0, 3.0])
+    assert np.array_equal(vec[0], [[0, 1, 0], [0, 0, 1], [1, 0, 0]])
+    ev, vec = oracle.cg_eigen(3, np.array([[1.0, np.nan, 0.0, 1.0, 0.0, 1.0]]))
+    assert np.all(np.isnan(ev)) and np.all(np.isnan(vec))
+    rng = np.random.default_rng(7)
+    cg = _random_spd(rng, 3, 200, 8)
+    ev, _ = oracle.cg_eigen(3, cg)
+    for i in range(200):
+        assert abs(ev[i, 2] - oracle.eigmax_sym3(*cg[i])) <= 1e-12 * ev[i, 2]
