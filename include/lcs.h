@@ -132,6 +132,14 @@ lcs_status lcs_cg_ftle(int32_t dim, int32_t dtype, const int32_t ng[3], const do
                        const void *flowmap, const uint8_t *exit_flag, double T,
                        void *cg, void *ftle, uint8_t *status, void *cuda_stream);
 
+/* All eigenvalues and eigenvectors of the Cauchy-Green tensor (the Cauchy-Green filter attaches
+ * "eigenvalues and eigenvectors"; hyperbolic-LCS criteria use the eigenvector fields).  Cyclic Jacobi
+ * in fp64 per seed (reading #27).  cg: device [n][3] or [n][6] of `dtype` as written by lcs_cg_ftle.
+ * evals: device [n][dim], ascending.  evecs: device [n][dim][dim], row i = unit eigenvector of evals[i], its component
+ * of largest magnitude positive.  A seed whose C holds a non-finite value gets NaN in both outputs.                */
+lcs_status lcs_cg_eigen(int32_t dim, int32_t dtype, int64_t n, const void *cg, void *evals, void *evecs,
+                        void *cuda_stream);
+
 /* End-to-end convenience with HOST buffers: copies the seeds to the device, runs lcs_advect and
  * lcs_cg_ftle and copies flow map (optional), flags (optional) and FTLE back; synchronous.
  * seeds_host/flowmap_host: [n][dim] of the field's compute_dtype; ftle_host: [n] of compute_dtype.

@@ -112,6 +112,97 @@ __global__ void __launch_bounds__(256) cg_ftle_kernel(const __grid_constant__ Cg
     if (status) status[idx] = st;
 }
 
+// ---------------------------------------------------------------------------------------------
+// Row f2: all eigenvalues and eigenvectors of C ("eigenvalues and eigenvectors"; the
+// eigenvector fields are what hyperbolic-LCS criteria need).  One thread per seed, cyclic Jacobi in fp64 registers
+// (reading #27): the closed forms are ill-conditioned for the small eigenvalues.  Streams 12-24 B in and
+// 24-48 B out per seed (fp32); the arithmetic is FP64-pipe bound.
+template <int D> __device__ __forceinline__ void jacobi_rotate(double (&a)[D][D], double (&v)[D][D], int p, int q)
+{
+    const double apq = a[p][q];
+    if (apq == 0.0) return;
+    const double theta = (a[q][q] - a[p][p]) / (2.0 * apq);
+    double t = copysign(1.0, theta) / (fabs(theta) + sqrt(fma(theta, theta, 1.0)));
+    if (!isfinite(theta)) t = 0.0;
+    const double c = rsqrt(fma(t, t, 1.0)), s = t * c;
+    a[p][p] -= t * apq;
+    a[q][q] += t * apq;
+    a[p][q] = a[q][p] = 0.0;
+#pragma unroll
+    for (int r = 0; r < D; ++r) {
+        if (r != p && r != q) {
+            const double arp = a[r][p], arq = a[r][q];
+            a[r][p] = a[p][r] = c * arp - s * arq;
+            a[r][q] = a[q][r] = s * arp + c * arq;
+        }
+        const double vrp = v[r][p], vrq = v[r][q];
+        v[r][p] = c * vrp - s * vrq;
+        v[r][q] = s * vrp + c * vrq;
+    }
+}
+
+template <int D, typename T>
+__global__ void __launch_bounds__(128) cg_eigen_kernel(const T *__restrict__ cg, T *__restrict__ evals, T *__restrict__ evecs, int64_t n)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    constexpr int NCG = D == 2 ? 3 : 6;
+    double c[NCG];
+    bool finite = true;
+#pragma unroll
+    for (int k = 0; k < NCG; ++k) { c[k] = (double)cg[i * NCG + k]; finite = finite && isfinite(c[k]); }
+    if (!finite) {
+        const T q = (T)nan("");
+#pragma unroll
+        for (int k = 0; k < D; ++k) evals[i * D + k] = q;
+#pragma unroll
+        for (int k = 0; k < D * D; ++k) evecs[i * D * D + k] = q;
+        return;
+    }
+    double a[D][D], v[D][D];
+    if constexpr (D == 2) { a[0][0] = c[0]; a[0][1] = a[1][0] = c[1]; a[1][1] = c[2]; }
+    else { a[0][0] = c[0]; a[0][1] = a[1][0] = c[1]; a[0][2] = a[2][0] = c[2]; a[1][1] = c[3]; a[1][2] = a[2][1] = c[4]; a[2][2] = c[5]; }
+#pragma unroll
+    for (int r = 0; r < D; ++r)
+#pragma unroll
+        for (int k = 0; k < D; ++k) v[r][k] = r == k ? 1.0 : 0.0;
+    for (int sweep = 0; sweep < 50; ++sweep) {
+        double off = fabs(a[0][1]);
+        if constexpr (D == 3) off += fabs(a[0][2]) + fabs(a[1][2]);
+        if (off == 0.0) break;
+        jacobi_rotate<D>(a, v, 0, 1);
+        if constexpr (D == 3) { jacobi_rotate<D>(a, v, 0, 2); jacobi_rotate<D>(a, v, 1, 2); }
+    }
+    // ascending order by a 2- or 3-element sorting network on (eigenvalue, column)
+    double ev[D], col[D][D];
+#pragma unroll
+    for (int k = 0; k < D; ++k) {
+        ev[k] = a[k][k];
+#pragma unroll
+        for (int r = 0; r < D; ++r) col[k][r] = v[r][k];
+    }
+    auto cswap = [&](int x, int y) {
+        if (ev[y] < ev[x]) {
+            double t = ev[x]; ev[x] = ev[y]; ev[y] = t;
+#pragma unroll
+            for (int r = 0; r < D; ++r) { double u = col[x][r]; col[x][r] = col[y][r]; col[y][r] = u; }
+        }
+    };
+    cswap(0, 1);
+    if constexpr (D == 3) { cswap(1, 2); cswap(0, 1); }
+#pragma unroll
+    for (int k = 0; k < D; ++k) {
+        double big = col[k][0];
+#pragma unroll
+        for (int r = 1; r < D; ++r)
+            if (fabs(col[k][r]) > fabs(big)) big = col[k][r];
+        const double sg = big < 0.0 ? -1.0 : 1.0;
+        evals[i * D + k] = (T)ev[k];
+#pragma unroll
+        for (int r = 0; r < D; ++r) evecs[(i * D + k) * D + r] = (T)(sg * col[k][r]);
+    }
+}
+
 }  // namespace
 
 extern "C" lcs_status lcs_cg_ftle(int32_t dim, int32_t dtype, const int32_t ng[3], const double seed_spacing[3],
@@ -139,6 +230,21 @@ extern "C" lcs_status lcs_cg_ftle(int32_t dim, int32_t dtype, const int32_t ng[3
     else if (dim == 2) LCS_LAUNCH((cg_ftle_kernel<2, float>), grid, 256, 0, st, g, (const float *)flowmap, exit_flag, (float *)cg, (float *)ftle, status, n);
     else if (dtype == LCS_F64) LCS_LAUNCH((cg_ftle_kernel<3, double>), grid, 256, 0, st, g, (const double *)flowmap, exit_flag, (double *)cg, (double *)ftle, status, n);
     else LCS_LAUNCH((cg_ftle_kernel<3, float>), grid, 256, 0, st, g, (const float *)flowmap, exit_flag, (float *)cg, (float *)ftle, status, n);
+    LCS_CUDA_OK(cudaGetLastError());
+    return LCS_OK;
+}
+
+extern "C" lcs_status lcs_cg_eigen(int32_t dim, int32_t dtype, int64_t n, const void *cg, void *evals, void *evecs, void *cuda_stream)
+{
+    if ((dim != 2 && dim != 3) || n < 0 || (n > 0 && (!cg || !evals || !evecs))) { lcs_set_error("null argument or bad dim"); return LCS_ERR_INVALID_ARG; }
+    if (dtype != LCS_F32 && dtype != LCS_F64) { lcs_set_error("bad dtype"); return LCS_ERR_INVALID_ARG; }
+    if (n == 0) return LCS_OK;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const unsigned grid = lcs_blocks(n, 128);
+    if (dim == 2 && dtype == LCS_F64) LCS_LAUNCH((cg_eigen_kernel<2, double>), grid, 128, 0, st, (const double *)cg, (double *)evals, (double *)evecs, n);
+    else if (dim == 2) LCS_LAUNCH((cg_eigen_kernel<2, float>), grid, 128, 0, st, (const float *)cg, (float *)evals, (float *)evecs, n);
+    else if (dtype == LCS_F64) LCS_LAUNCH((cg_eigen_kernel<3, double>), grid, 128, 0, st, (const double *)cg, (double *)evals, (double *)evecs, n);
+    else LCS_LAUNCH((cg_eigen_kernel<3, float>), grid, 128, 0, st, (const float *)cg, (float *)evals, (float *)evecs, n);
     LCS_CUDA_OK(cudaGetLastError());
     return LCS_OK;
 }

@@ -22,7 +22,7 @@ LCS_F32, LCS_F64 = 0, 1
 LCS_MESH_CARTESIAN, LCS_MESH_SIMPLEX = 0, 1
 
 EXPORTS = ["lcs_field_create", "lcs_field_set_snapshot", "lcs_field_sync", "lcs_field_destroy",
-           "lcs_field_set_option", "lcs_field_get_info", "lcs_locate", "lcs_advect", "lcs_cg_ftle",
+           "lcs_field_set_option", "lcs_field_get_info", "lcs_locate", "lcs_advect", "lcs_cg_ftle", "lcs_cg_eigen",
            "lcs_ftle_host", "lcs_kernel_launch_count", "lcs_last_error"]
 
 
@@ -68,6 +68,7 @@ def lib():
                                  C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.lcs_cg_ftle.argtypes = [C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                   C.c_void_p, C.c_void_p, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.lcs_cg_eigen.argtypes = [C.c_int32, C.c_int32, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.lcs_ftle_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                     C.c_double, C.c_double, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p]
         _lib = L
@@ -242,3 +243,16 @@ def cg_ftle(dim, ng, seed_spacing, seed_periodic, period, flowmap, exit_flag, T,
                              _tptr(flowmap), _tptr(exit_flag), float(T), _tptr(cg), _tptr(ftle), _tptr(status),
                              _stream_ptr(stream)))
     return cg, ftle, status
+
+
+def cg_eigen(dim, cg, stream=None):
+    """cg: torch CUDA [n][3|6] as returned by cg_ftle.  Returns (evals [n][dim] ascending, evecs [n][dim][dim], row i = unit
+    eigenvector of evals[i])."""
+    import torch
+    assert cg.is_cuda and cg.is_contiguous() and cg.shape[1] == (3 if dim == 2 else 6)
+    n = cg.shape[0]
+    dtype = LCS_F64 if cg.dtype == torch.float64 else LCS_F32
+    evals = torch.empty((n, dim), dtype=cg.dtype, device=cg.device)
+    evecs = torch.empty((n, dim, dim), dtype=cg.dtype, device=cg.device)
+    _check(lib().lcs_cg_eigen(int(dim), dtype, n, _tptr(cg), _tptr(evals), _tptr(evecs), _stream_ptr(stream)))
+    return evals, evecs

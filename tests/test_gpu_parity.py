@@ -539,3 +539,53 @@ def test_config5_full_size_one_volume_streamed(lcs, oracle):
     frac = np.mean(err <= 1e-3 * w.L)
     print("config5 full (volume 7): frac_ok %.5f median FTLE rel %.3e mean err %.3e max %.3e" % (frac, np.median(rel), err.mean(), err.max()))
     assert frac >= 0.999 and np.median(rel) <= 1e-3
+
+
+# -------------------------------------------------------------------------------------------------
+# row f2: full eigen-decomposition of C
+@pytest.mark.parametrize("dim", [2, 3])
+@pytest.mark.parametrize("dt", [np.float64, np.float32])
+def test_cg_eigen_vs_oracle(lcs, oracle, dim, dt):
+    """lcs_cg_eigen against oracle rule O8 on (i) C of a real flow map (config 1 / config 3 reduced, NaN rows included) and
+    (ii) random SPD matrices with condition numbers up to 1e10 (fp64) / 1e4 (fp32).  Eigenvalues within 1e-12 (fp64) or 2e-6
+    (fp32) of lambda_max; eigenvectors: residual |C v - lambda v| small, and equal to the oracle's up to rounding where the
+    eigenvalue is separated from the others (elsewhere any orthonormal basis of the eigenspace is correct)."""
+    import torch
+    rng = np.random.default_rng(160 + dim)
+    w = I.config1(ng=(64, 32), T=5.0) if dim == 2 else I.config3(ngrid=20, nn=16, T=1.0, n_snap=4)
+    f, sd, F, flag, es = gpu_run(w)
+    flag = flag.clone(); flag[::97] = 1                                     # some undefined seeds -> NaN rows
+    cgg, _, _ = gpu_cg(w, F, flag)
+    lc = 10 if dt == np.float64 else 4
+    from test_oracle_pins import _random_spd, _sym_from_upper
+    mats = np.concatenate([cpu(cgg).astype(np.float64), _random_spd(rng, dim, 4000, lc)]).astype(dt)
+    ev_g, vec_g = lcs.cg_eigen(dim, torch.from_numpy(mats).cuda())
+    torch.cuda.synchronize()
+    ev_g, vec_g = cpu(ev_g).astype(np.float64), cpu(vec_g).astype(np.float64)
+    ev_o, vec_o = oracle.cg_eigen(dim, mats.astype(np.float64))
+    nanrow = np.isnan(ev_o[:, 0])
+    assert nanrow.sum() > 5 and np.array_equal(np.isnan(ev_g[:, 0]), nanrow) and np.all(np.isnan(vec_g[nanrow]))
+    ok = ~nanrow
+    scale = np.abs(ev_o[ok]).max(axis=1, keepdims=True)
+    tol = 1e-12 if dt == np.float64 else 2e-6
+    assert np.max(np.abs(ev_g[ok] - ev_o[ok]) / scale) <= tol
+    checked = 0
+    for i in np.nonzero(ok)[0][::7]:
+        a = _sym_from_upper(dim, mats[i].astype(np.float64))
+        s = np.abs(ev_o[i]).max()
+        for k in range(dim):
+            assert np.linalg.norm(a @ vec_g[i, k] - ev_g[i, k] * vec_g[i, k]) <= 10 * tol * s
+            gap = min(abs(ev_o[i, k] - ev_o[i, m]) for m in range(dim) if m != k)
+            if gap > 1e-2 * s:
+                assert np.max(np.abs(vec_g[i, k] - vec_o[i, k])) <= (1e-9 if dt == np.float64 else 2e-4)
+                checked += 1
+    assert checked > 500
+
+
+def test_cg_eigen_arguments(lcs):
+    import torch
+    z = torch.zeros((0, 6), device="cuda")
+    ev, vec = lcs.cg_eigen(3, z)
+    assert ev.shape == (0, 3) and vec.shape == (0, 3, 3)
+    with pytest.raises(lcs.LcsError):
+        lcs._check(lcs.lib().lcs_cg_eigen(4, 0, 1, 1, 1, 1, None))
