@@ -598,6 +598,52 @@ void orc_cg_eigen(int32_t dim, int64_t n, const double *cg, double *evals, doubl
     }
 }
 
+/* ---- O9 (row f3): Cauchy-Green tensor from auxiliary points -------------------------------------------------
+ * "a structured grid of auxiliary points can be placed around each seed point" and the Cauchy-Green
+ * filter can use them "for the computation of the flow map gradient" instead of the neighbouring seeds.
+ * Reading (#28): 2 d auxiliary tracers per seed, released at x0 + delta_b e_b and x0 - delta_b e_b;
+ * Faux[i][2 b][.] / Faux[i][2 b + 1][.] are their final positions; G_ab = (F_a(+b) - F_a(-b)) / (2 delta_b), always
+ * central; if any of the 2 d auxiliary tracers of a seed has a non-zero exit flag: C, FTLE = NaN, status bit 0.
+ * C, lambda_max and FTLE then follow O6-O7.                                                                    */
+void orc_cg_ftle_aux(int32_t dim, int64_t n, const double *delta, const double *Faux, const uint8_t *flag_aux, double T,
+                     double *cg, double *ftle, uint8_t *status)
+{
+    const int d = dim, ncg = dim == 2 ? 3 : 6;
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n; ++i) {
+        double G[3][3], C[6], lam;
+        uint8_t st = 0;
+        for (int k = 0; k < 2 * d; ++k)
+            if (flag_aux && flag_aux[i * 2 * d + k] != 0) st = 1;
+        for (int b = 0; b < d; ++b)
+            for (int a = 0; a < d; ++a) {
+                double Fp = Faux[(i * 2 * d + 2 * b) * d + a], Fm = Faux[(i * 2 * d + 2 * b + 1) * d + a];
+                G[a][b] = (Fp - Fm) / (2.0 * delta[b]);
+            }
+        if (st) {
+            for (int k = 0; k < ncg; ++k) C[k] = NAN;
+            lam = NAN;
+        } else if (d == 2) {
+            C[0] = G[0][0] * G[0][0] + G[1][0] * G[1][0];
+            C[1] = G[0][0] * G[0][1] + G[1][0] * G[1][1];
+            C[2] = G[0][1] * G[0][1] + G[1][1] * G[1][1];
+            lam = orc_eigmax_sym2(C[0], C[1], C[2]);
+        } else {
+            int m = 0;
+            for (int b = 0; b < 3; ++b)
+                for (int c = b; c < 3; ++c) {
+                    double s = 0.0;
+                    for (int a = 0; a < 3; ++a) s = s + G[a][b] * G[a][c];
+                    C[m++] = s;
+                }
+            lam = orc_eigmax_sym3(C[0], C[1], C[2], C[3], C[4], C[5]);
+        }
+        if (cg) for (int k = 0; k < ncg; ++k) cg[i * ncg + k] = C[k];
+        ftle[i] = st ? NAN : log(lam) / (2.0 * fabs(T));
+        if (status) status[i] = st;
+    }
+}
+
 int orc_max_threads(void)
 {
 #ifdef _OPENMP

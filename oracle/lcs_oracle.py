@@ -201,6 +201,20 @@ def cg_ftle(dim, ng, seed_spacing, seed_periodic, period, flowmap, exit_flag, T)
     return cg, ftle, status
 
 
+def cg_ftle_aux(dim, delta, flow_aux, flag_aux, T):
+    """Rule O9.  flow_aux [n][2 dim][dim] (entry 2b: released at +delta_b, 2b+1: at -delta_b), flag_aux [n][2 dim] or None.
+    Returns (cg, ftle, status)."""
+    Fa = np.ascontiguousarray(flow_aux, dtype=np.float64).reshape(-1, 2 * dim, dim)
+    n = Fa.shape[0]
+    dl = np.ascontiguousarray(delta, dtype=np.float64)
+    fl = None if flag_aux is None else np.ascontiguousarray(flag_aux, dtype=np.uint8).reshape(n, 2 * dim)
+    cg = np.empty((n, 3 if dim == 2 else 6), dtype=np.float64)
+    ftle = np.empty(n, dtype=np.float64)
+    status = np.empty(n, dtype=np.uint8)
+    lib().orc_cg_ftle_aux(C.c_int32(dim), C.c_int64(n), _p(dl), _p(Fa), _p(fl), C.c_double(T), _p(cg), _p(ftle), _p(status))
+    return cg, ftle, status
+
+
 def cg_eigen(dim, cg):
     """All eigenvalues (ascending) and unit eigenvectors (row i belongs to eigenvalue i) of C: rule O8."""
     c = np.ascontiguousarray(cg, dtype=np.float64)

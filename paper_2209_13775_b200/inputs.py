@@ -353,3 +353,14 @@ def kuhn_mesh(dim: int, n: int, h: float = 1.0):
                 vs.append(vid(c))
             cells.append(vs)
     return np.ascontiguousarray(P), np.asarray(cells, dtype=np.int32)
+
+
+def aux_seeds(seeds: np.ndarray, delta: Sequence[float]) -> np.ndarray:
+    """Auxiliary points around each seed: [n][2 dim][dim], entry 2b = seed + delta_b e_b, 2b+1 = seed - delta_b e_b
+    (layout only; the difference quotient is formed by lcs_cg_ftle_aux / oracle rule O9)."""
+    n, dim = seeds.shape
+    out = np.repeat(seeds[:, None, :], 2 * dim, axis=1).astype(seeds.dtype)
+    for b in range(dim):
+        out[:, 2 * b, b] += seeds.dtype.type(delta[b])
+        out[:, 2 * b + 1, b] -= seeds.dtype.type(delta[b])
+    return out

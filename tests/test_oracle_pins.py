@@ -625,3 +625,51 @@ def test_P15_eigen_closed_forms(oracle):
     ev, _ = oracle.cg_eigen(3, cg)
     for i in range(200):
         assert abs(ev[i, 2] - oracle.eigmax_sym3(*cg[i])) <= 1e-12 * ev[i, 2]
+
+
+# -------------------------------------------------------------------------------------------------
+# O9 (row f3): gradient from auxiliary points
+def test_P16_aux_gradient_linear_flow_and_shear(oracle):
+    """Pin for O9: for u = A x the flow map is linear, so the auxiliary-point quotient is exact for ANY delta:
+    G = P(hA)^N, C = G^T G (pin P3); simple shear gives the closed-form FTLE of pin P5; a flagged auxiliary tracer gives
+    NaN + status 1; grid-neighbour (O5) and auxiliary (O9) gradients agree on a smooth flow to O(dx^2)."""
+    A = np.array([[0.1, 0.4], [-0.3, -0.1]])
+    h, N = 0.1, 50
+    w = I.analytic_cartesian(2, I.linear_flow(A), (41, 41), (-2.0, -2.0), (0.1, 0.1), (0.0, 5.0), ng=(6, 5), seed_lo=(-0.5, -0.5),
+                             seed_spacing=(0.2, 0.2), t0=0.0, tf=h * N, h=h)
+    fo = oracle.OracleField.from_workload(w)
+    delta = (1e-3, 2e-3)
+    aux = I.aux_seeds(w.seeds(), delta)
+    Fa, fla, _ = fo.advect(aux.reshape(-1, 2), w.t0, w.tf, w.h)
+    assert np.all(fla == 0)
+    cg, ftle, st = oracle.cg_ftle_aux(2, delta, Fa, fla, w.tf - w.t0)
+    hA = h * A
+    P = np.eye(2) + hA + hA @ hA / 2 + hA @ hA @ hA / 6 + hA @ hA @ hA @ hA / 24
+    G = np.linalg.matrix_power(P, N)
+    Cx = G.T @ G
+    assert np.max(np.abs(cg - np.array([Cx[0, 0], Cx[0, 1], Cx[1, 1]]))) <= 1e-9
+    assert np.all(st == 0)
+    lam = np.linalg.eigvalsh(Cx)[-1]
+    assert np.max(np.abs(ftle - np.log(lam) / (2 * h * N))) <= 1e-10
+    # shear: u = (gamma y, 0), gamma T = 5 -> FTLE of pin P5
+    w2 = I.analytic_cartesian(2, I.linear_flow(np.array([[0.0, 0.5], [0.0, 0.0]])), (41, 41), (-20.0, -2.0), (1.0, 0.1), (0.0, 10.0),
+                              ng=(4, 4), seed_lo=(-1.0, -1.0), seed_spacing=(0.5, 0.5), t0=0.0, tf=10.0, h=0.1)
+    fo2 = oracle.OracleField.from_workload(w2)
+    aux2 = I.aux_seeds(w2.seeds(), (0.01, 0.01))
+    F2, fl2, _ = fo2.advect(aux2.reshape(-1, 2), 0.0, 10.0, 0.1)
+    cg2, ft2, st2 = oracle.cg_ftle_aux(2, (0.01, 0.01), F2, fl2, 10.0)
+    assert np.max(np.abs(ft2 - 0.164723114637109571)) <= 1e-10           # tests/golden/closed_form_pins.txt, P5
+    fl2 = fl2.reshape(-1, 4).copy(); fl2[3, 2] = 1
+    cg3, ft3, st3 = oracle.cg_ftle_aux(2, (0.01, 0.01), F2, fl2, 10.0)
+    assert np.isnan(ft3[3]) and st3[3] == 1 and np.all(np.isnan(cg3[3])) and np.isfinite(ft3[2]) and st3[2] == 0
+    # against the grid-neighbour gradient on the double gyre (interior seeds): both approximate the same derivative
+    w3 = I.config1(ng=(64, 32), T=2.0)
+    fo3 = oracle.OracleField.from_workload(w3)
+    Fg, flg, _ = fo3.advect(w3.seeds(), w3.t0, w3.tf, w3.h)
+    _, ftg, _ = oracle.cg_ftle(2, w3.ng, w3.seed_spacing, w3.seed_periodic, w3.period, Fg, flg, w3.tf - w3.t0)
+    d3 = (w3.seed_spacing[0], w3.seed_spacing[1])
+    Fa3, fla3, _ = fo3.advect(I.aux_seeds(w3.seeds(), d3).reshape(-1, 2), w3.t0, w3.tf, w3.h)
+    _, fta, sta = oracle.cg_ftle_aux(2, d3, Fa3, fla3, w3.tf - w3.t0)
+    inner = np.zeros((32, 64), bool); inner[1:-1, 1:-1] = True
+    ok = inner.ravel() & (sta == 0)
+    assert ok.sum() > 1500 and np.max(np.abs(fta[ok] - ftg[ok])) <= 1e-12   # delta = seed spacing: the very same stencil
