@@ -132,6 +132,17 @@ lcs_status lcs_cg_ftle(int32_t dim, int32_t dtype, const int32_t ng[3], const do
                        const void *flowmap, const uint8_t *exit_flag, double T,
                        void *cg, void *ftle, uint8_t *status, void *cuda_stream);
 
+/* Cauchy-Green tensor and FTLE from AUXILIARY points instead of neighbouring seeds ("a structured grid
+ * of auxiliary points can be placed around each seed point"; the Cauchy-Green filter uses them "for the
+ * computation of the flow map gradient").  The caller advects, with lcs_advect, 2*dim auxiliary tracers per seed released
+ * at x0 + aux_delta[b] e_b (entry 2b) and x0 - aux_delta[b] e_b (entry 2b+1).
+ * flowmap_aux: device [n][2*dim][dim] of `dtype`; exit_flag_aux: device [n][2*dim] u8 or NULL.
+ * G_ab = (F_a(+b) - F_a(-b)) / (2 aux_delta[b]), always central; a seed with any flagged auxiliary tracer gets
+ * C, FTLE = NaN and status 1.  cg / ftle / status as in lcs_cg_ftle.  Errors: aux_delta[b] <= 0, T == 0.          */
+lcs_status lcs_cg_ftle_aux(int32_t dim, int32_t dtype, int64_t n, const double aux_delta[3], const void *flowmap_aux,
+                           const uint8_t *exit_flag_aux, double T, void *cg, void *ftle, uint8_t *status,
+                           void *cuda_stream);
+
 /* All eigenvalues and eigenvectors of the Cauchy-Green tensor (the Cauchy-Green filter attaches
  * "eigenvalues and eigenvectors"; hyperbolic-LCS criteria use the eigenvector fields).  Cyclic Jacobi
  * in fp64 per seed (reading #27).  cg: device [n][3] or [n][6] of `dtype` as written by lcs_cg_ftle.

@@ -113,6 +113,57 @@ __global__ void __launch_bounds__(256) cg_ftle_kernel(const __grid_constant__ Cg
 }
 
 // ---------------------------------------------------------------------------------------------
+// Row f3: gradient from auxiliary points ("auxiliary points can be placed around each seed point",
+// PAPER.md:67 "used for the computation of the flow map gradient").  Faux: [n][2 DIM][DIM], entry 2b / 2b+1 = final
+// position of the tracer released at x0 +/- delta_b e_b; always central; any flagged auxiliary tracer => NaN, status 1
+// (reading #28).  HBM streaming: 2 DIM^2 elements in per seed, read once, fully coalesced across the warp.
+template <int DIM, typename T>
+__global__ void __launch_bounds__(256) cg_ftle_aux_kernel(const T *__restrict__ Faux, const uint8_t *__restrict__ flag_aux,
+                                                           double i2d0, double i2d1, double i2d2, double inv_2T, T *__restrict__ cg,
+                                                           T *__restrict__ ftle, uint8_t *__restrict__ status, int64_t n)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    constexpr int NCG = (DIM == 2) ? 3 : 6;
+    const double i2d[3] = {i2d0, i2d1, i2d2};
+    uint8_t st = 0;
+    if (flag_aux) {
+#pragma unroll
+        for (int k = 0; k < 2 * DIM; ++k) st |= flag_aux[i * 2 * DIM + k] != 0 ? 1 : 0;
+    }
+    double G[DIM][DIM];
+    const T *f = Faux + i * (2 * DIM * DIM);
+#pragma unroll
+    for (int b = 0; b < DIM; ++b)
+#pragma unroll
+        for (int a = 0; a < DIM; ++a) G[a][b] = ((double)f[(2 * b) * DIM + a] - (double)f[(2 * b + 1) * DIM + a]) * i2d[b];
+    double C[NCG], lam;
+    if (st) {
+#pragma unroll
+        for (int k = 0; k < NCG; ++k) C[k] = nan("");
+        lam = nan("");
+    } else if constexpr (DIM == 2) {
+        C[0] = G[0][0] * G[0][0] + G[1][0] * G[1][0];
+        C[1] = G[0][0] * G[0][1] + G[1][0] * G[1][1];
+        C[2] = G[0][1] * G[0][1] + G[1][1] * G[1][1];
+        lam = eigmax_sym2(C[0], C[1], C[2]);
+    } else {
+        int m = 0;
+#pragma unroll
+        for (int b = 0; b < 3; ++b)
+#pragma unroll
+            for (int c = b; c < 3; ++c) C[m++] = G[0][b] * G[0][c] + G[1][b] * G[1][c] + G[2][b] * G[2][c];
+        lam = eigmax_sym3(C[0], C[1], C[2], C[3], C[4], C[5]);
+    }
+    if (cg) {
+#pragma unroll
+        for (int k = 0; k < NCG; ++k) cg[i * NCG + k] = (T)C[k];
+    }
+    ftle[i] = st ? (T)nan("") : (T)(log(lam) * inv_2T);
+    if (status) status[i] = st;
+}
+
+// ---------------------------------------------------------------------------------------------
 // Row f2: all eigenvalues and eigenvectors of C ("eigenvalues and eigenvectors"; the
 // eigenvector fields are what hyperbolic-LCS criteria need).  One thread per seed, cyclic Jacobi in fp64 registers
 // (reading #27): the closed forms are ill-conditioned for the small eigenvalues.  Streams 12-24 B in and
@@ -245,6 +296,29 @@ extern "C" lcs_status lcs_cg_eigen(int32_t dim, int32_t dtype, int64_t n, const 
     else if (dim == 2) LCS_LAUNCH((cg_eigen_kernel<2, float>), grid, 128, 0, st, (const float *)cg, (float *)evals, (float *)evecs, n);
     else if (dtype == LCS_F64) LCS_LAUNCH((cg_eigen_kernel<3, double>), grid, 128, 0, st, (const double *)cg, (double *)evals, (double *)evecs, n);
     else LCS_LAUNCH((cg_eigen_kernel<3, float>), grid, 128, 0, st, (const float *)cg, (float *)evals, (float *)evecs, n);
+    LCS_CUDA_OK(cudaGetLastError());
+    return LCS_OK;
+}
+
+extern "C" lcs_status lcs_cg_ftle_aux(int32_t dim, int32_t dtype, int64_t n, const double aux_delta[3], const void *flowmap_aux,
+                                      const uint8_t *exit_flag_aux, double T, void *cg, void *ftle, uint8_t *status, void *cuda_stream)
+{
+    if ((dim != 2 && dim != 3) || n < 0 || !aux_delta || (n > 0 && (!flowmap_aux || !ftle))) { lcs_set_error("null argument or bad dim"); return LCS_ERR_INVALID_ARG; }
+    if (dtype != LCS_F32 && dtype != LCS_F64) { lcs_set_error("bad dtype"); return LCS_ERR_INVALID_ARG; }
+    if (!(T != 0.0) || !isfinite(T)) { lcs_set_error("T must be finite and non-zero"); return LCS_ERR_INVALID_ARG; }
+    double i2d[3] = {1.0, 1.0, 1.0};
+    for (int a = 0; a < dim; ++a) {
+        if (!(aux_delta[a] > 0.0) || !isfinite(aux_delta[a])) { lcs_set_error("aux_delta[%d] must be positive", a); return LCS_ERR_INVALID_ARG; }
+        i2d[a] = 1.0 / (2.0 * aux_delta[a]);
+    }
+    if (n == 0) return LCS_OK;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const unsigned grid = lcs_blocks(n, 256);
+    const double inv_2T = 1.0 / (2.0 * fabs(T));
+    if (dim == 2 && dtype == LCS_F64) LCS_LAUNCH((cg_ftle_aux_kernel<2, double>), grid, 256, 0, st, (const double *)flowmap_aux, exit_flag_aux, i2d[0], i2d[1], i2d[2], inv_2T, (double *)cg, (double *)ftle, status, n);
+    else if (dim == 2) LCS_LAUNCH((cg_ftle_aux_kernel<2, float>), grid, 256, 0, st, (const float *)flowmap_aux, exit_flag_aux, i2d[0], i2d[1], i2d[2], inv_2T, (float *)cg, (float *)ftle, status, n);
+    else if (dtype == LCS_F64) LCS_LAUNCH((cg_ftle_aux_kernel<3, double>), grid, 256, 0, st, (const double *)flowmap_aux, exit_flag_aux, i2d[0], i2d[1], i2d[2], inv_2T, (double *)cg, (double *)ftle, status, n);
+    else LCS_LAUNCH((cg_ftle_aux_kernel<3, float>), grid, 256, 0, st, (const float *)flowmap_aux, exit_flag_aux, i2d[0], i2d[1], i2d[2], inv_2T, (float *)cg, (float *)ftle, status, n);
     LCS_CUDA_OK(cudaGetLastError());
     return LCS_OK;
 }

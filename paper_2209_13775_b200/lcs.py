@@ -22,7 +22,7 @@ LCS_F32, LCS_F64 = 0, 1
 LCS_MESH_CARTESIAN, LCS_MESH_SIMPLEX = 0, 1
 
 EXPORTS = ["lcs_field_create", "lcs_field_set_snapshot", "lcs_field_sync", "lcs_field_destroy",
-           "lcs_field_set_option", "lcs_field_get_info", "lcs_locate", "lcs_advect", "lcs_cg_ftle", "lcs_cg_eigen",
+           "lcs_field_set_option", "lcs_field_get_info", "lcs_locate", "lcs_advect", "lcs_cg_ftle", "lcs_cg_ftle_aux", "lcs_cg_eigen",
            "lcs_ftle_host", "lcs_kernel_launch_count", "lcs_last_error"]
 
 
@@ -68,6 +68,8 @@ def lib():
                                  C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.lcs_cg_ftle.argtypes = [C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                   C.c_void_p, C.c_void_p, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.lcs_cg_ftle_aux.argtypes = [C.c_int32, C.c_int32, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double,
+                                      C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.lcs_cg_eigen.argtypes = [C.c_int32, C.c_int32, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.lcs_ftle_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                     C.c_double, C.c_double, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p]
@@ -256,3 +258,18 @@ def cg_eigen(dim, cg, stream=None):
     evecs = torch.empty((n, dim, dim), dtype=cg.dtype, device=cg.device)
     _check(lib().lcs_cg_eigen(int(dim), dtype, n, _tptr(cg), _tptr(evals), _tptr(evecs), _stream_ptr(stream)))
     return evals, evecs
+
+
+def cg_ftle_aux(dim, aux_delta, flow_aux, flag_aux, T, want_cg=True, want_status=True, stream=None):
+    """flow_aux: torch CUDA [n][2 dim][dim] (final positions of the auxiliary tracers, see lcs.h); flag_aux [n][2 dim] u8 or
+    None.  Returns (cg or None, ftle, status or None)."""
+    import torch
+    assert flow_aux.is_cuda and flow_aux.is_contiguous()
+    n = flow_aux.numel() // (2 * dim * dim)
+    dtype = LCS_F64 if flow_aux.dtype == torch.float64 else LCS_F32
+    cg = torch.empty((n, 3 if dim == 2 else 6), dtype=flow_aux.dtype, device=flow_aux.device) if want_cg else None
+    ftle = torch.empty(n, dtype=flow_aux.dtype, device=flow_aux.device)
+    status = torch.empty(n, dtype=torch.uint8, device=flow_aux.device) if want_status else None
+    _check(lib().lcs_cg_ftle_aux(int(dim), dtype, n, _arr3(aux_delta, C.c_double, 1.0), _tptr(flow_aux), _tptr(flag_aux), float(T),
+                                 _tptr(cg), _tptr(ftle), _tptr(status), _stream_ptr(stream)))
+    return cg, ftle, status

@@ -589,3 +589,56 @@ def test_cg_eigen_arguments(lcs):
     assert ev.shape == (0, 3) and vec.shape == (0, 3, 3)
     with pytest.raises(lcs.LcsError):
         lcs._check(lcs.lib().lcs_cg_eigen(4, 0, 1, 1, 1, 1, None))
+
+
+# -------------------------------------------------------------------------------------------------
+# row f3: Cauchy-Green tensor from auxiliary points
+@pytest.mark.parametrize("case", ["cart2_f64", "tet_f32"])
+def test_cg_ftle_aux_vs_oracle(lcs, oracle, case):
+    """lcs_cg_ftle_aux against oracle rule O9: the auxiliary tracers are advected by lcs_advect (GPU) and by the oracle, then
+    differenced by each side.  fp64 double gyre: fp64 gate; fp32 pipe on tets with exits: statistical FTLE gate and equal
+    status wherever both sides agree on the flags of the auxiliary tracers."""
+    import torch
+    if case == "cart2_f64":
+        w = I.config1(ng=(48, 24), T=5.0)
+        delta = (1e-3, 1e-3)
+    else:
+        w = I.config4(ng=(16, 16, 24), delta=0.08, T=1.0, h=0.005, n_snap=8, length=4.0)
+        delta = (2e-2, 2e-2, 2e-2)
+    dim, T = w.dim, w.tf - w.t0
+    aux = I.aux_seeds(w.seeds(), delta).reshape(-1, dim)
+    fo, Fo, flo, eso = oracle_run(oracle, w, seeds=aux)
+    f, sd, F, flag, es = gpu_run(w, seeds=aux)
+    cgo, fto, sto = oracle.cg_ftle_aux(dim, delta, Fo, flo, T)
+    cgg, ftg, stg = lcs.cg_ftle_aux(dim, delta, F.reshape(-1, 2 * dim, dim), flag.reshape(-1, 2 * dim), T)
+    torch.cuda.synchronize()
+    cgg, ftg, stg = cpu(cgg).astype(np.float64), cpu(ftg).astype(np.float64), cpu(stg)
+    if case == "cart2_f64":
+        assert np.array_equal(cpu(flag), flo) and np.array_equal(stg, sto) and np.all(sto == 0)
+        assert np.max(np.abs(cpu(F) - Fo)) <= 1e-10
+        assert np.all(np.abs(ftg - fto) <= 1e-8 * np.abs(fto) + 1e-6)       # (1e-10 / delta) / (2 T): the quotient amplifies 1e-10
+        assert np.max(np.abs(cgg - cgo) / np.maximum(np.abs(cgo), 1.0)) <= 1e-5
+    else:
+        same = np.all(cpu(flag).reshape(-1, 2 * dim) == flo.reshape(-1, 2 * dim), axis=1)
+        assert same.mean() > 0.99 and np.array_equal(stg[same], sto[same])
+        assert (sto == 1).sum() > 50 and (sto == 0).sum() > 200
+        ok = same & (sto == 0)
+        assert np.all(np.isnan(ftg[same & (sto == 1)]))
+        # fp32 positions (1e-7 relative of L = 4) differenced over 2 delta = 0.04: FTLE absolute error budget 1e-4 / T
+        assert np.median(np.abs(ftg[ok] - fto[ok])) <= 2e-3
+    # the exact same device buffers through the oracle's arithmetic: the kernel's own differencing / eigenvalue is tight
+    cgx, ftx, stx = oracle.cg_ftle_aux(dim, delta, cpu(F).astype(np.float64), cpu(flag), T)
+    okx = stx == 0
+    assert np.array_equal(stg, stx)
+    assert np.max(np.abs(ftg[okx] - ftx[okx])) <= (1e-12 if case == "cart2_f64" else 2e-5)
+
+
+def test_cg_ftle_aux_arguments(lcs):
+    import torch
+    z = torch.zeros((4, 4, 2), device="cuda", dtype=torch.float64)
+    with pytest.raises(lcs.LcsError):
+        lcs.cg_ftle_aux(2, (0.0, 1e-3), z, None, 1.0)
+    with pytest.raises(lcs.LcsError):
+        lcs.cg_ftle_aux(2, (1e-3, 1e-3), z, None, 0.0)
+    cg, ft, st = lcs.cg_ftle_aux(2, (1e-3, 1e-3), torch.zeros((0, 4, 2), device="cuda", dtype=torch.float64), None, 1.0)
+    assert ft.shape == (0,)
