@@ -201,6 +201,54 @@ def cg_ftle(dim, ng, seed_spacing, seed_periodic, period, flowmap, exit_flag, T)
     return cg, ftle, status
 
 
+def early_cg(field, dim, ng, seed_spacing, seed_periodic, period, seeds, t0, tf, h, every):
+    """Rule O10 (row f1, reading #29): early evaluation of the Cauchy-Green tensor when a stencil member leaves.
+    All tracers advance synchronously (positions of all tracers exist at every step, so C "can be evaluated
+    at any time step"); when a tracer leaves the domain, "the computation of the CG tensor is performed" for the stencils it
+    belongs to with the positions at that time instead of discarding them.
+    Evaluation points are the step counts m = every, 2 every, ... and N.  At m a tracer is alive if it has completed m steps.
+    Seed i is (re-)evaluated at m iff it is alive and each of its 2 dim grid neighbours is alive or never started (flag 2 / outside
+    the grid: those are invalid neighbours in the sense of O5, i.e. one-sided differences); a neighbour that left freezes
+    the seed at its previous evaluation.  The evaluation is O5-O7 with T_eff = m h.  Returns
+    (flowmap, flag, exit_step, cg, ftle, t_eff, status); seeds never evaluated have NaN, t_eff = 0 and status bit 0."""
+    n = seeds.shape[0]
+    N = int(round((tf - t0) / h))
+    assert every >= 1
+    F, flag, es, traj = field.advect(seeds, t0, tf, h, rec_every=every)
+    ncg = 3 if dim == 2 else 6
+    cg = np.full((n, ncg), np.nan)
+    ftle = np.full(n, np.nan)
+    t_eff = np.zeros(n)
+    status = np.ones(n, dtype=np.uint8)
+    g = [int(ng[a]) if a < dim else 1 for a in range(3)]
+    idx = np.arange(n).reshape(g[2], g[1], g[0])
+    points = [(m, traj[m // every - 1]) for m in range(every, N + 1, every)]
+    if N % every != 0:
+        points.append((N, F))
+    for m, Fm in points:
+        alive = (flag == 0) | ((flag == 1) & (es >= m))
+        left = (flag == 1) & (es < m)
+        never = (flag == 2)
+        update = alive.copy()
+        for a in range(dim):
+            ax = 2 - a                                           # axis 0 is the fastest index
+            for sh in (1, -1):
+                nb = np.roll(idx, -sh, axis=ax)
+                nb_left = left[nb]
+                if not seed_periodic[a]:                         # outside the grid: no neighbour, never blocks
+                    sl = [slice(None)] * 3
+                    sl[ax] = -1 if sh == 1 else 0
+                    nb_left = nb_left.copy()
+                    nb_left[tuple(sl)] = False
+                update &= ~nb_left.ravel()
+        cgm, ftm, stm = cg_ftle(dim, ng, seed_spacing, seed_periodic, period, Fm, (never | left).astype(np.uint8), m * h)
+        cg[update] = cgm[update]
+        ftle[update] = ftm[update]
+        status[update] = stm[update]
+        t_eff[update] = m * h
+    return F, flag, es, cg, ftle, t_eff, status
+
+
 def cg_ftle_aux(dim, delta, flow_aux, flag_aux, T):
     """Rule O9.  flow_aux [n][2 dim][dim] (entry 2b: released at +delta_b, 2b+1: at -delta_b), flag_aux [n][2 dim] or None.
     Returns (cg, ftle, status)."""

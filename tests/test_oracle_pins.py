@@ -673,3 +673,45 @@ def test_P16_aux_gradient_linear_flow_and_shear(oracle):
     inner = np.zeros((32, 64), bool); inner[1:-1, 1:-1] = True
     ok = inner.ravel() & (sta == 0)
     assert ok.sum() > 1500 and np.max(np.abs(fta[ok] - ftg[ok])) <= 1e-12   # delta = seed spacing: the very same stencil
+
+
+# -------------------------------------------------------------------------------------------------
+# O10 (row f1): early evaluation of C when a stencil member leaves
+def test_P17_early_cg(oracle):
+    """Pins for O10.  (a) No exits: identical to the plain evaluation at T for any `every`.  (b) Uniform flow through an
+    open box: the exit step of every tracer follows from geometry, hence t_eff of every seed; C = I, FTLE = 0.  (c) Pure
+    strain u = (s x, -s y) in an open box: FTLE_RK4 = ln P(hs) / h whatever the evaluation time (pin P4), so every
+    evaluated seed carries the same value although their t_eff differ."""
+    w = I.config1(ng=(32, 16), T=3.0)
+    fo = oracle.OracleField.from_workload(w)
+    args = (2, w.ng, w.seed_spacing, w.seed_periodic, w.period)
+    F, fl, es, cg, ft, te, st = oracle.early_cg(fo, *args, w.seeds(), w.t0, w.tf, w.h, every=7)
+    cg0, ft0, st0 = oracle.cg_ftle(*args, F, fl, w.tf - w.t0)
+    assert np.all(fl == 0) and np.array_equal(cg, cg0) and np.array_equal(ft, ft0) and np.array_equal(st, st0)
+    assert np.all(te == w.tf - w.t0)
+    # (b) uniform flow c = (0.3, 0) in the box [0,4] x [0,4], seeds on an 8 x 6 grid, h = 0.25, 20 steps, every = 2
+    c, h, N, K = 0.3, 0.25, 20, 2
+    wu = I.analytic_cartesian(2, I.linear_flow(np.zeros((2, 2)), np.array([c, 0.0])), (5, 5), (0.0, 0.0), (1.0, 1.0), (0.0, 10.0),
+                              ng=(8, 6), seed_lo=(0.2, 0.5), seed_spacing=(0.45, 0.5), t0=0.0, tf=h * N, h=h)
+    fu = oracle.OracleField.from_workload(wu)
+    s = wu.seeds()
+    F, fl, es, cg, ft, te, st = oracle.early_cg(fu, 2, wu.ng, wu.seed_spacing, wu.seed_periodic, wu.period, s, 0.0, h * N, h, every=K)
+    # a step n succeeds iff x0 + c (n + 1) h <= 4 (the last stage point is the farthest): exit_step = number of such n
+    es_geo = np.minimum(N, np.floor((4.0 - s[:, 0]) / (c * h) + 1e-9)).astype(int)
+    assert np.array_equal(es, es_geo) and set(np.unique(fl)) == {0, 1}
+    esg = es_geo.reshape(6, 8)
+    stencil_min = esg.copy()
+    stencil_min[:, :-1] = np.minimum(stencil_min[:, :-1], esg[:, 1:])        # +x neighbour leaves first; y neighbours leave with the seed
+    te_geo = (stencil_min // K) * K * h
+    assert np.allclose(te.reshape(6, 8), te_geo, atol=1e-12)
+    ok = te > 0
+    assert ok.sum() > 30 and np.all(st[~ok] & 1) and np.all(np.isnan(ft[~ok]))
+    assert np.max(np.abs(cg[ok] - np.array([1.0, 0.0, 1.0]))) <= 1e-12 and np.max(np.abs(ft[ok])) <= 1e-12
+    # (c) pure strain, s = 1, h = 0.1: FTLE = 0.999999233219801983 at every evaluation time
+    ws = I.analytic_cartesian(2, I.linear_flow(np.array([[1.0, 0.0], [0.0, -1.0]])), (41, 41), (-4.0, -4.0), (0.2, 0.2), (0.0, 10.0),
+                              ng=(10, 8), seed_lo=(-0.9, -0.7), seed_spacing=(0.2, 0.2), t0=0.0, tf=3.0, h=0.1)
+    fs = oracle.OracleField.from_workload(ws)
+    F, fl, es, cg, ft, te, st = oracle.early_cg(fs, 2, ws.ng, ws.seed_spacing, ws.seed_periodic, ws.period, ws.seeds(), 0.0, 3.0, 0.1, every=5)
+    ok = te > 0
+    assert (fl == 1).sum() > 10 and len(np.unique(te[ok])) >= 3
+    assert np.max(np.abs(ft[ok] - 0.999999233219801983)) <= 1e-9
