@@ -132,6 +132,22 @@ lcs_status lcs_cg_ftle(int32_t dim, int32_t dtype, const int32_t ng[3], const do
                        const void *flowmap, const uint8_t *exit_flag, double T,
                        void *cg, void *ftle, uint8_t *status, void *cuda_stream);
 
+/* Flow map WITH early evaluation of the Cauchy-Green tensor (when a tracer leaves the domain "the
+ * computation of the CG tensor is performed" for the stencils it belongs to instead of discarding them; PAPER.md:85, 153:
+ * all tracers advance together, so C "can be evaluated at any time step").  Same integration as lcs_advect on the
+ * structured seed grid ng (n = ng0*ng1*ng2 seeds, layout as in lcs_cg_ftle).  Evaluation points are the step counts
+ * m = every, 2*every, ... and N.  At m a seed is (re-)evaluated iff it has completed m steps and none of its 2*dim grid
+ * neighbours has left; neighbours that never started (flag 2) or lie outside the grid are invalid neighbours as in
+ * lcs_cg_ftle (one-sided differences).  The evaluation is that of lcs_cg_ftle with T_eff = m*h.  A seed keeps the
+ * result of its last evaluation: t_eff[n] (compute_dtype) is m*h of it, 0 if it was never evaluated (then C, FTLE = NaN,
+ * status bit 0).  flowmap / exit_flag / exit_step: as lcs_advect (flowmap and exit_flag are required and must not alias
+ * seeds: they are rewritten at every evaluation point).  cg and status may be NULL.  every >= 1.                  */
+lcs_status lcs_advect_early_cg(lcs_field *f, const int32_t ng[3], const double seed_spacing[3],
+                               const int32_t seed_periodic[3], const double period[3], const void *seeds,
+                               double t0, double tf, double h, int32_t every, void *flowmap, uint8_t *exit_flag,
+                               int32_t *exit_step, void *cg, void *ftle, void *t_eff, uint8_t *status,
+                               void *cuda_stream);
+
 /* Cauchy-Green tensor and FTLE from AUXILIARY points instead of neighbouring seeds ("a structured grid
  * of auxiliary points can be placed around each seed point"; the Cauchy-Green filter uses them "for the
  * computation of the flow map gradient").  The caller advects, with lcs_advect, 2*dim auxiliary tracers per seed released

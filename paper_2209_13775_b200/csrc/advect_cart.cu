@@ -654,8 +654,9 @@ lcs_status cart_advect_impl(lcs_field *f, int64_t n, const void *seeds_, double 
         int chunk = w.count;
         if (blend) chunk = (int)f->opt_preblend_steps;
         else if (do_bundle && f->opt_bundle_steps > 0) chunk = (int)f->opt_bundle_steps;
-        for (int done = 0; done < w.count; done += chunk) {
-            Unit u{(int)wi, (int)w.first + done, w.count - done < chunk ? w.count - done : chunk, blend ? 1 : 0, (int)ftau.size(), 0};
+        for (int done = 0, cnt = 0; done < w.count; done += cnt) {
+            cnt = lcs_early_cut(f, w.first + done, w.count - done < chunk ? w.count - done : chunk);
+            Unit u{(int)wi, (int)w.first + done, cnt, blend ? 1 : 0, (int)ftau.size(), 0};
             if (blend) {
                 for (int s = u.first; s < u.first + u.count; ++s)
                     for (int k = 0; k < 3; ++k) {
@@ -715,6 +716,13 @@ lcs_status cart_advect_impl(lcs_field *f, int64_t n, const void *seeds_, double 
         return LCS_OK;
     };
 
+    // row f1: at an evaluation point, scatter positions and flags to the caller's order and evaluate C for complete stencils
+    auto early_eval = [&](int64_t end) -> lcs_status {
+        if (!lcs_early_due(f, end, N)) return LCS_OK;
+        LCS_LAUNCH((cart_final_kernel<DIM, TC>), lcs_blocks(n, 256), 256, 0, st, g, seeds, n, cur, (int32_t)N, (TC *)f->early.flowmap, f->early.flag,
+                   (int32_t *)nullptr);
+        return lcs_early_cg_eval(f, end, st);
+    };
     int cur_win = -1, since_bundle = 0;
     const void *p[3] = {nullptr, nullptr, nullptr}, *raw_a = nullptr, *raw_b = nullptr;
     for (size_t ui = 0; ui < units.size(); ++ui) {
@@ -758,6 +766,8 @@ lcs_status cart_advect_impl(lcs_field *f, int64_t n, const void *seeds_, double 
                 }
                 const bool last_of_win = ui + 1 == units.size() || units[ui + 1].win != u.win;
                 if (last_of_win) { rc = lcs_field_release_raw(f, w.s[0], st); if (rc != LCS_OK) return rc; }
+                rc = early_eval((int64_t)u.first + u.count);
+                if (rc != LCS_OK) return rc;
                 continue;
             }
         }
@@ -776,6 +786,8 @@ lcs_status cart_advect_impl(lcs_field *f, int64_t n, const void *seeds_, double 
                 else launch_split_step<DIM, TV, TC, false, false>(g, p, t3, s, n, cur, d_xi, d_acc, hs, block, st);
             }
         }
+        rc = early_eval((int64_t)u.first + u.count);
+        if (rc != LCS_OK) return rc;
     }
     LCS_LAUNCH((cart_final_kernel<DIM, TC>), lcs_blocks(n, 256), 256, 0, st, g, seeds, n, cur, (int32_t)N, flowmap, exit_flag, exit_step);
     LCS_CUDA_OK(cudaGetLastError());

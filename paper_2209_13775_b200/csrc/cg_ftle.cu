@@ -43,13 +43,19 @@ __device__ __forceinline__ double eigmax_sym3(double c11, double c12, double c13
     return q + 2.0 * p * cos(acos(r) / 3.0);
 }
 
-template <int DIM, typename T>
+// EARLY (row f1, reading #29): the kernel runs at an evaluation point of lcs_advect_early_cg with the flags of
+// that moment (0 alive, 1 left, 2 never started).  A seed is (re-)evaluated only if it is alive and none of its grid
+// neighbours has left; neighbours that never started stay invalid neighbours (one-sided differences).  Seeds that are
+// not evaluated keep the outputs of their previous evaluation; t_eff records the time of the last one.
+template <int DIM, typename T, bool EARLY>
 __global__ void __launch_bounds__(256) cg_ftle_kernel(const __grid_constant__ CgGrid g, const T *__restrict__ F,
                                                        const uint8_t *__restrict__ flag, T *__restrict__ cg,
-                                                       T *__restrict__ ftle, uint8_t *__restrict__ status, int64_t n)
+                                                       T *__restrict__ ftle, uint8_t *__restrict__ status, int64_t n,
+                                                       T *__restrict__ t_eff, double t_now)
 {
     int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= n) return;
+    if (EARLY && flag[idx] != 0) return;
     const int64_t n0 = g.ng[0], n1 = g.ng[1];
     int ijk[3] = {(int)(idx % n0), (int)((idx / n0) % n1), (int)(idx / (n0 * n1))};
     const int64_t stride[3] = {1, n0, n0 * n1};
@@ -68,6 +74,9 @@ __global__ void __launch_bounds__(256) cg_ftle_kernel(const __grid_constant__ Cg
         if (ip >= g.ng[b]) { if (g.per[b]) { ip -= g.ng[b]; shp = g.period[b]; } else okp = false; }
         if (im < 0) { if (g.per[b]) { im += g.ng[b]; shm = -g.period[b]; } else okm = false; }
         int64_t jp = idx + (int64_t)(ip - ijk[b]) * stride[b], jm = idx + (int64_t)(im - ijk[b]) * stride[b];
+        if constexpr (EARLY) {
+            if ((okp && flag[jp] == 1) || (okm && flag[jm] == 1)) return;
+        }
         if (okp && flag && flag[jp] != 0) okp = false;
         if (okm && flag && flag[jm] != 0) okm = false;
 #pragma unroll
@@ -110,6 +119,21 @@ __global__ void __launch_bounds__(256) cg_ftle_kernel(const __grid_constant__ Cg
     }
     ftle[idx] = (st & 1) ? (T)nan("") : (T)(log(lam) * g.inv_2T);
     if (status) status[idx] = st;
+    if constexpr (EARLY) t_eff[idx] = (T)t_now;
+}
+
+// outputs of seeds that are never evaluated: NaN, t_eff = 0, status bit 0
+template <typename T>
+__global__ void __launch_bounds__(256) early_init_kernel(T *__restrict__ cg, int ncg, T *__restrict__ ftle, T *__restrict__ t_eff,
+                                                          uint8_t *__restrict__ status, int64_t n)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const T q = (T)nan("");
+    if (cg) for (int k = 0; k < ncg; ++k) cg[i * ncg + k] = q;
+    ftle[i] = q;
+    t_eff[i] = T(0);
+    if (status) status[i] = 1;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -277,10 +301,10 @@ extern "C" lcs_status lcs_cg_ftle(int32_t dim, int32_t dtype, const int32_t ng[3
     if (n == 0) return LCS_OK;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const unsigned grid = lcs_blocks(n, 256);
-    if (dim == 2 && dtype == LCS_F64) LCS_LAUNCH((cg_ftle_kernel<2, double>), grid, 256, 0, st, g, (const double *)flowmap, exit_flag, (double *)cg, (double *)ftle, status, n);
-    else if (dim == 2) LCS_LAUNCH((cg_ftle_kernel<2, float>), grid, 256, 0, st, g, (const float *)flowmap, exit_flag, (float *)cg, (float *)ftle, status, n);
-    else if (dtype == LCS_F64) LCS_LAUNCH((cg_ftle_kernel<3, double>), grid, 256, 0, st, g, (const double *)flowmap, exit_flag, (double *)cg, (double *)ftle, status, n);
-    else LCS_LAUNCH((cg_ftle_kernel<3, float>), grid, 256, 0, st, g, (const float *)flowmap, exit_flag, (float *)cg, (float *)ftle, status, n);
+    if (dim == 2 && dtype == LCS_F64) LCS_LAUNCH((cg_ftle_kernel<2, double, false>), grid, 256, 0, st, g, (const double *)flowmap, exit_flag, (double *)cg, (double *)ftle, status, n, (double *)nullptr, 0.0);
+    else if (dim == 2) LCS_LAUNCH((cg_ftle_kernel<2, float, false>), grid, 256, 0, st, g, (const float *)flowmap, exit_flag, (float *)cg, (float *)ftle, status, n, (float *)nullptr, 0.0);
+    else if (dtype == LCS_F64) LCS_LAUNCH((cg_ftle_kernel<3, double, false>), grid, 256, 0, st, g, (const double *)flowmap, exit_flag, (double *)cg, (double *)ftle, status, n, (double *)nullptr, 0.0);
+    else LCS_LAUNCH((cg_ftle_kernel<3, float, false>), grid, 256, 0, st, g, (const float *)flowmap, exit_flag, (float *)cg, (float *)ftle, status, n, (float *)nullptr, 0.0);
     LCS_CUDA_OK(cudaGetLastError());
     return LCS_OK;
 }
@@ -321,4 +345,57 @@ extern "C" lcs_status lcs_cg_ftle_aux(int32_t dim, int32_t dtype, int64_t n, con
     else LCS_LAUNCH((cg_ftle_aux_kernel<3, float>), grid, 256, 0, st, (const float *)flowmap_aux, exit_flag_aux, i2d[0], i2d[1], i2d[2], inv_2T, (float *)cg, (float *)ftle, status, n);
     LCS_CUDA_OK(cudaGetLastError());
     return LCS_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Row f1: early evaluation of C when a stencil member leaves the domain
+lcs_status lcs_early_cg_eval(lcs_field *f, int64_t m, cudaStream_t st)
+{
+    const EarlyCg &e = f->early;
+    CgGrid g;
+    int64_t n = 1;
+    for (int a = 0; a < 3; ++a) {
+        g.ng[a] = e.ng[a]; g.per[a] = e.per[a]; g.period[a] = e.period[a]; g.inv_dx[a] = 1.0 / e.dx[a];
+        n *= e.ng[a];
+    }
+    const double t_now = (double)m * e.h;
+    g.inv_2T = 1.0 / (2.0 * fabs(t_now));
+    const unsigned grid = lcs_blocks(n, 256);
+    const bool f64 = f->compute_dtype == LCS_F64;
+    if (f->dim == 2 && f64) LCS_LAUNCH((cg_ftle_kernel<2, double, true>), grid, 256, 0, st, g, (const double *)e.flowmap, e.flag, (double *)e.cg, (double *)e.ftle, e.status, n, (double *)e.t_eff, t_now);
+    else if (f->dim == 2) LCS_LAUNCH((cg_ftle_kernel<2, float, true>), grid, 256, 0, st, g, (const float *)e.flowmap, e.flag, (float *)e.cg, (float *)e.ftle, e.status, n, (float *)e.t_eff, t_now);
+    else if (f64) LCS_LAUNCH((cg_ftle_kernel<3, double, true>), grid, 256, 0, st, g, (const double *)e.flowmap, e.flag, (double *)e.cg, (double *)e.ftle, e.status, n, (double *)e.t_eff, t_now);
+    else LCS_LAUNCH((cg_ftle_kernel<3, float, true>), grid, 256, 0, st, g, (const float *)e.flowmap, e.flag, (float *)e.cg, (float *)e.ftle, e.status, n, (float *)e.t_eff, t_now);
+    LCS_CUDA_OK(cudaGetLastError());
+    return LCS_OK;
+}
+
+extern "C" lcs_status lcs_advect_early_cg(lcs_field *f, const int32_t ng[3], const double seed_spacing[3], const int32_t seed_periodic[3],
+                                          const double period[3], const void *seeds, double t0, double tf, double h, int32_t every,
+                                          void *flowmap, uint8_t *exit_flag, int32_t *exit_step, void *cg, void *ftle, void *t_eff,
+                                          uint8_t *status, void *cuda_stream)
+{
+    if (!f || !ng || !seed_spacing || !seeds || !flowmap || !exit_flag || !ftle || !t_eff) { lcs_set_error("null argument"); return LCS_ERR_INVALID_ARG; }
+    if (every < 1) { lcs_set_error("every must be >= 1"); return LCS_ERR_INVALID_ARG; }
+    if (flowmap == seeds) { lcs_set_error("flowmap must not alias seeds (it is rewritten at every evaluation point)"); return LCS_ERR_INVALID_ARG; }
+    EarlyCg e;
+    int64_t n = 1;
+    for (int a = 0; a < 3; ++a) {
+        e.ng[a] = a < f->dim ? ng[a] : 1;
+        e.per[a] = (a < f->dim && seed_periodic) ? (seed_periodic[a] != 0) : 0;
+        e.period[a] = (a < f->dim && period) ? period[a] : 0.0;
+        e.dx[a] = a < f->dim ? seed_spacing[a] : 1.0;
+        if (a < f->dim && (ng[a] < 1 || !(seed_spacing[a] > 0))) { lcs_set_error("bad seed grid on axis %d", a); return LCS_ERR_INVALID_ARG; }
+        n *= e.ng[a];
+    }
+    e.on = true; e.every = every; e.h = h;
+    e.flowmap = flowmap; e.flag = exit_flag; e.cg = cg; e.ftle = ftle; e.t_eff = t_eff; e.status = status;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const int ncg = f->dim == 2 ? 3 : 6;
+    if (f->compute_dtype == LCS_F64) LCS_LAUNCH((early_init_kernel<double>), lcs_blocks(n, 256), 256, 0, st, (double *)cg, ncg, (double *)ftle, (double *)t_eff, status, n);
+    else LCS_LAUNCH((early_init_kernel<float>), lcs_blocks(n, 256), 256, 0, st, (float *)cg, ncg, (float *)ftle, (float *)t_eff, status, n);
+    f->early = e;
+    lcs_status rc = lcs_advect(f, n, seeds, t0, tf, h, flowmap, exit_flag, exit_step, cuda_stream);
+    f->early = EarlyCg();
+    return rc;
 }

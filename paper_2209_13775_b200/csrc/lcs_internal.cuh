@@ -74,6 +74,17 @@ struct TracerScratch {
     size_t bytes = 0;
 };
 
+// context of lcs_advect_early_cg (row f1): where and when the integrators evaluate C during the advection
+struct EarlyCg {
+    bool on = false;
+    int64_t every = 0;            // evaluation points: step counts that are multiples of `every`, and N
+    int32_t ng[3] = {1, 1, 1}, per[3] = {0, 0, 0};
+    double dx[3] = {1, 1, 1}, period[3] = {0, 0, 0};
+    double h = 0;
+    void *flowmap = nullptr, *cg = nullptr, *ftle = nullptr, *t_eff = nullptr;
+    uint8_t *flag = nullptr, *status = nullptr;
+};
+
 struct lcs_field {
     int dim = 0, kind = 0;
     int vel_dtype = 0, compute_dtype = 0;
@@ -108,6 +119,7 @@ struct lcs_field {
     void *h_seeds = nullptr, *h_flow = nullptr, *h_ftle = nullptr;
     uint8_t *h_flag = nullptr;
     int64_t h_cap = 0;
+    EarlyCg early;
     // options
     int64_t opt_integrator = 0;   // 0 auto, 1 fused, 2 split
     int64_t opt_bundle = -1;      // re-bundle tracers by cell: -1 auto (large seed sets), 0 off, 1 on
@@ -143,6 +155,17 @@ lcs_status lcs_field_prefetch(lcs_field *f, int s, int keep0, int keep1);
 lcs_status lcs_field_acquire_raw(lcs_field *f, int s, cudaStream_t stream, const void **a, const void **b);
 lcs_status lcs_field_release_raw(lcs_field *f, int s, cudaStream_t stream);
 lcs_status lcs_scratch_reserve(lcs_field *f, size_t bytes);
+
+// cg_ftle.cu: evaluate C for the stencils that are still complete after m steps (flow map + flags already scattered)
+lcs_status lcs_early_cg_eval(lcs_field *f, int64_t m, cudaStream_t st);
+// number of steps of a launch unit that starts at step `first` and would run `count` steps: cut at the next evaluation point
+static inline int lcs_early_cut(const lcs_field *f, int64_t first, int count)
+{
+    if (!f->early.on) return count;
+    int64_t next = (first / f->early.every + 1) * f->early.every;
+    return (int)(next - first < count ? next - first : count);
+}
+static inline bool lcs_early_due(const lcs_field *f, int64_t end, int64_t N) { return f->early.on && (end % f->early.every == 0 || end == N); }
 
 // simplex.cu
 lcs_status lcs_simplex_build(lcs_field *f, const double *verts_host, const int32_t *cells_host);

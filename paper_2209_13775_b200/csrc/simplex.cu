@@ -848,8 +848,8 @@ lcs_status simplex_advect_impl(lcs_field *f, int64_t n, const void *seeds_, doub
         }
         lcs_field_prefetch(f, dir > 0 ? w.s[2] + 2 : w.s[2] - 1, w.s[2], w.s[2] + 1);
         const int chunk = (do_bundle && f->opt_bundle_steps > 0 && f->opt_bundle_steps < w.count) ? (int)f->opt_bundle_steps : w.count;
-        for (int done = 0; done < w.count; done += chunk) {
-            const int cnt = w.count - done < chunk ? w.count - done : chunk;
+        for (int done = 0, cnt = 0; done < w.count; done += cnt) {
+            cnt = lcs_early_cut(f, w.first + done, w.count - done < chunk ? w.count - done : chunk);
             const int first = (int)w.first + done;
             if (do_bundle && (since_bundle < 0 || since_bundle >= bundle_every)) {
                 LCS_CUDA_OK(cudaMemsetAsync(d_cnt, 0, (size_t)nbins * 4, st));
@@ -862,6 +862,12 @@ lcs_status simplex_advect_impl(lcs_field *f, int64_t n, const void *seeds_, doub
             WindowTimer timer(f, st);
             LCS_LAUNCH((simplex_window_kernel<DIM, TV, TC>), lcs_blocks(n, block), block, 0, st, (const CellRec<DIM, TC> *)m.cellrec, m.neigh,
                        (const VRec *)p[0], (const VRec *)p[1], (const VRec *)p[2], d_tau + 3 * (size_t)first, cnt, first, n, cur, (TC)h);
+            if (lcs_early_due(f, (int64_t)first + cnt, N)) {         // row f1: evaluate C for the stencils that are still complete
+                LCS_LAUNCH((simplex_final_kernel<DIM, TC>), lcs_blocks(n, 256), 256, 0, st, n, cur, (int32_t)N, (TC *)f->early.flowmap,
+                           f->early.flag, (int32_t *)nullptr);
+                rc = lcs_early_cg_eval(f, (int64_t)first + cnt, st);
+                if (rc != LCS_OK) return rc;
+            }
         }
         f->info_windows++;
     }

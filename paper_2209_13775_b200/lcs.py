@@ -22,7 +22,7 @@ LCS_F32, LCS_F64 = 0, 1
 LCS_MESH_CARTESIAN, LCS_MESH_SIMPLEX = 0, 1
 
 EXPORTS = ["lcs_field_create", "lcs_field_set_snapshot", "lcs_field_sync", "lcs_field_destroy",
-           "lcs_field_set_option", "lcs_field_get_info", "lcs_locate", "lcs_advect", "lcs_cg_ftle", "lcs_cg_ftle_aux", "lcs_cg_eigen",
+           "lcs_field_set_option", "lcs_field_get_info", "lcs_locate", "lcs_advect", "lcs_advect_early_cg", "lcs_cg_ftle", "lcs_cg_ftle_aux", "lcs_cg_eigen",
            "lcs_ftle_host", "lcs_kernel_launch_count", "lcs_last_error"]
 
 
@@ -68,6 +68,9 @@ def lib():
                                  C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.lcs_cg_ftle.argtypes = [C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                   C.c_void_p, C.c_void_p, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.lcs_advect_early_cg.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_double,
+                                          C.c_double, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                          C.c_void_p, C.c_void_p]
         L.lcs_cg_ftle_aux.argtypes = [C.c_int32, C.c_int32, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double,
                                       C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.lcs_cg_eigen.argtypes = [C.c_int32, C.c_int32, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
@@ -273,3 +276,21 @@ def cg_ftle_aux(dim, aux_delta, flow_aux, flag_aux, T, want_cg=True, want_status
     _check(lib().lcs_cg_ftle_aux(int(dim), dtype, n, _arr3(aux_delta, C.c_double, 1.0), _tptr(flow_aux), _tptr(flag_aux), float(T),
                                  _tptr(cg), _tptr(ftle), _tptr(status), _stream_ptr(stream)))
     return cg, ftle, status
+
+
+def advect_early_cg(field, ng, seed_spacing, seed_periodic, period, seeds, t0, tf, h, every, stream=None):
+    """lcs_advect_early_cg: returns (flowmap, exit_flag, exit_step, cg, ftle, t_eff, status), torch CUDA tensors."""
+    import torch
+    assert seeds.is_cuda and seeds.is_contiguous()
+    n, dim = seeds.shape
+    F = torch.empty_like(seeds)
+    flag = torch.empty(n, dtype=torch.uint8, device=seeds.device)
+    es = torch.empty(n, dtype=torch.int32, device=seeds.device)
+    cg = torch.empty((n, 3 if dim == 2 else 6), dtype=seeds.dtype, device=seeds.device)
+    ftle = torch.empty(n, dtype=seeds.dtype, device=seeds.device)
+    t_eff = torch.empty(n, dtype=seeds.dtype, device=seeds.device)
+    status = torch.empty(n, dtype=torch.uint8, device=seeds.device)
+    _check(lib().lcs_advect_early_cg(field._h, _arr3(ng, C.c_int32, 1), _arr3(seed_spacing, C.c_double, 1.0), _arr3(seed_periodic, C.c_int32, 0),
+                                     _arr3(period, C.c_double, 0.0), _tptr(seeds), float(t0), float(tf), float(h), int(every), _tptr(F),
+                                     _tptr(flag), _tptr(es), _tptr(cg), _tptr(ftle), _tptr(t_eff), _tptr(status), _stream_ptr(stream)))
+    return F, flag, es, cg, ftle, t_eff, status

@@ -642,3 +642,82 @@ def test_cg_ftle_aux_arguments(lcs):
         lcs.cg_ftle_aux(2, (1e-3, 1e-3), z, None, 0.0)
     cg, ft, st = lcs.cg_ftle_aux(2, (1e-3, 1e-3), torch.zeros((0, 4, 2), device="cuda", dtype=torch.float64), None, 1.0)
     assert ft.shape == (0,)
+
+
+# -------------------------------------------------------------------------------------------------
+# row f1: early evaluation of C when a stencil member leaves
+@pytest.mark.parametrize("case", ["cart2_f64_open_box", "cart3_f32_preblend", "tet_f32_pipe"])
+def test_advect_early_cg_vs_oracle(lcs, oracle, case):
+    """lcs_advect_early_cg against oracle rule O10: same evaluation points, same update rule.  fp64 open box (a rotating strain
+    flow that pushes tracers out): flags, exit steps and t_eff identical, FTLE within the fp64 gate.  fp32 cases (non-periodic 3D
+    grid through the bundled pre-blended integrator; pipe flow on tets): t_eff identical wherever the flags of the whole stencil
+    agree, median FTLE error within the statistical gate."""
+    import torch
+    if case == "cart2_f64_open_box":
+        A = np.array([[0.25, 0.6], [-0.6, 0.25]])
+        w = I.analytic_cartesian(2, I.linear_flow(A), (41, 41), (-2.0, -2.0), (0.1, 0.1), (0.0, 2.0, 4.0), ng=(24, 20), seed_lo=(-2.1, -1.4),
+                                 seed_spacing=(0.175, 0.14), t0=0.0, tf=4.0, h=0.05)      # first and last seed columns lie outside
+        every, opts = 7, dict(bundle=1, bundle_steps=11)
+    elif case == "cart3_f32_preblend":
+        A = np.array([[0.05, 0.3, 0.0], [-0.3, 0.02, 0.1], [0.0, -0.1, 0.04]])
+        w = I.analytic_cartesian(3, I.linear_flow(A, np.array([0.2, -0.05, 0.1])), (21, 17, 13), (0.0, 0.0, 0.0), (0.1, 0.1, 0.1),
+                                 (0.0, 1.0, 2.0, 3.0), ng=(24, 20, 16), seed_lo=(0.1, 0.1, 0.1), seed_spacing=(1.8 / 24, 1.4 / 20, 1.0 / 16),
+                                 t0=0.0, tf=3.0, h=0.05, vel_dtype=np.float32, compute_dtype=np.float32)
+        every, opts = 10, dict(bundle=1, preblend=1, preblend_steps=6)
+    else:
+        w = I.config4(ng=(20, 20, 32), delta=0.08, T=1.5, h=0.005, n_snap=10, length=4.0)
+        every, opts = 40, dict(bundle=1, bundle_steps=60)
+    fo = oracle.OracleField.from_workload(w)
+    args = (w.dim, w.ng, w.seed_spacing, w.seed_periodic, w.period)
+    Fo, flo, eso, cgo, fto, teo, sto = oracle.early_cg(fo, *args, w.seeds().astype(np.float64), w.t0, w.tf, w.h, every)
+    f = lcs.Field.from_workload(w)
+    for k, v in opts.items():
+        f.set_option(k, v)
+    sd = torch.from_numpy(w.seeds()).cuda()
+    F, flag, es, cg, ft, te, stt = lcs.advect_early_cg(f, w.ng, w.seed_spacing, w.seed_periodic, w.period, sd, w.t0, w.tf, w.h, every)
+    torch.cuda.synchronize()
+    F2, flag2, es2 = f.advect(sd, w.t0, w.tf, w.h)                       # the plain call gives the same flow map
+    assert torch.equal(F, F2) and torch.equal(flag, flag2) and torch.equal(es, es2)
+    flag, es, ft, te, stt = cpu(flag), cpu(es), cpu(ft).astype(np.float64), cpu(te).astype(np.float64), cpu(stt)
+    early = (teo > 0) & (teo < (w.tf - w.t0) - 1e-9)
+    assert (flo == 1).sum() > 50 and early.sum() > 30 and (teo == 0).sum() > 0
+    if case == "cart2_f64_open_box":
+        assert np.array_equal(flag, flo) and np.array_equal(es, eso)
+        assert np.allclose(te, teo, atol=1e-12) and np.array_equal(stt, sto)
+        ok = teo > 0
+        assert np.all(np.abs(ft[ok] - fto[ok]) <= 1e-8 * np.abs(fto[ok]) + 1e-10 / teo[ok])
+        assert np.all(np.isnan(ft[~ok]))
+        assert np.max(np.abs(cpu(cg)[ok] - cgo[ok]) / np.maximum(np.abs(cgo[ok]), 1.0)) <= 1e-9
+    else:
+        g = [int(w.ng[a]) for a in range(3)]
+        agree = (flag == flo) & ((flag != 1) | (es == eso))
+        a3 = agree.reshape(g[2], g[1], g[0])
+        sten = a3.copy()
+        for ax in range(3):
+            for sh in (1, -1):
+                r = np.roll(a3, sh, axis=ax)
+                sl = [slice(None)] * 3; sl[ax] = 0 if sh == 1 else -1
+                r[tuple(sl)] = True
+                sten &= r
+        sten = sten.ravel()
+        assert sten.mean() > 0.97
+        assert np.allclose(te[sten], teo[sten], atol=1e-5)
+        ok = sten & (teo > 0) & np.isfinite(fto)
+        assert np.array_equal(np.isfinite(ft[sten]), np.isfinite(fto[sten]))
+        rel = np.abs(ft[ok] - fto[ok]) / np.maximum(np.abs(fto[ok]), 1e-3)
+        assert np.median(rel) <= 1e-3
+
+
+def test_advect_early_cg_arguments(lcs):
+    import torch
+    w = I.config1(ng=(8, 4), T=1.0)
+    f = lcs.Field.from_workload(w)
+    sd = torch.from_numpy(w.seeds()).cuda()
+    with pytest.raises(lcs.LcsError):
+        lcs.advect_early_cg(f, w.ng, w.seed_spacing, w.seed_periodic, w.period, sd, w.t0, w.tf, w.h, 0)
+    out = lcs.advect_early_cg(f, w.ng, w.seed_spacing, w.seed_periodic, w.period, sd, w.t0, w.tf, w.h, 3)
+    F0, fl0, es0 = f.advect(sd, w.t0, w.tf, w.h)
+    cg0, ft0, st0 = lcs.cg_ftle(w.dim, w.ng, w.seed_spacing, w.seed_periodic, w.period, F0, fl0, w.tf - w.t0)
+    torch.cuda.synchronize()
+    assert torch.equal(out[0], F0) and torch.equal(out[4], ft0) and torch.equal(out[3], cg0) and torch.equal(out[6], st0)
+    assert float(out[5].min()) == w.tf - w.t0
