@@ -340,6 +340,19 @@ def main():
                                       "note": "768 B per seed-step of the straightforward 4-stage scheme against 148 SMs x 128 B/clk; "
                                               "above 1 because the kernel gathers pre-blended fields and reuses corners in registers"},
                         **common}
+        elif w.kind == 1 and w.dim == 3 and w.compute_dtype == np.float32:
+            # tets in fp32 (config 4): measured DRAM 1.5% of peak, L2 hit 80-96%, issue slots 58%, L1 wavefronts 63%
+            # (profiles/r1_cfg4_simplex.md): not HBM-bound.  ALU roofline with SURVEY.md 8.3's 900 flop per seed-step.
+            flop_unit = 900.0
+            peak_tf = 148 * 128 * 2 * sm_max_mhz * 1e6 / 1e12
+            ach_tf = flop_unit * units_per_launch / max(kernel_s, 1e-12) / 1e12
+            roofline = {"bound": "alu", "kernel": "simplex_window_kernel", "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s",
+                        "frac": ach_tf / peak_tf, "peak_source": "derived: 148 SMs x 128 FP32 lanes x 2 x %.0f MHz (DESIGN.md)" % sm_max_mhz,
+                        "algorithmic_flop_per_seed_step": flop_unit,
+                        "hbm_gather": {"achieved": achieved, "peak": hbm_gbs, "unit": "GB/s", "frac": achieved / hbm_gbs,
+                                       "note": "640 B per seed-step of the straightforward scheme against the measured HBM copy peak; far "
+                                               "above 1 because the mesh is served by L1/L2 and the held cell skips most gathers"},
+                        **common}
         else:
             roofline = {"bound": "hbm", "kernel": "cart_window_kernel" if w.kind == 0 else "simplex_window_kernel",
                         "achieved": achieved, "peak": hbm_gbs, "unit": "GB/s", "frac": achieved / hbm_gbs, "peak_source": peak_src,

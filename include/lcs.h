@@ -14,6 +14,8 @@
  *  - The hot calls (lcs_locate, lcs_advect, lcs_cg_ftle) are asynchronous on `cuda_stream` (a
  *    cudaStream_t passed as void*, NULL = default stream); the caller synchronises.
  *  - Every step of the path runs in CUDA kernels; there is no CPU fallback.
+ *  - A field owns one set of tracer scratch buffers and one snapshot window: run one hot call at a time per field
+ *    (calls on the same stream serialise by themselves); different fields are independent.
  * Citations are PAPER.md lines (the paper text) and DESIGN.md readings where the paper is silent.
  */
 #ifndef LCS_H
