@@ -594,7 +594,7 @@ __device__ __forceinline__ bool simplex_velocity(const CellRec<DIM, TC> *__restr
 }
 
 template <int DIM, typename TV, typename TC>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(128, (sizeof(TC) == 4 ? 7 : 1))
 simplex_window_kernel(const CellRec<DIM, TC> *__restrict__ crec, const int32_t *__restrict__ neigh, const PairRec<DIM, TV> *__restrict__ pa,
                       const PairRec<DIM, TV> *__restrict__ pb, const PairRec<DIM, TV> *__restrict__ pc, const TC *__restrict__ tau,
                       int nsteps, int first_step, int64_t n, SimplexTracer<DIM, TC> *__restrict__ st, TC h)
