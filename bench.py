@@ -68,9 +68,6 @@ def algorithmic_bytes_per_seed_step(w) -> float:
     return 4.0 * ((w.dim + 1) * 2 * w.dim * es + mesh)
 
 
-FP32_INSTR_PER_SEED_STEP = None   # filled from SASS counts in DESIGN.md when the ALU roofline is quoted
-
-
 class ClockSampler:
     """nvidia-smi clocks + throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
     Q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
