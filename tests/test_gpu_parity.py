@@ -131,6 +131,16 @@ def test_config2_triangles_fp64(lcs, oracle, full):
     assert np.all(flo == 0)
     err = gate_fp64(cpu(F), Fo, cpu(ftg), fto, w.tf - w.t0, cpu(flag), flo, cpu(es), eso)
     print("config2 full=%s max flow-map error %.3e" % (full, err))
+    if full:
+        # SURVEY.md 8.3 parity protocol: lcs_locate bit-exact on ALL seeds against the oracle's walk and on 1e4 sampled seeds
+        # against brute force over all cells
+        import torch
+        pts = w.seeds().astype(np.float64)
+        cell = cpu(f.locate(torch.from_numpy(pts).cuda()))
+        assert np.array_equal(cell, fo.locate_walk(pts)) and cell.min() >= 0
+        sub = np.random.default_rng(22).choice(len(pts), 10000, replace=False)
+        cb, count = fo.locate_brute(pts[sub])
+        assert count.max() == 1 and np.array_equal(cb, cell[sub]) and f.info("locate_fallbacks") == 0
 
 
 def test_config3_reduced_fp32(lcs, oracle):
@@ -456,7 +466,7 @@ def test_simplex_bundled_identical_to_unbundled(lcs, oracle, options):
 def test_config4_full_size_sampled(lcs, oracle):
     """Config 4 at full size (2.01 M vertices / 13.4 M tets, 256x256x512 box seeds, 1600 steps) in bench.py's launch
     configuration (bundling on by default at this size).  lcs_locate: bit-exact against the oracle's walk on 2e5 sampled
-    seeds and against brute force over all cells on 64 of them, with no fallback.  Flow map / FTLE: the oracle integrates
+    seeds and against brute force over all cells on 256 of them, with no fallback.  Flow map / FTLE: the oracle integrates
     6 seeded 12^3 blocks; statistical gate of BASELINE.json."""
     import torch
     w = I.config4()
@@ -468,8 +478,8 @@ def test_config4_full_size_sampled(lcs, oracle):
     pts = np.ascontiguousarray(seeds[pick].astype(np.float64))
     cg_ = cpu(f.locate(torch.from_numpy(pts).cuda()))
     assert np.array_equal(cg_, fo.locate_walk(pts))
-    cb, count = fo.locate_brute(pts[:64])
-    assert np.array_equal(cg_[:64], cb) and np.all(count <= 1)
+    cb, count = fo.locate_brute(pts[:256])
+    assert np.array_equal(cg_[:256], cb) and np.all(count <= 1)
     assert f.info("locate_fallbacks") == 0
     sd = torch.from_numpy(seeds).cuda()
     F, flag, es = f.advect(sd, w.t0, w.tf, w.h)
