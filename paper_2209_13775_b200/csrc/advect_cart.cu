@@ -363,9 +363,10 @@ __global__ void __launch_bounds__(256) blend_xpair_kernel(const float *__restric
         float4 lo, hi;
         lo.x = fmaf(t, vd[0], va[0]); lo.y = fmaf(t, vd[1], va[1]); lo.z = fmaf(t, vd[2], va[2]); lo.w = 0.f;
         hi.x = fmaf(t, vd[3], va[3]); hi.y = fmaf(t, vd[4], va[4]); hi.z = fmaf(t, vd[5], va[5]); hi.w = 0.f;
-        float4 *dst = reinterpret_cast<float4 *>(fields + (int64_t)f * field_stride + i);
-        __stcs(dst, lo);
-        __stcs(dst + 1, hi);
+        // one 256-bit streaming store: a whole 32-byte sector per lane
+        asm volatile("st.global.cs.v8.f32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(fields + (int64_t)f * field_stride + i), "f"(lo.x),
+                     "f"(lo.y), "f"(lo.z), "f"(lo.w), "f"(hi.x), "f"(hi.y), "f"(hi.z), "f"(hi.w)
+                     : "memory");
     }
 }
 
