@@ -436,10 +436,11 @@ __device__ __forceinline__ bool cart_velocity_xpair(const CartDev &g, const XPai
     return true;
 }
 
-// fidx: [nsteps][3] index of the blended field of (ta, tb, tc) within `fields`
+// Step s of the chunk reads the blended fields 2s (ta), 2s+1 (tb), 2s+2 (tc = ta of step s+1): the host only uses this
+// kernel for chunks whose stage times have exactly that structure, so the field addresses are warp-uniform arithmetic.
 template <bool FASTWRAP>
 __global__ void __launch_bounds__(256)
-cart_xpair_kernel(const __grid_constant__ CartDev g, const XPair *__restrict__ fields, int64_t field_stride, const int *__restrict__ fidx,
+cart_xpair_kernel(const __grid_constant__ CartDev g, const XPair *__restrict__ fields, int64_t field_stride,
                   int nsteps, int first_step, int64_t n, CartTracer<3, float> *__restrict__ st, float hs0, float hs1, float hs2)
 {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -457,9 +458,9 @@ cart_xpair_kernel(const __grid_constant__ CartDev g, const XPair *__restrict__ f
     hc.idx = -1;
     const XPair *held_field = nullptr;
     for (; s < nsteps; ++s) {
-        const XPair *fa = fields + (int64_t)__ldg(fidx + 3 * s) * field_stride;
-        const XPair *fb = fields + (int64_t)__ldg(fidx + 3 * s + 1) * field_stride;
-        const XPair *fc = fields + (int64_t)__ldg(fidx + 3 * s + 2) * field_stride;
+        const XPair *fa = fields + (int64_t)(2 * s) * field_stride;
+        const XPair *fb = fa + field_stride;
+        const XPair *fc = fb + field_stride;
         float k1[3], k2[3], k3[3], k4[3], xi[3];
         if (fa != held_field) hc.idx = -1;                     // uniform: tc of the previous step is ta of this one
         ok = cart_velocity_xpair<FASTWRAP, true>(g, fa, ci, w, hc, k1);
@@ -647,7 +648,6 @@ lcs_status cart_advect_impl(lcs_field *f, int64_t n, const void *seeds_, double 
     struct Unit { int win, first, count, blend, ftau_off, nfields; };
     std::vector<Unit> units;
     std::vector<float> ftau;
-    std::vector<int> fidx((size_t)3 * N, 0);
     int max_fields = 0;
     for (size_t wi = 0; wi < windows.size(); ++wi) {
         const StepWindow &w = windows[wi];
@@ -659,13 +659,23 @@ lcs_status cart_advect_impl(lcs_field *f, int64_t n, const void *seeds_, double 
             cnt = lcs_early_cut(f, w.first + done, w.count - done < chunk ? w.count - done : chunk);
             Unit u{(int)wi, (int)w.first + done, cnt, blend ? 1 : 0, (int)ftau.size(), 0};
             if (blend) {
-                for (int s = u.first; s < u.first + u.count; ++s)
-                    for (int k = 0; k < 3; ++k) {
-                        const float t = (float)tau64[3 * (size_t)s + k];
-                        if (u.nfields == 0 || ftau.back() != t) { ftau.push_back(t); u.nfields++; }
-                        fidx[3 * (size_t)s + k] = u.nfields - 1;
+                // fields of the chunk: ta_0, tb_0, tc_0 (= ta_1), tb_1, tc_1, ...: 2 count + 1 of them.  tc of a step and ta of
+                // the next are the same product t0 + (n + 1) h in the same snapshot pair, hence the same tau bit for bit;
+                // should that ever fail, the chunk falls back to pair records.
+                bool regular = true;
+                for (int s = u.first; s + 1 < u.first + u.count; ++s)
+                    regular = regular && (float)tau64[3 * (size_t)s + 2] == (float)tau64[3 * (size_t)(s + 1)];
+                if (regular) {
+                    for (int s = u.first; s < u.first + u.count; ++s) {
+                        ftau.push_back((float)tau64[3 * (size_t)s]);
+                        ftau.push_back((float)tau64[3 * (size_t)s + 1]);
                     }
-                max_fields = u.nfields > max_fields ? u.nfields : max_fields;
+                    ftau.push_back((float)tau64[3 * (size_t)(u.first + u.count - 1) + 2]);
+                    u.nfields = 2 * u.count + 1;
+                    max_fields = u.nfields > max_fields ? u.nfields : max_fields;
+                } else {
+                    u.blend = 0;
+                }
             }
             units.push_back(u);
         }
@@ -683,7 +693,6 @@ lcs_status cart_advect_impl(lcs_field *f, int64_t n, const void *seeds_, double 
     const size_t o_cnt = off; if (do_bundle) off = align_up(off + (size_t)nbins * 4);
     const size_t o_tile = off; if (do_bundle) off = align_up(off + (size_t)ntiles * 4);
     const size_t o_ftau = off; off = align_up(off + ftau.size() * 4 + 4);
-    const size_t o_fidx = off; if (max_fields) off = align_up(off + fidx.size() * 4);
     const size_t o_fields = off; off = align_up(off + (size_t)max_fields * (size_t)f->nrec * 32);
     rc = lcs_scratch_reserve(f, off);
     if (rc != LCS_OK) return rc;
@@ -692,11 +701,9 @@ lcs_status cart_advect_impl(lcs_field *f, int64_t n, const void *seeds_, double 
     TC *d_xi = (TC *)(base + o_xi), *d_acc = (TC *)(base + o_acc), *d_tau = (TC *)(base + o_tau);
     uint32_t *d_key = (uint32_t *)(base + o_key), *d_cnt = (uint32_t *)(base + o_cnt), *d_tile = (uint32_t *)(base + o_tile);
     float *d_ftau = (float *)(base + o_ftau);
-    int *d_fidx = (int *)(base + o_fidx);
     LCS_CUDA_OK(cudaMemcpyAsync(d_tau, tau.data(), tau.size() * sizeof(TC), cudaMemcpyHostToDevice, st));
     if (max_fields) {
         LCS_CUDA_OK(cudaMemcpyAsync(d_ftau, ftau.data(), ftau.size() * 4, cudaMemcpyHostToDevice, st));
-        LCS_CUDA_OK(cudaMemcpyAsync(d_fidx, fidx.data(), fidx.size() * 4, cudaMemcpyHostToDevice, st));
     }
 
     CartDev g = make_dev(f);
@@ -731,10 +738,14 @@ lcs_status cart_advect_impl(lcs_field *f, int64_t n, const void *seeds_, double 
         const StepWindow &w = windows[u.win];
         const bool new_win = u.win != cur_win;
         if (new_win) {
-            if (u.blend) {
+            // what the units of this window gather from: raw snapshots (blended chunks) and / or pair records
+            bool need_raw = false, need_pairs = false;
+            for (size_t uj = ui; uj < units.size() && units[uj].win == u.win; ++uj) (units[uj].blend ? need_raw : need_pairs) = true;
+            if (need_raw) {
                 rc = lcs_field_acquire_raw(f, w.s[0], st, &raw_a, &raw_b);
                 if (rc != LCS_OK) return rc;
-            } else {
+            }
+            if (need_pairs) {
                 for (int k = 0; k < 3; ++k) {
                     rc = lcs_field_require_pair(f, w.s[k], st, &p[k]);
                     if (rc != LCS_OK) return rc;
@@ -760,13 +771,14 @@ lcs_status cart_advect_impl(lcs_field *f, int64_t n, const void *seeds_, double 
                     WindowTimer timer(f, st);
                     if (fast)
                         LCS_LAUNCH((cart_xpair_kernel<true>), lcs_blocks(n, block), block, 0, st, g, (const XPair *)fields, f->nrec,
-                                   d_fidx + 3 * (size_t)u.first, u.count, u.first, n, cur, hs[0], hs[1], hs[2]);
+                                   u.count, u.first, n, cur, hs[0], hs[1], hs[2]);
                     else
                         LCS_LAUNCH((cart_xpair_kernel<false>), lcs_blocks(n, block), block, 0, st, g, (const XPair *)fields, f->nrec,
-                                   d_fidx + 3 * (size_t)u.first, u.count, u.first, n, cur, hs[0], hs[1], hs[2]);
+                                   u.count, u.first, n, cur, hs[0], hs[1], hs[2]);
                 }
-                const bool last_of_win = ui + 1 == units.size() || units[ui + 1].win != u.win;
-                if (last_of_win) { rc = lcs_field_release_raw(f, w.s[0], st); if (rc != LCS_OK) return rc; }
+                bool last_blend_of_win = true;
+                for (size_t uj = ui + 1; uj < units.size() && units[uj].win == u.win; ++uj) last_blend_of_win = last_blend_of_win && !units[uj].blend;
+                if (last_blend_of_win) { rc = lcs_field_release_raw(f, w.s[0], st); if (rc != LCS_OK) return rc; }
                 rc = early_eval((int64_t)u.first + u.count);
                 if (rc != LCS_OK) return rc;
                 continue;
