@@ -327,12 +327,12 @@ cart_window_kernel(const __grid_constant__ CartDev g, const PairRec<DIM, TV> *__
 // Pre-blended variant (3D, fp32): the time blend u(node, t) = a + tau (b - a) does not depend on the tracer, and the
 // integrator is bound by the bytes the L1 delivers into registers (128 B per cycle per SM), so the blend is hoisted
 // out of the gather: for a chunk of k RK4 steps the 2k+1 distinct stage times are blended once per node into
-// "x-pair" records {u(i0,i1,i2), u(i0+1,i1,i2)} (2 x float4 = one 32-byte sector, one 256-bit load), and a stage
+// "x-pair" records {u(i0,i1,i2), u(i0+1,i1,i2) - u(i0,i1,i2)} (2 x float4 = one 32-byte sector, one 256-bit load), and a stage
 // gathers 4 records = 128 B per tracer instead of 8 pair records = 256 B.  The arithmetic per tracer is unchanged
 // (fma(tau, b - a, a) per node, then the nested lerps), so results are bit-identical to the pair-record path.
 struct alignas(32) XPair {
-    float lo[4];
-    float hi[4];
+    float lo[4];           // u(i0, i1, i2) at the field's stage time
+    float hi[4];           // u(i0+1, i1, i2) - u(i0, i1, i2): the x-lerp is one FMA
 };
 
 constexpr int kMaxBlendFields = 2 * 256 + 1;
@@ -362,7 +362,7 @@ __global__ void __launch_bounds__(256) blend_xpair_kernel(const float *__restric
         const float t = __ldg(tau + f);
         float4 lo, hi;
         lo.x = fmaf(t, vd[0], va[0]); lo.y = fmaf(t, vd[1], va[1]); lo.z = fmaf(t, vd[2], va[2]); lo.w = 0.f;
-        hi.x = fmaf(t, vd[3], va[3]); hi.y = fmaf(t, vd[4], va[4]); hi.z = fmaf(t, vd[5], va[5]); hi.w = 0.f;
+        hi.x = fmaf(t, vd[3], va[3]) - lo.x; hi.y = fmaf(t, vd[4], va[4]) - lo.y; hi.z = fmaf(t, vd[5], va[5]) - lo.z; hi.w = 0.f;
         // one 256-bit streaming store: a whole 32-byte sector per lane
         asm volatile("st.global.cs.v8.f32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(fields + (int64_t)f * field_stride + i), "f"(lo.x),
                      "f"(lo.y), "f"(lo.z), "f"(lo.w), "f"(hi.x), "f"(hi.y), "f"(hi.z), "f"(hi.w)
@@ -425,10 +425,10 @@ __device__ __forceinline__ bool cart_velocity_xpair(const CartDev &g, const XPai
     }
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-        float a00 = fmaf(wl[0], hc.v[1][c] - hc.v[0][c], hc.v[0][c]);
-        float a10 = fmaf(wl[0], hc.v[3][c] - hc.v[2][c], hc.v[2][c]);
-        float a01 = fmaf(wl[0], hc.v[5][c] - hc.v[4][c], hc.v[4][c]);
-        float a11 = fmaf(wl[0], hc.v[7][c] - hc.v[6][c], hc.v[6][c]);
+        float a00 = fmaf(wl[0], hc.v[1][c], hc.v[0][c]);       // v[odd] holds the x-difference rounded in fp32 by the blend kernel
+        float a10 = fmaf(wl[0], hc.v[3][c], hc.v[2][c]);
+        float a01 = fmaf(wl[0], hc.v[5][c], hc.v[4][c]);
+        float a11 = fmaf(wl[0], hc.v[7][c], hc.v[6][c]);
         float b0 = fmaf(wl[1], a10 - a00, a00);
         float b1 = fmaf(wl[1], a11 - a01, a01);
         u[c] = fmaf(wl[2], b1 - b0, b0);
