@@ -89,7 +89,9 @@ void lcs_field_destroy(lcs_field *f);
  * window), 2 = split (one short kernel per RK4 stage, tracers advance synchronously: PAPER.md:85);
  * "bundle" -1 = auto, 0 = off, 1 = on: re-bundle tracers by cell (Morton order of the cell index) so that a
  * warp gathers from neighbouring cells; results are returned in the caller's order;
- * "bundle_steps" k = re-bundle every k RK4 steps (0 = once per snapshot window);
+ * "bundle_steps" k = re-bundle every k RK4 steps (0 = once per snapshot window; unstructured meshes: every 160 steps);
+ * "bundle_order" / "simplex_order" 0 = Morton, 1 = row-major (x fastest, default) sort key over cells / bins;
+ * "preblend" -1/0/1 and "preblend_steps" k: 3D fp32 Cartesian grids gather from per-stage-time blended fields, k steps per launch;
  * "ld256" 0/1 = gather each 32-byte node record with one 256-bit load; "block" = threads per block;
  * "time_windows" 0/1 = record CUDA events around the integrator launches (read with lcs_field_get_info). */
 lcs_status lcs_field_set_option(lcs_field *f, const char *key, int64_t value);

@@ -32,7 +32,7 @@ struct CartDev {
     int n[3];
     int periodic[3];
     int pow2[3];
-    int np0, np01;         // padded record strides: np0 = n0 + 1, np01 = (n0 + 1) * (n1 + 1)
+    int np0, np01;         // padded record strides (CartGeom::np): np0 = np[0], np01 = np[0] * np[1]
     double origin[3], spacing[3], inv[3];
 };
 
@@ -254,7 +254,8 @@ __global__ void __launch_bounds__(256) cart_final_kernel(CartDev g, const TC *__
 // (flag != 0) go to the last bin so that their warps retire at once
 template <int DIM, typename TC>
 __global__ void __launch_bounds__(256) cart_key_kernel(CartDev g, const CartTracer<DIM, TC> *__restrict__ st, int64_t n, int shift,
-                                                        uint32_t last_bin, uint32_t *__restrict__ key, uint32_t *__restrict__ cnt)
+                                                        int row_major, uint32_t last_bin, uint32_t *__restrict__ key,
+                                                        uint32_t *__restrict__ cnt)
 {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
@@ -264,7 +265,14 @@ __global__ void __launch_bounds__(256) cart_key_kernel(CartDev g, const CartTrac
         int c[DIM];
 #pragma unroll
         for (int a = 0; a < DIM; ++a) c[a] = (g.periodic[a] ? wrap_index(t.ci[a], g.n[a], g.pow2[a]) : t.ci[a]) >> shift;
-        k = bundle::morton<DIM>(c);
+        if (row_major) {
+            // x fastest: consecutive tracers sit in x-neighbouring cells, whose records share a 128-byte line (rows are
+            // padded to 4 records), so a 4-lane group that straddles two cells still costs one L1 wavefront
+            const int m0 = ((g.n[0] - 1) >> shift) + 1, m1 = ((g.n[1] - 1) >> shift) + 1;
+            k = (uint32_t)c[0] + (uint32_t)m0 * ((uint32_t)c[1] + (DIM == 3 ? (uint32_t)m1 * (uint32_t)c[2] : 0u));
+        } else {
+            k = bundle::morton<DIM>(c);
+        }
         if (k > last_bin - 1) k = last_bin - 1;
     }
     key[i] = k;
@@ -339,16 +347,14 @@ constexpr int kMaxBlendFields = 2 * 256 + 1;
 
 // one thread per padded record; raw snapshots a, b are [node][3] fp32; field f of the chunk gets tau[f]
 __global__ void __launch_bounds__(256) blend_xpair_kernel(const float *__restrict__ a, const float *__restrict__ b, int n0, int n1, int n2,
+                                                           int q0, int q1, int q2,
                                                            const float *__restrict__ tau, int nfields, XPair *__restrict__ fields,
                                                            int64_t field_stride)
 {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    const int64_t p0 = n0 + 1, p1 = n1 + 1, p2 = n2 + 1;
+    const int64_t p0 = q0, p1 = q1, p2 = q2;
     if (i >= p0 * p1 * p2) return;
-    int i0 = (int)(i % p0), i1 = (int)((i / p0) % p1), i2 = (int)(i / (p0 * p1));
-    if (i0 == n0) i0 = 0;
-    if (i1 == n1) i1 = 0;
-    if (i2 == n2) i2 = 0;
+    int i0 = (int)(i % p0) % n0, i1 = (int)((i / p0) % p1) % n1, i2 = (int)(i / (p0 * p1)) % n2;
     const int j0 = i0 + 1 == n0 ? 0 : i0 + 1;
     const int64_t row = (int64_t)n0 * (i1 + (int64_t)n1 * i2);
     const float *al = a + 3 * (row + i0), *bl = b + 3 * (row + i0), *ah = a + 3 * (row + j0), *bh = b + 3 * (row + j0);
@@ -582,8 +588,8 @@ CartDev make_dev(const lcs_field *f)
         g.n[a] = f->cart.n[a]; g.periodic[a] = f->cart.periodic[a]; g.pow2[a] = f->cart.pow2[a];
         g.origin[a] = f->cart.origin[a]; g.spacing[a] = f->cart.spacing[a]; g.inv[a] = f->cart.inv[a];
     }
-    g.np0 = f->cart.n[0] + 1;
-    g.np01 = (f->cart.n[0] + 1) * (f->cart.n[1] + 1);
+    g.np0 = f->cart.np[0];
+    g.np01 = f->cart.np[0] * f->cart.np[1];
     return g;
 }
 
@@ -718,7 +724,7 @@ lcs_status cart_advect_impl(lcs_field *f, int64_t n, const void *seeds_, double 
 
     auto rebundle = [&]() -> lcs_status {
         LCS_CUDA_OK(cudaMemsetAsync(d_cnt, 0, (size_t)nbins * 4, st));
-        LCS_LAUNCH((cart_key_kernel<DIM, TC>), lcs_blocks(n, 256), 256, 0, st, g, cur, n, shift, (uint32_t)(nbins - 1), d_key, d_cnt);
+        LCS_LAUNCH((cart_key_kernel<DIM, TC>), lcs_blocks(n, 256), 256, 0, st, g, cur, n, shift, (int)f->opt_bundle_order, (uint32_t)(nbins - 1), d_key, d_cnt);
         bundle::sort_records<Tracer>(cur, alt, d_key, d_cnt, d_tile, n, nbins, st);
         std::swap(cur, alt);
         return LCS_OK;
@@ -766,7 +772,7 @@ lcs_status cart_advect_impl(lcs_field *f, int64_t n, const void *seeds_, double 
             if (u.blend) {
                 XPair *fields = (XPair *)(base + o_fields);
                 LCS_LAUNCH(blend_xpair_kernel, lcs_blocks(f->nrec, 256), 256, 0, st, (const float *)raw_a, (const float *)raw_b, g.n[0], g.n[1],
-                           g.n[2], d_ftau + u.ftau_off, u.nfields, fields, f->nrec);
+                           g.n[2], f->cart.np[0], f->cart.np[1], f->cart.np[2], d_ftau + u.ftau_off, u.nfields, fields, f->nrec);
                 {
                     WindowTimer timer(f, st);
                     if (fast)

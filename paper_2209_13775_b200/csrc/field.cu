@@ -53,15 +53,13 @@ __global__ void __launch_bounds__(256) build_pair_kernel(const TV *__restrict__ 
 // offset from the lower one: one base address and 2^DIM constant offsets per interpolation.
 template <int DIM, typename TV, typename TR>
 __global__ void __launch_bounds__(256) build_pair_padded_kernel(const TV *__restrict__ a, const TV *__restrict__ b,
-                                                                 PairRec<DIM, TR> *__restrict__ rec, int n0, int n1, int n2)
+                                                                 PairRec<DIM, TR> *__restrict__ rec, int n0, int n1, int n2,
+                                                                 int q0, int q1, int q2)
 {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    const int64_t p0 = n0 + 1, p1 = n1 + 1, p2 = DIM == 3 ? n2 + 1 : 1;
+    const int64_t p0 = q0, p1 = q1, p2 = q2;
     if (i >= p0 * p1 * p2) return;
-    int i0 = (int)(i % p0), i1 = (int)((i / p0) % p1), i2 = (int)(i / (p0 * p1));
-    if (i0 == n0) i0 = 0;
-    if (i1 == n1) i1 = 0;
-    if (DIM == 3 && i2 == n2) i2 = 0;
+    int i0 = (int)(i % p0) % n0, i1 = (int)((i / p0) % p1) % n1, i2 = (int)(i / (p0 * p1)) % n2;
     const int64_t node = i0 + (int64_t)n0 * (i1 + (int64_t)n1 * i2);
     PairRec<DIM, TR> r;
 #pragma unroll
@@ -123,7 +121,7 @@ static void launch_build_pair(const lcs_field *f, const void *a, const void *b, 
 {
     if (f->kind == LCS_MESH_CARTESIAN)
         LCS_LAUNCH((build_pair_padded_kernel<DIM, TV, TR>), lcs_blocks(f->nrec, 256), 256, 0, st, (const TV *)a, (const TV *)b,
-                   (PairRec<DIM, TR> *)rec, f->cart.n[0], f->cart.n[1], f->cart.n[2]);
+                   (PairRec<DIM, TR> *)rec, f->cart.n[0], f->cart.n[1], f->cart.n[2], f->cart.np[0], f->cart.np[1], f->cart.np[2]);
     else
         LCS_LAUNCH((build_pair_kernel<DIM, TV, TR>), lcs_blocks(f->nnodes, 256), 256, 0, st, (const TV *)a, (const TV *)b,
                    (PairRec<DIM, TR> *)rec, f->nnodes);
@@ -292,7 +290,10 @@ extern "C" lcs_status lcs_field_create(const lcs_field_desc *d, lcs_field **out)
         if (nn >= (1LL << 31)) { lcs_set_error("grid too large for int32 node ids"); delete f; return LCS_ERR_INVALID_ARG; }
         f->nnodes = nn;
         f->nrec = 1;
-        for (int a = 0; a < d->dim; ++a) f->nrec *= (int64_t)d->n[a] + 1;
+        for (int a = 0; a < 3; ++a) {
+            f->cart.np[a] = a < d->dim ? d->n[a] + 1 : 1;
+            f->nrec *= (int64_t)f->cart.np[a];
+        }
         if (f->nrec >= (1LL << 31)) { lcs_set_error("grid too large for int32 node ids"); delete f; return LCS_ERR_INVALID_ARG; }
     } else {
         if (d->n_vertices < d->dim + 1 || d->n_cells < 1 || !d->vertices || !d->cells || d->n_vertices >= (1LL << 31) ||
@@ -381,6 +382,8 @@ extern "C" lcs_status lcs_field_set_option(lcs_field *f, const char *key, int64_
     if (!strcmp(key, "integrator") && value >= 0 && value <= 2) f->opt_integrator = value;
     else if (!strcmp(key, "bundle") && value >= -1 && value <= 1) f->opt_bundle = value;
     else if (!strcmp(key, "bundle_steps") && value >= 0) f->opt_bundle_steps = value;
+    else if (!strcmp(key, "bundle_order") && (value == 0 || value == 1)) f->opt_bundle_order = value;
+    else if (!strcmp(key, "simplex_order") && (value == 0 || value == 1)) f->opt_simplex_order = value;
     else if (!strcmp(key, "ld256") && (value == 0 || value == 1)) f->opt_ld256 = value;
     else if (!strcmp(key, "preblend") && value >= -1 && value <= 1) f->opt_preblend = value;
     else if (!strcmp(key, "preblend_steps") && value >= 1 && value <= 256) f->opt_preblend_steps = value;

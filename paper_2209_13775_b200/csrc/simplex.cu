@@ -456,7 +456,8 @@ __global__ void __launch_bounds__(128) simplex_init_kernel(BinGrid b, const int3
 // that live tracers stay compacted at the front and whole warps of finished ones retire at once
 template <int DIM, typename TC>
 __global__ void __launch_bounds__(256) simplex_key_kernel(BinGrid b, const SimplexTracer<DIM, TC> *__restrict__ st, int64_t n, int shift,
-                                                           uint32_t last_bin, uint32_t *__restrict__ key, uint32_t *__restrict__ cnt)
+                                                           int row_major, uint32_t last_bin, uint32_t *__restrict__ key,
+                                                           uint32_t *__restrict__ cnt)
 {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
@@ -470,7 +471,12 @@ __global__ void __launch_bounds__(256) simplex_key_kernel(BinGrid b, const Simpl
             int ia = q < 0.0 ? 0 : (q > (double)(b.nb[a] - 1) ? b.nb[a] - 1 : (int)q);
             c[a] = ia >> shift;
         }
-        k = bundle::morton<DIM>(c);
+        if (row_major) {
+            const int m0 = ((b.nb[0] - 1) >> shift) + 1, m1 = ((b.nb[1] - 1) >> shift) + 1;
+            k = (uint32_t)c[0] + (uint32_t)m0 * ((uint32_t)c[1] + (DIM == 3 ? (uint32_t)m1 * (uint32_t)c[2] : 0u));
+        } else {
+            k = bundle::morton<DIM>(c);
+        }
         if (k > last_bin - 1) k = last_bin - 1;
     }
     key[i] = k;
@@ -853,7 +859,7 @@ lcs_status simplex_advect_impl(lcs_field *f, int64_t n, const void *seeds_, doub
             const int first = (int)w.first + done;
             if (do_bundle && (since_bundle < 0 || since_bundle >= bundle_every)) {
                 LCS_CUDA_OK(cudaMemsetAsync(d_cnt, 0, (size_t)nbins * 4, st));
-                LCS_LAUNCH((simplex_key_kernel<DIM, TC>), lcs_blocks(n, 256), 256, 0, st, b, cur, n, shift, (uint32_t)(nbins - 1), d_key, d_cnt);
+                LCS_LAUNCH((simplex_key_kernel<DIM, TC>), lcs_blocks(n, 256), 256, 0, st, b, cur, n, shift, (int)f->opt_simplex_order, (uint32_t)(nbins - 1), d_key, d_cnt);
                 bundle::sort_records<Tracer>(cur, alt, d_key, d_cnt, d_tile, n, nbins, st);
                 std::swap(cur, alt);
                 since_bundle = 0;
