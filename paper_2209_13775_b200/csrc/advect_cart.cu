@@ -633,7 +633,7 @@ lcs_status cart_advect_impl(lcs_field *f, int64_t n, const void *seeds_, double 
     for (size_t k = 0; k < tau.size(); ++k) tau[k] = (TC)tau64[k];
 
     const bool split = f->opt_integrator == 2;
-    const bool do_bundle = f->opt_bundle == 1 || (f->opt_bundle < 0 && n >= (1 << 20));
+    const bool do_bundle = f->opt_bundle == 1 || (f->opt_bundle < 0 && n >= (1 << 18));
     // sort bins: Morton code of the cell index, coarsened so that the histogram stays <= 2^24 bins
     int shift = 0, bits = 0;
     for (;; ++shift) {

@@ -807,7 +807,7 @@ lcs_status simplex_advect_impl(lcs_field *f, int64_t n, const void *seeds_, doub
     for (size_t k = 0; k < tau.size(); ++k) tau[k] = (TC)tau64[k];
 
     // re-bundling by bin (Morton order of the coarsened bin grid), histogram <= 2^24 bins
-    const bool do_bundle = f->opt_bundle == 1 || (f->opt_bundle < 0 && n >= (1 << 20));
+    const bool do_bundle = f->opt_bundle == 1 || (f->opt_bundle < 0 && n >= (1 << 18));
     int shift = 0, bits = 0;
     for (;; ++shift) {
         bits = 0;
