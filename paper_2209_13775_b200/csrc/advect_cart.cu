@@ -16,9 +16,11 @@
 //  * gathers read "pair records" {a, b-a}: both time levels of a node in one 32-byte sector (one 256-bit
 //    load), the time blend is one FMA per component.  The record array is padded by one node per axis so
 //    that the 2^d corners of a cell sit at constant offsets from one base address.
-//  * tracers are re-bundled by cell (Morton order) once per snapshot window, so that the 32 tracers of a
-//    warp gather from 2x2x1 neighbouring cells: the kernel is bound by L1 wavefronts, and a wavefront
-//    serves one 128-byte line per instruction (profiles/r1_cfg3_baseline.md).
+//  * tracers are re-bundled by cell once per snapshot window, in row-major cell order (x fastest; Morton order is the
+//    other option): the kernel is bound by L1 wavefronts, a load costs one wavefront per distinct 128-byte line that
+//    each group of 4 lanes touches, and x-neighbouring cells share a line (profiles/r1_cfg3_baseline.md).
+//  * 3D fp32: the time blend is hoisted out of the gather into per-stage-time "x-pair" fields and the corners of the
+//    last gathered cell stay in registers (cart_xpair_kernel below).
 //  * fused variant: one thread runs every RK4 step of a snapshot window; split variant (the paper's): one
 //    short kernel per RK4 stage with the stage state in global memory.
 #include <math.h>

@@ -3,8 +3,9 @@
 //
 // Why: the paper notes that tracers "disperse" so that sorting the velocity data gave no gain
 // and cites re-bundling of tracers for coherence (ref [6]).  On B200 the integrator is bound by
-// L1 wavefronts (one 128-byte line per cycle per SM): a warp whose 32 tracers sit in 2x2x1 neighbouring
-// cells touches 2-4 lines per gather instruction, a warp of dispersed tracers touches up to 32.  Tracer
+// L1 wavefronts (one 128-byte line per cycle per SM): a 256-bit gather costs one wavefront per distinct line that each
+// group of 4 lanes touches -- 8 per warp when neighbouring lanes sit in the same or x-neighbouring cells, up to 32 when
+// the tracers of a warp are dispersed.  Tracer
 // results do not depend on the order (every tracer is independent), so the scatter may place
 // equal keys in any order (atomic slot allocation).
 #pragma once
