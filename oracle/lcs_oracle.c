@@ -644,6 +644,43 @@ void orc_cg_ftle_aux(int32_t dim, int64_t n, const double *delta, const double *
     }
 }
 
+/* ---- O11 (row f4, first part): Gaussian smoothing of the FTLE field ------------------------------------------
+ * The LCS filter smooths the FTLE field with a Gaussian before extracting ridges; no parameters given.
+ * Reading (#30): one normalised 1D convolution per axis, axis 0 first, on the structured seed grid:
+ *   out(i) = sum_k w_k f(i+k) / sum_k w_k over |k| <= R = ceil(3 sigma) with f(i+k) finite and inside the grid
+ *   (index wrapped on a periodic axis), w_k = exp(-k^2 / (2 sigma^2)), sigma in seed-grid cells;
+ * a NaN centre stays NaN (undefined seeds are not filled in), NaN neighbours are skipped.  fp64 throughout.       */
+void orc_smooth_gaussian(int32_t dim, const int32_t *ng, const int32_t *sper, double sigma, const double *in, double *out)
+{
+    int64_t n[3] = {ng[0], ng[1], dim == 3 ? ng[2] : 1};
+    int64_t total = n[0] * n[1] * n[2], stride[3] = {1, n[0], n[0] * n[1]};
+    int R = (int)ceil(3.0 * sigma);
+    double *a = (double *)malloc(sizeof(double) * (size_t)total), *b = (double *)malloc(sizeof(double) * (size_t)total);
+    memcpy(a, in, sizeof(double) * (size_t)total);
+    for (int ax = 0; ax < dim; ++ax) {
+#pragma omp parallel for schedule(static)
+        for (int64_t idx = 0; idx < total; ++idx) {
+            int64_t i = (idx / stride[ax]) % n[ax];
+            if (!isfinite(a[idx])) { b[idx] = a[idx]; continue; }
+            double num = 0.0, den = 0.0;
+            for (int k = -R; k <= R; ++k) {
+                int64_t j = i + k;
+                if (sper[ax]) j = ((j % n[ax]) + n[ax]) % n[ax];
+                else if (j < 0 || j >= n[ax]) continue;
+                double v = a[idx + (j - i) * stride[ax]];
+                if (!isfinite(v)) continue;
+                double w = exp(-(double)(k * k) / (2.0 * sigma * sigma));
+                num += w * v;
+                den += w;
+            }
+            b[idx] = num / den;
+        }
+        double *t = a; a = b; b = t;
+    }
+    memcpy(out, a, sizeof(double) * (size_t)total);
+    free(a); free(b);
+}
+
 int orc_max_threads(void)
 {
 #ifdef _OPENMP

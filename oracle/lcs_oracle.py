@@ -263,6 +263,16 @@ def cg_ftle_aux(dim, delta, flow_aux, flag_aux, T):
     return cg, ftle, status
 
 
+def smooth_gaussian(dim, ng, seed_periodic, sigma, field):
+    """Rule O11: NaN-aware normalised Gaussian smoothing of a scalar field on the seed grid, one pass per axis."""
+    f = np.ascontiguousarray(field, dtype=np.float64).ravel()
+    ng_ = np.asarray(list(ng) + [1] * (3 - len(ng)), dtype=np.int32)
+    sp = np.asarray(list(seed_periodic) + [0] * (3 - len(seed_periodic)), dtype=np.int32)
+    out = np.empty_like(f)
+    lib().orc_smooth_gaussian(C.c_int32(dim), _p(ng_), _p(sp), C.c_double(sigma), _p(f), _p(out))
+    return out
+
+
 def cg_eigen(dim, cg):
     """All eigenvalues (ascending) and unit eigenvectors (row i belongs to eigenvalue i) of C: rule O8."""
     c = np.ascontiguousarray(cg, dtype=np.float64)

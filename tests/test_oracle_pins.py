@@ -715,3 +715,35 @@ def test_P17_early_cg(oracle):
     ok = te > 0
     assert (fl == 1).sum() > 10 and len(np.unique(te[ok])) >= 3
     assert np.max(np.abs(ft[ok] - 0.999999233219801983)) <= 1e-9
+
+
+# -------------------------------------------------------------------------------------------------
+# O11 (row f4, first part): Gaussian smoothing of the FTLE field
+def test_P18_gaussian_smoothing(oracle):
+    """Pins for O11: equal to scipy.ndimage.gaussian_filter1d (mode wrap, truncate 3) applied axis by axis on periodic grids;
+    constants are fixed points; the sum is conserved on periodic grids; a linear ramp is reproduced in the interior of a
+    non-periodic grid; NaN centres stay NaN and NaN neighbours are skipped with renormalisation; impulse response = weights."""
+    from scipy.ndimage import gaussian_filter1d
+    rng = np.random.default_rng(18)
+    f3 = rng.standard_normal((12, 10, 14))                                 # [z][y][x]
+    for sigma in (1.0, 2.0):
+        ref = f3
+        for ax in (2, 1, 0):                                              # axis 0 of the seed grid is the fastest (last) index
+            ref = gaussian_filter1d(ref, sigma, axis=ax, mode="wrap", truncate=3.0)
+        out = oracle.smooth_gaussian(3, (14, 10, 12), (1, 1, 1), sigma, f3).reshape(f3.shape)
+        assert np.max(np.abs(out - ref)) <= 1e-13
+        assert abs(out.sum() - f3.sum()) <= 1e-10
+    c = oracle.smooth_gaussian(2, (9, 7), (0, 1), 1.5, np.full(63, 3.25))
+    assert np.max(np.abs(c - 3.25)) <= 1e-15
+    ramp = np.tile(np.arange(40, dtype=np.float64), (6, 1))               # f = x on a 40 x 6 grid, non-periodic in x
+    out = oracle.smooth_gaussian(2, (40, 6), (0, 0), 2.0, ramp).reshape(6, 40)
+    assert np.max(np.abs(out[:, 6:-6] - ramp[:, 6:-6])) <= 1e-12 and out[0, 0] > 0.0     # one-sided average at the edge
+    imp = np.zeros(21); imp[10] = 1.0
+    out = oracle.smooth_gaussian(2, (21, 1), (0, 0), 1.0, imp)
+    w = np.exp(-np.arange(-3, 4) ** 2 / 2.0); w /= w.sum()
+    assert np.max(np.abs(out[7:14] - w)) <= 1e-15 and np.all(out[:7] == 0) and np.all(out[14:] == 0)
+    g = rng.standard_normal(30); g[11] = np.nan
+    out = oracle.smooth_gaussian(2, (30, 1), (1, 0), 1.0, g)
+    assert np.isnan(out[11]) and np.isfinite(np.delete(out, 11)).all()
+    k = np.arange(-3, 4); wk = np.exp(-k ** 2 / 2.0); vals = g[(12 + k) % 30]; ok = np.isfinite(vals)
+    assert abs(out[12] - (wk[ok] * vals[ok]).sum() / wk[ok].sum()) <= 1e-15
