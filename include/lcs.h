@@ -171,6 +171,14 @@ lcs_status lcs_cg_ftle_aux(int32_t dim, int32_t dtype, int64_t n, const double a
 lcs_status lcs_cg_eigen(int32_t dim, int32_t dtype, int64_t n, const void *cg, void *evals, void *evecs,
                         void *cuda_stream);
 
+/* Gaussian smoothing of a scalar field (the FTLE) on the structured seed grid, the first step of the LCS filter
+ * ("Gaussian smoothing of FTLE" before ridge extraction; reading #30).  One normalised 1D convolution
+ * per axis, axis 0 first: out(i) = sum_k w_k f(i+k) / sum_k w_k over |k| <= ceil(3 sigma) with f(i+k) finite and inside the grid
+ * (wrapped on a periodic axis), w_k = exp(-k^2 / (2 sigma^2)), sigma in seed-grid cells, 0 < sigma <= 21.33.  A NaN centre
+ * stays NaN; NaN neighbours are skipped.  field, out, work: three distinct device buffers of [n] `dtype` (work is scratch). */
+lcs_status lcs_smooth_gaussian(int32_t dim, int32_t dtype, const int32_t ng[3], const int32_t seed_periodic[3],
+                               double sigma, const void *field, void *out, void *work, void *cuda_stream);
+
 /* End-to-end convenience with HOST buffers: copies the seeds to the device, runs lcs_advect and
  * lcs_cg_ftle and copies flow map (optional), flags (optional) and FTLE back; synchronous.
  * seeds_host/flowmap_host: [n][dim] of the field's compute_dtype; ftle_host: [n] of compute_dtype.

@@ -188,6 +188,37 @@ __global__ void __launch_bounds__(256) cg_ftle_aux_kernel(const T *__restrict__ 
 }
 
 // ---------------------------------------------------------------------------------------------
+// Row f4 (first part): Gaussian smoothing of the FTLE field before ridge extraction, reading #30.
+// One normalised 1D convolution per axis (radius ceil(3 sigma) <= 64, weights in shared memory), NaN centres kept, NaN and
+// out-of-grid neighbours skipped with renormalisation, fp64 accumulation.  HBM streaming: one read + one write per pass;
+// the 2R+1 taps of neighbouring threads hit L1 / L2.
+template <typename T>
+__global__ void __launch_bounds__(256) smooth_axis_kernel(const T *__restrict__ in, T *__restrict__ out, int64_t total, int64_t stride,
+                                                           int64_t len, int periodic, int R, double inv_2s2)
+{
+    __shared__ double w[65];
+    for (int k = threadIdx.x; k <= R; k += blockDim.x) w[k] = exp(-(double)(k * k) * inv_2s2);
+    __syncthreads();
+    const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= total) return;
+    const T centre = in[idx];
+    if (!isfinite((double)centre)) { out[idx] = centre; return; }
+    const int64_t i = (idx / stride) % len;
+    double num = 0.0, den = 0.0;
+    for (int k = -R; k <= R; ++k) {
+        int64_t j = i + k;
+        if (periodic) { j %= len; if (j < 0) j += len; }
+        else if (j < 0 || j >= len) continue;
+        const double v = (double)in[idx + (j - i) * stride];
+        if (!isfinite(v)) continue;
+        const double wk = w[k < 0 ? -k : k];
+        num = fma(wk, v, num);
+        den += wk;
+    }
+    out[idx] = (T)(num / den);
+}
+
+// ---------------------------------------------------------------------------------------------
 // Row f2: all eigenvalues and eigenvectors of C ("eigenvalues and eigenvectors"; the
 // eigenvector fields are what hyperbolic-LCS criteria need).  One thread per seed, cyclic Jacobi in fp64 registers
 // (reading #27): the closed forms are ill-conditioned for the small eigenvalues.  Streams 12-24 B in and
@@ -398,4 +429,30 @@ extern "C" lcs_status lcs_advect_early_cg(lcs_field *f, const int32_t ng[3], con
     lcs_status rc = lcs_advect(f, n, seeds, t0, tf, h, flowmap, exit_flag, exit_step, cuda_stream);
     f->early = EarlyCg();
     return rc;
+}
+
+extern "C" lcs_status lcs_smooth_gaussian(int32_t dim, int32_t dtype, const int32_t ng[3], const int32_t seed_periodic[3], double sigma,
+                                          const void *field, void *out, void *work, void *cuda_stream)
+{
+    if ((dim != 2 && dim != 3) || !ng || !field || !out || !work) { lcs_set_error("null argument or bad dim"); return LCS_ERR_INVALID_ARG; }
+    if (dtype != LCS_F32 && dtype != LCS_F64) { lcs_set_error("bad dtype"); return LCS_ERR_INVALID_ARG; }
+    if (!(sigma > 0.0) || ceil(3.0 * sigma) > 64.0) { lcs_set_error("sigma must be in (0, 21.33] seed-grid cells"); return LCS_ERR_INVALID_ARG; }
+    if (out == field || work == field || work == out) { lcs_set_error("field, out and work must be distinct buffers"); return LCS_ERR_INVALID_ARG; }
+    int64_t n[3] = {1, 1, 1}, total = 1;
+    for (int a = 0; a < dim; ++a) { if (ng[a] < 1) { lcs_set_error("bad seed grid"); return LCS_ERR_INVALID_ARG; } n[a] = ng[a]; total *= n[a]; }
+    const int64_t stride[3] = {1, n[0], n[0] * n[1]};
+    const int R = (int)ceil(3.0 * sigma);
+    const double inv_2s2 = 1.0 / (2.0 * sigma * sigma);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    // dim passes ending in `out`: 2D: field -> work -> out; 3D: field -> out -> work -> out
+    const void *src = field;
+    for (int a = 0; a < dim; ++a) {
+        void *dst = ((dim - a) % 2 == 1) ? out : work;
+        const int per = seed_periodic ? (seed_periodic[a] != 0) : 0;
+        if (dtype == LCS_F64) LCS_LAUNCH((smooth_axis_kernel<double>), lcs_blocks(total, 256), 256, 0, st, (const double *)src, (double *)dst, total, stride[a], n[a], per, R, inv_2s2);
+        else LCS_LAUNCH((smooth_axis_kernel<float>), lcs_blocks(total, 256), 256, 0, st, (const float *)src, (float *)dst, total, stride[a], n[a], per, R, inv_2s2);
+        src = dst;
+    }
+    LCS_CUDA_OK(cudaGetLastError());
+    return LCS_OK;
 }

@@ -22,7 +22,7 @@ LCS_F32, LCS_F64 = 0, 1
 LCS_MESH_CARTESIAN, LCS_MESH_SIMPLEX = 0, 1
 
 EXPORTS = ["lcs_field_create", "lcs_field_set_snapshot", "lcs_field_sync", "lcs_field_destroy",
-           "lcs_field_set_option", "lcs_field_get_info", "lcs_locate", "lcs_advect", "lcs_advect_early_cg", "lcs_cg_ftle", "lcs_cg_ftle_aux", "lcs_cg_eigen",
+           "lcs_field_set_option", "lcs_field_get_info", "lcs_locate", "lcs_advect", "lcs_advect_early_cg", "lcs_cg_ftle", "lcs_cg_ftle_aux", "lcs_cg_eigen", "lcs_smooth_gaussian",
            "lcs_ftle_host", "lcs_kernel_launch_count", "lcs_last_error"]
 
 
@@ -73,6 +73,8 @@ def lib():
                                           C.c_void_p, C.c_void_p]
         L.lcs_cg_ftle_aux.argtypes = [C.c_int32, C.c_int32, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double,
                                       C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.lcs_smooth_gaussian.argtypes = [C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p,
+                                          C.c_void_p]
         L.lcs_cg_eigen.argtypes = [C.c_int32, C.c_int32, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.lcs_ftle_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                     C.c_double, C.c_double, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p]
@@ -294,3 +296,14 @@ def advect_early_cg(field, ng, seed_spacing, seed_periodic, period, seeds, t0, t
                                      _arr3(period, C.c_double, 0.0), _tptr(seeds), float(t0), float(tf), float(h), int(every), _tptr(F),
                                      _tptr(flag), _tptr(es), _tptr(cg), _tptr(ftle), _tptr(t_eff), _tptr(status), _stream_ptr(stream)))
     return F, flag, es, cg, ftle, t_eff, status
+
+
+def smooth_gaussian(dim, ng, seed_periodic, sigma, field, stream=None):
+    """lcs_smooth_gaussian on a torch CUDA tensor [n]; returns the smoothed field."""
+    import torch
+    assert field.is_cuda and field.is_contiguous()
+    dtype = LCS_F64 if field.dtype == torch.float64 else LCS_F32
+    out, work = torch.empty_like(field), torch.empty_like(field)
+    _check(lib().lcs_smooth_gaussian(int(dim), dtype, _arr3(ng, C.c_int32, 1), _arr3(seed_periodic, C.c_int32, 0), float(sigma),
+                                     _tptr(field), _tptr(out), _tptr(work), _stream_ptr(stream)))
+    return out

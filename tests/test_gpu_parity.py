@@ -731,3 +731,33 @@ def test_advect_early_cg_arguments(lcs):
     torch.cuda.synchronize()
     assert torch.equal(out[0], F0) and torch.equal(out[4], ft0) and torch.equal(out[3], cg0) and torch.equal(out[6], st0)
     assert float(out[5].min()) == w.tf - w.t0
+
+
+# -------------------------------------------------------------------------------------------------
+# row f4 (first part): Gaussian smoothing of the FTLE field
+@pytest.mark.parametrize("dt", [np.float64, np.float32])
+def test_smooth_gaussian_vs_oracle(lcs, oracle, dt):
+    """lcs_smooth_gaussian against oracle rule O11 on (i) the FTLE field of config 1 reduced with undefined (NaN) seeds punched
+    in, non-periodic 2D, and (ii) the FTLE field of config 3 reduced, periodic 3D; ragged sizes, two sigmas."""
+    import torch
+    tol = 1e-13 if dt == np.float64 else 2e-6
+    w = I.config1(ng=(70, 37), T=4.0)
+    f, sd, F, flag, es = gpu_run(w)
+    flag = flag.clone(); flag[::53] = 1
+    _, ft, _ = gpu_cg(w, F, flag)
+    w3 = I.config3(ngrid=22, nn=16, T=1.0, n_snap=4)
+    f3, sd3, F3, flag3, es3 = gpu_run(w3)
+    _, ft3, _ = gpu_cg(w3, F3, flag3)
+    for (dim, ng, per, field) in ((2, w.ng, w.seed_periodic, ft), (3, w3.ng, w3.seed_periodic, ft3)):
+        field = field.to(torch.float64 if dt == np.float64 else torch.float32).contiguous()
+        for sigma in (0.8, 2.5):
+            out = cpu(lcs.smooth_gaussian(dim, ng, per, sigma, field)).astype(np.float64)
+            ref = oracle.smooth_gaussian(dim, ng[:dim], per[:dim], sigma, cpu(field).astype(np.float64))
+            assert np.array_equal(np.isnan(out), np.isnan(ref))
+            ok = np.isfinite(ref)
+            assert ok.sum() > 1000 and np.max(np.abs(out[ok] - ref[ok])) <= tol * max(1.0, np.abs(ref[ok]).max())
+    assert np.isnan(cpu(ft)).sum() > 10
+    with pytest.raises(lcs.LcsError):
+        lcs.smooth_gaussian(2, w.ng, w.seed_periodic, 0.0, ft)
+    with pytest.raises(lcs.LcsError):
+        lcs.smooth_gaussian(2, w.ng, w.seed_periodic, 30.0, ft)
