@@ -361,7 +361,7 @@ def main():
                         "achieved": achieved, "peak": hbm_gbs, "unit": "GB/s", "frac": achieved / hbm_gbs, "peak_source": peak_src,
                         "note": "algorithmic gather bytes; small fields are served by L1/L2, so this can exceed the HBM copy peak "
                                 "(DESIGN.md section 6)", **common}
-        tr = os.path.join(ROOT, "profiles", "traffic_cfg%d.json" % args.config)
+        tr = os.path.join(ROOT, "profiles", "traffic_cfg%d.txt" % args.config)
         if os.path.exists(tr):
             roofline["traffic"] = json.load(open(tr)).get("dram_bytes_per_launch")
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
