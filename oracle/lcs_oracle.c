@@ -428,6 +428,59 @@ void orc_advect(const orc_field *f, int64_t npts, const double *seeds, double t0
     }
 }
 
+/* ---- O12 (row f4, second part): multi-step integrator ------------------------------------------------------
+ * The Flow Map filter can use "Runge-Kutta (single-step)" or "Adams-Bashforth (multi-step)" integrators;
+ * no order or start-up is given.  Reading (#31): 4-step Adams-Bashforth, started with three classical RK4
+ * steps (rule O4).  f_n = u(x_n, t_n), t_n = t0 + n h (by multiplication);
+ *   n >= 3:  x_{n+1} = x_n + (h / 24) (55 f_n - 59 f_{n-1} + 37 f_{n-2} - 9 f_{n-3}).
+ * One velocity evaluation per step after the start-up.  Exit: an evaluation point outside the domain => x keeps its
+ * start-of-step value, flag 1, exit_step n (as O4; an AB step can carry x_{n+1} itself outside, which the next step's
+ * evaluation then reports).  Same argument conventions as orc_advect.                                              */
+void orc_advect_ab4(const orc_field *f, int64_t npts, const double *seeds, double t0, double tf, double h,
+                    const int32_t *cell0, double *flowmap, uint8_t *flag, int32_t *exit_step)
+{
+    int d = f->dim;
+    int64_t N = llround((tf - t0) / h);
+    #pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t p = 0; p < npts; ++p) {
+        double x[3] = {0, 0, 0}, hist[3][3];             /* hist[0] = f_{n-1}, hist[1] = f_{n-2}, hist[2] = f_{n-3} */
+        for (int k = 0; k < d; ++k) x[k] = seeds[p * d + k];
+        int64_t cell = 0;
+        uint8_t fl = 0; int32_t es = (int32_t)N;
+        if (f->kind == 1) {
+            cell = cell0 ? cell0[p] : simplex_locate_brute1(f, x, NULL);
+            if (cell < 0) { fl = 2; es = 0; }
+        } else {
+            int64_t lo[3], hi[3]; double w[3];
+            if (!cart_locate(f, x, lo, hi, w)) { fl = 2; es = 0; }
+        }
+        for (int64_t n = 0; n < N && fl == 0; ++n) {
+            double ta = t0 + (double)n * h, tb = t0 + ((double)n + 0.5) * h, tc = t0 + ((double)n + 1.0) * h;
+            double k1[3], k2[3], k3[3], k4[3], y[3];
+            int64_t c = cell;
+            int ok = velocity(f, x, ta, &c, k1);            /* f_n */
+            if (ok && n < 3) {
+                for (int k = 0; k < d; ++k) y[k] = x[k] + (h / 2) * k1[k];
+                ok = velocity(f, y, tb, &c, k2);
+                if (ok) { for (int k = 0; k < d; ++k) y[k] = x[k] + (h / 2) * k2[k]; ok = velocity(f, y, tb, &c, k3); }
+                if (ok) { for (int k = 0; k < d; ++k) y[k] = x[k] + h * k3[k];       ok = velocity(f, y, tc, &c, k4); }
+            }
+            if (!ok) { fl = 1; es = (int32_t)n; break; }
+            if (n < 3) {
+                for (int k = 0; k < d; ++k) x[k] = x[k] + (h / 6) * (k1[k] + 2 * k2[k] + 2 * k3[k] + k4[k]);
+            } else {
+                for (int k = 0; k < d; ++k)
+                    x[k] = x[k] + (h / 24) * (55 * k1[k] - 59 * hist[0][k] + 37 * hist[1][k] - 9 * hist[2][k]);
+            }
+            for (int k = 0; k < d; ++k) { hist[2][k] = hist[1][k]; hist[1][k] = hist[0][k]; hist[0][k] = k1[k]; }
+            cell = c;
+        }
+        for (int k = 0; k < d; ++k) flowmap[p * d + k] = x[k];
+        if (flag) flag[p] = fl;
+        if (exit_step) exit_step[p] = es;
+    }
+}
+
 /* ------------------------------------------------------------------------------------------ */
 /* O7 largest eigenvalue of a symmetric matrix, closed form.
  * 2x2: lambda = (C11+C22)/2 + sqrt(((C11-C22)/2)^2 + C12^2).

@@ -182,6 +182,18 @@ class OracleField:
             return F, flag, es, traj
         return F, flag, es
 
+    def advect_ab4(self, seeds, t0, tf, h):
+        """Rule O12: 4-step Adams-Bashforth with an RK4 start-up."""
+        seeds = np.ascontiguousarray(seeds, dtype=np.float64)
+        n = seeds.shape[0]
+        cell0 = self.locate_walk(seeds) if self.kind == 1 else None
+        F = np.empty_like(seeds)
+        flag = np.empty(n, dtype=np.uint8)
+        es = np.empty(n, dtype=np.int32)
+        lib().orc_advect_ab4(C.byref(self._f), C.c_int64(n), _p(seeds), C.c_double(t0), C.c_double(tf), C.c_double(h), _p(cell0),
+                             _p(F), _p(flag), _p(es))
+        return F, flag, es
+
 
 def cg_ftle(dim, ng, seed_spacing, seed_periodic, period, flowmap, exit_flag, T):
     """Returns (cg [n][3|6], ftle [n], status [n])."""

@@ -747,3 +747,50 @@ def test_P18_gaussian_smoothing(oracle):
     assert np.isnan(out[11]) and np.isfinite(np.delete(out, 11)).all()
     k = np.arange(-3, 4); wk = np.exp(-k ** 2 / 2.0); vals = g[(12 + k) % 30]; ok = np.isfinite(vals)
     assert abs(out[12] - (wk[ok] * vals[ok]).sum() / wk[ok].sum()) <= 1e-15
+
+
+# -------------------------------------------------------------------------------------------------
+# O12 (row f4, second part): Adams-Bashforth 4 with RK4 start-up
+def test_P19_adams_bashforth(oracle):
+    """Pins for O12.  (a) u = a + b t (time-linear, uniform in space): AB4 integrates cubics in t exactly, RK4 too, and
+    linear time interpolation is exact with steps aligned to snapshots: x(T) = x0 + a T + b T^2 / 2.  (b) u = A x: the scheme
+    is the linear recurrence x_{n+1} = x_n + (h/24) A (55 x_n - 59 x_{n-1} + 37 x_{n-2} - 9 x_{n-3}) after three P(hA)
+    steps; the oracle must reproduce it to rounding.  (c) Fourth order: the error against exp(A T) x0 falls about 16x per
+    halving of h.  (d) Exit handling: flags 0/1/2 and frozen positions in an open box."""
+    a, b, T = np.array([0.3, -0.2]), np.array([0.05, 0.1]), 4.0
+    w = I.analytic_cartesian(2, I.time_linear_uniform(a, b), (9, 9), (-4.0, -4.0), (1.0, 1.0), np.arange(0.0, 5.0, 1.0), ng=(5, 4),
+                             seed_lo=(-1.0, -1.0), seed_spacing=(0.3, 0.3), t0=0.0, tf=T, h=0.25)
+    fo = oracle.OracleField.from_workload(w)
+    F, fl, es = fo.advect_ab4(w.seeds(), 0.0, T, 0.25)
+    assert np.all(fl == 0) and np.max(np.abs(F - (w.seeds() + a * T + b * T * T / 2))) <= 1e-13
+    A = np.array([[0.1, 0.7], [-0.6, -0.2]])
+    def run(h, N):
+        wl = I.analytic_cartesian(2, I.linear_flow(A), (81, 81), (-4.0, -4.0), (0.1, 0.1), (0.0, 8.0), ng=(3, 3), seed_lo=(-0.4, -0.3),
+                                  seed_spacing=(0.35, 0.3), t0=0.0, tf=h * N, h=h)
+        return wl, oracle.OracleField.from_workload(wl).advect_ab4(wl.seeds(), 0.0, h * N, h)
+    h, N = 0.05, 40
+    wl, (F, fl, es) = run(h, N)
+    hA = h * A
+    P = np.eye(2) + hA + hA @ hA / 2 + hA @ hA @ hA / 6 + hA @ hA @ hA @ hA / 24
+    xs = [wl.seeds().T]
+    for n in range(N):
+        if n < 3:
+            xs.append(P @ xs[-1])
+        else:
+            xs.append(xs[-1] + (h / 24) * (A @ (55 * xs[-1] - 59 * xs[-2] + 37 * xs[-3] - 9 * xs[-4])))
+    assert np.all(fl == 0) and np.max(np.abs(F - xs[-1].T)) <= 1e-13
+    from scipy.linalg import expm
+    errs = []
+    for h, N in ((0.1, 20), (0.05, 40), (0.025, 80)):
+        wl, (F, fl, es) = run(h, N)
+        errs.append(np.max(np.abs(F - (expm(A * 2.0) @ wl.seeds().T).T)))
+    assert 11 <= errs[0] / errs[1] <= 20 and 13 <= errs[1] / errs[2] <= 19
+    c = np.array([0.3, 0.13])
+    wb = I.analytic_cartesian(2, I.linear_flow(np.zeros((2, 2)), c), (5, 5), (0.0, 0.0), (1.0, 1.0), (0.0, 10.0), ng=(16, 16),
+                              seed_lo=(-0.5, -0.5), seed_spacing=(0.31, 0.31), t0=0.0, tf=5.0, h=0.25)
+    fb = oracle.OracleField.from_workload(wb)
+    F, fl, es = fb.advect_ab4(wb.seeds(), 0.0, 5.0, 0.25)
+    assert set(np.unique(fl)) == {0, 1, 2}
+    inside = fl != 2
+    assert np.max(np.abs(F[inside] - (wb.seeds()[inside] + np.outer(es[inside] * 0.25, c)))) <= 1e-12   # uniform flow: exact until the exit
+    assert np.array_equal(F[~inside], wb.seeds()[~inside]) and np.all(es[fl == 2] == 0) and np.all(es[fl == 0] == 20)
