@@ -86,7 +86,8 @@ lcs_status lcs_field_sync(lcs_field *f);
 void lcs_field_destroy(lcs_field *f);
 
 /* Integer options.  Keys: "integrator" 0 = auto, 1 = fused (one persistent per-seed loop per snapshot
- * window), 2 = split (one short kernel per RK4 stage, tracers advance synchronously: PAPER.md:85);
+ * window), 2 = split (one short kernel per RK4 stage, tracers advance synchronously: PAPER.md:85), 3 = 4-step
+ * Adams-Bashforth with three RK4 start-up steps ("Adams-Bashforth (multi-step)"; one velocity evaluation per step);
  * "bundle" -1 = auto, 0 = off, 1 = on: re-bundle tracers by cell (Morton order of the cell index) so that a
  * warp gathers from neighbouring cells; results are returned in the caller's order;
  * "bundle_steps" k = re-bundle every k RK4 steps (0 = once per snapshot window; unstructured meshes: every 160 steps);

@@ -501,6 +501,75 @@ cart_xpair_kernel(const __grid_constant__ CartDev g, const XPair *__restrict__ f
 }
 
 // ---------------------------------------------------------------------------------------------
+// Adams-Bashforth 4 with an RK4 start-up (row f4; "Adams-Bashforth (multi-step)"; reading #31): one
+// velocity evaluation per step once three RK4 steps have filled the history.  hist: [n][3][DIM] physical velocities
+// f_{n-1}, f_{n-2}, f_{n-3} of each tracer, carried across launches (tracers are not re-bundled in this mode).
+template <int DIM, typename TV, typename TC, bool FASTWRAP, bool LD256>
+__global__ void __launch_bounds__(256)
+cart_ab4_kernel(const __grid_constant__ CartDev g, const PairRec<DIM, TV> *__restrict__ pa, const PairRec<DIM, TV> *__restrict__ pb,
+                const PairRec<DIM, TV> *__restrict__ pc, const TC *__restrict__ tau, int nsteps, int first_step, int64_t n,
+                CartTracer<DIM, TC> *__restrict__ st, TC *__restrict__ hist, TC hs0, TC hs1, TC hs2)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    CartTracer<DIM, TC> t = load_record(st + i);
+    if ((t.meta >> 30) != 0) return;
+    const TC hs[3] = {hs0, hs1, hs2};
+    int ci[DIM];
+    TC w[DIM], h0[DIM], h1[DIM], h2[DIM];
+#pragma unroll
+    for (int a = 0; a < DIM; ++a) {
+        ci[a] = t.ci[a]; w[a] = t.w[a];
+        h0[a] = first_step > 0 ? hist[(i * 3 + 0) * DIM + a] : TC(0);
+        h1[a] = first_step > 0 ? hist[(i * 3 + 1) * DIM + a] : TC(0);
+        h2[a] = first_step > 0 ? hist[(i * 3 + 2) * DIM + a] : TC(0);
+    }
+    int s = 0;
+    bool ok = true;
+    for (; s < nsteps; ++s) {
+        const TC ta = __ldg(tau + 3 * s), tb = __ldg(tau + 3 * s + 1), tc = __ldg(tau + 3 * s + 2);
+        TC k1[DIM], inc[DIM];
+        ok = cart_velocity<DIM, TV, TC, FASTWRAP, LD256>(g, pa, ta, ci, w, k1);
+        if (!ok) break;
+        if (first_step + s < 3) {
+            TC k2[DIM], k3[DIM], k4[DIM], xi[DIM];
+#pragma unroll
+            for (int a = 0; a < DIM; ++a) xi[a] = fma(TC(0.5) * hs[a], k1[a], w[a]);
+            ok = cart_velocity<DIM, TV, TC, FASTWRAP, LD256>(g, pb, tb, ci, xi, k2);
+            if (!ok) break;
+#pragma unroll
+            for (int a = 0; a < DIM; ++a) xi[a] = fma(TC(0.5) * hs[a], k2[a], w[a]);
+            ok = cart_velocity<DIM, TV, TC, FASTWRAP, LD256>(g, pb, tb, ci, xi, k3);
+            if (!ok) break;
+#pragma unroll
+            for (int a = 0; a < DIM; ++a) xi[a] = fma(hs[a], k3[a], w[a]);
+            ok = cart_velocity<DIM, TV, TC, FASTWRAP, LD256>(g, pc, tc, ci, xi, k4);
+            if (!ok) break;
+#pragma unroll
+            for (int a = 0; a < DIM; ++a) inc[a] = TC(1.0 / 6.0) * ((k1[a] + k4[a]) + TC(2) * (k2[a] + k3[a]));
+        } else {
+#pragma unroll
+            for (int a = 0; a < DIM; ++a)
+                inc[a] = TC(1.0 / 24.0) * (((TC(55) * k1[a] - TC(59) * h0[a]) + TC(37) * h1[a]) - TC(9) * h2[a]);
+        }
+#pragma unroll
+        for (int a = 0; a < DIM; ++a) {
+            int ifl;
+            floor_split<TC>(fma(hs[a], inc[a], w[a]), ifl, w[a]);
+            ci[a] += ifl;
+            h2[a] = h1[a]; h1[a] = h0[a]; h0[a] = k1[a];
+        }
+    }
+#pragma unroll
+    for (int a = 0; a < DIM; ++a) {
+        t.ci[a] = ci[a]; t.w[a] = w[a];
+        hist[(i * 3 + 0) * DIM + a] = h0[a]; hist[(i * 3 + 1) * DIM + a] = h1[a]; hist[(i * 3 + 2) * DIM + a] = h2[a];
+    }
+    if (!ok) t.meta = (1u << 30) | (uint32_t)(first_step + s);
+    store_record(st + i, t);
+}
+
+// ---------------------------------------------------------------------------------------------
 // Split variant (the paper's design: "the RK4 computation was divided into several short
 // kernels"; all tracers advance one stage at a time).  One launch per RK4 stage; between the launches the
 // stage point (xi) and the running sum k1 + 2 k2 + 2 k3 (acc) live in global memory as [n][DIM] arrays.
@@ -634,8 +703,8 @@ lcs_status cart_advect_impl(lcs_field *f, int64_t n, const void *seeds_, double 
     std::vector<TC> tau(tau64.size());
     for (size_t k = 0; k < tau.size(); ++k) tau[k] = (TC)tau64[k];
 
-    const bool split = f->opt_integrator == 2;
-    const bool do_bundle = f->opt_bundle == 1 || (f->opt_bundle < 0 && n >= (1 << 18));
+    const bool split = f->opt_integrator == 2, ab4 = f->opt_integrator == 3;
+    const bool do_bundle = !ab4 && (f->opt_bundle == 1 || (f->opt_bundle < 0 && n >= (1 << 18)));
     // sort bins: Morton code of the cell index, coarsened so that the histogram stays <= 2^24 bins
     int shift = 0, bits = 0;
     for (;; ++shift) {
@@ -652,7 +721,7 @@ lcs_status cart_advect_impl(lcs_field *f, int64_t n, const void *seeds_, double 
     // launch units: a snapshot window is cut into chunks (pre-blended variant: <= preblend_steps steps, whose
     // distinct stage times are blended once per node; otherwise <= bundle_steps steps between re-bundlings)
     constexpr bool kCanBlend = DIM == 3 && sizeof(TC) == 4 && sizeof(TV) == 4;
-    const bool preblend = kCanBlend && !split && (f->opt_preblend == 1 || (f->opt_preblend < 0 && n >= (1 << 20)));
+    const bool preblend = kCanBlend && !split && !ab4 && (f->opt_preblend == 1 || (f->opt_preblend < 0 && n >= (1 << 20)));
     struct Unit { int win, first, count, blend, ftau_off, nfields; };
     std::vector<Unit> units;
     std::vector<float> ftau;
@@ -695,6 +764,7 @@ lcs_status cart_advect_impl(lcs_field *f, int64_t n, const void *seeds_, double 
     const size_t o_b = off; if (do_bundle) off = align_up(off + (size_t)n * sizeof(Tracer));
     const size_t o_xi = off; if (split) off = align_up(off + (size_t)n * DIM * sizeof(TC));
     const size_t o_acc = off; if (split) off = align_up(off + (size_t)n * DIM * sizeof(TC));
+    const size_t o_hist = off; if (ab4) off = align_up(off + (size_t)n * 3 * DIM * sizeof(TC));
     const size_t o_tau = off; off = align_up(off + tau.size() * sizeof(TC));
     const int64_t ntiles = (nbins + bundle::kScanTile - 1) / bundle::kScanTile;
     const size_t o_key = off; if (do_bundle) off = align_up(off + (size_t)n * 4);
@@ -793,7 +863,17 @@ lcs_status cart_advect_impl(lcs_field *f, int64_t n, const void *seeds_, double 
             }
         }
         WindowTimer timer(f, st);
-        if (!split) {
+        if (ab4) {
+            using Rec = PairRec<DIM, TV>;
+            TC *d_hist = (TC *)(base + o_hist);
+#define LCS_AB4(FW, LD) LCS_LAUNCH((cart_ab4_kernel<DIM, TV, TC, FW, LD>), lcs_blocks(n, block), block, 0, st, g, (const Rec *)p[0], (const Rec *)p[1], \
+                                   (const Rec *)p[2], d_tau + 3 * (size_t)u.first, u.count, u.first, n, cur, d_hist, hs[0], hs[1], hs[2])
+            if (fast && ld256) LCS_AB4(true, true);
+            else if (fast) LCS_AB4(true, false);
+            else if (ld256) LCS_AB4(false, true);
+            else LCS_AB4(false, false);
+#undef LCS_AB4
+        } else if (!split) {
             if (fast && ld256) launch_window<DIM, TV, TC, true, true>(g, p, d_tau, u.first, u.count, n, cur, hs, block, st);
             else if (fast) launch_window<DIM, TV, TC, true, false>(g, p, d_tau, u.first, u.count, n, cur, hs, block, st);
             else if (ld256) launch_window<DIM, TV, TC, false, true>(g, p, d_tau, u.first, u.count, n, cur, hs, block, st);

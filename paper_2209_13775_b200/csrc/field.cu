@@ -379,7 +379,7 @@ extern "C" lcs_status lcs_field_sync(lcs_field *f)
 extern "C" lcs_status lcs_field_set_option(lcs_field *f, const char *key, int64_t value)
 {
     if (!f || !key) { lcs_set_error("null argument"); return LCS_ERR_INVALID_ARG; }
-    if (!strcmp(key, "integrator") && value >= 0 && value <= 2) f->opt_integrator = value;
+    if (!strcmp(key, "integrator") && value >= 0 && value <= 3) f->opt_integrator = value;
     else if (!strcmp(key, "bundle") && value >= -1 && value <= 1) f->opt_bundle = value;
     else if (!strcmp(key, "bundle_steps") && value >= 0) f->opt_bundle_steps = value;
     else if (!strcmp(key, "bundle_order") && (value == 0 || value == 1)) f->opt_bundle_order = value;

@@ -645,6 +645,73 @@ simplex_window_kernel(const CellRec<DIM, TC> *__restrict__ crec, const int32_t *
     store_tracer(st + i, t);
 }
 
+// Adams-Bashforth 4 with an RK4 start-up on simplicial meshes (row f4, reading #31): as simplex_window_kernel,
+// one velocity evaluation (walk + interpolation) per step after the first three; hist [n][3][DIM] as in cart_ab4_kernel.
+template <int DIM, typename TV, typename TC>
+__global__ void __launch_bounds__(128)
+simplex_ab4_kernel(const CellRec<DIM, TC> *__restrict__ crec, const int32_t *__restrict__ neigh, const PairRec<DIM, TV> *__restrict__ pa,
+                   const PairRec<DIM, TV> *__restrict__ pb, const PairRec<DIM, TV> *__restrict__ pc, const TC *__restrict__ tau,
+                   int nsteps, int first_step, int64_t n, SimplexTracer<DIM, TC> *__restrict__ st, TC *__restrict__ hist, TC h)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    SimplexTracer<DIM, TC> t = load_tracer(st + i);
+    if ((t.meta >> 30) != 0) return;
+    TC x[DIM], h0[DIM], h1[DIM], h2[DIM];
+#pragma unroll
+    for (int k = 0; k < DIM; ++k) {
+        x[k] = t.x[k];
+        h0[k] = first_step > 0 ? hist[(i * 3 + 0) * DIM + k] : TC(0);
+        h1[k] = first_step > 0 ? hist[(i * 3 + 1) * DIM + k] : TC(0);
+        h2[k] = first_step > 0 ? hist[(i * 3 + 2) * DIM + k] : TC(0);
+    }
+    int32_t cell = t.cell;
+    int s = 0;
+    bool ok = true;
+    HeldSimplex<DIM, TV, TC> held;
+    for (; s < nsteps; ++s) {
+        const TC ta = __ldg(tau + 3 * s), tb = __ldg(tau + 3 * s + 1), tc = __ldg(tau + 3 * s + 2);
+        TC k1[DIM], inc[DIM];
+        int32_t c = cell;
+        ok = simplex_velocity<DIM, TV, TC>(crec, neigh, pa, ta, x, &c, held, k1);
+        if (!ok) break;
+        if (first_step + s < 3) {
+            TC k2[DIM], k3[DIM], k4[DIM], y[DIM];
+#pragma unroll
+            for (int k = 0; k < DIM; ++k) y[k] = fma(TC(0.5) * h, k1[k], x[k]);
+            ok = simplex_velocity<DIM, TV, TC>(crec, neigh, pb, tb, y, &c, held, k2);
+            if (!ok) break;
+#pragma unroll
+            for (int k = 0; k < DIM; ++k) y[k] = fma(TC(0.5) * h, k2[k], x[k]);
+            ok = simplex_velocity<DIM, TV, TC>(crec, neigh, pb, tb, y, &c, held, k3);
+            if (!ok) break;
+#pragma unroll
+            for (int k = 0; k < DIM; ++k) y[k] = fma(h, k3[k], x[k]);
+            ok = simplex_velocity<DIM, TV, TC>(crec, neigh, pc, tc, y, &c, held, k4);
+            if (!ok) break;
+#pragma unroll
+            for (int k = 0; k < DIM; ++k) inc[k] = TC(1.0 / 6.0) * ((k1[k] + k4[k]) + TC(2) * (k2[k] + k3[k]));
+        } else {
+#pragma unroll
+            for (int k = 0; k < DIM; ++k) inc[k] = TC(1.0 / 24.0) * (((TC(55) * k1[k] - TC(59) * h0[k]) + TC(37) * h1[k]) - TC(9) * h2[k]);
+        }
+#pragma unroll
+        for (int k = 0; k < DIM; ++k) {
+            x[k] = fma(h, inc[k], x[k]);
+            h2[k] = h1[k]; h1[k] = h0[k]; h0[k] = k1[k];
+        }
+        cell = c;
+    }
+#pragma unroll
+    for (int k = 0; k < DIM; ++k) {
+        t.x[k] = x[k];
+        hist[(i * 3 + 0) * DIM + k] = h0[k]; hist[(i * 3 + 1) * DIM + k] = h1[k]; hist[(i * 3 + 2) * DIM + k] = h2[k];
+    }
+    t.cell = cell;
+    if (!ok) t.meta = (1u << 30) | (uint32_t)(first_step + s);
+    store_tracer(st + i, t);
+}
+
 template <int DIM, typename TC>
 __global__ void __launch_bounds__(256) simplex_final_kernel(int64_t n, const SimplexTracer<DIM, TC> *__restrict__ st, int32_t N,
                                                              TC *__restrict__ flowmap, uint8_t *__restrict__ exit_flag,
@@ -807,7 +874,8 @@ lcs_status simplex_advect_impl(lcs_field *f, int64_t n, const void *seeds_, doub
     for (size_t k = 0; k < tau.size(); ++k) tau[k] = (TC)tau64[k];
 
     // re-bundling by bin (Morton order of the coarsened bin grid), histogram <= 2^24 bins
-    const bool do_bundle = f->opt_bundle == 1 || (f->opt_bundle < 0 && n >= (1 << 18));
+    const bool ab4 = f->opt_integrator == 3;
+    const bool do_bundle = !ab4 && (f->opt_bundle == 1 || (f->opt_bundle < 0 && n >= (1 << 18)));
     int shift = 0, bits = 0;
     for (;; ++shift) {
         bits = 0;
@@ -825,6 +893,7 @@ lcs_status simplex_advect_impl(lcs_field *f, int64_t n, const void *seeds_, doub
     const size_t o_a = off; off = align_up(off + (size_t)n * sizeof(Tracer));
     const size_t o_b = off; if (do_bundle) off = align_up(off + (size_t)n * sizeof(Tracer));
     const size_t o_tau = off; off = align_up(off + tau.size() * sizeof(TC));
+    const size_t o_hist = off; if (ab4) off = align_up(off + (size_t)n * 3 * DIM * sizeof(TC));
     const size_t o_key = off; if (do_bundle) off = align_up(off + (size_t)n * 4);
     const size_t o_cnt = off; if (do_bundle) off = align_up(off + (size_t)nbins * 4);
     const size_t o_tile = off; if (do_bundle) off = align_up(off + (size_t)ntiles * 4);
@@ -866,8 +935,13 @@ lcs_status simplex_advect_impl(lcs_field *f, int64_t n, const void *seeds_, doub
             }
             since_bundle += cnt;
             WindowTimer timer(f, st);
-            LCS_LAUNCH((simplex_window_kernel<DIM, TV, TC>), lcs_blocks(n, block), block, 0, st, (const CellRec<DIM, TC> *)m.cellrec, m.neigh,
-                       (const VRec *)p[0], (const VRec *)p[1], (const VRec *)p[2], d_tau + 3 * (size_t)first, cnt, first, n, cur, (TC)h);
+            if (ab4)
+                LCS_LAUNCH((simplex_ab4_kernel<DIM, TV, TC>), lcs_blocks(n, block), block, 0, st, (const CellRec<DIM, TC> *)m.cellrec, m.neigh,
+                           (const VRec *)p[0], (const VRec *)p[1], (const VRec *)p[2], d_tau + 3 * (size_t)first, cnt, first, n, cur,
+                           (TC *)(base + o_hist), (TC)h);
+            else
+                LCS_LAUNCH((simplex_window_kernel<DIM, TV, TC>), lcs_blocks(n, block), block, 0, st, (const CellRec<DIM, TC> *)m.cellrec, m.neigh,
+                           (const VRec *)p[0], (const VRec *)p[1], (const VRec *)p[2], d_tau + 3 * (size_t)first, cnt, first, n, cur, (TC)h);
             if (lcs_early_due(f, (int64_t)first + cnt, N)) {         // row f1: evaluate C for the stencils that are still complete
                 LCS_LAUNCH((simplex_final_kernel<DIM, TC>), lcs_blocks(n, 256), 256, 0, st, n, cur, (int32_t)N, (TC *)f->early.flowmap,
                            f->early.flag, (int32_t *)nullptr);

@@ -761,3 +761,42 @@ def test_smooth_gaussian_vs_oracle(lcs, oracle, dt):
         lcs.smooth_gaussian(2, w.ng, w.seed_periodic, 0.0, ft)
     with pytest.raises(lcs.LcsError):
         lcs.smooth_gaussian(2, w.ng, w.seed_periodic, 30.0, ft)
+
+
+# -------------------------------------------------------------------------------------------------
+# row f4 (second part): Adams-Bashforth 4 integrator
+@pytest.mark.parametrize("case", ["cart2_f64", "cart3_f32_periodic", "tri_f64", "tet_f32", "cart2_f64_exits"])
+def test_adams_bashforth_vs_oracle(lcs, oracle, case):
+    """integrator = 3 (AB4 with RK4 start-up) against oracle rule O12 on every mesh kind: fp64 cases within the fp64 gate
+    (flags and exit steps identical), fp32 cases within the statistical gate.  Windows of several launches exercise the
+    velocity history that is carried across launches."""
+    if case == "cart2_f64":
+        w = I.config1(ng=(64, 32), T=6.0)
+    elif case == "cart3_f32_periodic":
+        w = I.config3(ngrid=24, nn=16, T=2.0, h=0.01, n_snap=9)
+    elif case == "tri_f64":
+        w = I.config2(ng=(64, 32), lattice=(50, 25), T=4.0)
+    elif case == "tet_f32":
+        w = I.config4(ng=(16, 16, 24), delta=0.08, T=1.5, h=0.005, n_snap=10, length=4.0)
+    else:
+        A = np.array([[0.25, 0.6], [-0.6, 0.25]])
+        w = I.analytic_cartesian(2, I.linear_flow(A), (41, 41), (-2.0, -2.0), (0.1, 0.1), (0.0, 2.0, 4.0), ng=(24, 20), seed_lo=(-2.1, -1.4),
+                                 seed_spacing=(0.175, 0.14), t0=0.0, tf=4.0, h=0.05)
+    fo = oracle.OracleField.from_workload(w)
+    Fo, flo, eso = fo.advect_ab4(w.seeds().astype(np.float64), w.t0, w.tf, w.h)
+    f, sd, F, flag, es = gpu_run(w, options=dict(integrator=3))
+    cgo, fto, sto = oracle_cg(oracle, w, Fo, flo)
+    cgg, ftg, stg = gpu_cg(w, F, flag)
+    if w.compute_dtype == np.float64 and case != "tri_f64":
+        gate_fp64(cpu(F), Fo, cpu(ftg), fto, w.tf - w.t0, cpu(flag), flo, cpu(es), eso)
+    elif case == "tri_f64":
+        assert np.array_equal(cpu(flag), flo) and np.max(np.abs(cpu(F) - Fo)) <= 1e-10
+    else:
+        gate_statistical(cpu(F), Fo, cpu(ftg), fto, w.L, cpu(flag), flo)
+    if case == "cart2_f64_exits":
+        assert set(np.unique(flo)) == {0, 1, 2}
+    # and it is a different scheme from RK4: the two flow maps differ by the truncation error, not by rounding
+    f2, sd2, F2, flag2, es2 = gpu_run(w)
+    both = (cpu(flag) == 0) & (cpu(flag2) == 0)
+    d = np.max(np.abs(cpu(F)[both].astype(np.float64) - cpu(F2)[both].astype(np.float64)))
+    assert d > (1e-9 if w.compute_dtype == np.float64 else 0.0)
