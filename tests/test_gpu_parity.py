@@ -800,3 +800,59 @@ def test_adams_bashforth_vs_oracle(lcs, oracle, case):
     both = (cpu(flag) == 0) & (cpu(flag2) == 0)
     d = np.max(np.abs(cpu(F)[both].astype(np.float64) - cpu(F2)[both].astype(np.float64)))
     assert d > (1e-9 if w.compute_dtype == np.float64 else 0.0)
+
+
+# -------------------------------------------------------------------------------------------------
+# randomized small Cartesian configurations: every integrator variant against the oracle
+def test_random_cartesian_configs_all_variants(lcs, oracle):
+    """24 seeded random small workloads: 2D / 3D, ragged non-power-of-two grids, any mix of periodic axes, fp64 or fp32,
+    forward or backward time, step sizes that do or do not divide the snapshot spacing, seeds partly outside.  Each runs
+    through a random integrator variant (fused, split, bundled, pre-blended, Adams-Bashforth) and is compared with the oracle:
+    fp64 to 1e-9 with identical flags and exit steps, fp32 statistically."""
+    rng = np.random.default_rng(777)
+    n_exit_cases = 0
+    for case in range(24):
+        dim = int(rng.integers(2, 4))
+        n = tuple(int(v) for v in rng.integers(5, 20, dim))
+        per = tuple(int(v) for v in rng.integers(0, 2, dim))
+        f32 = bool(rng.integers(0, 2))
+        spacing = tuple(float(v) for v in rng.uniform(0.05, 0.2, dim))
+        origin = tuple(float(v) for v in rng.uniform(-1, 1, dim))
+        ext = [spacing[a] * (n[a] if per[a] else n[a] - 1) for a in range(dim)]
+        A = rng.uniform(-0.4, 0.4, (dim, dim))
+        b = rng.uniform(-0.3, 0.3, dim)
+        times = np.arange(0.0, 2.01, 0.5)
+        h = float(rng.choice([0.05, 0.0625, 0.03]))
+        nsteps = int(rng.integers(8, 30))
+        backward = bool(rng.integers(0, 2))
+        t0 = 2.0 if backward else 0.0
+        tf = t0 + (-h if backward else h) * nsteps
+        ng = tuple(int(v) for v in rng.integers(6, 14, dim))
+        margin = 0.0 if all(per) else 0.08
+        seed_lo = tuple(origin[a] - margin * ext[a] for a in range(dim))
+        seed_sp = tuple((1 + 2 * margin) * ext[a] / ng[a] for a in range(dim))
+        dt = np.float32 if f32 else np.float64
+        w = I.analytic_cartesian(dim, I.linear_flow(A, b), n, origin, spacing, times, ng=ng, seed_lo=seed_lo, seed_spacing=seed_sp,
+                                 t0=t0, tf=tf, h=(-h if backward else h), periodic=per + (0,) * (3 - dim), seed_periodic=(0, 0, 0),
+                                 vel_dtype=dt, compute_dtype=dt)
+        variant = [dict(bundle=0), dict(bundle=1, bundle_steps=int(rng.integers(1, 9))), dict(integrator=2, bundle=int(rng.integers(0, 2))),
+                   dict(bundle=1, preblend=1, preblend_steps=int(rng.integers(1, 9))), dict(integrator=3),
+                   dict(bundle=1, bundle_order=0, ld256=0)][case % 6]
+        fo = oracle.OracleField.from_workload(w)
+        s64 = w.seeds().astype(np.float64)
+        if variant.get("integrator") == 3:
+            Fo, flo, eso = fo.advect_ab4(s64, w.t0, w.tf, w.h)
+        else:
+            Fo, flo, eso = fo.advect(s64, w.t0, w.tf, w.h)
+        f, sd, F, flag, es = gpu_run(w, options=variant)
+        Fg, fg, eg = cpu(F).astype(np.float64), cpu(flag), cpu(es)
+        n_exit_cases += int((flo == 1).any())
+        tag = "case %d dim %d n %s per %s f32 %s variant %s" % (case, dim, n, per, f32, variant)
+        if not f32:
+            assert np.array_equal(fg, flo) and np.array_equal(eg, eso), tag
+            assert np.max(np.abs(Fg - Fo)) <= 1e-9, tag
+        else:
+            same = (fg == flo)
+            assert same.mean() >= 0.98, tag
+            assert np.max(np.linalg.norm(Fg[same] - Fo[same], axis=1)) <= 2e-4 * max(ext), tag
+    assert n_exit_cases >= 8
