@@ -734,6 +734,69 @@ void orc_smooth_gaussian(int32_t dim, const int32_t *ng, const int32_t *sper, do
     free(a); free(b);
 }
 
+/* ---- O13 (row f4, third part): ridges of the (smoothed) FTLE field ---------------------------------------------
+ * The LCS filter extracts "C-ridges" of the smoothed FTLE field; the paper gives no definition.
+ * Reading (#32): the second-derivative ridge of the FTLE literature (the paper's ref [29]): with g the gradient
+ * and H the Hessian of the field s, n the unit eigenvector of the SMALLEST eigenvalue kappa of H, a ridge point has
+ * kappa < 0 and g . n = 0.  On the seed grid, per seed:
+ *   g_a  = (s(+a) - s(-a)) / (2 dx_a);  H_aa = (s(+a) - 2 s + s(-a)) / dx_a^2;
+ *   H_ab = (s(+a+b) - s(+a-b) - s(-a+b) + s(-a-b)) / (4 dx_a dx_b);   neighbours wrapped on periodic axes;
+ *   (kappa, n) by the Jacobi iteration of O8 (sign of n: component of largest magnitude positive);  d = g . n;
+ *   mask = 1 iff kappa < -kappa_min and s >= s_min and |d| <= |kappa| * delta / 2,  delta = min_a dx_a
+ *   (to first order |d| / |kappa| is the distance to the ridge along n: the ridge passes within half a cell).
+ * A seed whose stencil (the 3^d block) leaves the grid on a non-periodic axis or contains a non-finite value gets
+ * kappa = d = NaN, mask = 0.                                                                                       */
+void orc_ridge(int32_t dim, const int32_t *ng, const double *dx, const int32_t *sper, double kappa_min, double s_min,
+               const double *field, double *kappa, double *dgn, uint8_t *mask)
+{
+    int64_t n[3] = {ng[0], ng[1], dim == 3 ? ng[2] : 1};
+    int64_t total = n[0] * n[1] * n[2], stride[3] = {1, n[0], n[0] * n[1]};
+    double delta = dx[0];
+    for (int a = 1; a < dim; ++a) if (dx[a] < delta) delta = dx[a];
+#pragma omp parallel for schedule(static)
+    for (int64_t idx = 0; idx < total; ++idx) {
+        int64_t ijk[3] = {idx % n[0], (idx / n[0]) % n[1], idx / (n[0] * n[1])};
+        int64_t off[3][3];                               /* off[a][0|1|2] = index offset of the -1 | 0 | +1 neighbour on axis a */
+        int ok = 1;
+        for (int a = 0; a < dim; ++a)
+            for (int k = -1; k <= 1; ++k) {
+                int64_t j = ijk[a] + k;
+                if (j < 0 || j >= n[a]) { if (sper[a]) j = (j + n[a]) % n[a]; else ok = 0; }
+                off[a][k + 1] = (j - ijk[a]) * stride[a];
+            }
+        double g[3], H[3][3], v[3][3];
+        if (ok) {
+#define S2(a, ka, b, kb) field[idx + off[a][(ka) + 1] + off[b][(kb) + 1]]
+            double s0 = field[idx];
+            ok = isfinite(s0);
+            for (int a = 0; a < dim && ok; ++a) {
+                double sp = field[idx + off[a][2]], sm = field[idx + off[a][0]];
+                ok = isfinite(sp) && isfinite(sm);
+                g[a] = (sp - sm) / (2.0 * dx[a]);
+                H[a][a] = (sp - 2.0 * s0 + sm) / (dx[a] * dx[a]);
+                for (int b = a + 1; b < dim && ok; ++b) {
+                    double pp = S2(a, 1, b, 1), pm = S2(a, 1, b, -1), mp = S2(a, -1, b, 1), mm = S2(a, -1, b, -1);
+                    ok = isfinite(pp) && isfinite(pm) && isfinite(mp) && isfinite(mm);
+                    H[a][b] = H[b][a] = (pp - pm - mp + mm) / (4.0 * dx[a] * dx[b]);
+                }
+            }
+#undef S2
+        }
+        if (!ok) { kappa[idx] = NAN; dgn[idx] = NAN; mask[idx] = 0; continue; }
+        jacobi_sym(dim, H, v);
+        int col = 0;
+        for (int k = 1; k < dim; ++k) if (H[k][k] < H[col][col]) col = k;
+        int big = 0;
+        for (int r = 1; r < dim; ++r) if (fabs(v[r][col]) > fabs(v[big][col])) big = r;
+        double sg = v[big][col] < 0.0 ? -1.0 : 1.0, d = 0.0;
+        for (int r = 0; r < dim; ++r) d += g[r] * (sg * v[r][col]);
+        double kap = H[col][col];
+        kappa[idx] = kap;
+        dgn[idx] = d;
+        mask[idx] = (kap < -kappa_min && field[idx] >= s_min && fabs(d) <= fabs(kap) * delta / 2.0) ? 1 : 0;
+    }
+}
+
 int orc_max_threads(void)
 {
 #ifdef _OPENMP

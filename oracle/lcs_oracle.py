@@ -285,6 +285,17 @@ def smooth_gaussian(dim, ng, seed_periodic, sigma, field):
     return out
 
 
+def ridge(dim, ng, seed_spacing, seed_periodic, kappa_min, s_min, field):
+    """Rule O13: second-derivative ridge indicator of a scalar field on the seed grid.  Returns (kappa, d, mask)."""
+    f = np.ascontiguousarray(field, dtype=np.float64).ravel()
+    ng_ = np.asarray(list(ng) + [1] * (3 - len(ng)), dtype=np.int32)
+    dx = np.asarray(list(seed_spacing) + [1.0] * (3 - len(seed_spacing)), dtype=np.float64)
+    sp = np.asarray(list(seed_periodic) + [0] * (3 - len(seed_periodic)), dtype=np.int32)
+    kappa, d, mask = np.empty_like(f), np.empty_like(f), np.empty(f.size, dtype=np.uint8)
+    lib().orc_ridge(C.c_int32(dim), _p(ng_), _p(dx), _p(sp), C.c_double(kappa_min), C.c_double(s_min), _p(f), _p(kappa), _p(d), _p(mask))
+    return kappa, d, mask
+
+
 def cg_eigen(dim, cg):
     """All eigenvalues (ascending) and unit eigenvectors (row i belongs to eigenvalue i) of C: rule O8."""
     c = np.ascontiguousarray(cg, dtype=np.float64)

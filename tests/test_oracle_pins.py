@@ -794,3 +794,53 @@ def test_P19_adams_bashforth(oracle):
     inside = fl != 2
     assert np.max(np.abs(F[inside] - (wb.seeds()[inside] + np.outer(es[inside] * 0.25, c)))) <= 1e-12   # uniform flow: exact until the exit
     assert np.array_equal(F[~inside], wb.seeds()[~inside]) and np.all(es[fl == 2] == 0) and np.all(es[fl == 0] == 20)
+
+
+# -------------------------------------------------------------------------------------------------
+# O13 (row f4, third part): ridges of the smoothed FTLE field
+def test_P20_ridge_indicator(oracle):
+    """Pins for O13 on analytic fields.  (a) Straight ridge s = exp(-(y - y0)^2 / (2 b^2)): kappa = -s / b^2 on the ridge row,
+    n = (0, 1), d = ds/dy, and the mask marks exactly the grid row(s) within half a cell of y0.  (b) Quadratic field
+    s = c - (p x^2 + q y^2 + r x y)/2: central differences are exact, so kappa is the smallest eigenvalue of -[[p, r/2],[r/2, q]]
+    and d = g . n to rounding.  (c) Circular ridge: the mask is a closed ring of radius R.  (d) Planar ridge sheet in 3D.
+    (e) NaN in the stencil or a stencil leaving a non-periodic grid gives NaN / mask 0; a valley (kappa > 0) is not marked."""
+    nx, ny, dx, dy = 60, 41, 0.05, 0.04
+    X, Y = np.meshgrid((np.arange(nx) + 0.5) * dx, (np.arange(ny) + 0.5) * dy)
+    y0, b = 0.83, 0.2
+    s = np.exp(-(Y - y0) ** 2 / (2 * b * b))
+    kap, d, m = (a.reshape(ny, nx) for a in oracle.ridge(2, (nx, ny), (dx, dy), (0, 0), 0.0, 0.5, s))
+    jr = int(np.argmin(np.abs(Y[:, 0] - y0)))
+    assert abs(kap[jr, 10] + s[jr, 10] / (b * b)) <= 0.03 / (b * b)                      # O(dy^2) finite-difference error
+    rows = np.nonzero(m[:, 10])[0]
+    assert set(rows) == set(np.nonzero(np.abs(Y[:, 0] - y0) <= dy / 2 * 1.02)[0]) and len(rows) >= 1
+    assert np.all(m[1:-1, 1:-1] == m[1:-1, 10:11])                                       # the same rows at every interior x
+    assert np.all(np.isnan(kap[0])) and np.all(np.isnan(kap[:, 0])) and m[0].sum() == 0   # stencil leaves the grid
+    p, q, r = 1.3, 0.4, 0.5
+    s2 = 2.0 - (p * X * X + q * Y * Y + r * X * Y) / 2
+    kap, d, m = (a.reshape(ny, nx) for a in oracle.ridge(2, (nx, ny), (dx, dy), (0, 0), 0.0, -1e9, s2))
+    Hm = -np.array([[p, r / 2], [r / 2, q]])
+    wv, vv = np.linalg.eigh(Hm)
+    nvec = vv[:, 0] * np.sign(vv[np.argmax(np.abs(vv[:, 0])), 0])
+    gx, gy = -(p * X + r * Y / 2), -(q * Y + r * X / 2)
+    assert np.nanmax(np.abs(kap[1:-1, 1:-1] - wv[0])) <= 1e-10
+    assert np.nanmax(np.abs(d[1:-1, 1:-1] - (gx * nvec[0] + gy * nvec[1])[1:-1, 1:-1])) <= 1e-10
+    n2 = 81
+    Xc, Yc = np.meshgrid((np.arange(n2) - 40) * 0.05, (np.arange(n2) - 40) * 0.05)
+    R = np.hypot(Xc, Yc)
+    s3 = np.exp(-(R - 1.2) ** 2 / (2 * 0.25 ** 2))
+    kap, d, m = (a.reshape(n2, n2) for a in oracle.ridge(2, (n2, n2), (0.05, 0.05), (0, 0), 1.0, 0.8, s3))   # s_min = 0.8 cuts the shoulders beyond the inflection circle, where the
+    # tangential curvature s'/r < 0 is the smallest eigenvalue and g . n vanishes identically (a known artefact of height ridges)
+    assert m.sum() > 100 and np.all(np.abs(R[m == 1] - 1.2) <= 0.05) and np.all(m[np.abs(R - 1.2) > 0.06] == 0)
+    ang = np.arctan2(Yc[m == 1], Xc[m == 1])
+    assert np.max(np.diff(np.sort(ang))) < 0.12                                           # a closed ring, no gaps
+    nz = 30
+    Z = ((np.arange(nz) + 0.5) * 0.1)[:, None, None] * np.ones((nz, 12, 14))
+    s4 = np.exp(-(Z - 1.42) ** 2 / (2 * 0.4 ** 2))
+    kap, d, m = (a.reshape(nz, 12, 14) for a in oracle.ridge(3, (14, 12, nz), (0.1, 0.1, 0.1), (1, 1, 0), 0.0, 0.5, s4))
+    kr = int(np.argmin(np.abs(Z[:, 0, 0] - 1.42)))
+    assert np.all(m[kr] == 1) and m.sum() == 12 * 14 and np.all(np.isfinite(kap[1:-1]))   # periodic in x, y: whole sheet
+    s5 = s.copy(); s5[20, 30] = np.nan
+    kap, d, m = (a.reshape(ny, nx) for a in oracle.ridge(2, (nx, ny), (dx, dy), (0, 0), 0.0, 0.0, s5))
+    assert np.all(np.isnan(kap[19:22, 29:32])) and m[19:22, 29:32].sum() == 0 and np.isfinite(kap[20, 33])
+    kap, d, m = oracle.ridge(2, (nx, ny), (dx, dy), (0, 0), 0.0, -1e9, -s)
+    assert m.reshape(ny, nx)[jr, 5:-5].sum() == 0                                         # a valley is not a ridge
