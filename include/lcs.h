@@ -180,6 +180,17 @@ lcs_status lcs_cg_eigen(int32_t dim, int32_t dtype, int64_t n, const void *cg, v
 lcs_status lcs_smooth_gaussian(int32_t dim, int32_t dtype, const int32_t ng[3], const int32_t seed_periodic[3],
                                double sigma, const void *field, void *out, void *work, void *cuda_stream);
 
+/* Ridge indicator of a scalar field (the smoothed FTLE) on the structured seed grid, the second step of the LCS filter
+ * ("C-ridge extraction"; the paper gives no definition: DESIGN.md reading #32, second-derivative ridge).
+ * Per seed: gradient g and Hessian H by central differences on the 3^dim stencil (wrapped on periodic axes), kappa = smallest
+ * eigenvalue of H with unit eigenvector n (component of largest magnitude positive), d = g . n,
+ * mask = (kappa < -kappa_min) && (field >= s_min) && (|d| <= |kappa| * min(seed_spacing) / 2): the ridge passes within half
+ * a cell of the seed.  A seed whose stencil leaves a non-periodic grid or holds a non-finite value gets kappa = d = NaN,
+ * mask = 0.  field, kappa, dgn: device [n] of `dtype`; mask: device [n] u8.  fp64 arithmetic.  kappa_min >= 0.          */
+lcs_status lcs_ridge(int32_t dim, int32_t dtype, const int32_t ng[3], const double seed_spacing[3],
+                     const int32_t seed_periodic[3], double kappa_min, double s_min, const void *field,
+                     void *kappa, void *dgn, uint8_t *mask, void *cuda_stream);
+
 /* End-to-end convenience with HOST buffers: copies the seeds to the device, runs lcs_advect and
  * lcs_cg_ftle and copies flow map (optional), flags (optional) and FTLE back; synchronous.
  * seeds_host/flowmap_host: [n][dim] of the field's compute_dtype; ftle_host: [n] of compute_dtype.

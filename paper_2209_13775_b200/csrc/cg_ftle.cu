@@ -247,6 +247,93 @@ template <int D> __device__ __forceinline__ void jacobi_rotate(double (&a)[D][D]
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Row f4 (third part): ridge indicator of the (smoothed) FTLE field ("C-ridge extraction"; DESIGN.md reading
+// #32: second-derivative ridge).  Per seed: gradient and Hessian by central differences on the 3^d stencil, smallest
+// Hessian eigenvalue kappa and its eigenvector n by Jacobi in fp64, d = g . n, mask = kappa < -kappa_min && s >= s_min &&
+// |d| <= |kappa| delta / 2.  Streams the field once (stencil taps hit L1/L2); FP64-pipe bound like the eigen kernels.
+struct RidgeGrid {
+    int ng[3], per[3];
+    double dx[3];
+    double kappa_min, s_min, delta;
+};
+
+template <int D, typename T>
+__global__ void __launch_bounds__(128) ridge_kernel(const __grid_constant__ RidgeGrid g, const T *__restrict__ field, T *__restrict__ kappa,
+                                                     T *__restrict__ dgn, uint8_t *__restrict__ mask, int64_t total)
+{
+    const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= total) return;
+    const int64_t n0 = g.ng[0], n1 = g.ng[1];
+    const int64_t ijk[3] = {idx % n0, (idx / n0) % n1, idx / (n0 * n1)};
+    const int64_t stride[3] = {1, n0, n0 * n1};
+    int64_t off[D][3];
+    bool ok = true;
+#pragma unroll
+    for (int a = 0; a < D; ++a)
+#pragma unroll
+        for (int k = -1; k <= 1; ++k) {
+            int64_t j = ijk[a] + k;
+            if (j < 0 || j >= g.ng[a]) { if (g.per[a]) j = (j + g.ng[a]) % g.ng[a]; else ok = false; }
+            off[a][k + 1] = (j - ijk[a]) * stride[a];
+        }
+    double gr[D], H[D][D], v[D][D];
+    const double s0 = ok ? (double)field[idx] : 0.0;
+    ok = ok && isfinite(s0);
+    if (ok) {
+#pragma unroll
+        for (int a = 0; a < D; ++a) {
+            const double sp = (double)field[idx + off[a][2]], sm = (double)field[idx + off[a][0]];
+            ok = ok && isfinite(sp) && isfinite(sm);
+            gr[a] = (sp - sm) / (2.0 * g.dx[a]);
+            H[a][a] = (sp - 2.0 * s0 + sm) / (g.dx[a] * g.dx[a]);
+#pragma unroll
+            for (int b = a + 1; b < D; ++b) {
+                const double pp = (double)field[idx + off[a][2] + off[b][2]], pm = (double)field[idx + off[a][2] + off[b][0]];
+                const double mp = (double)field[idx + off[a][0] + off[b][2]], mm = (double)field[idx + off[a][0] + off[b][0]];
+                ok = ok && isfinite(pp) && isfinite(pm) && isfinite(mp) && isfinite(mm);
+                H[a][b] = H[b][a] = (pp - pm - mp + mm) / (4.0 * g.dx[a] * g.dx[b]);
+            }
+        }
+    }
+    if (!ok) {
+        kappa[idx] = (T)nan(""); dgn[idx] = (T)nan(""); mask[idx] = 0;
+        return;
+    }
+#pragma unroll
+    for (int r = 0; r < D; ++r)
+#pragma unroll
+        for (int k = 0; k < D; ++k) v[r][k] = r == k ? 1.0 : 0.0;
+    for (int sweep = 0; sweep < 50; ++sweep) {
+        double offd = fabs(H[0][1]);
+        if constexpr (D == 3) offd += fabs(H[0][2]) + fabs(H[1][2]);
+        if (offd == 0.0) break;
+        jacobi_rotate<D>(H, v, 0, 1);
+        if constexpr (D == 3) { jacobi_rotate<D>(H, v, 0, 2); jacobi_rotate<D>(H, v, 1, 2); }
+    }
+    double kap = H[0][0], nv[D];
+#pragma unroll
+    for (int r = 0; r < D; ++r) nv[r] = v[r][0];
+#pragma unroll
+    for (int k = 1; k < D; ++k)
+        if (H[k][k] < kap) {
+            kap = H[k][k];
+#pragma unroll
+            for (int r = 0; r < D; ++r) nv[r] = v[r][k];
+        }
+    double big = nv[0];
+#pragma unroll
+    for (int r = 1; r < D; ++r)
+        if (fabs(nv[r]) > fabs(big)) big = nv[r];
+    const double sg = big < 0.0 ? -1.0 : 1.0;
+    double d = 0.0;
+#pragma unroll
+    for (int r = 0; r < D; ++r) d += gr[r] * (sg * nv[r]);
+    kappa[idx] = (T)kap;
+    dgn[idx] = (T)d;
+    mask[idx] = (kap < -g.kappa_min && s0 >= g.s_min && fabs(d) <= fabs(kap) * g.delta * 0.5) ? 1 : 0;
+}
+
 template <int D, typename T>
 __global__ void __launch_bounds__(128) cg_eigen_kernel(const T *__restrict__ cg, T *__restrict__ evals, T *__restrict__ evecs, int64_t n)
 {
@@ -453,6 +540,34 @@ extern "C" lcs_status lcs_smooth_gaussian(int32_t dim, int32_t dtype, const int3
         else LCS_LAUNCH((smooth_axis_kernel<float>), lcs_blocks(total, 256), 256, 0, st, (const float *)src, (float *)dst, total, stride[a], n[a], per, R, inv_2s2);
         src = dst;
     }
+    LCS_CUDA_OK(cudaGetLastError());
+    return LCS_OK;
+}
+
+extern "C" lcs_status lcs_ridge(int32_t dim, int32_t dtype, const int32_t ng[3], const double seed_spacing[3], const int32_t seed_periodic[3],
+                                double kappa_min, double s_min, const void *field, void *kappa, void *dgn, uint8_t *mask, void *cuda_stream)
+{
+    if ((dim != 2 && dim != 3) || !ng || !seed_spacing || !field || !kappa || !dgn || !mask) { lcs_set_error("null argument or bad dim"); return LCS_ERR_INVALID_ARG; }
+    if (dtype != LCS_F32 && dtype != LCS_F64) { lcs_set_error("bad dtype"); return LCS_ERR_INVALID_ARG; }
+    if (!(kappa_min >= 0.0) || !isfinite(s_min) && !(s_min < 0)) { lcs_set_error("kappa_min must be >= 0 and s_min a number"); return LCS_ERR_INVALID_ARG; }
+    RidgeGrid g;
+    int64_t total = 1;
+    g.delta = 1e300;
+    for (int a = 0; a < 3; ++a) {
+        g.ng[a] = a < dim ? ng[a] : 1;
+        g.per[a] = (a < dim && seed_periodic) ? (seed_periodic[a] != 0) : 0;
+        g.dx[a] = a < dim ? seed_spacing[a] : 1.0;
+        if (a < dim && (ng[a] < 1 || !(seed_spacing[a] > 0))) { lcs_set_error("bad seed grid on axis %d", a); return LCS_ERR_INVALID_ARG; }
+        if (a < dim && g.dx[a] < g.delta) g.delta = g.dx[a];
+        total *= g.ng[a];
+    }
+    g.kappa_min = kappa_min; g.s_min = s_min;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const unsigned grid = lcs_blocks(total, 128);
+    if (dim == 2 && dtype == LCS_F64) LCS_LAUNCH((ridge_kernel<2, double>), grid, 128, 0, st, g, (const double *)field, (double *)kappa, (double *)dgn, mask, total);
+    else if (dim == 2) LCS_LAUNCH((ridge_kernel<2, float>), grid, 128, 0, st, g, (const float *)field, (float *)kappa, (float *)dgn, mask, total);
+    else if (dtype == LCS_F64) LCS_LAUNCH((ridge_kernel<3, double>), grid, 128, 0, st, g, (const double *)field, (double *)kappa, (double *)dgn, mask, total);
+    else LCS_LAUNCH((ridge_kernel<3, float>), grid, 128, 0, st, g, (const float *)field, (float *)kappa, (float *)dgn, mask, total);
     LCS_CUDA_OK(cudaGetLastError());
     return LCS_OK;
 }

@@ -22,7 +22,7 @@ LCS_F32, LCS_F64 = 0, 1
 LCS_MESH_CARTESIAN, LCS_MESH_SIMPLEX = 0, 1
 
 EXPORTS = ["lcs_field_create", "lcs_field_set_snapshot", "lcs_field_sync", "lcs_field_destroy",
-           "lcs_field_set_option", "lcs_field_get_info", "lcs_locate", "lcs_advect", "lcs_advect_early_cg", "lcs_cg_ftle", "lcs_cg_ftle_aux", "lcs_cg_eigen", "lcs_smooth_gaussian",
+           "lcs_field_set_option", "lcs_field_get_info", "lcs_locate", "lcs_advect", "lcs_advect_early_cg", "lcs_cg_ftle", "lcs_cg_ftle_aux", "lcs_cg_eigen", "lcs_smooth_gaussian", "lcs_ridge",
            "lcs_ftle_host", "lcs_kernel_launch_count", "lcs_last_error"]
 
 
@@ -75,6 +75,8 @@ def lib():
                                       C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.lcs_smooth_gaussian.argtypes = [C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p,
                                           C.c_void_p]
+        L.lcs_ridge.argtypes = [C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.c_void_p, C.c_void_p,
+                                C.c_void_p, C.c_void_p, C.c_void_p]
         L.lcs_cg_eigen.argtypes = [C.c_int32, C.c_int32, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.lcs_ftle_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                     C.c_double, C.c_double, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p]
@@ -307,3 +309,15 @@ def smooth_gaussian(dim, ng, seed_periodic, sigma, field, stream=None):
     _check(lib().lcs_smooth_gaussian(int(dim), dtype, _arr3(ng, C.c_int32, 1), _arr3(seed_periodic, C.c_int32, 0), float(sigma),
                                      _tptr(field), _tptr(out), _tptr(work), _stream_ptr(stream)))
     return out
+
+
+def ridge(dim, ng, seed_spacing, seed_periodic, kappa_min, s_min, field, stream=None):
+    """lcs_ridge on a torch CUDA tensor [n]; returns (kappa, d, mask)."""
+    import torch
+    assert field.is_cuda and field.is_contiguous()
+    dtype = LCS_F64 if field.dtype == torch.float64 else LCS_F32
+    kappa, d = torch.empty_like(field), torch.empty_like(field)
+    mask = torch.empty(field.numel(), dtype=torch.uint8, device=field.device)
+    _check(lib().lcs_ridge(int(dim), dtype, _arr3(ng, C.c_int32, 1), _arr3(seed_spacing, C.c_double, 1.0), _arr3(seed_periodic, C.c_int32, 0),
+                           float(kappa_min), float(s_min), _tptr(field), _tptr(kappa), _tptr(d), _tptr(mask), _stream_ptr(stream)))
+    return kappa, d, mask

@@ -905,3 +905,46 @@ def test_random_simplex_configs_all_variants(lcs, oracle):
         assert exact.mean() >= 0.97, tag
         assert np.max(np.linalg.norm(Fg[exact] - Fo[exact], axis=1)) <= (2e-4 if f32 else 1e-9), tag
         assert f.info("locate_fallbacks") == 0, tag
+
+
+# -------------------------------------------------------------------------------------------------
+# row f4 (third part): ridge indicator of the smoothed FTLE field
+@pytest.mark.parametrize("dt", [np.float64, np.float32])
+def test_ridge_vs_oracle(lcs, oracle, dt):
+    """lcs_ridge against oracle rule O13 on the smoothed FTLE fields of config 1 (2D, non-periodic, with undefined seeds) and
+    config 3 (3D, periodic), both produced by the GPU path, and on an analytic ring.  kappa and d within tolerance; the mask is
+    an integer decided by fp64 comparisons on both sides: it must be identical wherever none of the three comparisons is within
+    the tolerance of its threshold."""
+    import torch
+    tol = 1e-9 if dt == np.float64 else 2e-5     # fp32 field values differenced over dx^2: 4 x 1e-7 s / dx^2 relative to max |kappa|
+    tdt = torch.float64 if dt == np.float64 else torch.float32
+    w = I.config1(ng=(96, 48), T=8.0)
+    f, sd, F, flag, es = gpu_run(w)
+    flag = flag.clone(); flag[::211] = 1
+    _, ft, _ = gpu_cg(w, F, flag)
+    s1 = lcs.smooth_gaussian(2, w.ng, w.seed_periodic, 1.5, ft.to(tdt).contiguous())
+    w3 = I.config3(ngrid=24, nn=16, T=2.0, n_snap=6)
+    f3, sd3, F3, flag3, es3 = gpu_run(w3)
+    _, ft3, _ = gpu_cg(w3, F3, flag3)
+    s3 = lcs.smooth_gaussian(3, w3.ng, w3.seed_periodic, 1.0, ft3.to(tdt).contiguous())
+    n2 = 81
+    Xc, Yc = np.meshgrid((np.arange(n2) - 40) * 0.05, (np.arange(n2) - 40) * 0.05)
+    ring = torch.from_numpy(np.exp(-(np.hypot(Xc, Yc) - 1.2) ** 2 / (2 * 0.25 ** 2)).ravel().astype(dt)).cuda()
+    n_masked = 0
+    for (dim, ng, dx, per, field, kmin, smin) in ((2, w.ng, w.seed_spacing, w.seed_periodic, s1, 0.0, 0.05),
+                                                   (3, w3.ng, w3.seed_spacing, w3.seed_periodic, s3, 0.0, 0.1),
+                                                   (2, (n2, n2, 1), (0.05, 0.05, 1.0), (0, 0, 0), ring, 1.0, 0.8)):
+        kap, d, m = (cpu(t) for t in lcs.ridge(dim, ng, dx, per, kmin, smin, field))
+        ko, do, mo = oracle.ridge(dim, ng[:dim], dx[:dim], per[:dim], kmin, smin, cpu(field).astype(np.float64))
+        assert np.array_equal(np.isnan(kap), np.isnan(ko))
+        ok = np.isfinite(ko)
+        scale = max(1.0, np.abs(ko[ok]).max())
+        assert ok.sum() > 1000 and np.max(np.abs(kap[ok] - ko[ok])) <= tol * scale and np.max(np.abs(d[ok] - do[ok])) <= tol * scale
+        delta = min(dx[:dim])
+        sv = cpu(field).astype(np.float64)
+        margin = np.minimum(np.abs(ko + kmin), np.abs(np.abs(do) - np.abs(ko) * delta / 2))
+        clear = ok & (margin > 10 * tol * scale) & (np.abs(sv - smin) > 1e-6)
+        assert clear.sum() > 0.5 * ok.sum(), (clear.sum(), ok.sum(), scale)     # the flat far field of the ring sits at the thresholds
+        assert np.array_equal(m[clear], mo[clear]) and np.all(m[~ok] == 0)
+        n_masked += int(mo.sum())
+    assert n_masked > 300
