@@ -10,7 +10,7 @@
  * The method is an iteration (RK4 on interpolated data) and an approximation (finite-difference
  * gradient), so the oracle follows the algorithm step by step in the paper's order; readings of
  * points where the paper is silent are the numbered "O" rules of SURVEY.md 8.2 / DESIGN.md.
- * Every function is pinned by tests/test_oracle_pins.py (closed forms P1-P14); nothing here is
+ * Every function is pinned by tests/test_oracle_pins.py (pins P1-P20); nothing here is
  * "parity unpinned".
  *
  * Build: gcc -O2 -ffp-contract=off -fopenmp -shared -fPIC  (no FMA contraction: the canonical
