@@ -92,6 +92,9 @@ void lcs_field_destroy(lcs_field *f);
  * warp gathers from neighbouring cells; results are returned in the caller's order;
  * "bundle_steps" k = re-bundle every k RK4 steps (0 = once per snapshot window; unstructured meshes: every 160 steps);
  * "bundle_order" / "simplex_order" 0 = Morton, 1 = row-major (x fastest, default) sort key over cells / bins;
+ * "field_sets" m = keep the blended fields of the last m chunks resident (about 7 GB each for a 128^3 grid and 50-step chunks)
+ * and reuse them when a later lcs_advect needs the same snapshot pair and stage times (FTLE time series: volumes released one
+ * snapshot interval apart share most windows); "field_sets_clear" = forget them;
  * "preblend" -1/0/1 and "preblend_steps" k: 3D fp32 Cartesian grids gather from per-stage-time blended fields, k steps per launch;
  * "ld256" 0/1 = gather each 32-byte node record with one 256-bit load; "block" = threads per block;
  * "time_windows" 0/1 = record CUDA events around the integrator launches (read with lcs_field_get_info). */

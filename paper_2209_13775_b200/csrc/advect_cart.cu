@@ -25,6 +25,8 @@
 //    short kernel per RK4 stage with the stage state in global memory.
 #include <math.h>
 
+#include <algorithm>
+
 #include "bundle_sort.cuh"
 #include "lcs_internal.cuh"
 
@@ -843,8 +845,36 @@ lcs_status cart_advect_impl(lcs_field *f, int64_t n, const void *seeds_, double 
         if constexpr (kCanBlend) {
             if (u.blend) {
                 XPair *fields = (XPair *)(base + o_fields);
-                LCS_LAUNCH(blend_xpair_kernel, lcs_blocks(f->nrec, 256), 256, 0, st, (const float *)raw_a, (const float *)raw_b, g.n[0], g.n[1],
-                           g.n[2], f->cart.np[0], f->cart.np[1], f->cart.np[2], d_ftau + u.ftau_off, u.nfields, fields, f->nrec);
+                bool need_blend = true;
+                if (f->opt_field_sets > 0) {
+                    // resident field sets: reuse the set blended for the same snapshot pair and the same stage times
+                    const float *tb = ftau.data() + u.ftau_off;
+                    const size_t bytes = (size_t)u.nfields * (size_t)f->nrec * 32;
+                    FieldSet *hit = nullptr, *victim = nullptr;
+                    for (FieldSet &fs : f->field_sets)
+                        if (fs.pair == w.s[0] && fs.tau.size() == (size_t)u.nfields && std::equal(fs.tau.begin(), fs.tau.end(), tb)) hit = &fs;
+                    if (!hit) {
+                        if ((int64_t)f->field_sets.size() < f->opt_field_sets) { f->field_sets.emplace_back(); victim = &f->field_sets.back(); }
+                        else for (FieldSet &fs : f->field_sets) if (!victim || fs.age < victim->age) victim = &fs;
+                        if (victim->bytes < bytes) {
+                            if (victim->buf) { cudaStreamSynchronize(st); cudaFree(victim->buf); victim->buf = nullptr; victim->bytes = 0; }
+                            LCS_CUDA_OK(cudaMalloc(&victim->buf, bytes));
+                            victim->bytes = bytes;
+                        }
+                        victim->pair = w.s[0];
+                        victim->tau.assign(tb, tb + u.nfields);
+                        f->info_field_set_misses++;
+                        hit = victim;
+                    } else {
+                        need_blend = false;
+                        f->info_field_set_hits++;
+                    }
+                    hit->age = ++f->field_set_clock;
+                    fields = (XPair *)hit->buf;
+                }
+                if (need_blend)
+                    LCS_LAUNCH(blend_xpair_kernel, lcs_blocks(f->nrec, 256), 256, 0, st, (const float *)raw_a, (const float *)raw_b, g.n[0],
+                               g.n[1], g.n[2], f->cart.np[0], f->cart.np[1], f->cart.np[2], d_ftau + u.ftau_off, u.nfields, fields, f->nrec);
                 {
                     WindowTimer timer(f, st);
                     if (fast)

@@ -336,6 +336,7 @@ extern "C" void lcs_field_destroy(lcs_field *f)
     for (cudaEvent_t ev : f->win_ev) cudaEventDestroy(ev);
     for (int k = 0; k < lcs_field::kPairCache; ++k) if (f->pair_buf[k]) cudaFree(f->pair_buf[k]);
     if (f->scratch.buf) cudaFree(f->scratch.buf);
+    for (FieldSet &fs : f->field_sets) if (fs.buf) cudaFree(fs.buf);
     if (f->h_seeds) cudaFree(f->h_seeds);
     if (f->h_flow) cudaFree(f->h_flow);
     if (f->h_ftle) cudaFree(f->h_ftle);
@@ -352,6 +353,8 @@ extern "C" lcs_status lcs_field_set_snapshot(lcs_field *f, int32_t s, const void
     // any cached pair built from the old contents is stale
     for (int k = 0; k < lcs_field::kPairCache; ++k)
         if (f->pair_snap[k] == s || f->pair_snap[k] == s - 1) f->pair_snap[k] = -1;
+    for (FieldSet &fs : f->field_sets)
+        if (fs.pair == s || fs.pair == s - 1) { fs.pair = -1; fs.tau.clear(); }
     if (f->ring) {
         if (is_device_ptr) { lcs_set_error("ring mode streams snapshots from HOST memory"); return LCS_ERR_INVALID_ARG; }
         f->host_src[s] = vel;
@@ -386,6 +389,13 @@ extern "C" lcs_status lcs_field_set_option(lcs_field *f, const char *key, int64_
     else if (!strcmp(key, "simplex_order") && (value == 0 || value == 1)) f->opt_simplex_order = value;
     else if (!strcmp(key, "ld256") && (value == 0 || value == 1)) f->opt_ld256 = value;
     else if (!strcmp(key, "preblend") && value >= -1 && value <= 1) f->opt_preblend = value;
+    else if (!strcmp(key, "field_sets") && value >= 0 && value <= 64) {
+        f->opt_field_sets = value;
+        cudaDeviceSynchronize();
+        for (FieldSet &fs : f->field_sets) if (fs.buf) cudaFree(fs.buf);
+        f->field_sets.clear();
+    }
+    else if (!strcmp(key, "field_sets_clear")) { for (FieldSet &fs : f->field_sets) { fs.pair = -1; fs.tau.clear(); } }
     else if (!strcmp(key, "preblend_steps") && value >= 1 && value <= 256) f->opt_preblend_steps = value;
     else if (!strcmp(key, "time_windows") && (value == 0 || value == 1)) { f->opt_time_windows = value; f->win_ev_used = 0; }
     else if (!strcmp(key, "block") && (value == 0 || (value >= 32 && value <= 1024 && value % 32 == 0))) f->opt_block = value;
@@ -402,6 +412,8 @@ extern "C" lcs_status lcs_field_get_info(const lcs_field *f, const char *key, in
     else if (!strcmp(key, "n_cells")) *value = f->kind == LCS_MESH_SIMPLEX ? f->mesh.nc : 0;
     else if (!strcmp(key, "n_bins")) *value = f->kind == LCS_MESH_SIMPLEX ? (int64_t)f->mesh.nb[0] * f->mesh.nb[1] * f->mesh.nb[2] : 0;
     else if (!strcmp(key, "ring")) *value = f->ring;
+    else if (!strcmp(key, "field_set_hits")) *value = f->info_field_set_hits;
+    else if (!strcmp(key, "field_set_misses")) *value = f->info_field_set_misses;
     else if (!strcmp(key, "window_launches")) *value = (int64_t)(f->win_ev_used / 2);
     else if (!strcmp(key, "window_time_ns")) {          // synchronises; sum of the bracketed launch durations
         double ms = 0.0;

@@ -88,6 +88,17 @@ struct EarlyCg {
     uint8_t *flag = nullptr, *status = nullptr;
 };
 
+// A resident set of blended x-pair fields (one chunk of the pre-blended integrator): FTLE time series release one seed grid
+// per snapshot interval, and consecutive volumes share nine tenths of their stage times; with 180 GB of HBM the sets of the
+// last windows stay resident and are reused instead of blended again (option "field_sets" = how many to keep, 0 = off).
+struct FieldSet {
+    int pair = -1;                // snapshot pair the set was blended from
+    std::vector<float> tau;       // stage-time weights of its fields, compared exactly
+    void *buf = nullptr;
+    size_t bytes = 0;
+    int64_t age = 0;
+};
+
 struct lcs_field {
     int dim = 0, kind = 0;
     int vel_dtype = 0, compute_dtype = 0;
@@ -123,6 +134,8 @@ struct lcs_field {
     uint8_t *h_flag = nullptr;
     int64_t h_cap = 0;
     EarlyCg early;
+    std::vector<FieldSet> field_sets;
+    int64_t field_set_clock = 0, info_field_set_hits = 0, info_field_set_misses = 0;
     // options
     int64_t opt_integrator = 0;   // 0 auto, 1 fused, 2 split
     int64_t opt_bundle = -1;      // re-bundle tracers by cell: -1 auto (large seed sets), 0 off, 1 on
@@ -131,6 +144,7 @@ struct lcs_field {
     int64_t opt_bundle_steps = 0; // RK4 steps between re-bundlings (0 = once per snapshot window)
     int64_t opt_preblend = -1;    // 3D fp32 Cartesian: gather from per-stage-time blended fields (-1 auto, 0 off, 1 on)
     int64_t opt_preblend_steps = 50; // RK4 steps per launch of the pre-blended integrator (2k+1 blended fields resident)
+    int64_t opt_field_sets = 0;   // number of resident blended-field sets (0 = blend every chunk into scratch)
     int64_t opt_ld256 = 1;        // gather pair records with one 256-bit load instead of two 128-bit loads
     int64_t opt_block = 0;        // threads per block override (0 = default)
     int64_t opt_time_windows = 0; // record CUDA events around every window (hot) kernel launch
