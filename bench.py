@@ -4,18 +4,27 @@
 A "step" is one pass of the whole hot path over one batch of synthetic input: with the velocity field resident,
 lcs_advect (RK4 flow map of the whole seed grid) followed by lcs_cg_ftle (gradient, Cauchy-Green tensor, FTLE).
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--extra-configs 4,5|none] [--impl reference]
 
 N = 1: the workload is BASELINE.json config 3 (3D ABC flow, 128^3 periodic grid, 256^3 seeds, 500 RK4 steps, fp32),
-the 3D Cartesian configuration north_star's roofline target is stated for; --config picks another one.
+the 3D Cartesian configuration north_star's roofline target is stated for; --config picks another one.  The default
+line also carries, under "configs", the same figures for configs 4 and 5 (the other two 3D configs of the >= 50% target).
 N > 1 (torchrun, one rank per GPU): the path shards with NO data-path collective -- rank r computes an independent
 FTLE volume (the seed grid released at t0 = 0.5 r: the time series of PAPER.md:37) -- so scaling is "weak"; the only
 communication is the barrier and the max-over-ranks of the device time.
 --impl reference times the CPU oracle (oracle/, test infrastructure) on a bounded sample of the same workload.
+
+Roofline: every peak is MEASURED in this run by the library's own micro-kernels (lcs_measure_peak: FP32 / FP64 FMA, L1-hit
+256-bit gathers, shared-memory gathers, L2 sequential and random-sector reads, random 32-byte HBM gathers, launch latency);
+the HBM streaming peak is the driver's MEASURED_PEAKS.json.  `bound` names the resource that the committed ncu counters
+(profiles/roofline_cfgN.json, extracted from the --set full tables beside them) show closest to saturation; `frac` is the
+useful work the kernel gets out of that resource (bytes its gathers deliver to registers per seed-step x rate) over the
+measured peak; the 720 / 900-flop and 768 / 640-byte model figures of SURVEY.md 8.3 are kept beside it.
 """
 from __future__ import annotations
 
 import argparse
+import gc
 import json
 import os
 import subprocess
@@ -31,6 +40,7 @@ if ROOT not in sys.path:
 
 METRIC = "seed_rk4_steps_per_s"
 UNIT = "seed-steps/s"
+L2_BYTES = 126e6
 
 
 # ------------------------------------------------------------------------------------------------
@@ -112,12 +122,35 @@ class ClockSampler:
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def measured_peaks():
-    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
-    if os.path.exists(p):
-        d = json.load(open(p))
-        return float(d["hbm_gbs"]), float(d.get("sm_max_mhz", 1965.0)), "measured (MEASURED_PEAKS.json)"
-    return 6650.0, 1965.0, "fallback (B200_PROFILING.md)"
+_PEAKS = None
+
+
+def measured_peaks(lcs):
+    """Peaks measured in THIS run by the library's micro-kernels, plus the driver's HBM copy figure."""
+    global _PEAKS
+    if _PEAKS is None:
+        p = {k: lcs.measure_peak(k) for k in lcs.PEAK_KINDS}
+        path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+        if os.path.exists(path):
+            d = json.load(open(path))
+            p["hbm_copy_driver_gbs"] = float(d["hbm_gbs"])
+            p["hbm_source"] = "measured (MEASURED_PEAKS.json)"
+        else:
+            p["hbm_copy_driver_gbs"] = 6650.0
+            p["hbm_source"] = "fallback (B200_PROFILING.md)"
+        _PEAKS = p
+    return _PEAKS
+
+
+def profile_constants(cfg: int):
+    """Per-kernel constants taken from the committed ncu tables (profiles/roofline_cfgN.json names its source table):
+    DRAM bytes per launch, bytes the gathers deliver to registers per seed-step, executed warp instructions per seed-step and
+    the pipe utilisations that decide which resource binds."""
+    for name in ("roofline_cfg%d.json" % cfg, "traffic_cfg%d.txt" % cfg):
+        path = os.path.join(ROOT, "profiles", name)
+        if os.path.exists(path):
+            return json.load(open(path))
+    return {}
 
 
 # ------------------------------------------------------------------------------------------------
@@ -203,12 +236,204 @@ def reduce_over_ranks(elapsed_ms, seed_steps, seeds, device, world):
 
 
 # ------------------------------------------------------------------------------------------------
+def roofline_block(lcs, cfg, w, kernel_s, units_per_launch, share, win_launches, win_s_per_pass):
+    """The roofline object of one config (see the module docstring)."""
+    pk = measured_peaks(lcs)
+    prof = profile_constants(cfg)
+    rate = units_per_launch / max(kernel_s, 1e-12)                         # seed-steps per second inside the dominant kernel
+    bytes_unit = algorithmic_bytes_per_seed_step(w)
+    common = {"traffic": prof.get("dram_bytes_per_launch"), "seed_steps_per_launch": units_per_launch, "avg_launch_ms": kernel_s * 1e3,
+              "launches_timed": int(win_launches), "kernel_share_of_step": share, "algorithmic_bytes_per_seed_step": bytes_unit,
+              "peak_source": "measured in this run (lcs_measure_peak); HBM copy: " + pk["hbm_source"],
+              "peaks": {k: v for k, v in pk.items() if k != "hbm_source"},
+              "counters": {k: prof[k] for k in ("l1_data_pipe_pct", "issue_slots_pct", "fma_pipe_pct", "fp64_pipe_pct", "dram_pct", "l1_hit_pct",
+                                                "lanes_per_instruction", "executed_inst_per_seed_step", "source") if k in prof}}
+    three_d_f32 = w.dim == 3 and w.compute_dtype == np.float32
+    if three_d_f32:
+        cart = w.kind == 0
+        flop_unit = 720.0 if cart else 900.0
+        model_alu = {"flop_per_seed_step": flop_unit, "achieved": flop_unit * rate / 1e12, "peak": pk["fp32_fma_tflops"], "unit": "TFLOP/s",
+                     "frac": flop_unit * rate / 1e12 / pk["fp32_fma_tflops"],
+                     "note": "SURVEY.md 8.3 model flop count of the straightforward scheme (not what the kernel executes) over the measured FFMA peak"}
+        model_gather = {"bytes_per_seed_step": bytes_unit, "achieved": bytes_unit * rate / 1e9, "unit": "GB/s",
+                        "note": "SURVEY.md 8.3 model gather bytes of the straightforward 4-stage scheme; the kernel loads less (pre-blended "
+                                "fields / held cell), so this is a statement about the method, not a utilisation"}
+        delivered = prof.get("l1_bytes_to_registers_per_seed_step")
+        kern = prof.get("kernel", "cart_xpair_kernel" if cart else "simplex_window_kernel")
+        staged = "tma" in kern
+        peak_key = "smem_records_swizzled_gbs" if staged else "l1_gather_line_gbs"
+        if delivered:
+            ach = delivered * rate / 1e9
+            return {"bound": "l1", "kernel": kern, "achieved": ach, "peak": pk[peak_key], "unit": "GB/s", "frac": ach / pk[peak_key],
+                    "bytes_to_registers_per_seed_step": delivered,
+                    "note": "L1 / shared-memory data pipe (128 B per clock per SM into registers): bytes the kernel's gathers actually deliver to "
+                            "registers per seed-step (ncu request counts, profiles/) x rate, over the measured best-case gather rate (%s)" % peak_key,
+                    "model_alu": model_alu, "model_gather": model_gather, **common}
+        return {"bound": "alu", "kernel": kern, "achieved": model_alu["achieved"], "peak": model_alu["peak"], "unit": "TFLOP/s",
+                "frac": model_alu["frac"], "note": "no ncu table for this kernel yet: model flop count over the measured FFMA peak",
+                "model_gather": model_gather, **common}
+    # configs 1-2 (and other small fp64 cases): under / near one wave of threads, fields resident in L1 / L2: latency-bound.
+    # SURVEY.md 8.3: report time-to-solution and microseconds per RK4 step (FP64 pipe share for config 2), no HBM fraction.
+    us_per_step = win_s_per_pass * 1e6 / max(w.n_steps, 1)
+    flop_unit = 250.0 if w.kind == 0 else 400.0
+    return {"bound": "latency", "kernel": "cart_window_kernel" if w.kind == 0 else "simplex_window_kernel",
+            "achieved": us_per_step, "peak": pk["launch_us"], "unit": "us per RK4 step (all seeds)", "frac": None,
+            "fp64_pipe": {"flop_per_seed_step": flop_unit, "achieved": flop_unit * rate / 1e12, "peak": pk["fp64_fma_tflops"], "unit": "TFLOP/s",
+                          "frac": flop_unit * rate / 1e12 / pk["fp64_fma_tflops"]},
+            "note": "fewer seeds than (or about) one wave of 148 SMs x 2048 threads and fields that live in L1 / L2: bound by launch and "
+                    "dependent-load latency; `peak` is the measured empty-launch latency for scale", **common}
+
+
+def run_config(args, lcs, cfg, steps, warmup, rank, world, local, with_e2e, with_cpu):
+    """Times `steps` passes of the hot path on one config; returns the fields of the JSON line (rank 0) or None."""
+    import torch
+    import torch.distributed as dist
+    w, runs = make_workload(cfg, rank)
+    ring = 4 if cfg == 5 else 0
+    field = lcs.Field.from_workload(w, max_resident_snapshots=ring, pinned=True)
+    if cfg == 5:
+        field.set_option("field_sets", 12)               # time series: consecutive volumes share 9 of their 10 windows (DESIGN.md)
+    for kv in args.option:
+        k, v = kv.split("=")
+        field.set_option(k, int(v))
+    tdt = torch.float32 if w.compute_dtype == np.float32 else torch.float64
+    seeds_h = torch.from_numpy(w.seeds()).pin_memory()
+    seeds_d = seeds_h.cuda()
+    n = w.n_seeds
+    flow = torch.empty_like(seeds_d)
+    flag = torch.empty(n, dtype=torch.uint8, device="cuda")
+    es = torch.empty(n, dtype=torch.int32, device="cuda")
+    stream = torch.cuda.current_stream()
+    # set-up: everything lcs_advect needs is allocated here, once (the hot calls never allocate)
+    field.reserve(n, max(int(round((tf - t0) / h)) for (t0, tf, h) in runs))
+
+    def one_pass(count=None):
+        """All rows of the hot path over one batch: flow map(s) -> CG -> FTLE."""
+        if cfg == 5:
+            field.set_option("field_sets_clear", 0)      # every pass starts without resident blended fields: reuse only WITHIN a pass
+        for (t0, tf, h) in runs:
+            field.advect(seeds_d, t0, tf, h, flowmap=flow, exit_flag=flag, exit_step=es, reserve=False)
+            lcs.cg_ftle(w.dim, w.ng, w.seed_spacing, w.seed_periodic, w.period, flow, flag, tf - t0, want_cg=True, want_status=False)
+            if count is not None:
+                count.append(float(es.sum(dtype=torch.int64).item()))
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # inputs of one pass: tracer records (two buffers when re-bundled) + seeds + outputs + the fields gathered from
+    state_bytes = n * (32 * 2 + w.dim * 2 * seeds_h.element_size() + 5) + float(np.asarray(w.vel[0]).nbytes) * 2
+    flush = state_bytes < L2_BYTES
+    flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device="cuda") if flush else None
+    for _ in range(max(warmup - 1, 0)):
+        one_pass()
+    counts = []
+    one_pass(counts)                                     # last warm-up pass: seed-steps actually taken (exits shorten trajectories),
+    steps_per_pass = float(sum(counts))                  # summed over EVERY run of the pass
+    field.set_option("time_windows", 1)
+    sampler = ClockSampler(local)
+    sampler.start()
+    l0 = lcs.kernel_launch_count()
+    barrier()
+    if flush:
+        # small configs: the whole working set would stay in the 126 MB L2 between passes; write a 256 MB buffer between
+        # timed passes (outside the per-pass event brackets)
+        elapsed_ms = 0.0
+        for _ in range(steps):
+            flush_buf.fill_(1)
+            ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            ev0.record(stream)
+            one_pass()
+            ev1.record(stream)
+            torch.cuda.synchronize()
+            elapsed_ms += ev0.elapsed_time(ev1)
+        barrier()
+    else:
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev0.record(stream)
+        for _ in range(steps):
+            one_pass()
+        ev1.record(stream)
+        barrier()
+        elapsed_ms = ev0.elapsed_time(ev1)
+    launches = lcs.kernel_launch_count() - l0
+    clocks = sampler.stop()
+    win_ns = field.info("window_time_ns")
+    win_launches = field.info("window_launches")
+    field.set_option("time_windows", 0)
+    elapsed_ms, steps_all, seeds_all = reduce_over_ranks(elapsed_ms, steps_per_pass, float(n * len(runs)), "cuda", world)
+    sec_per_step = elapsed_ms * 1e-3 / steps
+    value = steps_all / sec_per_step
+
+    # end to end through the C-ABI with HOST buffers: H2D of the seeds, D2H of the Cauchy-Green tensor and the FTLE inside the
+    # timed region (the same outputs the device-timed pass writes)
+    e2e = None
+    if with_e2e:
+        ncg = 3 if w.dim == 2 else 6
+        ftle_h = torch.empty(n, dtype=tdt).pin_memory()
+        cg_h = torch.empty((n, ncg), dtype=tdt).pin_memory()
+        esz = seeds_h.element_size()
+        e_steps = steps if cfg == args.config else min(steps, 5)
+
+        def e2e_pass():
+            if cfg == 5:
+                field.set_option("field_sets_clear", 0)
+            for (t0, tf, h) in runs:
+                field.ftle_host(w.ng, w.seed_spacing, w.seed_periodic, w.period, seeds_h.numpy(), t0, tf, h, ftle=ftle_h.numpy(), cg=cg_h.numpy())
+        e2e_pass()
+        barrier()
+        t0w = time.perf_counter()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev0.record(stream)
+        for _ in range(e_steps):
+            e2e_pass()
+        ev1.record(stream)
+        barrier()
+        e_ms = max(ev0.elapsed_time(ev1), 0.0)
+        e_wall = (time.perf_counter() - t0w) * 1e3
+        e_ms = max(e_ms, e_wall)                          # copies on the legacy stream: wall clock bounds the region
+        te = torch.tensor([e_ms], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(te, op=dist.ReduceOp.MAX)
+        e2e = {"value": steps_all / (float(te.item()) * 1e-3 / e_steps), "unit": UNIT, "steps": e_steps,
+               "h2d_bytes_per_step": int(n * w.dim * esz * len(runs)), "d2h_bytes_per_step": int(n * (1 + ncg) * esz * len(runs)),
+               "outputs": "cg + ftle", "seeds_per_s_to_ftle": seeds_all / (float(te.item()) * 1e-3 / e_steps)}
+        del ftle_h, cg_h
+
+    line = None
+    if rank == 0:
+        kernel_s = win_ns * 1e-9 / max(win_launches, 1)                    # average launch duration of the dominant kernel
+        units_per_launch = steps_per_pass * steps / max(win_launches, 1)
+        share = (win_ns * 1e-9) / (elapsed_ms * 1e-3) if world == 1 else None
+        roofline = roofline_block(lcs, cfg, w, kernel_s, units_per_launch, share, win_launches, win_ns * 1e-9 / steps)
+        l2_note = ("flushed: a 256 MB buffer is written between timed passes (working set %.1f MB < L2)" % (state_bytes / 1e6)) if flush else \
+                  ("inputs larger than L2: tracer records, seeds, outputs and fields are %.0f MB per pass" % (state_bytes / 1e6))
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warmup,
+                "ms_per_step": sec_per_step * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f32" if w.compute_dtype == np.float32 else "f64", "data": "synthetic",
+                "config": {"workload": w.name, "baseline_config": cfg, "seeds": n * len(runs), "rk4_steps": w.n_steps,
+                           "seed_steps_per_pass": steps_per_pass, "parallelism": "independent FTLE volumes per rank, no collective",
+                           "options": dict(kv.split("=") for kv in args.option), "l2": l2_note},
+                "seeds_per_s_to_ftle": seeds_all / sec_per_step, "roofline": roofline, "clocks": clocks, "gpu_launches": int(launches),
+                "e2e": e2e}
+        if with_cpu and world == 1:
+            line["cpu_baseline"] = cpu_baseline(w, runs)
+    field.close()
+    del field, seeds_d, flow, flag, es, flush_buf, seeds_h, w
+    gc.collect()
+    torch.cuda.empty_cache()
+    return line
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--extra-configs", default="4,5", help="configs whose figures ride along under `configs` (N = 1, default config only)")
     ap.add_argument("--impl", default="ours")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -234,152 +459,18 @@ def main():
         dist.barrier()
     lcs.lib()
 
-    w, runs = make_workload(args.config, rank)
-    ring = 4 if args.config == 5 else 0
-    field = lcs.Field.from_workload(w, max_resident_snapshots=ring, pinned=True)
-    if args.config == 5:
-        field.set_option("field_sets", 12)               # time series: consecutive volumes share 9 of their 10 windows
-    for kv in args.option:
-        k, v = kv.split("=")
-        field.set_option(k, int(v))
-    tdt = torch.float32 if w.compute_dtype == np.float32 else torch.float64
-    seeds_h = torch.from_numpy(w.seeds()).pin_memory()
-    seeds_d = seeds_h.cuda()
-    n = w.n_seeds
-    flow = torch.empty_like(seeds_d)
-    flag = torch.empty(n, dtype=torch.uint8, device="cuda")
-    es = torch.empty(n, dtype=torch.int32, device="cuda")
-    stream = torch.cuda.current_stream()
-
-    def one_pass():
-        """All rows of the hot path over one batch: flow map(s) -> CG -> FTLE.  Returns seed-steps taken."""
-        ftles = []
-        if args.config == 5:
-            field.set_option("field_sets_clear", 0)      # every pass starts without resident blended fields: reuse only WITHIN a pass
-        for (t0, tf, h) in runs:
-            field.advect(seeds_d, t0, tf, h, flowmap=flow, exit_flag=flag, exit_step=es)
-            cg, ftle, st = lcs.cg_ftle(w.dim, w.ng, w.seed_spacing, w.seed_periodic, w.period, flow, flag, tf - t0,
-                                       want_cg=True, want_status=False)
-            ftles.append(ftle)
-        return ftles
-
-    def barrier():
-        torch.cuda.synchronize()
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    for _ in range(args.warmup):
-        one_pass()
-    # seed-steps actually taken in one pass (exits shorten trajectories): sum of exit_step
-    torch.cuda.synchronize()
-    steps_per_pass = 0.0
-    for (t0, tf, h) in runs[-1:]:
-        steps_per_pass = float(es.sum(dtype=torch.int64).item()) * len(runs) if len(runs) > 1 else float(es.sum(dtype=torch.int64).item())
-    field.set_option("time_windows", 1)
-    sampler = ClockSampler(local)
-    sampler.start()
-    l0 = lcs.kernel_launch_count()
-    barrier()
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    ev0.record(stream)
-    for _ in range(args.steps):
-        one_pass()
-    ev1.record(stream)
-    barrier()
-    elapsed_ms = ev0.elapsed_time(ev1)
-    launches = lcs.kernel_launch_count() - l0
-    clocks = sampler.stop()
-    win_ns = field.info("window_time_ns")
-    win_launches = field.info("window_launches")
-    field.set_option("time_windows", 0)
-    elapsed_ms, steps_all, seeds_all = reduce_over_ranks(elapsed_ms, steps_per_pass, float(n * len(runs)), "cuda", world)
-    sec_per_step = elapsed_ms * 1e-3 / args.steps
-    value = steps_all / sec_per_step
-
-    # end to end through the C-ABI with HOST buffers (H2D seeds + D2H FTLE inside the timed region)
-    e2e = None
-    if not args.no_e2e:
-        ftle_h = torch.empty(n, dtype=tdt).pin_memory()
-        esz = seeds_h.element_size()
-        def e2e_pass():
-            if args.config == 5:
-                field.set_option("field_sets_clear", 0)
-            for (t0, tf, h) in runs:
-                field.ftle_host(w.ng, w.seed_spacing, w.seed_periodic, w.period, seeds_h.numpy(), t0, tf, h, ftle=ftle_h.numpy())
-        e2e_pass()
-        barrier()
-        t0w = time.perf_counter()
-        ev0.record(stream)
-        for _ in range(args.steps):
-            e2e_pass()
-        ev1.record(stream)
-        barrier()
-        e_ms = max(ev0.elapsed_time(ev1), 0.0)
-        e_wall = (time.perf_counter() - t0w) * 1e3
-        e_ms = max(e_ms, e_wall)                          # copies on the legacy stream: wall clock bounds the region
-        te = torch.tensor([e_ms], dtype=torch.float64, device="cuda")
-        if world > 1:
-            dist.all_reduce(te, op=dist.ReduceOp.MAX)
-        e2e = {"value": steps_all / (float(te.item()) * 1e-3 / args.steps), "unit": UNIT,
-               "h2d_bytes_per_step": int(n * w.dim * esz * len(runs)), "d2h_bytes_per_step": int(n * esz * len(runs)),
-               "seeds_per_s_to_ftle": seeds_all / (float(te.item()) * 1e-3 / args.steps)}
-
-    if rank == 0:
-        hbm_gbs, sm_max_mhz, peak_src = measured_peaks()
-        kernel_s = win_ns * 1e-9 / max(win_launches, 1)                    # average launch duration of the dominant kernel
-        bytes_unit = algorithmic_bytes_per_seed_step(w)
-        units_per_launch = steps_per_pass * args.steps / max(win_launches, 1)
-        achieved = bytes_unit * units_per_launch / max(kernel_s, 1e-12) / 1e9
-        share = (win_ns * 1e-9) / (elapsed_ms * 1e-3) if world == 1 else None
-        common = {"traffic": None, "seed_steps_per_launch": units_per_launch, "avg_launch_ms": kernel_s * 1e3,
-                  "kernel_share_of_step": share, "algorithmic_bytes_per_seed_step": bytes_unit}
-        if w.kind == 0 and w.dim == 3 and w.compute_dtype == np.float32:
-            # DESIGN.md section 6: the 3D fp32 Cartesian integrator gathers from L1 (DRAM < 20% of peak) and is bound by
-            # FP32 issue slots + L1 wavefronts.  ALU roofline: SURVEY.md 8.3's 720 flop per seed-step against
-            # 148 SMs x 128 FP32 lanes x 2 flop x max SM clock.
-            flop_unit = 720.0
-            peak_tf = 148 * 128 * 2 * sm_max_mhz * 1e6 / 1e12
-            ach_tf = flop_unit * units_per_launch / max(kernel_s, 1e-12) / 1e12
-            l1_peak = 148 * 128 * sm_max_mhz * 1e6 / 1e9
-            roofline = {"bound": "alu", "kernel": "cart_xpair_kernel", "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s",
-                        "frac": ach_tf / peak_tf, "peak_source": "derived: 148 SMs x 128 FP32 lanes x 2 x %.0f MHz (DESIGN.md)" % sm_max_mhz,
-                        "algorithmic_flop_per_seed_step": flop_unit,
-                        "l1_gather": {"achieved": achieved, "peak": l1_peak, "unit": "GB/s", "frac": achieved / l1_peak,
-                                      "note": "768 B per seed-step of the straightforward 4-stage scheme against 148 SMs x 128 B/clk; "
-                                              "above 1 because the kernel gathers pre-blended fields and reuses corners in registers"},
-                        **common}
-        elif w.kind == 1 and w.dim == 3 and w.compute_dtype == np.float32:
-            # tets in fp32 (config 4): measured DRAM 1.5% of peak, L2 hit 80-96%, issue slots 58%, L1 wavefronts 63%
-            # (profiles/r1_cfg4_simplex.md): not HBM-bound.  ALU roofline with SURVEY.md 8.3's 900 flop per seed-step.
-            flop_unit = 900.0
-            peak_tf = 148 * 128 * 2 * sm_max_mhz * 1e6 / 1e12
-            ach_tf = flop_unit * units_per_launch / max(kernel_s, 1e-12) / 1e12
-            roofline = {"bound": "alu", "kernel": "simplex_window_kernel", "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s",
-                        "frac": ach_tf / peak_tf, "peak_source": "derived: 148 SMs x 128 FP32 lanes x 2 x %.0f MHz (DESIGN.md)" % sm_max_mhz,
-                        "algorithmic_flop_per_seed_step": flop_unit,
-                        "hbm_gather": {"achieved": achieved, "peak": hbm_gbs, "unit": "GB/s", "frac": achieved / hbm_gbs,
-                                       "note": "640 B per seed-step of the straightforward scheme against the measured HBM copy peak; far "
-                                               "above 1 because the mesh is served by L1/L2 and the held cell skips most gathers"},
-                        **common}
-        else:
-            roofline = {"bound": "hbm", "kernel": "cart_window_kernel" if w.kind == 0 else "simplex_window_kernel",
-                        "achieved": achieved, "peak": hbm_gbs, "unit": "GB/s", "frac": achieved / hbm_gbs, "peak_source": peak_src,
-                        "note": "algorithmic gather bytes; small fields are served by L1/L2, so this can exceed the HBM copy peak "
-                                "(DESIGN.md section 6)", **common}
-        tr = os.path.join(ROOT, "profiles", "traffic_cfg%d.txt" % args.config)
-        if os.path.exists(tr):
-            roofline["traffic"] = json.load(open(tr)).get("dram_bytes_per_launch")
-        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-                "ms_per_step": sec_per_step * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-                "dtype": "f32" if w.compute_dtype == np.float32 else "f64", "data": "synthetic",
-                "config": {"workload": w.name, "baseline_config": args.config, "seeds": n * len(runs), "rk4_steps": w.n_steps,
-                           "seed_steps_per_pass": steps_per_pass, "parallelism": "independent FTLE volumes per rank, no collective",
-                           "l2": "inputs larger than L2: seeds + tracer state are %.0f MB per pass" % (n * (w.dim * 2 + 3) * 4 / 1e6)},
-                "seeds_per_s_to_ftle": seeds_all / sec_per_step, "roofline": roofline, "clocks": clocks, "gpu_launches": int(launches),
-                "e2e": e2e}
-        if not args.no_cpu_baseline and world == 1:
-            line["cpu_baseline"] = cpu_baseline(w, runs)
+    line = run_config(args, lcs, args.config, args.steps, max(args.warmup, 1), rank, world, local, not args.no_e2e, not args.no_cpu_baseline)
+    extras = []
+    if world == 1 and args.config == 3 and args.extra_configs not in ("", "none") and not args.option:
+        extras = [int(c) for c in args.extra_configs.split(",") if int(c) != args.config]
+    if extras and line is not None:
+        line["configs"] = {}
+        for c in extras:
+            # the other 3D configs of the >= 50% target, same passes / timing rules, fewer passes so that the default run stays short
+            sub = run_config(args, lcs, c, min(args.steps, 10), min(max(args.warmup, 1), 3), rank, world, local, not args.no_e2e, False)
+            line["configs"][str(c)] = {k: sub[k] for k in ("value", "unit", "steps", "warmup", "ms_per_step", "dtype", "config", "seeds_per_s_to_ftle",
+                                                              "roofline", "clocks", "gpu_launches", "e2e")}
+    if rank == 0 and line is not None:
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

@@ -12,7 +12,9 @@
  *    caller (the Python binding uses torch tensors); "host" pointers are ordinary memory.  The library
  *    owns only what lives behind lcs_field (mesh, snapshots, tracer scratch).
  *  - The hot calls (lcs_locate, lcs_advect, lcs_cg_ftle) are asynchronous on `cuda_stream` (a
- *    cudaStream_t passed as void*, NULL = default stream); the caller synchronises.
+ *    cudaStream_t passed as void*, NULL = default stream); the caller synchronises.  They never allocate or
+ *    free device memory and never synchronise the device: everything lcs_advect needs is allocated by
+ *    lcs_field_reserve (a set-up call), and lcs_advect returns LCS_ERR_OOM if the reservation is too small.
  *  - Every step of the path runs in CUDA kernels; there is no CPU fallback.
  *  - A field owns one set of tracer scratch buffers and one snapshot window: run one hot call at a time per field
  *    (calls on the same stream serialise by themselves); different fields are independent.
@@ -84,6 +86,18 @@ lcs_status lcs_field_create(const lcs_field_desc *desc, lcs_field **out);
 lcs_status lcs_field_set_snapshot(lcs_field *f, int32_t s, const void *vel, int32_t is_device_ptr);
 lcs_status lcs_field_sync(lcs_field *f);
 void lcs_field_destroy(lcs_field *f);
+
+/* Set-up call: allocates everything lcs_advect / lcs_advect_early_cg need for up to n_seeds tracers and n_steps RK4
+ * steps per call under the CURRENT options: tracer records and sort scratch, stage-time tables, the pair-record cache,
+ * the blended stage-time fields of one chunk (3D fp32 Cartesian grids) and the resident field sets (option
+ * "field_sets").  The paper loads velocity data into GPU memory "only every time a new velocity data file is needed"
+ * (PAPER.md:85); nothing else may stall the stream, so the hot calls themselves never allocate.  Grow-only and
+ * idempotent: a call that asks for no more than what is reserved returns at once; growing synchronises the device, frees
+ * and re-allocates.  Options that change the footprint ("field_sets", "preblend_steps", "integrator", "bundle", "tma")
+ * must be set BEFORE the reservation they are meant for; lcs_advect returns LCS_ERR_OOM ("call lcs_field_reserve") when
+ * the reservation does not cover a call.  Errors: LCS_ERR_INVALID_ARG (n_seeds < 1, n_steps < 1, n_seeds >= 2^31,
+ * n_steps >= 2^24), LCS_ERR_OOM.                                                                                  */
+lcs_status lcs_field_reserve(lcs_field *f, int64_t n_seeds, int64_t n_steps);
 
 /* Integer options.  Keys: "integrator" 0 = auto, 1 = fused (one persistent per-seed loop per snapshot
  * window), 2 = split (one short kernel per RK4 stage, tracers advance synchronously: PAPER.md:85), 3 = 4-step
@@ -195,13 +209,39 @@ lcs_status lcs_ridge(int32_t dim, int32_t dtype, const int32_t ng[3], const doub
                      void *kappa, void *dgn, uint8_t *mask, void *cuda_stream);
 
 /* End-to-end convenience with HOST buffers: copies the seeds to the device, runs lcs_advect and
- * lcs_cg_ftle and copies flow map (optional), flags (optional) and FTLE back; synchronous.
- * seeds_host/flowmap_host: [n][dim] of the field's compute_dtype; ftle_host: [n] of compute_dtype.
+ * lcs_cg_ftle and copies the flow map, flags, exit steps, Cauchy-Green tensor (each optional, NULL = not
+ * wanted) and the FTLE back; synchronous (it reserves what it needs: lcs_field_reserve + its own staging).
+ * seeds_host/flowmap_host: [n][dim] of the field's compute_dtype; cg_host: [n][3 or 6]; ftle_host: [n] of
+ * compute_dtype; exit_flag_host [n] u8; exit_step_host [n] i32.
  * Pinned host memory makes the copies asynchronous with respect to each other.                      */
 lcs_status lcs_ftle_host(lcs_field *f, const int32_t ng[3], const double seed_spacing[3],
                          const int32_t seed_periodic[3], const double period[3],
                          const void *seeds_host, double t0, double tf, double h,
-                         void *flowmap_host, uint8_t *exit_flag_host, void *ftle_host);
+                         void *flowmap_host, uint8_t *exit_flag_host, int32_t *exit_step_host,
+                         void *cg_host, void *ftle_host);
+
+/* Measured peaks of the device the roofline fractions are quoted against ("Peaks to measure on the box
+ * before quoting any %"; the paper's claim under test is "limited by memory bandwidth").  Runs a
+ * micro-kernel (warm-up + best of 3, CUDA events), synchronous, allocates and frees its own buffers (up to 2 GB).
+ * value: TFLOP/s for the FMA kinds, microseconds for LCS_PEAK_LAUNCH_US, GB/s otherwise (bytes delivered to registers for
+ * the gather kinds: 32 bytes per lane and load).                                                                   */
+typedef enum {
+    LCS_PEAK_FP32_FMA = 0,            /* dependent-free FFMA chains, all SMs                                        */
+    LCS_PEAK_FP64_FMA = 1,
+    LCS_PEAK_LAUNCH_US = 2,           /* back-to-back empty kernel launches, microseconds per launch                */
+    LCS_PEAK_HBM_COPY = 3,            /* 1 GiB streaming copy, read + write bytes                                   */
+    LCS_PEAK_L2_SEQ = 4,              /* sequential 128-bit reads of a 48 MB buffer, L1 bypassed                    */
+    LCS_PEAK_L2_SECTOR = 5,           /* random 32-byte sectors of a 32 MB buffer (L2-resident), L1 bypassed        */
+    LCS_PEAK_HBM_SECTOR = 6,          /* random 32-byte sectors of a 2 GB buffer                                    */
+    LCS_PEAK_L1_GATHER_LINE = 7,      /* L1-resident 256-bit gathers, the 4 lanes of a group read one 128-byte line */
+    LCS_PEAK_L1_GATHER_SAME = 8,      /* ... the 4 lanes of a group read the same 32-byte record                    */
+    LCS_PEAK_L1_GATHER_SPREAD = 9,    /* ... every lane reads a line of its own                                     */
+    LCS_PEAK_SMEM_CONTIGUOUS = 10,    /* shared memory, LDS.128, lane L reads chunk base + L (conflict-free)        */
+    LCS_PEAK_SMEM_RECORDS = 11,       /* shared memory, lane L reads the 32-byte record base + L as 2 x LDS.128     */
+    LCS_PEAK_SMEM_RECORDS_SWIZZLED = 12, /* ... with the 16-byte chunks laid out as TMA's 32-byte swizzle does      */
+    LCS_PEAK_SMEM_RECORDS_SAME = 13   /* ... swizzled, the 4 lanes of a group read the same record (broadcast)      */
+} lcs_peak_kind;
+lcs_status lcs_measure_peak(int32_t kind, double *value);
 
 /* Number of kernels this library has launched in this process (bench.py's gpu_launches).           */
 int64_t lcs_kernel_launch_count(void);

@@ -9,7 +9,7 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liblcs.so")
-SOURCES = ["field.cu", "advect_cart.cu", "cg_ftle.cu", "simplex.cu"]
+SOURCES = ["field.cu", "advect_cart.cu", "cg_ftle.cu", "simplex.cu", "peaks.cu"]
 HEADERS = [os.path.join(CSRC, "lcs_internal.cuh"), os.path.join(CSRC, "bundle_sort.cuh"), os.path.join(HERE, "..", "include", "lcs.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr", "-Xcudafe", "--diag_suppress=177"]

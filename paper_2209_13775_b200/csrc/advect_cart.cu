@@ -254,11 +254,16 @@ __global__ void __launch_bounds__(256) cart_final_kernel(CartDev g, const TC *__
     if (exit_step) exit_step[i] = fl == 0 ? N : (fl == 2 ? 0 : (int32_t)(t.meta & 0x3fffffffu));
 }
 
-// sort key of a tracer: Morton code of its (wrapped) cell, coarsened by `shift` bits per axis; finished tracers
-// (flag != 0) go to the last bin so that their warps retire at once
+// sort key of a tracer; finished tracers (flag != 0) go to the last bin so that their warps retire at once.
+// order 0: Morton code of the (wrapped) cell, coarsened by `shift` bits per axis; order 1: row-major cell index, x fastest
+// (x-neighbouring cells share a 128-byte line of records).  order 2 (3D, shift == 0): row-major over PAIRS of x-neighbouring
+// cells, and inside a pair by (z half, y half, x quarter) of the tracer's offset: a 256-bit gather costs one L1 wavefront per
+// distinct 128-byte line that each group of 4 lanes touches, and with 8 tracers per cell in arbitrary order every group
+// straddles two rows in y about half of the time (13 instead of 8 wavefronts per request, profiles/r1_cfg3_final.md);
+// ordered like this the 4 lanes of a group are x-neighbours in one (y, z) row.
 template <int DIM, typename TC>
 __global__ void __launch_bounds__(256) cart_key_kernel(CartDev g, const CartTracer<DIM, TC> *__restrict__ st, int64_t n, int shift,
-                                                        int row_major, uint32_t last_bin, uint32_t *__restrict__ key,
+                                                        int order, uint32_t last_bin, uint32_t *__restrict__ key,
                                                         uint32_t *__restrict__ cnt)
 {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -269,11 +274,14 @@ __global__ void __launch_bounds__(256) cart_key_kernel(CartDev g, const CartTrac
         int c[DIM];
 #pragma unroll
         for (int a = 0; a < DIM; ++a) c[a] = (g.periodic[a] ? wrap_index(t.ci[a], g.n[a], g.pow2[a]) : t.ci[a]) >> shift;
-        if (row_major) {
-            // x fastest: consecutive tracers sit in x-neighbouring cells, whose records share a 128-byte line (rows are
-            // padded to 4 records), so a 4-lane group that straddles two cells still costs one L1 wavefront
-            const int m0 = ((g.n[0] - 1) >> shift) + 1, m1 = ((g.n[1] - 1) >> shift) + 1;
-            k = (uint32_t)c[0] + (uint32_t)m0 * ((uint32_t)c[1] + (DIM == 3 ? (uint32_t)m1 * (uint32_t)c[2] : 0u));
+        const int m0 = ((g.n[0] - 1) >> shift) + 1, m1 = ((g.n[1] - 1) >> shift) + 1;
+        if (order == 2 && DIM == 3) {
+            const uint32_t m0p = (uint32_t)(m0 + 1) >> 1;
+            const uint32_t sub = ((t.w[DIM - 1] >= TC(0.5)) ? 8u : 0u) | ((t.w[1] >= TC(0.5)) ? 4u : 0u) | (((uint32_t)c[0] & 1u) << 1) |
+                                 ((t.w[0] >= TC(0.5)) ? 1u : 0u);
+            k = (((uint32_t)c[0] >> 1) + m0p * ((uint32_t)c[1] + (uint32_t)m1 * (uint32_t)c[DIM - 1])) * 16u + sub;
+        } else if (order >= 1) {
+            k = (uint32_t)c[0] + (uint32_t)m0 * ((uint32_t)c[1] + (DIM == 3 ? (uint32_t)m1 * (uint32_t)c[DIM - 1] : 0u));
         } else {
             k = bundle::morton<DIM>(c);
         }
@@ -668,6 +676,70 @@ CartDev make_dev(const lcs_field *f)
 
 size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 
+// How lcs_advect carves the field's scratch for n tracers and N steps under the current options.  lcs_field_reserve sizes
+// the allocation with the same function (worst case over the windows of any [t0, tf]), so the hot call never allocates.
+struct CartLayout {
+    bool split, ab4, do_bundle, preblend;
+    int shift, order, max_fields;
+    int64_t nbins, ntiles;
+    size_t o_a, o_b, o_xi, o_acc, o_hist, o_tau, o_key, o_cnt, o_tile, o_ftau, o_fields, total;
+};
+
+size_t cart_tracer_bytes(const lcs_field *f)
+{
+    const bool c64 = f->compute_dtype == LCS_F64;
+    if (f->dim == 2) return c64 ? sizeof(CartTracer<2, double>) : sizeof(CartTracer<2, float>);
+    return c64 ? sizeof(CartTracer<3, double>) : sizeof(CartTracer<3, float>);
+}
+
+CartLayout cart_layout(const lcs_field *f, int64_t n, int64_t N)
+{
+    CartLayout L{};
+    const int DIM = f->dim;
+    const size_t tcb = lcs_esize(f->compute_dtype), trb = cart_tracer_bytes(f);
+    L.split = f->opt_integrator == 2;
+    L.ab4 = f->opt_integrator == 3;
+    L.do_bundle = !L.ab4 && (f->opt_bundle == 1 || (f->opt_bundle < 0 && n >= (1 << 18)));
+    // sort bins: cell index coarsened so that the histogram stays <= 2^24 bins
+    int bits = 0;
+    for (L.shift = 0;; ++L.shift) {
+        bits = 0;
+        for (int a = 0; a < DIM; ++a) {
+            int cells = ((f->cart.n[a] - 1) >> L.shift) + 1, b = 0;
+            while ((1 << b) < cells) ++b;
+            bits = b > bits ? b : bits;
+        }
+        if (bits * DIM <= 24) break;
+    }
+    L.order = (int)f->opt_bundle_order;
+    int64_t nkeys = (int64_t)1 << (bits * DIM);
+    if (L.order == 2) {
+        const int64_t sub = (int64_t)((f->cart.n[0] + 1) / 2) * f->cart.n[1] * f->cart.n[2] * 16;
+        if (DIM == 3 && L.shift == 0 && sub <= (1 << 24)) nkeys = sub;
+        else L.order = 1;
+    }
+    L.nbins = L.do_bundle ? nkeys + 1 : 0;
+    L.ntiles = (L.nbins + bundle::kScanTile - 1) / bundle::kScanTile;
+    const bool can_blend = DIM == 3 && f->compute_dtype == LCS_F32 && f->vel_dtype == LCS_F32;
+    L.preblend = can_blend && !L.split && !L.ab4 && (f->opt_preblend == 1 || (f->opt_preblend < 0 && n >= (1 << 20)));
+    L.max_fields = L.preblend ? 2 * (int)(f->opt_preblend_steps < N ? f->opt_preblend_steps : N) + 1 : 0;
+    size_t off = 0;
+    L.o_a = off; off = align_up(off + (size_t)n * trb);
+    L.o_b = off; if (L.do_bundle) off = align_up(off + (size_t)n * trb);
+    L.o_xi = off; if (L.split) off = align_up(off + (size_t)n * DIM * tcb);
+    L.o_acc = off; if (L.split) off = align_up(off + (size_t)n * DIM * tcb);
+    L.o_hist = off; if (L.ab4) off = align_up(off + (size_t)n * 3 * DIM * tcb);
+    L.o_tau = off; off = align_up(off + (size_t)3 * N * tcb);
+    L.o_key = off; if (L.do_bundle) off = align_up(off + (size_t)n * 4);
+    L.o_cnt = off; if (L.do_bundle) off = align_up(off + (size_t)L.nbins * 4);
+    L.o_tile = off; if (L.do_bundle) off = align_up(off + (size_t)L.ntiles * 4);
+    L.o_ftau = off; if (L.preblend) off = align_up(off + ((size_t)3 * N + 8) * 4);
+    // one chunk of blended fields, unless resident field sets hold them
+    L.o_fields = off; if (L.preblend && f->opt_field_sets == 0) off = align_up(off + (size_t)L.max_fields * (size_t)f->nrec * 32);
+    L.total = off;
+    return L;
+}
+
 template <int DIM, typename TV, typename TC, bool FASTWRAP, bool LD256>
 void launch_window(const CartDev &g, const void *const p[3], const TC *d_tau, int first, int count, int64_t n, CartTracer<DIM, TC> *S,
                    const TC *hs, int block, cudaStream_t st)
@@ -697,37 +769,22 @@ lcs_status cart_advect_impl(lcs_field *f, int64_t n, const void *seeds_, double 
     using Tracer = CartTracer<DIM, TC>;
     const TC *seeds = (const TC *)seeds_;
     TC *flowmap = (TC *)flowmap_;
-    if (n >= (1LL << 31) || N >= (1LL << 30)) { lcs_set_error("too many seeds or steps for 32-bit tracer records"); return LCS_ERR_INVALID_ARG; }
+    if (n >= (1LL << 31) || N >= (1LL << 24)) { lcs_set_error("too many seeds or steps for 32-bit tracer records"); return LCS_ERR_INVALID_ARG; }
     std::vector<StepWindow> windows;
-    std::vector<double> tau64;
-    lcs_status rc = lcs_plan_windows(f, t0, h, N, windows, tau64);
+    lcs_status rc = lcs_plan_windows(f, t0, h, N, windows);
     if (rc != LCS_OK) return rc;
-    std::vector<TC> tau(tau64.size());
-    for (size_t k = 0; k < tau.size(); ++k) tau[k] = (TC)tau64[k];
-
-    const bool split = f->opt_integrator == 2, ab4 = f->opt_integrator == 3;
-    const bool do_bundle = !ab4 && (f->opt_bundle == 1 || (f->opt_bundle < 0 && n >= (1 << 18)));
-    // sort bins: Morton code of the cell index, coarsened so that the histogram stays <= 2^24 bins
-    int shift = 0, bits = 0;
-    for (;; ++shift) {
-        bits = 0;
-        for (int a = 0; a < DIM; ++a) {
-            int cells = ((f->cart.n[a] - 1) >> shift) + 1, b = 0;
-            while ((1 << b) < cells) ++b;
-            bits = b > bits ? b : bits;
-        }
-        if (bits * DIM <= 24) break;
-    }
-    const int64_t nbins = do_bundle ? ((int64_t)1 << (bits * DIM)) + 1 : 0;
+    const CartLayout L = cart_layout(f, n, N);
+    rc = lcs_scratch_check(f, L.total);
+    if (rc != LCS_OK) return rc;
+    const bool split = L.split, ab4 = L.ab4, do_bundle = L.do_bundle, preblend = L.preblend;
+    const int64_t nbins = L.nbins;
 
     // launch units: a snapshot window is cut into chunks (pre-blended variant: <= preblend_steps steps, whose
     // distinct stage times are blended once per node; otherwise <= bundle_steps steps between re-bundlings)
     constexpr bool kCanBlend = DIM == 3 && sizeof(TC) == 4 && sizeof(TV) == 4;
-    const bool preblend = kCanBlend && !split && !ab4 && (f->opt_preblend == 1 || (f->opt_preblend < 0 && n >= (1 << 20)));
     struct Unit { int win, first, count, blend, ftau_off, nfields; };
     std::vector<Unit> units;
-    std::vector<float> ftau;
-    int max_fields = 0;
+    std::vector<float> ftau;                          // host copy of the blended stage-time weights: keys of the resident field sets
     for (size_t wi = 0; wi < windows.size(); ++wi) {
         const StepWindow &w = windows[wi];
         const bool blend = preblend && w.s[0] == w.s[1] && w.s[1] == w.s[2];
@@ -743,15 +800,14 @@ lcs_status cart_advect_impl(lcs_field *f, int64_t n, const void *seeds_, double 
                 // should that ever fail, the chunk falls back to pair records.
                 bool regular = true;
                 for (int s = u.first; s + 1 < u.first + u.count; ++s)
-                    regular = regular && (float)tau64[3 * (size_t)s + 2] == (float)tau64[3 * (size_t)(s + 1)];
+                    regular = regular && (float)lcs_stage_tau(f, t0, h, s, 2, w.s[2]) == (float)lcs_stage_tau(f, t0, h, s + 1, 0, w.s[0]);
                 if (regular) {
                     for (int s = u.first; s < u.first + u.count; ++s) {
-                        ftau.push_back((float)tau64[3 * (size_t)s]);
-                        ftau.push_back((float)tau64[3 * (size_t)s + 1]);
+                        ftau.push_back((float)lcs_stage_tau(f, t0, h, s, 0, w.s[0]));
+                        ftau.push_back((float)lcs_stage_tau(f, t0, h, s, 1, w.s[1]));
                     }
-                    ftau.push_back((float)tau64[3 * (size_t)(u.first + u.count - 1) + 2]);
+                    ftau.push_back((float)lcs_stage_tau(f, t0, h, u.first + u.count - 1, 2, w.s[2]));
                     u.nfields = 2 * u.count + 1;
-                    max_fields = u.nfields > max_fields ? u.nfields : max_fields;
                 } else {
                     u.blend = 0;
                 }
@@ -760,31 +816,11 @@ lcs_status cart_advect_impl(lcs_field *f, int64_t n, const void *seeds_, double 
         }
     }
 
-    // carve the tracer scratch
-    size_t off = 0;
-    const size_t o_a = off; off = align_up(off + (size_t)n * sizeof(Tracer));
-    const size_t o_b = off; if (do_bundle) off = align_up(off + (size_t)n * sizeof(Tracer));
-    const size_t o_xi = off; if (split) off = align_up(off + (size_t)n * DIM * sizeof(TC));
-    const size_t o_acc = off; if (split) off = align_up(off + (size_t)n * DIM * sizeof(TC));
-    const size_t o_hist = off; if (ab4) off = align_up(off + (size_t)n * 3 * DIM * sizeof(TC));
-    const size_t o_tau = off; off = align_up(off + tau.size() * sizeof(TC));
-    const int64_t ntiles = (nbins + bundle::kScanTile - 1) / bundle::kScanTile;
-    const size_t o_key = off; if (do_bundle) off = align_up(off + (size_t)n * 4);
-    const size_t o_cnt = off; if (do_bundle) off = align_up(off + (size_t)nbins * 4);
-    const size_t o_tile = off; if (do_bundle) off = align_up(off + (size_t)ntiles * 4);
-    const size_t o_ftau = off; off = align_up(off + ftau.size() * 4 + 4);
-    const size_t o_fields = off; off = align_up(off + (size_t)max_fields * (size_t)f->nrec * 32);
-    rc = lcs_scratch_reserve(f, off);
-    if (rc != LCS_OK) return rc;
     char *base = (char *)f->scratch.buf;
-    Tracer *cur = (Tracer *)(base + o_a), *alt = (Tracer *)(base + o_b);
-    TC *d_xi = (TC *)(base + o_xi), *d_acc = (TC *)(base + o_acc), *d_tau = (TC *)(base + o_tau);
-    uint32_t *d_key = (uint32_t *)(base + o_key), *d_cnt = (uint32_t *)(base + o_cnt), *d_tile = (uint32_t *)(base + o_tile);
-    float *d_ftau = (float *)(base + o_ftau);
-    LCS_CUDA_OK(cudaMemcpyAsync(d_tau, tau.data(), tau.size() * sizeof(TC), cudaMemcpyHostToDevice, st));
-    if (max_fields) {
-        LCS_CUDA_OK(cudaMemcpyAsync(d_ftau, ftau.data(), ftau.size() * 4, cudaMemcpyHostToDevice, st));
-    }
+    Tracer *cur = (Tracer *)(base + L.o_a), *alt = (Tracer *)(base + L.o_b);
+    TC *d_xi = (TC *)(base + L.o_xi), *d_acc = (TC *)(base + L.o_acc), *d_tau = (TC *)(base + L.o_tau);
+    uint32_t *d_key = (uint32_t *)(base + L.o_key), *d_cnt = (uint32_t *)(base + L.o_cnt), *d_tile = (uint32_t *)(base + L.o_tile);
+    float *d_ftau = (float *)(base + L.o_ftau);
 
     CartDev g = make_dev(f);
     const int block = f->opt_block ? (int)(f->opt_block > 256 ? 256 : f->opt_block) : 256;
@@ -798,7 +834,7 @@ lcs_status cart_advect_impl(lcs_field *f, int64_t n, const void *seeds_, double 
 
     auto rebundle = [&]() -> lcs_status {
         LCS_CUDA_OK(cudaMemsetAsync(d_cnt, 0, (size_t)nbins * 4, st));
-        LCS_LAUNCH((cart_key_kernel<DIM, TC>), lcs_blocks(n, 256), 256, 0, st, g, cur, n, shift, (int)f->opt_bundle_order, (uint32_t)(nbins - 1), d_key, d_cnt);
+        LCS_LAUNCH((cart_key_kernel<DIM, TC>), lcs_blocks(n, 256), 256, 0, st, g, cur, n, L.shift, L.order, (uint32_t)(nbins - 1), d_key, d_cnt);
         bundle::sort_records<Tracer>(cur, alt, d_key, d_cnt, d_tile, n, nbins, st);
         std::swap(cur, alt);
         return LCS_OK;
@@ -830,6 +866,9 @@ lcs_status cart_advect_impl(lcs_field *f, int64_t n, const void *seeds_, double 
                     rc = lcs_field_require_pair(f, w.s[k], st, &p[k]);
                     if (rc != LCS_OK) return rc;
                 }
+                // stage-time weights of the window's steps, computed on the device (no host-to-device copy in the hot call)
+                rc = lcs_fill_stage_tau(f, t0, h, w.first, w.count, w.s, d_tau, nullptr, st);
+                if (rc != LCS_OK) return rc;
             }
             // stream the snapshot the NEXT window will need while this one computes (side stream)
             lcs_field_prefetch(f, dir > 0 ? w.s[2] + 2 : w.s[2] - 1, w.s[2], w.s[2] + 1);
@@ -844,27 +883,27 @@ lcs_status cart_advect_impl(lcs_field *f, int64_t n, const void *seeds_, double 
         since_bundle += u.count;
         if constexpr (kCanBlend) {
             if (u.blend) {
-                XPair *fields = (XPair *)(base + o_fields);
+                XPair *fields = (XPair *)(base + L.o_fields);
                 bool need_blend = true;
+                FieldSet *filling = nullptr;
+                const float *tb = ftau.data() + u.ftau_off;
                 if (f->opt_field_sets > 0) {
-                    // resident field sets: reuse the set blended for the same snapshot pair and the same stage times
-                    const float *tb = ftau.data() + u.ftau_off;
+                    // resident field sets (allocated by lcs_field_reserve): reuse the set blended from the same snapshot pair
+                    // for the same stage times, else blend into the least recently used one
                     const size_t bytes = (size_t)u.nfields * (size_t)f->nrec * 32;
                     FieldSet *hit = nullptr, *victim = nullptr;
                     for (FieldSet &fs : f->field_sets)
-                        if (fs.pair == w.s[0] && fs.tau.size() == (size_t)u.nfields && std::equal(fs.tau.begin(), fs.tau.end(), tb)) hit = &fs;
+                        if (fs.buf && fs.pair == w.s[0] && fs.tau.size() == (size_t)u.nfields && std::equal(fs.tau.begin(), fs.tau.end(), tb)) hit = &fs;
                     if (!hit) {
-                        if ((int64_t)f->field_sets.size() < f->opt_field_sets) { f->field_sets.emplace_back(); victim = &f->field_sets.back(); }
-                        else for (FieldSet &fs : f->field_sets) if (!victim || fs.age < victim->age) victim = &fs;
-                        if (victim->bytes < bytes) {
-                            if (victim->buf) { cudaStreamSynchronize(st); cudaFree(victim->buf); victim->buf = nullptr; victim->bytes = 0; }
-                            LCS_CUDA_OK(cudaMalloc(&victim->buf, bytes));
-                            victim->bytes = bytes;
+                        for (FieldSet &fs : f->field_sets) if (fs.buf && fs.bytes >= bytes && (!victim || fs.age < victim->age)) victim = &fs;
+                        if (!victim) {
+                            lcs_set_error("no resident field set of %zu bytes is reserved: call lcs_field_reserve after setting field_sets", bytes);
+                            return LCS_ERR_OOM;
                         }
-                        victim->pair = w.s[0];
-                        victim->tau.assign(tb, tb + u.nfields);
+                        victim->pair = -1;                           // the old key dies BEFORE the buffer is overwritten;
+                        victim->tau.clear();                         // the new one is set once the blend is enqueued
                         f->info_field_set_misses++;
-                        hit = victim;
+                        hit = filling = victim;
                     } else {
                         need_blend = false;
                         f->info_field_set_hits++;
@@ -872,9 +911,14 @@ lcs_status cart_advect_impl(lcs_field *f, int64_t n, const void *seeds_, double 
                     hit->age = ++f->field_set_clock;
                     fields = (XPair *)hit->buf;
                 }
-                if (need_blend)
+                if (need_blend) {
+                    rc = lcs_fill_stage_tau(f, t0, h, u.first, u.count, w.s, nullptr, d_ftau + u.ftau_off, st);
+                    if (rc != LCS_OK) return rc;
                     LCS_LAUNCH(blend_xpair_kernel, lcs_blocks(f->nrec, 256), 256, 0, st, (const float *)raw_a, (const float *)raw_b, g.n[0],
                                g.n[1], g.n[2], f->cart.np[0], f->cart.np[1], f->cart.np[2], d_ftau + u.ftau_off, u.nfields, fields, f->nrec);
+                    LCS_CUDA_OK(cudaGetLastError());
+                    if (filling) { filling->pair = w.s[0]; filling->tau.assign(tb, tb + u.nfields); }
+                }
                 {
                     WindowTimer timer(f, st);
                     if (fast)
@@ -895,7 +939,7 @@ lcs_status cart_advect_impl(lcs_field *f, int64_t n, const void *seeds_, double 
         WindowTimer timer(f, st);
         if (ab4) {
             using Rec = PairRec<DIM, TV>;
-            TC *d_hist = (TC *)(base + o_hist);
+            TC *d_hist = (TC *)(base + L.o_hist);
 #define LCS_AB4(FW, LD) LCS_LAUNCH((cart_ab4_kernel<DIM, TV, TC, FW, LD>), lcs_blocks(n, block), block, 0, st, g, (const Rec *)p[0], (const Rec *)p[1], \
                                    (const Rec *)p[2], d_tau + 3 * (size_t)u.first, u.count, u.first, n, cur, d_hist, hs[0], hs[1], hs[2])
             if (fast && ld256) LCS_AB4(true, true);
@@ -910,7 +954,8 @@ lcs_status cart_advect_impl(lcs_field *f, int64_t n, const void *seeds_, double 
             else launch_window<DIM, TV, TC, false, false>(g, p, d_tau, u.first, u.count, n, cur, hs, block, st);
         } else {
             for (int s = u.first; s < u.first + u.count; ++s) {
-                const TC *t3 = tau.data() + 3 * (size_t)s;
+                const TC t3[3] = {(TC)lcs_stage_tau(f, t0, h, s, 0, w.s[0]), (TC)lcs_stage_tau(f, t0, h, s, 1, w.s[1]),
+                                  (TC)lcs_stage_tau(f, t0, h, s, 2, w.s[2])};
                 if (fast && ld256) launch_split_step<DIM, TV, TC, true, true>(g, p, t3, s, n, cur, d_xi, d_acc, hs, block, st);
                 else if (fast) launch_split_step<DIM, TV, TC, true, false>(g, p, t3, s, n, cur, d_xi, d_acc, hs, block, st);
                 else if (ld256) launch_split_step<DIM, TV, TC, false, true>(g, p, t3, s, n, cur, d_xi, d_acc, hs, block, st);
@@ -926,6 +971,14 @@ lcs_status cart_advect_impl(lcs_field *f, int64_t n, const void *seeds_, double 
 }
 
 }  // namespace
+
+size_t lcs_cart_scratch_bytes(const lcs_field *f, int64_t n, int64_t N) { return cart_layout(f, n, N).total; }
+
+size_t lcs_cart_field_set_bytes(const lcs_field *f, int64_t N)
+{
+    const CartLayout L = cart_layout(f, (int64_t)1 << 20, N);      // sets are used by the pre-blended integrator only
+    return (f->opt_preblend != 0 && L.max_fields > 0) ? (size_t)L.max_fields * (size_t)f->nrec * 32 : 0;
+}
 
 lcs_status lcs_cart_locate(lcs_field *f, int64_t n, const double *pos, int32_t *cell, double *w, cudaStream_t st)
 {

@@ -11,6 +11,8 @@
 #include <stdio.h>
 #include <string.h>
 
+#include <new>
+
 #include "lcs_internal.cuh"
 
 std::atomic<int64_t> g_lcs_launches{0};
@@ -94,7 +96,6 @@ static lcs_status ensure_slot(lcs_field *f, int s, int keep0, int keep1, int *sl
     }
     if (best < 0) { lcs_set_error("no free snapshot slot"); return LCS_ERR_INVALID_ARG; }
     if (f->slot_snap[best] >= 0) f->snap_slot[f->slot_snap[best]] = -1;
-    if (!f->slot[best]) LCS_CUDA_OK(cudaMalloc(&f->slot[best], raw_bytes(f)));
     // do not overwrite the slot before its last reader (a pair build on the compute stream) is done
     if (f->slot_free_valid[best]) LCS_CUDA_OK(cudaStreamWaitEvent(f->side, f->slot_free[best], 0));
     LCS_CUDA_OK(cudaMemcpyAsync(f->slot[best], f->host_src[s], raw_bytes(f), cudaMemcpyHostToDevice, f->side));
@@ -141,7 +142,6 @@ lcs_status lcs_field_require_pair(lcs_field *f, int s, cudaStream_t st, const vo
     int k = 0;
     for (int j = 1; j < lcs_field::kPairCache; ++j)
         if (f->pair_age[j] < f->pair_age[k]) k = j;
-    if (!f->pair_buf[k]) LCS_CUDA_OK(cudaMalloc(&f->pair_buf[k], pair_bytes(f)));
     LCS_CUDA_OK(cudaStreamWaitEvent(st, f->slot_ready[s0], 0));
     LCS_CUDA_OK(cudaStreamWaitEvent(st, f->slot_ready[s1], 0));
     const bool v64 = f->vel_dtype == LCS_F64, r64 = rec_dtype(f) == LCS_F64;
@@ -197,12 +197,50 @@ lcs_status lcs_field_release_raw(lcs_field *f, int s, cudaStream_t st)
     return LCS_OK;
 }
 
-lcs_status lcs_scratch_reserve(lcs_field *f, size_t bytes)
+lcs_status lcs_scratch_check(lcs_field *f, size_t bytes)
 {
     if (f->scratch.bytes >= bytes) return LCS_OK;
-    if (f->scratch.buf) { cudaDeviceSynchronize(); cudaFree(f->scratch.buf); f->scratch.buf = nullptr; f->scratch.bytes = 0; }
-    LCS_CUDA_OK(cudaMalloc(&f->scratch.buf, bytes));
-    f->scratch.bytes = bytes;
+    lcs_set_error("the reservation (%zu bytes for %lld seeds, %lld steps) does not cover this call (%zu bytes): call lcs_field_reserve first "
+                  "(the hot calls never allocate)", f->scratch.bytes, (long long)f->scratch.n_seeds, (long long)f->scratch.n_steps, bytes);
+    return LCS_ERR_OOM;
+}
+
+// ---------------------------------------------------------------------------------------------
+// stage-time tables, filled on the device so that lcs_advect issues no host-to-device copy.  Same operations as
+// lcs_stage_tau on the host, every one rounded separately (no FMA contraction), hence the same bits.
+template <typename TC>
+__global__ void __launch_bounds__(128) stage_tau_kernel(double t0, double h, int64_t first, int count, double ts0, double ts1, double ts2,
+                                                         double dt0, double dt1, double dt2, TC *__restrict__ tau, float *__restrict__ ftau)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= count) return;
+    const double n = (double)(first + i);
+    const double ts[3] = {ts0, ts1, ts2}, dts[3] = {dt0, dt1, dt2};
+    double v[3];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        const double t = __dadd_rn(t0, __dmul_rn(__dadd_rn(n, 0.5 * (double)k), h));
+        v[k] = __ddiv_rn(__dsub_rn(t, ts[k]), dts[k]);
+    }
+    if (tau) { tau[3 * (first + i)] = (TC)v[0]; tau[3 * (first + i) + 1] = (TC)v[1]; tau[3 * (first + i) + 2] = (TC)v[2]; }
+    if (ftau) {
+        ftau[2 * i] = (float)v[0];
+        ftau[2 * i + 1] = (float)v[1];
+        if (i == count - 1) ftau[2 * count] = (float)v[2];
+    }
+}
+
+lcs_status lcs_fill_stage_tau(const lcs_field *f, double t0, double h, int64_t first, int count, const int32_t s[3], void *tau,
+                              float *ftau, cudaStream_t st)
+{
+    double ts[3], dts[3];
+    for (int k = 0; k < 3; ++k) { ts[k] = f->times[s[k]]; dts[k] = f->times[s[k] + 1] - f->times[s[k]]; }
+    if (f->compute_dtype == LCS_F64)
+        LCS_LAUNCH((stage_tau_kernel<double>), lcs_blocks(count, 128), 128, 0, st, t0, h, first, count, ts[0], ts[1], ts[2], dts[0], dts[1], dts[2],
+                   (double *)tau, ftau);
+    else
+        LCS_LAUNCH((stage_tau_kernel<float>), lcs_blocks(count, 128), 128, 0, st, t0, h, first, count, ts[0], ts[1], ts[2], dts[0], dts[1], dts[2],
+                   (float *)tau, ftau);
     return LCS_OK;
 }
 
@@ -212,8 +250,7 @@ lcs_status lcs_scratch_reserve(lcs_field *f, size_t bytes)
 // tolerance of 1e-9 intervals: a stage time that lands on a snapshot is evaluated with tau = 1 in the
 // earlier interval instead of tau = 0 in the later one -- the same value, reading #17); otherwise each
 // stage time takes its own interval s = clamp(floor((t - times[0]) / dt), 0, ns-2) as the oracle does.
-lcs_status lcs_plan_windows(const lcs_field *f, double t0, double h, int64_t N, std::vector<StepWindow> &windows,
-                            std::vector<double> &tau)
+lcs_status lcs_plan_windows(const lcs_field *f, double t0, double h, int64_t N, std::vector<StepWindow> &windows)
 {
     const double T0 = f->times[0], dt = f->dt_snap, eps = 1e-9 * dt;
     auto bracket = [&](double t) {
@@ -222,7 +259,6 @@ lcs_status lcs_plan_windows(const lcs_field *f, double t0, double h, int64_t N, 
         return s;
     };
     windows.clear();
-    tau.resize((size_t)3 * N);
     for (int64_t n = 0; n < N; ++n) {
         double t[3] = {t0 + (double)n * h, t0 + ((double)n + 0.5) * h, t0 + ((double)n + 1.0) * h};
         int sm = bracket(t[1]);
@@ -230,7 +266,6 @@ lcs_status lcs_plan_windows(const lcs_field *f, double t0, double h, int64_t N, 
         int s[3];
         if (t[0] >= lo && t[0] <= hi && t[2] >= lo && t[2] <= hi) s[0] = s[1] = s[2] = sm;
         else for (int k = 0; k < 3; ++k) s[k] = bracket(t[k]);
-        for (int k = 0; k < 3; ++k) tau[3 * n + k] = (t[k] - f->times[s[k]]) / (f->times[s[k] + 1] - f->times[s[k]]);
         if (!windows.empty()) {
             StepWindow &w = windows.back();
             if (w.s[0] == s[0] && w.s[1] == s[1] && w.s[2] == s[2] && w.count < (1 << 30)) { w.count++; continue; }
@@ -322,6 +357,14 @@ extern "C" lcs_status lcs_field_create(const lcs_field_desc *d, lcs_field **out)
         if (e == cudaSuccess) e = cudaEventCreateWithFlags(&f->slot_free[k], cudaEventDisableTiming);
     }
     if (e != cudaSuccess) { lcs_set_error("stream/event creation failed: %s", cudaGetErrorString(e)); lcs_field_destroy(f); return LCS_ERR_CUDA; }
+    // the snapshot window and the pair-record cache are allocated here, once: the hot calls never allocate
+    for (int k = 0; k < f->nslots && e == cudaSuccess; ++k) e = cudaMalloc(&f->slot[k], raw_bytes(f));
+    for (int k = 0; k < lcs_field::kPairCache && e == cudaSuccess; ++k) e = cudaMalloc(&f->pair_buf[k], pair_bytes(f));
+    if (e != cudaSuccess) {
+        lcs_set_error("allocating the snapshot window failed: %s", cudaGetErrorString(e));
+        lcs_field_destroy(f);
+        return e == cudaErrorMemoryAllocation ? LCS_ERR_OOM : LCS_ERR_CUDA;
+    }
     *out = f;
     return LCS_OK;
 }
@@ -341,6 +384,8 @@ extern "C" void lcs_field_destroy(lcs_field *f)
     if (f->h_flow) cudaFree(f->h_flow);
     if (f->h_ftle) cudaFree(f->h_ftle);
     if (f->h_flag) cudaFree(f->h_flag);
+    if (f->h_cg) cudaFree(f->h_cg);
+    if (f->h_step) cudaFree(f->h_step);
     lcs_simplex_free(f);
     if (f->side) cudaStreamDestroy(f->side);
     delete f;
@@ -362,7 +407,6 @@ extern "C" lcs_status lcs_field_set_snapshot(lcs_field *f, int32_t s, const void
         if (f->snap_slot[s] >= 0) { f->slot_snap[f->snap_slot[s]] = -1; f->snap_slot[s] = -1; }
         return LCS_OK;
     }
-    if (!f->slot[s]) LCS_CUDA_OK(cudaMalloc(&f->slot[s], raw_bytes(f)));
     LCS_CUDA_OK(cudaMemcpyAsync(f->slot[s], vel, raw_bytes(f), is_device_ptr ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, f->side));
     LCS_CUDA_OK(cudaEventRecord(f->slot_ready[s], f->side));
     if (!is_device_ptr) f->info_h2d_bytes += (int64_t)raw_bytes(f);
@@ -385,11 +429,11 @@ extern "C" lcs_status lcs_field_set_option(lcs_field *f, const char *key, int64_
     if (!strcmp(key, "integrator") && value >= 0 && value <= 3) f->opt_integrator = value;
     else if (!strcmp(key, "bundle") && value >= -1 && value <= 1) f->opt_bundle = value;
     else if (!strcmp(key, "bundle_steps") && value >= 0) f->opt_bundle_steps = value;
-    else if (!strcmp(key, "bundle_order") && (value == 0 || value == 1)) f->opt_bundle_order = value;
+    else if (!strcmp(key, "bundle_order") && value >= 0 && value <= 2) f->opt_bundle_order = value;
     else if (!strcmp(key, "simplex_order") && (value == 0 || value == 1)) f->opt_simplex_order = value;
     else if (!strcmp(key, "ld256") && (value == 0 || value == 1)) f->opt_ld256 = value;
     else if (!strcmp(key, "preblend") && value >= -1 && value <= 1) f->opt_preblend = value;
-    else if (!strcmp(key, "field_sets") && value >= 0 && value <= 64) {
+    else if (!strcmp(key, "field_sets") && value >= 0 && value <= 64) {      // set-up: the next lcs_field_reserve allocates the sets
         f->opt_field_sets = value;
         cudaDeviceSynchronize();
         for (FieldSet &fs : f->field_sets) if (fs.buf) cudaFree(fs.buf);
@@ -426,14 +470,17 @@ extern "C" lcs_status lcs_field_get_info(const lcs_field *f, const char *key, in
         }
         *value = (int64_t)(ms * 1e6);
     }
-    else if (!strcmp(key, "locate_fallbacks") || !strcmp(key, "locate_hops") || !strcmp(key, "locate_max_hops") || !strcmp(key, "locate_random_walks")) {
+    else if (!strcmp(key, "locate_fallbacks") || !strcmp(key, "locate_hops") || !strcmp(key, "locate_max_hops") || !strcmp(key, "locate_random_walks") ||
+             !strcmp(key, "walk_cap_hits")) {
         *value = 0;
         if (f->kind == LCS_MESH_SIMPLEX) {
-            unsigned long long h[4] = {0, 0, 0, 0};
+            unsigned long long h[8] = {0, 0, 0, 0, 0, 0, 0, 0};
             cudaMemcpy(h, f->mesh.stats, sizeof h, cudaMemcpyDeviceToHost);
-            *value = (int64_t)h[!strcmp(key, "locate_fallbacks") ? 0 : (!strcmp(key, "locate_hops") ? 1 : (!strcmp(key, "locate_max_hops") ? 2 : 3))];
+            *value = (int64_t)h[!strcmp(key, "locate_fallbacks") ? 0 : (!strcmp(key, "locate_hops") ? 1 : (!strcmp(key, "locate_max_hops") ? 2 :
+                                (!strcmp(key, "locate_random_walks") ? 3 : 4)))];
         }
     }
+    else if (!strcmp(key, "scratch_bytes")) *value = (int64_t)f->scratch.bytes;
     else if (!strcmp(key, "n_boundary_faces")) {
         *value = 0;
         if (f->kind == LCS_MESH_SIMPLEX) {
@@ -463,10 +510,47 @@ static lcs_status check_interval(const lcs_field *f, double t0, double tf, doubl
     if (T == 0.0 || (T > 0) != (h > 0)) { lcs_set_error("sign(h) must equal sign(tf - t0)"); return LCS_ERR_INVALID_ARG; }
     int64_t n = llround(T / h);
     if (n < 1 || fabs((double)n * h - T) > 1e-9 * fabs(T)) { lcs_set_error("(tf-t0)/h must be a positive integer (no partial last step)"); return LCS_ERR_INVALID_ARG; }
+    if (n >= (1LL << 24)) { lcs_set_error("more than 2^24 - 1 steps per call: split the interval (the flow map of one call seeds the next)"); return LCS_ERR_INVALID_ARG; }
     double eps = 1e-9 * f->dt_snap, lo = f->times.front() - eps, hi = f->times.back() + eps;
     if (t0 < lo || t0 > hi || tf < lo || tf > hi) { lcs_set_error("[t0,tf] = [%g,%g] outside the snapshot times [%g,%g]", t0, tf, f->times.front(), f->times.back()); return LCS_ERR_TIME_RANGE; }
     *N = n;
     return LCS_OK;
+}
+
+// no C++ exception crosses the boundary (std::vector storage of the window plan, of the field-set keys, ...)
+#define LCS_GUARD(...)                                                                           \
+    try { __VA_ARGS__ } catch (const std::bad_alloc &) { lcs_set_error("host allocation failed"); return LCS_ERR_OOM; } \
+    catch (...) { lcs_set_error("unexpected C++ exception"); return LCS_ERR_CUDA; }
+
+extern "C" lcs_status lcs_field_reserve(lcs_field *f, int64_t n_seeds, int64_t n_steps)
+{
+    if (!f) { lcs_set_error("null field"); return LCS_ERR_INVALID_ARG; }
+    if (n_seeds < 1 || n_steps < 1 || n_seeds >= (1LL << 31) || n_steps >= (1LL << 24)) {
+        lcs_set_error("lcs_field_reserve: need 1 <= n_seeds < 2^31 and 1 <= n_steps < 2^24"); return LCS_ERR_INVALID_ARG;
+    }
+    LCS_GUARD(
+        const size_t need = f->kind == LCS_MESH_CARTESIAN ? lcs_cart_scratch_bytes(f, n_seeds, n_steps) : lcs_simplex_scratch_bytes(f, n_seeds, n_steps);
+        if (need > f->scratch.bytes) {
+            if (f->scratch.buf) { cudaDeviceSynchronize(); cudaFree(f->scratch.buf); f->scratch.buf = nullptr; f->scratch.bytes = 0; }
+            LCS_CUDA_OK(cudaMalloc(&f->scratch.buf, need));
+            f->scratch.bytes = need;
+        }
+        if (n_seeds > f->scratch.n_seeds) f->scratch.n_seeds = n_seeds;
+        if (n_steps > f->scratch.n_steps) f->scratch.n_steps = n_steps;
+        // resident sets of blended fields (option "field_sets"): all of them, now
+        const size_t set_bytes = f->kind == LCS_MESH_CARTESIAN ? lcs_cart_field_set_bytes(f, n_steps) : 0;
+        if (f->opt_field_sets > 0 && set_bytes > 0) {
+            f->field_sets.resize((size_t)f->opt_field_sets);
+            for (FieldSet &fs : f->field_sets) {
+                if (fs.bytes >= set_bytes) continue;
+                fs.pair = -1; fs.tau.clear();
+                if (fs.buf) { cudaDeviceSynchronize(); cudaFree(fs.buf); fs.buf = nullptr; fs.bytes = 0; }
+                LCS_CUDA_OK(cudaMalloc(&fs.buf, set_bytes));
+                fs.bytes = set_bytes;
+            }
+        }
+        return LCS_OK;
+    )
 }
 
 extern "C" lcs_status lcs_advect(lcs_field *f, int64_t n, const void *seeds, double t0, double tf, double h, void *flowmap,
@@ -478,40 +562,55 @@ extern "C" lcs_status lcs_advect(lcs_field *f, int64_t n, const void *seeds, dou
     if (rc != LCS_OK) return rc;
     if (n == 0) return LCS_OK;
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    return f->kind == LCS_MESH_CARTESIAN ? lcs_cart_advect(f, n, seeds, t0, h, N, flowmap, exit_flag, exit_step, st)
-                                         : lcs_simplex_advect(f, n, seeds, t0, h, N, flowmap, exit_flag, exit_step, st);
+    LCS_GUARD(
+        return f->kind == LCS_MESH_CARTESIAN ? lcs_cart_advect(f, n, seeds, t0, h, N, flowmap, exit_flag, exit_step, st)
+                                             : lcs_simplex_advect(f, n, seeds, t0, h, N, flowmap, exit_flag, exit_step, st);
+    )
 }
 
 // ---------------------------------------------------------------------------------------------
 extern "C" lcs_status lcs_ftle_host(lcs_field *f, const int32_t ng[3], const double seed_spacing[3], const int32_t seed_periodic[3],
                                     const double period[3], const void *seeds_host, double t0, double tf, double h,
-                                    void *flowmap_host, uint8_t *exit_flag_host, void *ftle_host)
+                                    void *flowmap_host, uint8_t *exit_flag_host, int32_t *exit_step_host, void *cg_host, void *ftle_host)
 {
     if (!f || !ng || !seeds_host || !ftle_host) { lcs_set_error("null argument"); return LCS_ERR_INVALID_ARG; }
     int64_t n = (int64_t)ng[0] * ng[1] * (f->dim == 3 ? ng[2] : 1);
     if (n <= 0) { lcs_set_error("empty seed grid"); return LCS_ERR_INVALID_ARG; }
-    size_t es = lcs_esize(f->compute_dtype);
-    if (f->h_cap < n) {
+    int64_t N = 0;
+    lcs_status rc = check_interval(f, t0, tf, h, &N);
+    if (rc != LCS_OK) return rc;
+    rc = lcs_field_reserve(f, n, N);                       // this convenience call is synchronous set-up + run
+    if (rc != LCS_OK) return rc;
+    const size_t es = lcs_esize(f->compute_dtype), ncg = f->dim == 2 ? 3 : 6;
+    if (f->h_cap < n || (cg_host && !f->h_cg) || (exit_step_host && !f->h_step)) {
         cudaDeviceSynchronize();
         if (f->h_seeds) cudaFree(f->h_seeds);
         if (f->h_ftle) cudaFree(f->h_ftle);
         if (f->h_flag) cudaFree(f->h_flag);
-        f->h_seeds = f->h_ftle = nullptr; f->h_flag = nullptr; f->h_cap = 0;
-        LCS_CUDA_OK(cudaMalloc(&f->h_seeds, (size_t)n * f->dim * es));
-        LCS_CUDA_OK(cudaMalloc(&f->h_ftle, (size_t)n * es));
-        LCS_CUDA_OK(cudaMalloc((void **)&f->h_flag, (size_t)n));
-        f->h_cap = n;
+        if (f->h_cg) cudaFree(f->h_cg);
+        if (f->h_step) cudaFree(f->h_step);
+        f->h_seeds = f->h_ftle = f->h_cg = nullptr; f->h_flag = nullptr; f->h_step = nullptr;
+        const int64_t cap = n > f->h_cap ? n : f->h_cap;
+        f->h_cap = 0;
+        LCS_CUDA_OK(cudaMalloc(&f->h_seeds, (size_t)cap * f->dim * es));
+        LCS_CUDA_OK(cudaMalloc(&f->h_ftle, (size_t)cap * es));
+        LCS_CUDA_OK(cudaMalloc((void **)&f->h_flag, (size_t)cap));
+        if (cg_host) LCS_CUDA_OK(cudaMalloc(&f->h_cg, (size_t)cap * ncg * es));
+        if (exit_step_host) LCS_CUDA_OK(cudaMalloc((void **)&f->h_step, (size_t)cap * 4));
+        f->h_cap = cap;
     }
     cudaStream_t st = 0;
     LCS_CUDA_OK(cudaMemcpyAsync(f->h_seeds, seeds_host, (size_t)n * f->dim * es, cudaMemcpyHostToDevice, st));
-    lcs_status rc = lcs_advect(f, n, f->h_seeds, t0, tf, h, f->h_seeds, f->h_flag, nullptr, st);   // flow map in place
+    rc = lcs_advect(f, n, f->h_seeds, t0, tf, h, f->h_seeds, f->h_flag, exit_step_host ? f->h_step : nullptr, st);   // flow map in place
     if (rc != LCS_OK) return rc;
-    rc = lcs_cg_ftle(f->dim, f->compute_dtype, ng, seed_spacing, seed_periodic, period, f->h_seeds, f->h_flag, tf - t0, nullptr,
-                     f->h_ftle, nullptr, st);
+    rc = lcs_cg_ftle(f->dim, f->compute_dtype, ng, seed_spacing, seed_periodic, period, f->h_seeds, f->h_flag, tf - t0,
+                     cg_host ? f->h_cg : nullptr, f->h_ftle, nullptr, st);
     if (rc != LCS_OK) return rc;
     LCS_CUDA_OK(cudaMemcpyAsync(ftle_host, f->h_ftle, (size_t)n * es, cudaMemcpyDeviceToHost, st));
+    if (cg_host) LCS_CUDA_OK(cudaMemcpyAsync(cg_host, f->h_cg, (size_t)n * ncg * es, cudaMemcpyDeviceToHost, st));
     if (flowmap_host) LCS_CUDA_OK(cudaMemcpyAsync(flowmap_host, f->h_seeds, (size_t)n * f->dim * es, cudaMemcpyDeviceToHost, st));
     if (exit_flag_host) LCS_CUDA_OK(cudaMemcpyAsync(exit_flag_host, f->h_flag, (size_t)n, cudaMemcpyDeviceToHost, st));
+    if (exit_step_host) LCS_CUDA_OK(cudaMemcpyAsync(exit_step_host, f->h_step, (size_t)n * 4, cudaMemcpyDeviceToHost, st));
     LCS_CUDA_OK(cudaStreamSynchronize(st));
     return LCS_OK;
 }

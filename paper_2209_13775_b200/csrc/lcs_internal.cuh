@@ -67,14 +67,15 @@ struct SimplexMesh {
     double bin_lo[3] = {0, 0, 0};
     double bin_inv[3] = {0, 0, 0};
     int64_t hop_cap = 64;
-    unsigned long long *stats = nullptr;   // [0] brute-force fallbacks, [1] walk hops, [2] max hops of one walk (lcs_locate + seeds)
+    unsigned long long *stats = nullptr;   // [0] brute-force fallbacks, [1] walk hops, [2] max hops of one walk (lcs_locate + seeds),
+                                           // [3] random-walk fallbacks, [4] in-advect walks stopped by the hop cap (tracer flagged)
 };
 
-// tracer scratch owned by the field, grown on demand
+// tracer scratch owned by the field: one allocation made by lcs_field_reserve and carved by the advect code
 struct TracerScratch {
-    int64_t cap = 0;
-    void *buf = nullptr;          // one allocation, carved by the advect code
+    void *buf = nullptr;
     size_t bytes = 0;
+    int64_t n_seeds = 0, n_steps = 0;     // what the last lcs_field_reserve asked for
 };
 
 // context of lcs_advect_early_cg (row f1): where and when the integrators evaluate C during the advection
@@ -130,8 +131,9 @@ struct lcs_field {
     cudaStream_t side = nullptr;
     TracerScratch scratch;
     // host-API scratch
-    void *h_seeds = nullptr, *h_flow = nullptr, *h_ftle = nullptr;
+    void *h_seeds = nullptr, *h_flow = nullptr, *h_ftle = nullptr, *h_cg = nullptr;
     uint8_t *h_flag = nullptr;
+    int32_t *h_step = nullptr;
     int64_t h_cap = 0;
     EarlyCg early;
     std::vector<FieldSet> field_sets;
@@ -173,7 +175,8 @@ lcs_status lcs_field_require_pair(lcs_field *f, int s, cudaStream_t stream, cons
 lcs_status lcs_field_prefetch(lcs_field *f, int s, int keep0, int keep1);
 lcs_status lcs_field_acquire_raw(lcs_field *f, int s, cudaStream_t stream, const void **a, const void **b);
 lcs_status lcs_field_release_raw(lcs_field *f, int s, cudaStream_t stream);
-lcs_status lcs_scratch_reserve(lcs_field *f, size_t bytes);
+// lcs_advect never allocates: it checks that lcs_field_reserve made the scratch large enough (LCS_ERR_OOM otherwise)
+lcs_status lcs_scratch_check(lcs_field *f, size_t bytes);
 
 // cg_ftle.cu: evaluate C for the stencils that are still complete after m steps (flow map + flags already scattered)
 lcs_status lcs_early_cg_eval(lcs_field *f, int64_t m, cudaStream_t st);
@@ -206,6 +209,21 @@ struct StepWindow {
     int32_t count = 0;      // steps in the window
     int32_t s[3] = {0, 0, 0};   // snapshot pair index used by the stage times ta, tb, tc
 };
-// tau[3*n + {0,1,2}] = (t - times[s]) / dt for ta, tb, tc of step n (fp64, as the oracle computes them)
-lcs_status lcs_plan_windows(const lcs_field *f, double t0, double h, int64_t N,
-                            std::vector<StepWindow> &windows, std::vector<double> &tau);
+lcs_status lcs_plan_windows(const lcs_field *f, double t0, double h, int64_t N, std::vector<StepWindow> &windows);
+// time weight of stage k (0: ta, 1: tb, 2: tc) of step n in snapshot pair s: (t - times[s]) / (times[s+1] - times[s]) with
+// t = t0 + (n + k/2) h by multiplication (fp64, exactly as the oracle computes it; the device tables are filled by
+// lcs_fill_stage_tau with the same operations, rounded separately)
+static inline double lcs_stage_tau(const lcs_field *f, double t0, double h, int64_t n, int k, int s)
+{
+    const double t = t0 + ((double)n + 0.5 * (double)k) * h;
+    return (t - f->times[s]) / (f->times[s + 1] - f->times[s]);
+}
+// device tables, no host copy: tau[3 i + k] (TC = float or double) for the `count` steps from `first` of window w, and
+// (is_blend) ftau[0 .. 2 count] = (float) tau of ta_0, tb_0, ta_1, tb_1, ..., tc_last for a chunk of the pre-blended integrator
+lcs_status lcs_fill_stage_tau(const lcs_field *f, double t0, double h, int64_t first, int count, const int32_t s[3], void *tau,
+                              float *ftau, cudaStream_t st);
+// bytes lcs_advect carves out of the scratch for n seeds and N steps under the current options (the two integrators and
+// lcs_field_reserve use the same function, so a reservation always covers the call it was made for)
+size_t lcs_cart_scratch_bytes(const lcs_field *f, int64_t n, int64_t N);
+size_t lcs_simplex_scratch_bytes(const lcs_field *f, int64_t n, int64_t N);
+size_t lcs_cart_field_set_bytes(const lcs_field *f, int64_t N);     // one resident set of blended fields (0: not applicable)

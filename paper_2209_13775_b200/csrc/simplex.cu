@@ -549,9 +549,12 @@ __device__ __forceinline__ void load_vertex(const PairRec<DIM, TV> *__restrict__
     for (int k = 0; k < DIM; ++k) { a[k] = (TC)word_value<TV>(w, k); d[k] = (TC)word_value<TV>(w, P + k); }
 }
 
-// u(p, tau) with the walk from *cell; false = p left the mesh through a hull face
+// u(p, tau) with the walk from *cell.  Returns 0 = evaluated, 1 = p left the mesh through a hull face, 2 = the walk did not
+// reach a cell containing p within kWalkCap hops (a stage point many cells away, or a walk cycling among slivers): the
+// tracer is stopped like an exit and counted (info key "walk_cap_hits"), never interpolated in a cell that does not hold it.
+constexpr int kWalkCap = 64;
 template <int DIM, typename TV, typename TC>
-__device__ __forceinline__ bool simplex_velocity(const CellRec<DIM, TC> *__restrict__ crec, const int32_t *__restrict__ neigh,
+__device__ __forceinline__ int simplex_velocity(const CellRec<DIM, TC> *__restrict__ crec, const int32_t *__restrict__ neigh,
                                                  const PairRec<DIM, TV> *__restrict__ vrec, TC tau, const TC *p, int32_t *cell,
                                                  HeldSimplex<DIM, TV, TC> &h, TC *u)
 {
@@ -578,9 +581,10 @@ __device__ __forceinline__ bool simplex_velocity(const CellRec<DIM, TC> *__restr
 #pragma unroll
         for (int i = 1; i <= DIM; ++i)
             if (lam[i] < lmin) { lmin = lam[i]; jmin = i; }
-        if (lmin >= -WalkTol<TC>::eps || hop >= 64) break;
+        if (lmin >= -WalkTol<TC>::eps) break;
+        if (hop >= kWalkCap) return 2;
         int32_t nb = __ldg(neigh + (int64_t)c * (DIM + 1) + jmin);
-        if (nb < 0) return false;
+        if (nb < 0) return 1;
         c = nb;
     }
     *cell = c;
@@ -596,14 +600,15 @@ __device__ __forceinline__ bool simplex_velocity(const CellRec<DIM, TC> *__restr
 #pragma unroll
         for (int k = 0; k < DIM; ++k) u[k] = fma(lam[i], fma(tau, h.d[i][k], h.a[i][k]), u[k]);
     }
-    return true;
+    return 0;
 }
 
 template <int DIM, typename TV, typename TC>
 __global__ void __launch_bounds__(128, (sizeof(TC) == 4 ? 7 : 1))
 simplex_window_kernel(const CellRec<DIM, TC> *__restrict__ crec, const int32_t *__restrict__ neigh, const PairRec<DIM, TV> *__restrict__ pa,
                       const PairRec<DIM, TV> *__restrict__ pb, const PairRec<DIM, TV> *__restrict__ pc, const TC *__restrict__ tau,
-                      int nsteps, int first_step, int64_t n, SimplexTracer<DIM, TC> *__restrict__ st, TC h)
+                      int nsteps, int first_step, int64_t n, SimplexTracer<DIM, TC> *__restrict__ st, TC h,
+                      unsigned long long *__restrict__ stats)
 {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
@@ -613,27 +618,26 @@ simplex_window_kernel(const CellRec<DIM, TC> *__restrict__ crec, const int32_t *
 #pragma unroll
     for (int k = 0; k < DIM; ++k) x[k] = t.x[k];
     int32_t cell = t.cell;
-    int s = 0;
-    bool ok = true;
+    int s = 0, rc = 0;
     HeldSimplex<DIM, TV, TC> held;
     for (; s < nsteps; ++s) {
         const TC ta = __ldg(tau + 3 * s), tb = __ldg(tau + 3 * s + 1), tc = __ldg(tau + 3 * s + 2);
         TC k1[DIM], k2[DIM], k3[DIM], k4[DIM], y[DIM];
         int32_t c = cell;
-        ok = simplex_velocity<DIM, TV, TC>(crec, neigh, pa, ta, x, &c, held, k1);
-        if (!ok) break;
+        rc = simplex_velocity<DIM, TV, TC>(crec, neigh, pa, ta, x, &c, held, k1);
+        if (rc) break;
 #pragma unroll
         for (int k = 0; k < DIM; ++k) y[k] = fma(TC(0.5) * h, k1[k], x[k]);
-        ok = simplex_velocity<DIM, TV, TC>(crec, neigh, pb, tb, y, &c, held, k2);
-        if (!ok) break;
+        rc = simplex_velocity<DIM, TV, TC>(crec, neigh, pb, tb, y, &c, held, k2);
+        if (rc) break;
 #pragma unroll
         for (int k = 0; k < DIM; ++k) y[k] = fma(TC(0.5) * h, k2[k], x[k]);
-        ok = simplex_velocity<DIM, TV, TC>(crec, neigh, pb, tb, y, &c, held, k3);
-        if (!ok) break;
+        rc = simplex_velocity<DIM, TV, TC>(crec, neigh, pb, tb, y, &c, held, k3);
+        if (rc) break;
 #pragma unroll
         for (int k = 0; k < DIM; ++k) y[k] = fma(h, k3[k], x[k]);
-        ok = simplex_velocity<DIM, TV, TC>(crec, neigh, pc, tc, y, &c, held, k4);
-        if (!ok) break;
+        rc = simplex_velocity<DIM, TV, TC>(crec, neigh, pc, tc, y, &c, held, k4);
+        if (rc) break;
 #pragma unroll
         for (int k = 0; k < DIM; ++k) x[k] = fma(h * TC(1.0 / 6.0), (k1[k] + k4[k]) + TC(2) * (k2[k] + k3[k]), x[k]);
         cell = c;
@@ -641,7 +645,8 @@ simplex_window_kernel(const CellRec<DIM, TC> *__restrict__ crec, const int32_t *
 #pragma unroll
     for (int k = 0; k < DIM; ++k) t.x[k] = x[k];
     t.cell = cell;
-    if (!ok) t.meta = (1u << 30) | (uint32_t)(first_step + s);
+    if (rc) t.meta = (1u << 30) | (uint32_t)(first_step + s);
+    if (rc == 2) atomicAdd(stats + 4, 1ull);
     store_tracer(st + i, t);
 }
 
@@ -651,7 +656,8 @@ template <int DIM, typename TV, typename TC>
 __global__ void __launch_bounds__(128)
 simplex_ab4_kernel(const CellRec<DIM, TC> *__restrict__ crec, const int32_t *__restrict__ neigh, const PairRec<DIM, TV> *__restrict__ pa,
                    const PairRec<DIM, TV> *__restrict__ pb, const PairRec<DIM, TV> *__restrict__ pc, const TC *__restrict__ tau,
-                   int nsteps, int first_step, int64_t n, SimplexTracer<DIM, TC> *__restrict__ st, TC *__restrict__ hist, TC h)
+                   int nsteps, int first_step, int64_t n, SimplexTracer<DIM, TC> *__restrict__ st, TC *__restrict__ hist, TC h,
+                   unsigned long long *__restrict__ stats)
 {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
@@ -667,28 +673,28 @@ simplex_ab4_kernel(const CellRec<DIM, TC> *__restrict__ crec, const int32_t *__r
     }
     int32_t cell = t.cell;
     int s = 0;
-    bool ok = true;
+    int rc = 0;
     HeldSimplex<DIM, TV, TC> held;
     for (; s < nsteps; ++s) {
         const TC ta = __ldg(tau + 3 * s), tb = __ldg(tau + 3 * s + 1), tc = __ldg(tau + 3 * s + 2);
         TC k1[DIM], inc[DIM];
         int32_t c = cell;
-        ok = simplex_velocity<DIM, TV, TC>(crec, neigh, pa, ta, x, &c, held, k1);
-        if (!ok) break;
+        rc = simplex_velocity<DIM, TV, TC>(crec, neigh, pa, ta, x, &c, held, k1);
+        if (rc) break;
         if (first_step + s < 3) {
             TC k2[DIM], k3[DIM], k4[DIM], y[DIM];
 #pragma unroll
             for (int k = 0; k < DIM; ++k) y[k] = fma(TC(0.5) * h, k1[k], x[k]);
-            ok = simplex_velocity<DIM, TV, TC>(crec, neigh, pb, tb, y, &c, held, k2);
-            if (!ok) break;
+            rc = simplex_velocity<DIM, TV, TC>(crec, neigh, pb, tb, y, &c, held, k2);
+            if (rc) break;
 #pragma unroll
             for (int k = 0; k < DIM; ++k) y[k] = fma(TC(0.5) * h, k2[k], x[k]);
-            ok = simplex_velocity<DIM, TV, TC>(crec, neigh, pb, tb, y, &c, held, k3);
-            if (!ok) break;
+            rc = simplex_velocity<DIM, TV, TC>(crec, neigh, pb, tb, y, &c, held, k3);
+            if (rc) break;
 #pragma unroll
             for (int k = 0; k < DIM; ++k) y[k] = fma(h, k3[k], x[k]);
-            ok = simplex_velocity<DIM, TV, TC>(crec, neigh, pc, tc, y, &c, held, k4);
-            if (!ok) break;
+            rc = simplex_velocity<DIM, TV, TC>(crec, neigh, pc, tc, y, &c, held, k4);
+            if (rc) break;
 #pragma unroll
             for (int k = 0; k < DIM; ++k) inc[k] = TC(1.0 / 6.0) * ((k1[k] + k4[k]) + TC(2) * (k2[k] + k3[k]));
         } else {
@@ -708,7 +714,8 @@ simplex_ab4_kernel(const CellRec<DIM, TC> *__restrict__ crec, const int32_t *__r
         hist[(i * 3 + 0) * DIM + k] = h0[k]; hist[(i * 3 + 1) * DIM + k] = h1[k]; hist[(i * 3 + 2) * DIM + k] = h2[k];
     }
     t.cell = cell;
-    if (!ok) t.meta = (1u << 30) | (uint32_t)(first_step + s);
+    if (rc) t.meta = (1u << 30) | (uint32_t)(first_step + s);
+    if (rc == 2) atomicAdd(stats + 4, 1ull);
     store_tracer(st + i, t);
 }
 
@@ -759,8 +766,8 @@ template <int DIM> lcs_status build_impl(lcs_field *f, const double *vh, const i
     LCS_CUDA_OK(cudaMalloc((void **)&m.cells, (size_t)nf * 4));
     LCS_CUDA_OK(cudaMalloc((void **)&m.neigh, (size_t)nf * 4));
     LCS_CUDA_OK(cudaMalloc((void **)&m.oppside, (size_t)nc));
-    LCS_CUDA_OK(cudaMalloc((void **)&m.stats, 4 * sizeof(unsigned long long)));
-    LCS_CUDA_OK(cudaMemset(m.stats, 0, 4 * sizeof(unsigned long long)));
+    LCS_CUDA_OK(cudaMalloc((void **)&m.stats, 8 * sizeof(unsigned long long)));
+    LCS_CUDA_OK(cudaMemset(m.stats, 0, 8 * sizeof(unsigned long long)));
     LCS_CUDA_OK(cudaMemcpy(m.verts, vh, (size_t)nv * DIM * 8, cudaMemcpyHostToDevice));
     LCS_CUDA_OK(cudaMemcpy(m.cells, ch, (size_t)nf * 4, cudaMemcpyHostToDevice));
     LCS_CUDA_OK(cudaMemset(m.neigh, 0xff, (size_t)nf * 4));
@@ -857,6 +864,54 @@ template <int DIM> lcs_status build_impl(lcs_field *f, const double *vh, const i
     return LCS_OK;
 }
 
+// how lcs_advect carves the scratch on a simplicial mesh (shared with lcs_field_reserve, see CartLayout)
+struct SimplexLayout {
+    bool ab4, do_bundle;
+    int shift;
+    int64_t nbins, ntiles;
+    size_t o_a, o_b, o_tau, o_hist, o_key, o_cnt, o_tile, total;
+};
+
+size_t simplex_tracer_bytes(const lcs_field *f)
+{
+    const bool c64 = f->compute_dtype == LCS_F64;
+    if (f->dim == 2) return c64 ? sizeof(SimplexTracer<2, double>) : sizeof(SimplexTracer<2, float>);
+    return c64 ? sizeof(SimplexTracer<3, double>) : sizeof(SimplexTracer<3, float>);
+}
+
+SimplexLayout simplex_layout(const lcs_field *f, int64_t n, int64_t N)
+{
+    SimplexLayout L{};
+    const SimplexMesh &m = f->mesh;
+    const int DIM = f->dim;
+    const size_t tcb = lcs_esize(f->compute_dtype), trb = simplex_tracer_bytes(f);
+    // re-bundling by bin (Morton or row-major order of the coarsened bin grid), histogram <= 2^24 bins
+    L.ab4 = f->opt_integrator == 3;
+    L.do_bundle = !L.ab4 && (f->opt_bundle == 1 || (f->opt_bundle < 0 && n >= (1 << 18)));
+    int bits = 0;
+    for (L.shift = 0;; ++L.shift) {
+        bits = 0;
+        for (int a = 0; a < DIM; ++a) {
+            int cells = ((m.nb[a] - 1) >> L.shift) + 1, b = 0;
+            while ((1 << b) < cells) ++b;
+            bits = b > bits ? b : bits;
+        }
+        if (bits * DIM <= 24) break;
+    }
+    L.nbins = L.do_bundle ? ((int64_t)1 << (bits * DIM)) + 1 : 0;
+    L.ntiles = (L.nbins + bundle::kScanTile - 1) / bundle::kScanTile;
+    size_t off = 0;
+    L.o_a = off; off = align_up(off + (size_t)n * trb);
+    L.o_b = off; if (L.do_bundle) off = align_up(off + (size_t)n * trb);
+    L.o_tau = off; off = align_up(off + (size_t)3 * N * tcb);
+    L.o_hist = off; if (L.ab4) off = align_up(off + (size_t)n * 3 * DIM * tcb);
+    L.o_key = off; if (L.do_bundle) off = align_up(off + (size_t)n * 4);
+    L.o_cnt = off; if (L.do_bundle) off = align_up(off + (size_t)L.nbins * 4);
+    L.o_tile = off; if (L.do_bundle) off = align_up(off + (size_t)L.ntiles * 4);
+    L.total = off;
+    return L;
+}
+
 template <int DIM, typename TV, typename TC>
 lcs_status simplex_advect_impl(lcs_field *f, int64_t n, const void *seeds_, double t0, double h, int64_t N, void *flowmap_,
                                uint8_t *exit_flag, int32_t *exit_step, cudaStream_t st)
@@ -865,45 +920,23 @@ lcs_status simplex_advect_impl(lcs_field *f, int64_t n, const void *seeds_, doub
     const TC *seeds = (const TC *)seeds_;
     TC *flowmap = (TC *)flowmap_;
     SimplexMesh &m = f->mesh;
-    if (n >= (1LL << 31) || N >= (1LL << 30)) { lcs_set_error("too many seeds or steps for 32-bit tracer records"); return LCS_ERR_INVALID_ARG; }
-    std::vector<StepWindow> windows;
-    std::vector<double> tau64;
-    lcs_status rc = lcs_plan_windows(f, t0, h, N, windows, tau64);
-    if (rc != LCS_OK) return rc;
-    std::vector<TC> tau(tau64.size());
-    for (size_t k = 0; k < tau.size(); ++k) tau[k] = (TC)tau64[k];
-
-    // re-bundling by bin (Morton order of the coarsened bin grid), histogram <= 2^24 bins
-    const bool ab4 = f->opt_integrator == 3;
-    const bool do_bundle = !ab4 && (f->opt_bundle == 1 || (f->opt_bundle < 0 && n >= (1 << 18)));
-    int shift = 0, bits = 0;
-    for (;; ++shift) {
-        bits = 0;
-        for (int a = 0; a < DIM; ++a) {
-            int cells = ((m.nb[a] - 1) >> shift) + 1, b = 0;
-            while ((1 << b) < cells) ++b;
-            bits = b > bits ? b : bits;
-        }
-        if (bits * DIM <= 24) break;
+    if (n >= (1LL << 31) || N >= (1LL << 24)) { lcs_set_error("too many seeds or steps for 32-bit tracer records"); return LCS_ERR_INVALID_ARG; }
+    if (f->opt_integrator == 2) {
+        lcs_set_error("integrator = 2 (split per-stage kernels) is not available on simplicial meshes in this build");
+        return LCS_ERR_INVALID_ARG;
     }
-    const int64_t nbins = do_bundle ? ((int64_t)1 << (bits * DIM)) + 1 : 0;
-    const int64_t ntiles = (nbins + bundle::kScanTile - 1) / bundle::kScanTile;
-
-    size_t off = 0;
-    const size_t o_a = off; off = align_up(off + (size_t)n * sizeof(Tracer));
-    const size_t o_b = off; if (do_bundle) off = align_up(off + (size_t)n * sizeof(Tracer));
-    const size_t o_tau = off; off = align_up(off + tau.size() * sizeof(TC));
-    const size_t o_hist = off; if (ab4) off = align_up(off + (size_t)n * 3 * DIM * sizeof(TC));
-    const size_t o_key = off; if (do_bundle) off = align_up(off + (size_t)n * 4);
-    const size_t o_cnt = off; if (do_bundle) off = align_up(off + (size_t)nbins * 4);
-    const size_t o_tile = off; if (do_bundle) off = align_up(off + (size_t)ntiles * 4);
-    rc = lcs_scratch_reserve(f, off);
+    std::vector<StepWindow> windows;
+    lcs_status rc = lcs_plan_windows(f, t0, h, N, windows);
     if (rc != LCS_OK) return rc;
+    const SimplexLayout L = simplex_layout(f, n, N);
+    rc = lcs_scratch_check(f, L.total);
+    if (rc != LCS_OK) return rc;
+    const bool ab4 = L.ab4, do_bundle = L.do_bundle;
+    const int64_t nbins = L.nbins;
     char *base = (char *)f->scratch.buf;
-    Tracer *cur = (Tracer *)(base + o_a), *alt = (Tracer *)(base + o_b);
-    TC *d_tau = (TC *)(base + o_tau);
-    uint32_t *d_key = (uint32_t *)(base + o_key), *d_cnt = (uint32_t *)(base + o_cnt), *d_tile = (uint32_t *)(base + o_tile);
-    LCS_CUDA_OK(cudaMemcpyAsync(d_tau, tau.data(), tau.size() * sizeof(TC), cudaMemcpyHostToDevice, st));
+    Tracer *cur = (Tracer *)(base + L.o_a), *alt = (Tracer *)(base + L.o_b);
+    TC *d_tau = (TC *)(base + L.o_tau);
+    uint32_t *d_key = (uint32_t *)(base + L.o_key), *d_cnt = (uint32_t *)(base + L.o_cnt), *d_tile = (uint32_t *)(base + L.o_tile);
     BinGrid b = make_bins(f);
     LCS_LAUNCH((simplex_init_kernel<DIM, TC>), lcs_blocks(n, 128), 128, 0, st, b, m.bins, m.verts, m.cells, m.neigh, m.oppside, m.nc,
                m.hop_cap, seeds, n, cur, m.stats);
@@ -921,6 +954,9 @@ lcs_status simplex_advect_impl(lcs_field *f, int64_t n, const void *seeds_, doub
             rc = lcs_field_require_pair(f, w.s[k], st, &p[k]);
             if (rc != LCS_OK) return rc;
         }
+        // stage-time weights of the window's steps, computed on the device (no host-to-device copy in the hot call)
+        rc = lcs_fill_stage_tau(f, t0, h, w.first, w.count, w.s, d_tau, nullptr, st);
+        if (rc != LCS_OK) return rc;
         lcs_field_prefetch(f, dir > 0 ? w.s[2] + 2 : w.s[2] - 1, w.s[2], w.s[2] + 1);
         const int chunk = (do_bundle && f->opt_bundle_steps > 0 && f->opt_bundle_steps < w.count) ? (int)f->opt_bundle_steps : w.count;
         for (int done = 0, cnt = 0; done < w.count; done += cnt) {
@@ -928,7 +964,7 @@ lcs_status simplex_advect_impl(lcs_field *f, int64_t n, const void *seeds_, doub
             const int first = (int)w.first + done;
             if (do_bundle && (since_bundle < 0 || since_bundle >= bundle_every)) {
                 LCS_CUDA_OK(cudaMemsetAsync(d_cnt, 0, (size_t)nbins * 4, st));
-                LCS_LAUNCH((simplex_key_kernel<DIM, TC>), lcs_blocks(n, 256), 256, 0, st, b, cur, n, shift, (int)f->opt_simplex_order, (uint32_t)(nbins - 1), d_key, d_cnt);
+                LCS_LAUNCH((simplex_key_kernel<DIM, TC>), lcs_blocks(n, 256), 256, 0, st, b, cur, n, L.shift, (int)f->opt_simplex_order, (uint32_t)(nbins - 1), d_key, d_cnt);
                 bundle::sort_records<Tracer>(cur, alt, d_key, d_cnt, d_tile, n, nbins, st);
                 std::swap(cur, alt);
                 since_bundle = 0;
@@ -938,10 +974,10 @@ lcs_status simplex_advect_impl(lcs_field *f, int64_t n, const void *seeds_, doub
             if (ab4)
                 LCS_LAUNCH((simplex_ab4_kernel<DIM, TV, TC>), lcs_blocks(n, block), block, 0, st, (const CellRec<DIM, TC> *)m.cellrec, m.neigh,
                            (const VRec *)p[0], (const VRec *)p[1], (const VRec *)p[2], d_tau + 3 * (size_t)first, cnt, first, n, cur,
-                           (TC *)(base + o_hist), (TC)h);
+                           (TC *)(base + L.o_hist), (TC)h, m.stats);
             else
                 LCS_LAUNCH((simplex_window_kernel<DIM, TV, TC>), lcs_blocks(n, block), block, 0, st, (const CellRec<DIM, TC> *)m.cellrec, m.neigh,
-                           (const VRec *)p[0], (const VRec *)p[1], (const VRec *)p[2], d_tau + 3 * (size_t)first, cnt, first, n, cur, (TC)h);
+                           (const VRec *)p[0], (const VRec *)p[1], (const VRec *)p[2], d_tau + 3 * (size_t)first, cnt, first, n, cur, (TC)h, m.stats);
             if (lcs_early_due(f, (int64_t)first + cnt, N)) {         // row f1: evaluate C for the stencils that are still complete
                 LCS_LAUNCH((simplex_final_kernel<DIM, TC>), lcs_blocks(n, 256), 256, 0, st, n, cur, (int32_t)N, (TC *)f->early.flowmap,
                            f->early.flag, (int32_t *)nullptr);
@@ -957,6 +993,8 @@ lcs_status simplex_advect_impl(lcs_field *f, int64_t n, const void *seeds_, doub
 }
 
 }  // namespace
+
+size_t lcs_simplex_scratch_bytes(const lcs_field *f, int64_t n, int64_t N) { return simplex_layout(f, n, N).total; }
 
 lcs_status lcs_simplex_build(lcs_field *f, const double *verts_host, const int32_t *cells_host)
 {

@@ -21,9 +21,12 @@ STATUS_NAMES = {0: "LCS_OK", 1: "LCS_ERR_INVALID_ARG", 2: "LCS_ERR_TIME_RANGE", 
 LCS_F32, LCS_F64 = 0, 1
 LCS_MESH_CARTESIAN, LCS_MESH_SIMPLEX = 0, 1
 
-EXPORTS = ["lcs_field_create", "lcs_field_set_snapshot", "lcs_field_sync", "lcs_field_destroy",
+EXPORTS = ["lcs_field_create", "lcs_field_set_snapshot", "lcs_field_sync", "lcs_field_destroy", "lcs_field_reserve",
            "lcs_field_set_option", "lcs_field_get_info", "lcs_locate", "lcs_advect", "lcs_advect_early_cg", "lcs_cg_ftle", "lcs_cg_ftle_aux", "lcs_cg_eigen", "lcs_smooth_gaussian", "lcs_ridge",
-           "lcs_ftle_host", "lcs_kernel_launch_count", "lcs_last_error"]
+           "lcs_ftle_host", "lcs_measure_peak", "lcs_kernel_launch_count", "lcs_last_error"]
+PEAK_KINDS = {"fp32_fma_tflops": 0, "fp64_fma_tflops": 1, "launch_us": 2, "hbm_copy_gbs": 3, "l2_seq_gbs": 4, "l2_sector_gbs": 5,
+              "hbm_sector_gbs": 6, "l1_gather_line_gbs": 7, "l1_gather_same_gbs": 8, "l1_gather_spread_gbs": 9,
+              "smem_contiguous_gbs": 10, "smem_records_gbs": 11, "smem_records_swizzled_gbs": 12, "smem_records_same_gbs": 13}
 
 
 class LcsError(RuntimeError):
@@ -61,6 +64,8 @@ def lib():
         L.lcs_field_sync.argtypes = [C.c_void_p]
         L.lcs_field_destroy.argtypes = [C.c_void_p]
         L.lcs_field_destroy.restype = None
+        L.lcs_field_reserve.argtypes = [C.c_void_p, C.c_int64, C.c_int64]
+        L.lcs_measure_peak.argtypes = [C.c_int32, C.POINTER(C.c_double)]
         L.lcs_field_set_option.argtypes = [C.c_void_p, C.c_char_p, C.c_int64]
         L.lcs_field_get_info.argtypes = [C.c_void_p, C.c_char_p, C.POINTER(C.c_int64)]
         L.lcs_locate.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
@@ -79,7 +84,7 @@ def lib():
                                 C.c_void_p, C.c_void_p, C.c_void_p]
         L.lcs_cg_eigen.argtypes = [C.c_int32, C.c_int32, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.lcs_ftle_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
-                                    C.c_double, C.c_double, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p]
+                                    C.c_double, C.c_double, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         _lib = L
     return _lib
 
@@ -114,6 +119,17 @@ def _arr3(vals, ctype, fill, dim=3):
 
 def kernel_launch_count() -> int:
     return int(lib().lcs_kernel_launch_count())
+
+
+def measure_peak(kind) -> float:
+    """lcs_measure_peak: kind is an lcs_peak_kind value or a PEAK_KINDS name (TFLOP/s, microseconds or GB/s, see lcs.h)."""
+    v = C.c_double()
+    _check(lib().lcs_measure_peak(int(PEAK_KINDS.get(kind, kind)), C.byref(v)))
+    return float(v.value)
+
+
+def _n_steps(t0, tf, h) -> int:
+    return max(1, int(round((float(tf) - float(t0)) / float(h)))) if h else 1
 
 
 class Field:
@@ -180,6 +196,11 @@ class Field:
     def set_option(self, key, value):
         _check(lib().lcs_field_set_option(self._h, key.encode(), int(value)))
 
+    def reserve(self, n_seeds, n_steps):
+        """lcs_field_reserve: set-up call that allocates what lcs_advect needs for up to n_seeds tracers and n_steps steps under
+        the current options (the hot calls never allocate).  advect() below calls it, so Python users need not."""
+        _check(lib().lcs_field_reserve(self._h, int(n_seeds), int(n_steps)))
+
     def info(self, key) -> int:
         v = C.c_int64()
         _check(lib().lcs_field_get_info(self._h, key.encode(), C.byref(v)))
@@ -208,8 +229,9 @@ class Field:
         _check(lib().lcs_locate(self._h, n, _tptr(pos), _tptr(cell), _tptr(bary), _stream_ptr(stream)))
         return (cell, bary) if want_bary else cell
 
-    def advect(self, seeds, t0, tf, h, flowmap=None, exit_flag=None, exit_step=None, stream=None, want_flags=True):
-        """seeds: torch CUDA [n][dim] of compute_dtype.  Returns (flowmap, exit_flag, exit_step)."""
+    def advect(self, seeds, t0, tf, h, flowmap=None, exit_flag=None, exit_step=None, stream=None, want_flags=True, reserve=True):
+        """seeds: torch CUDA [n][dim] of compute_dtype.  Returns (flowmap, exit_flag, exit_step).  reserve=False skips the
+        lcs_field_reserve call (lcs_advect then fails with LCS_ERR_OOM unless an earlier reservation covers it)."""
         import torch
         tdt = torch.float64 if self.compute_dtype == np.float64 else torch.float32
         assert seeds.is_cuda and seeds.dtype == tdt and seeds.is_contiguous()
@@ -221,12 +243,16 @@ class Field:
                 exit_flag = torch.empty(n, dtype=torch.uint8, device=seeds.device)
             if exit_step is None:
                 exit_step = torch.empty(n, dtype=torch.int32, device=seeds.device)
+        if reserve and n > 0 and 0 < _n_steps(t0, tf, h) < (1 << 24):
+            self.reserve(n, _n_steps(t0, tf, h))             # no-op once the reservation covers the call
         _check(lib().lcs_advect(self._h, n, _tptr(seeds), float(t0), float(tf), float(h), _tptr(flowmap),
                                 _tptr(exit_flag), _tptr(exit_step), _stream_ptr(stream)))
         return flowmap, exit_flag, exit_step
 
-    def ftle_host(self, ng, seed_spacing, seed_periodic, period, seeds, t0, tf, h, flowmap=None, exit_flag=None, ftle=None):
-        """End-to-end with HOST numpy buffers (H2D + advect + cg_ftle + D2H inside the call)."""
+    def ftle_host(self, ng, seed_spacing, seed_periodic, period, seeds, t0, tf, h, flowmap=None, exit_flag=None, ftle=None,
+                  exit_step=None, cg=None):
+        """End-to-end with HOST numpy buffers (H2D + advect + cg_ftle + D2H inside the call); flowmap, exit_flag, exit_step
+        and cg are optional outputs."""
         seeds = np.ascontiguousarray(seeds, dtype=self.compute_dtype)
         n = seeds.shape[0]
         if ftle is None:
@@ -234,7 +260,7 @@ class Field:
         _check(lib().lcs_ftle_host(self._h, _arr3(ng, C.c_int32, 1), _arr3(seed_spacing, C.c_double, 1.0),
                                    _arr3(seed_periodic, C.c_int32, 0), _arr3(period, C.c_double, 0.0),
                                    _np_ptr(seeds), float(t0), float(tf), float(h), _np_ptr(flowmap), _np_ptr(exit_flag),
-                                   _np_ptr(ftle)))
+                                   _np_ptr(exit_step), _np_ptr(cg), _np_ptr(ftle)))
         return ftle
 
 
@@ -294,6 +320,8 @@ def advect_early_cg(field, ng, seed_spacing, seed_periodic, period, seeds, t0, t
     ftle = torch.empty(n, dtype=seeds.dtype, device=seeds.device)
     t_eff = torch.empty(n, dtype=seeds.dtype, device=seeds.device)
     status = torch.empty(n, dtype=torch.uint8, device=seeds.device)
+    if n > 0 and 0 < _n_steps(t0, tf, h) < (1 << 24):
+        field.reserve(n, _n_steps(t0, tf, h))
     _check(lib().lcs_advect_early_cg(field._h, _arr3(ng, C.c_int32, 1), _arr3(seed_spacing, C.c_double, 1.0), _arr3(seed_periodic, C.c_int32, 0),
                                      _arr3(period, C.c_double, 0.0), _tptr(seeds), float(t0), float(tf), float(h), int(every), _tptr(F),
                                      _tptr(flag), _tptr(es), _tptr(cg), _tptr(ftle), _tptr(t_eff), _tptr(status), _stream_ptr(stream)))

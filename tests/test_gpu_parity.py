@@ -141,6 +141,7 @@ def test_config2_triangles_fp64(lcs, oracle, full):
         sub = np.random.default_rng(22).choice(len(pts), 10000, replace=False)
         cb, count = fo.locate_brute(pts[sub])
         assert count.max() == 1 and np.array_equal(cb, cell[sub]) and f.info("locate_fallbacks") == 0
+    assert f.info("walk_cap_hits") == 0
 
 
 def test_config3_reduced_fp32(lcs, oracle):
@@ -155,34 +156,58 @@ def test_config3_reduced_fp32(lcs, oracle):
     print("config3 reduced", stats)
 
 
+def periodic_block(w, S32, n, B, k0, j0, i0):
+    """Seeds of the B^3 block of an n^3 periodic cell-centred seed grid whose lowest index is (i0, j0, k0) (x fastest),
+    indices wrapping past n - 1: the stored fp32 seeds, shifted by whole periods so that the block is contiguous in space
+    (the field is periodic and positions are never wrapped, reading #13).  Returns (seeds fp64 [B^3][3], wrapped
+    flat seed indices [B^3], period shift [B^3][3])."""
+    kk, jj, ii = np.meshgrid(k0 + np.arange(B), j0 + np.arange(B), i0 + np.arange(B), indexing="ij")
+    idx = np.stack([ii.ravel(), jj.ravel(), kk.ravel()], 1)
+    wrapped = idx % n
+    flat = wrapped[:, 0] + n * (wrapped[:, 1] + n * wrapped[:, 2])
+    shift = (idx // n).astype(np.float64) * np.asarray(w.period, dtype=np.float64)[None, :]
+    return S32[flat].astype(np.float64) + shift, flat, shift
+
+
+def compare_periodic_blocks(oracle, w, fo, F, ftle, blocks, B, t0, tf, h):
+    """SURVEY.md 8.3 parity protocol for the periodic 3D configs at full size: the oracle integrates seeded contiguous B^3
+    blocks (B - 2 interior + 1-seed halo so that the FTLE is comparable); returns per-seed flow-map errors and per-interior-seed
+    relative FTLE errors.  Blocks may straddle the periodic seam of the seed grid (indices wrapping n-1 -> 0): there the GPU's
+    FTLE went through lcs_cg_ftle's +-period seam path while the oracle differentiates a contiguous block."""
+    n = w.ng[0]
+    S32 = w.seeds()
+    Fh, fth = cpu(F), cpu(ftle)
+    errs, rels = [], []
+    for (k0, j0, i0) in blocks:
+        blk, flat, shift = periodic_block(w, S32, n, B, k0, j0, i0)
+        Fo, flo, _ = fo.advect(blk, t0, tf, h)
+        assert np.all(flo == 0)
+        errs.append(np.linalg.norm(Fh[flat].astype(np.float64) + shift - Fo, axis=1))
+        cgo, fto, sto = oracle.cg_ftle(3, (B, B, B), w.seed_spacing, (0, 0, 0), (0, 0, 0), Fo, flo, tf - t0)
+        inner = np.zeros((B, B, B), bool)
+        inner[1:-1, 1:-1, 1:-1] = True
+        inner = inner.ravel()
+        rels.append(np.abs(fth[flat][inner].astype(np.float64) - fto[inner]) / np.maximum(np.abs(fto[inner]), 1e-300))
+    return np.concatenate(errs), np.concatenate(rels)
+
+
 def test_config3_full_size_sampled_blocks(lcs, oracle):
-    """Config 3 at full size (128^3 grid, 256^3 seeds, 500 steps) in bench.py's launch configuration; the
-    oracle integrates 8 seeded 18^3 blocks (16^3 + halo) and FTLE is compared on their interiors."""
-    import torch
+    """Config 3 at full size (128^3 grid, 256^3 seeds, 500 steps) in bench.py's launch configuration (options as bench.py
+    leaves them: the defaults).  SURVEY.md 8.3 protocol: the oracle integrates 8 seeded contiguous 34^3 blocks (32^3 + halo);
+    two of them straddle the periodic seam of the seed grid on every axis, so the seam path of lcs_cg_ftle is compared at
+    full size."""
     w = I.config3()
     f, sd, F, flag, es = gpu_run(w)
     cgg, ftg, stg = gpu_cg(w, F, flag)
-    assert int(flag.max()) == 0
-    Fh = cpu(F).reshape(256, 256, 256, 3)
-    fth = cpu(ftg).reshape(256, 256, 256)
-    seeds = w.seeds().reshape(256, 256, 256, 3)
+    assert int(flag.max()) == 0 and int(es.min()) == 500
     fo = oracle.OracleField.from_workload(w)
     rng = np.random.default_rng(34)
-    B = 18
-    errs, rels = [], []
-    for b in range(8):
-        k0, j0, i0 = rng.integers(0, 256 - B, 3)
-        blk = np.ascontiguousarray(seeds[k0:k0 + B, j0:j0 + B, i0:i0 + B].reshape(-1, 3))
-        Fo, flo, _ = fo.advect(blk.astype(np.float64), w.t0, w.tf, w.h)
-        Fg = Fh[k0:k0 + B, j0:j0 + B, i0:i0 + B].reshape(-1, 3)
-        errs.append(np.linalg.norm(Fg.astype(np.float64) - Fo, axis=1))
-        cgo, fto, sto = oracle.cg_ftle(3, (B, B, B), w.seed_spacing, (0, 0, 0), (0, 0, 0), Fo, flo, w.tf - w.t0)
-        fto = fto.reshape(B, B, B)[1:-1, 1:-1, 1:-1]
-        ftb = fth[k0 + 1:k0 + B - 1, j0 + 1:j0 + B - 1, i0 + 1:i0 + B - 1].astype(np.float64)
-        rels.append((np.abs(ftb - fto) / np.maximum(np.abs(fto), 1e-300)).ravel())
-    err, rel = np.concatenate(errs), np.concatenate(rels)
+    B = 34
+    blocks = [tuple(int(v) for v in rng.integers(0, 256 - B, 3)) for _ in range(6)]
+    blocks += [(240, 245, 250), (int(rng.integers(0, 200)), 230, int(rng.integers(0, 200)))]       # wrap 255 -> 0
+    err, rel = compare_periodic_blocks(oracle, w, fo, F, ftg, blocks, B, w.t0, w.tf, w.h)
     frac = np.mean(err <= 1e-3 * w.L)
-    print("config3 full: frac_ok %.5f median FTLE rel %.3e mean err %.3e max %.3e" % (frac, np.median(rel), err.mean(), err.max()))
+    print("config3 full: %d seeds, frac_ok %.5f median FTLE rel %.3e mean err %.3e max %.3e" % (err.size, frac, np.median(rel), err.mean(), err.max()))
     assert frac >= 0.999 and np.median(rel) <= 1e-3
 
 
@@ -199,6 +224,7 @@ def test_config4_reduced_tets_fp32(lcs, oracle):
     stats = gate_statistical(cpu(F), Fo, cpu(ftg), fto, w.L, fl, flo)
     both1 = (fl == 1) & (flo == 1)
     assert np.mean(np.abs(cpu(es)[both1] - eso[both1]) <= 1) > 0.999
+    assert f.info("walk_cap_hits") == 0 and f.info("locate_fallbacks") == 0
     print("config4 reduced", stats, "flag mismatches", int((fl != flo).sum()))
 
 
@@ -364,6 +390,96 @@ def test_aliasing_and_host_api(lcs, oracle):
     assert np.array_equal(Fh, cpu(F)) and np.array_equal(ft, cpu(ftg), equal_nan=True) and np.array_equal(flh, cpu(flag))
 
 
+def test_host_api_returns_cg_and_exit_steps(lcs, oracle):
+    """lcs_ftle_host with every optional output: Cauchy-Green tensor, exit flags and exit steps equal the device path
+    (open box: flags 0 / 1 / 2)."""
+    A = np.array([[0.03, 0.05], [-0.02, 0.04]])
+    w = I.analytic_cartesian(2, I.linear_flow(A, np.array([0.25, -0.1])), (41, 31), (0.0, 0.0), (0.05, 0.05),
+                             (0.0, 2.0, 4.0), ng=(64, 48), seed_lo=(-0.2, -0.1), seed_spacing=(2.4 / 64, 1.7 / 48),
+                             t0=0.0, tf=4.0, h=0.05)
+    f, sd, F, flag, es = gpu_run(w)
+    cgg, ftg, stg = gpu_cg(w, F, flag)
+    n = w.n_seeds
+    Fh, flh, esh, cgh = np.empty((n, 2)), np.empty(n, np.uint8), np.empty(n, np.int32), np.empty((n, 3))
+    ft = f.ftle_host(w.ng, w.seed_spacing, w.seed_periodic, w.period, w.seeds(), w.t0, w.tf, w.h, flowmap=Fh, exit_flag=flh,
+                     exit_step=esh, cg=cgh)
+    assert set(np.unique(flh)) == {0, 1, 2}
+    assert np.array_equal(Fh, cpu(F)) and np.array_equal(flh, cpu(flag)) and np.array_equal(esh, cpu(es))
+    assert np.array_equal(ft, cpu(ftg), equal_nan=True) and np.array_equal(cgh, cpu(cgg), equal_nan=True)
+
+
+def test_reserve_then_hot_calls_do_not_allocate(lcs, oracle):
+    """the library allocates its scratch in a set-up call, none inside lcs_advect.  After lcs_field_reserve,
+    lcs_advect with growing seed counts (and a different integration length) leaves cudaMemGetInfo unchanged; without a
+    covering reservation it returns LCS_ERR_OOM instead of allocating; results do not depend on who reserved."""
+    import torch
+    w = I.config3(ngrid=64, nn=32, T=1.0, h=0.01, n_snap=5)
+    f = lcs.Field.from_workload(w)
+    for k, v in (("bundle", 1), ("preblend", 1), ("preblend_steps", 10), ("field_sets", 12)):
+        f.set_option(k, v)
+    sd = torch.from_numpy(w.seeds()).cuda()
+    n = sd.shape[0]
+    with pytest.raises(lcs.LcsError) as e:
+        f.advect(sd, w.t0, w.tf, w.h, reserve=False)
+    assert e.value.status == 4 and "lcs_field_reserve" in str(e.value)
+    f.reserve(n, 100)
+    outs = [(torch.empty_like(sd[:m]), torch.empty(m, dtype=torch.uint8, device="cuda"), torch.empty(m, dtype=torch.int32, device="cuda"))
+            for m in (n // 4, n // 2, n)]
+    f.advect(sd[:n // 4], w.t0, w.tf, w.h, flowmap=outs[0][0], exit_flag=outs[0][1], exit_step=outs[0][2], reserve=False)   # loads the kernels
+    torch.cuda.synchronize()
+    free0 = torch.cuda.mem_get_info()[0]
+    scratch0 = f.info("scratch_bytes")
+    for (m, tf), (Fm, flm, esm) in zip(((n // 4, 1.0), (n // 2, 0.5), (n, 1.0)), outs):
+        f.advect(sd[:m], w.t0, tf, w.h, flowmap=Fm, exit_flag=flm, exit_step=esm, reserve=False)
+    torch.cuda.synchronize()
+    assert torch.cuda.mem_get_info()[0] == free0 and f.info("scratch_bytes") == scratch0
+    assert f.info("field_set_hits") > 0
+    with pytest.raises(lcs.LcsError) as e:
+        f.advect(sd, w.t0, 2.0, w.h, reserve=False)                      # 200 steps > the 100 reserved
+    assert e.value.status == 4
+    f1, sd1, F1, fl1, es1 = gpu_run(w, options=dict(bundle=1, preblend=1, preblend_steps=10))
+    assert torch.equal(outs[2][0], F1) and torch.equal(outs[2][2], es1)
+    for bad in ((0, 10), (10, 0), (1 << 31, 10), (10, 1 << 24)):
+        with pytest.raises(lcs.LcsError) as e:
+            f.reserve(*bad)
+        assert e.value.status == 1
+
+
+def test_walk_cap_stops_the_tracer_and_is_counted(lcs, oracle):
+    """A step so long that a stage point lies hundreds of cells away: the in-advect walk gives up after its hop cap; the
+    tracer is stopped (flag 1 at the start of that step) and counted under walk_cap_hits -- never interpolated in a cell
+    that does not contain the point.  Ordinary runs keep the counter at zero (asserted in the config 2 / 4 tests)."""
+    w = I.config2(ng=(32, 16), lattice=(300, 150), T=10.0)
+    w.vel = I.sample_field(I.linear_flow(np.zeros((2, 2)), [0.1, 0.0]), w.vertices, w.times, np.float64)
+    f, sd, F, flag, es = gpu_run(w, t0=0.0, tf=10.0, h=10.0)              # one step: stage points 0.5 and 1.0 domain units = 75 / 150 cells away
+    hits = f.info("walk_cap_hits")
+    fl = cpu(flag)
+    assert hits > 0 and int((fl == 1).sum()) >= hits
+    stopped = fl == 1
+    assert np.array_equal(cpu(F)[stopped], w.seeds()[stopped]) and np.all(cpu(es)[stopped] == 0)
+    f2, sd2, F2, flag2, es2 = gpu_run(w, t0=0.0, tf=10.0, h=0.05)
+    assert f2.info("walk_cap_hits") == 0
+    fo, Fo, flo, eso = oracle_run(oracle, w, t0=0.0, tf=10.0, h=0.05)
+    same = cpu(flag2) == flo
+    assert same.mean() > 0.995 and np.max(np.abs(cpu(F2)[same] - Fo[same])) < 1e-9
+
+
+def test_measured_peaks_are_plausible(lcs):
+    """lcs_measure_peak (peaks measured on the box): every kind runs and lands in the range a B200 can
+    deliver; bench.py quotes its roofline fractions against these."""
+    v = {k: lcs.measure_peak(k) for k in lcs.PEAK_KINDS}
+    print("measured peaks:", {k: round(x, 2) for k, x in v.items()})
+    assert 40.0 < v["fp32_fma_tflops"] < 90.0 and 15.0 < v["fp64_fma_tflops"] < 45.0
+    assert 0.5 < v["launch_us"] < 30.0
+    assert 3000.0 < v["hbm_copy_gbs"] < 8500.0
+    assert v["l2_seq_gbs"] > v["hbm_copy_gbs"] and v["l2_sector_gbs"] > v["hbm_sector_gbs"] > 300.0
+    assert v["l1_gather_line_gbs"] > v["l1_gather_spread_gbs"] and 10000.0 < v["l1_gather_line_gbs"] < 45000.0
+    assert 5000.0 < v["smem_records_gbs"] <= 1.05 * v["smem_contiguous_gbs"] < 45000.0
+    with pytest.raises(lcs.LcsError) as e:
+        lcs.measure_peak(99)
+    assert e.value.status == 1
+
+
 def test_cg_ftle_patterns_vs_oracle(lcs, oracle):
     """lcs_cg_ftle alone on synthetic flow maps: random exit flags (one-sided / NaN patterns), periodic seams,
     2D and 3D, fp64 and fp32 storage, ragged grid sizes."""
@@ -463,7 +579,7 @@ def test_simplex_bundled_identical_to_unbundled(lcs, oracle, options):
         f0, sd0, F0, flag0, es0 = gpu_run(w, options=dict(bundle=0))
         f1, sd1, F1, flag1, es1 = gpu_run(w, options=options)
         assert torch.equal(F0, F1) and torch.equal(flag0, flag1) and torch.equal(es0, es1)
-        assert f1.info("locate_fallbacks") == 0
+        assert f1.info("locate_fallbacks") == 0 and f1.info("walk_cap_hits") == 0 and f0.info("walk_cap_hits") == 0
 
 
 @pytest.mark.slow
@@ -471,7 +587,8 @@ def test_config4_full_size_sampled(lcs, oracle):
     """Config 4 at full size (2.01 M vertices / 13.4 M tets, 256x256x512 box seeds, 1600 steps) in bench.py's launch
     configuration (bundling on by default at this size).  lcs_locate: bit-exact against the oracle's walk on 2e5 sampled
     seeds and against brute force over all cells on 256 of them, with no fallback.  Flow map / FTLE: the oracle integrates
-    6 seeded 12^3 blocks; statistical gate of BASELINE.json."""
+    10 seeded random 16^3 blocks of the box grid; statistical gate of BASELINE.json with flag mismatches counted as
+    failures; the in-advect walk never hits its hop cap."""
     import torch
     w = I.config4()
     f = lcs.Field.from_workload(w)
@@ -489,24 +606,22 @@ def test_config4_full_size_sampled(lcs, oracle):
     F, flag, es = f.advect(sd, w.t0, w.tf, w.h)
     cgg, ftg, stg = gpu_cg(w, F, flag)
     torch.cuda.synchronize()
-    assert f.info("locate_fallbacks") == 0
+    assert f.info("locate_fallbacks") == 0 and f.info("walk_cap_hits") == 0
     nx, ny, nz = w.ng
     Fh = cpu(F).reshape(nz, ny, nx, 3); fth = cpu(ftg).reshape(nz, ny, nx); flh = cpu(flag).reshape(nz, ny, nx)
     S = seeds.reshape(nz, ny, nx, 3)
-    B = 12
-    errs, rels, mism, tot = [], [], 0, 0
-    for b in range(6):
-        if b < 3:      # slow tracers near the wall (r ~ 0.8, u_z ~ 0.7): stay inside for all 1600 steps, FTLE is defined
-            k0, j0, i0 = int(rng.integers(10, 150)), int(rng.integers(110, 134)), 228
-        else:          # core of the pipe: leave through the outlet (flag 1), early or late
-            k0 = int(rng.integers(0, nz // 3)) if b < 5 else int(rng.integers(nz // 2, nz - B))
-            j0, i0 = (int(v) for v in rng.integers(ny // 4, 3 * ny // 4 - B, 2))
+    B = 16
+    errs, rels, mism, flag_mism, tot, counts = [], [], 0, 0, 0, np.zeros(3, int)
+    for b in range(10):
+        k0, j0, i0 = int(rng.integers(0, nz - B)), int(rng.integers(0, ny - B)), int(rng.integers(0, nx - B))
         blk = np.ascontiguousarray(S[k0:k0 + B, j0:j0 + B, i0:i0 + B].reshape(-1, 3))
         Fo, flo, eso = fo.advect(blk.astype(np.float64), w.t0, w.tf, w.h)
         Fg = Fh[k0:k0 + B, j0:j0 + B, i0:i0 + B].reshape(-1, 3).astype(np.float64)
         fg = flh[k0:k0 + B, j0:j0 + B, i0:i0 + B].ravel()
+        assert np.array_equal(fg == 2, flo == 2)                         # the seeds' cells are canonical: exact
         bad = (np.linalg.norm(Fg - Fo, axis=1) > 1e-3 * w.L) | (fg != flo)
-        mism += int(bad.sum()); tot += bad.size
+        mism += int(bad.sum()); flag_mism += int((fg != flo).sum()); tot += bad.size
+        counts += np.bincount(flo, minlength=3)[:3]
         errs.append(np.linalg.norm(Fg - Fo, axis=1)[fg == flo])
         cgo, fto, sto = oracle.cg_ftle(3, (B, B, B), w.seed_spacing, (0, 0, 0), (0, 0, 0), Fo, flo, w.tf - w.t0)
         fto = fto.reshape(B, B, B)[1:-1, 1:-1, 1:-1]
@@ -514,44 +629,48 @@ def test_config4_full_size_sampled(lcs, oracle):
         ok = np.isfinite(fto) & np.isfinite(ftb)
         rels.append((np.abs(ftb[ok] - fto[ok]) / np.maximum(np.abs(fto[ok]), 1e-300)).ravel())
     err = np.concatenate(errs); rel = np.concatenate(rels)
-    print("config4 full: frac_ok %.5f (n=%d) median FTLE rel %.3e (n=%d) mean err %.3e max %.3e" %
-          (1 - mism / tot, tot, np.median(rel) if rel.size else 0.0, rel.size, err.mean(), err.max()))
+    print("config4 full: %d seeds (flags 0/1/2: %s), frac_ok %.5f, flag mismatches %d, median FTLE rel %.3e (n=%d) mean err %.3e max %.3e" %
+          (tot, counts.tolist(), 1 - mism / tot, flag_mism, np.median(rel) if rel.size else 0.0, rel.size, err.mean(), err.max()))
+    assert counts.min() > 500                                            # the sample holds stayers, leavers and outside seeds
     assert 1 - mism / tot >= 0.999
-    assert rel.size > 1000 and np.median(rel) <= 1e-3
+    assert rel.size > 500 and np.median(rel) <= 1e-3
 
 
 @pytest.mark.slow
-def test_config5_full_size_one_volume_streamed(lcs, oracle):
-    """Config 5 at full size for one of its 16 volumes (192^3 seeds, backward 500 steps, ring of 4 slots fed from pinned
-    host memory, pre-blended integrator): the oracle integrates 6 seeded 14^3 blocks; statistical gate."""
+def test_config5_full_size_series_with_field_sets(lcs, oracle):
+    """Config 5 at full size in the configuration bench.py times: ring of 4 device slots fed from pinned host memory and 12
+    resident sets of blended fields.  Three consecutive volumes (192^3 seeds, backward 500 steps) on ONE field: the later
+    volumes reuse the sets cached by the earlier ones (9 of their 10 windows).  The last volume must equal, bit for bit, the
+    same volume from a fresh field WITHOUT field sets, and passes the statistical gate against 6 seeded 18^3 oracle blocks,
+    one of them across the periodic seam."""
     import torch
     w = I.config5()
     f = lcs.Field.from_workload(w, max_resident_snapshots=4, pinned=True)
-    t_rel, t_end = w.meta["windows"][7]
+    f.set_option("field_sets", 12)
     sd = torch.from_numpy(w.seeds()).cuda()
-    F, flag, es = f.advect(sd, t_rel, t_end, w.h)
+    vols = w.meta["windows"][6:9]
+    for (t_rel, t_end) in vols:
+        F, flag, es = f.advect(sd, t_rel, t_end, w.h)
     cgg, ftg, stg = gpu_cg(w, F, flag, T=t_end - t_rel)
     torch.cuda.synchronize()
+    hits, misses = f.info("field_set_hits"), f.info("field_set_misses")
+    print("config5 field sets: hits %d misses %d" % (hits, misses))
+    assert hits == 18 and misses == 12                                   # 10 windows per volume, 9 shared with the previous one
     assert int(flag.max()) == 0 and f.info("ring") == 1 and f.info("h2d_bytes") > 0
-    n = w.ng[0]
-    Fh = cpu(F).reshape(n, n, n, 3); fth = cpu(ftg).reshape(n, n, n); S = w.seeds().reshape(n, n, n, 3)
+    f.close()
+    f0 = lcs.Field.from_workload(w, max_resident_snapshots=4, pinned=True)
+    F0, flag0, es0 = f0.advect(sd, t_rel, t_end, w.h)
+    torch.cuda.synchronize()
+    assert f0.info("field_set_hits") == 0 and torch.equal(F0, F) and torch.equal(flag0, flag) and torch.equal(es0, es)
+    f0.close()
     fo = oracle.OracleField.from_workload(w)
     rng = np.random.default_rng(55)
-    B = 14
-    errs, rels = [], []
-    for b in range(6):
-        k0, j0, i0 = (int(v) for v in rng.integers(0, n - B, 3))
-        blk = np.ascontiguousarray(S[k0:k0 + B, j0:j0 + B, i0:i0 + B].reshape(-1, 3))
-        Fo, flo, _ = fo.advect(blk.astype(np.float64), t_rel, t_end, w.h)
-        Fg = Fh[k0:k0 + B, j0:j0 + B, i0:i0 + B].reshape(-1, 3)
-        errs.append(np.linalg.norm(Fg.astype(np.float64) - Fo, axis=1))
-        cgo, fto, sto = oracle.cg_ftle(3, (B, B, B), w.seed_spacing, (0, 0, 0), (0, 0, 0), Fo, flo, t_end - t_rel)
-        fto = fto.reshape(B, B, B)[1:-1, 1:-1, 1:-1]
-        ftb = fth[k0 + 1:k0 + B - 1, j0 + 1:j0 + B - 1, i0 + 1:i0 + B - 1].astype(np.float64)
-        rels.append((np.abs(ftb - fto) / np.maximum(np.abs(fto), 1e-300)).ravel())
-    err, rel = np.concatenate(errs), np.concatenate(rels)
+    B = 18
+    n = w.ng[0]
+    blocks = [tuple(int(v) for v in rng.integers(0, n - B, 3)) for _ in range(5)] + [(n - 9, n - 5, n - 12)]
+    err, rel = compare_periodic_blocks(oracle, w, fo, F, ftg, blocks, B, t_rel, t_end, w.h)
     frac = np.mean(err <= 1e-3 * w.L)
-    print("config5 full (volume 7): frac_ok %.5f median FTLE rel %.3e mean err %.3e max %.3e" % (frac, np.median(rel), err.mean(), err.max()))
+    print("config5 full (volume 8 of a 3-volume series): frac_ok %.5f median FTLE rel %.3e mean err %.3e max %.3e" % (frac, np.median(rel), err.mean(), err.max()))
     assert frac >= 0.999 and np.median(rel) <= 1e-3
 
 

@@ -45,14 +45,26 @@ def test_reduce_single_rank_is_identity():
     assert bench.reduce_over_ranks(12.5, 7.0, 3.0, "cpu", 1) == (12.5, 7.0, 3.0)
 
 
-def test_rank_shards_are_independent_volumes_of_equal_size():
-    """Weak scaling: rank r integrates the seed grid released at t0 = 0.5 r over the same T; every window stays inside the
-    snapshot times for the 8 ranks of one node, and all ranks do the same amount of work."""
+def test_rank_shards_are_independent_volumes_of_equal_size(monkeypatch):
+    """Weak scaling: bench.make_workload(3, rank) gives rank r the seed grid released at its own t0 over the same T.  The eight
+    windows of one node are distinct, lie inside the snapshot times, have the same number of steps (same work per rank) and
+    share the seeds and the field (replicated, no data-path collective)."""
     sys.path.insert(0, ROOT)
+    import bench
     from paper_2209_13775_b200 import inputs as I
-    w = I.config3(ngrid=8, nn=8)
+    small = I.config3(ngrid=8, nn=8)
+    monkeypatch.setattr(I, "config3", lambda *a, **k: small)
+    seen = []
     for rank in range(8):
-        t0 = 0.5 * rank
-        assert w.times[0] <= t0 and t0 + 5.0 <= w.times[-1] + 1e-12
-    src = open(os.path.join(ROOT, "bench.py")).read()
-    assert "t0 = 0.5 * rank" in src and "\"scaling\": \"weak\"" in src
+        w, runs = bench.make_workload(3, rank)
+        assert w is small and len(runs) == 1
+        t0, tf, h = runs[0]
+        assert w.times[0] <= t0 < tf <= w.times[-1] + 1e-12 and h == w.h
+        assert int(round((tf - t0) / h)) == w.n_steps
+        seen.append((t0, tf))
+    assert len(set(seen)) == 8
+    # the single-volume configs give every rank the same, complete workload (replicas: they do not shard further)
+    for cfg, name in ((1, "config1"), (2, "config2")):
+        tiny = getattr(I, name)(ng=(8, 4)) if cfg == 1 else I.config2(ng=(8, 4), lattice=(9, 5))
+        monkeypatch.setattr(I, name, lambda *a, _t=tiny, **k: _t)
+        assert bench.make_workload(cfg, 0)[1] == bench.make_workload(cfg, 5)[1]
