@@ -471,13 +471,18 @@ extern "C" lcs_status lcs_field_get_info(const lcs_field *f, const char *key, in
         *value = (int64_t)(ms * 1e6);
     }
     else if (!strcmp(key, "locate_fallbacks") || !strcmp(key, "locate_hops") || !strcmp(key, "locate_max_hops") || !strcmp(key, "locate_random_walks") ||
-             !strcmp(key, "walk_cap_hits")) {
+             !strcmp(key, "walk_cap_hits") || !strcmp(key, "walk_fallbacks")) {
         *value = 0;
         if (f->kind == LCS_MESH_SIMPLEX) {
-            unsigned long long h[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+            unsigned long long h[16] = {0};
             cudaMemcpy(h, f->mesh.stats, sizeof h, cudaMemcpyDeviceToHost);
-            *value = (int64_t)h[!strcmp(key, "locate_fallbacks") ? 0 : (!strcmp(key, "locate_hops") ? 1 : (!strcmp(key, "locate_max_hops") ? 2 :
-                                (!strcmp(key, "locate_random_walks") ? 3 : 4)))];
+            // fallbacks of the in-advect re-locations ([8], [11]) count as locate fallbacks / random walks too
+            if (!strcmp(key, "locate_fallbacks")) *value = (int64_t)(h[0] + h[8]);
+            else if (!strcmp(key, "locate_hops")) *value = (int64_t)h[1];
+            else if (!strcmp(key, "locate_max_hops")) *value = (int64_t)h[2];
+            else if (!strcmp(key, "locate_random_walks")) *value = (int64_t)(h[3] + h[11]);
+            else if (!strcmp(key, "walk_cap_hits")) *value = (int64_t)h[4];
+            else *value = (int64_t)h[5];
         }
     }
     else if (!strcmp(key, "scratch_bytes")) *value = (int64_t)f->scratch.bytes;

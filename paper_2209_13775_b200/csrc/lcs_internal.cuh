@@ -68,7 +68,9 @@ struct SimplexMesh {
     double bin_inv[3] = {0, 0, 0};
     int64_t hop_cap = 64;
     unsigned long long *stats = nullptr;   // [0] brute-force fallbacks, [1] walk hops, [2] max hops of one walk (lcs_locate + seeds),
-                                           // [3] random-walk fallbacks, [4] in-advect walks stopped by the hop cap (tracer flagged)
+                                           // [3] random-walk fallbacks, [4] in-advect walks that ended in a cell not holding the point
+                                           // (0 by construction), [5] in-advect walks re-located with the canonical predicate,
+                                           // [8..11] as [0..3] for those re-locations
 };
 
 // tracer scratch owned by the field: one allocation made by lcs_field_reserve and carved by the advect code

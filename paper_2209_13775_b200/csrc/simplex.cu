@@ -549,18 +549,45 @@ __device__ __forceinline__ void load_vertex(const PairRec<DIM, TV> *__restrict__
     for (int k = 0; k < DIM; ++k) { a[k] = (TC)word_value<TV>(w, k); d[k] = (TC)word_value<TV>(w, P + k); }
 }
 
-// u(p, tau) with the walk from *cell.  Returns 0 = evaluated, 1 = p left the mesh through a hull face, 2 = the walk did not
-// reach a cell containing p within kWalkCap hops (a stage point many cells away, or a walk cycling among slivers): the
-// tracer is stopped like an exit and counted (info key "walk_cap_hits"), never interpolated in a cell that does not hold it.
-constexpr int kWalkCap = 64;
-template <int DIM, typename TV, typename TC>
+// What the in-advect walk needs when it gives up: the canonical (fp64) locator of lcs_locate.
+struct CanonCtx {
+    BinGrid b;
+    const int32_t *bins;
+    const double *verts;
+    const int32_t *cells;
+    const int32_t *neigh;
+    const uint8_t *oppside;
+    int64_t nc, hop_cap;
+    unsigned long long *stats;
+};
+
+// canonical owner of p (or -1 = outside the mesh)
+template <int DIM, typename TC> __device__ __forceinline__ int32_t walk_fallback(const CanonCtx &cx, const TC *p)
+{
+    double q[DIM];
+#pragma unroll
+    for (int k = 0; k < DIM; ++k) q[k] = (double)p[k];
+    atomicAdd(cx.stats + 5, 1ull);
+    return locate_canonical<DIM>(cx.b, cx.bins, cx.verts, cx.cells, cx.neigh, cx.oppside, cx.nc, cx.hop_cap, q, cx.stats + 8);
+}
+
+// u(p, tau) with the walk from *cell.  Returns 0 = evaluated, 1 = p left the mesh through a hull face, 2 (SLOW == false
+// only) = the walk on the per-cell affine maps (compute type) has not reached a cell that holds p, to the tolerance, within
+// kWalkCap hops: a stage point many cells away, or two slivers whose rounded maps each push the point into the other.  The
+// integrator then hands the tracer to its SLOW instantiation (a second, small launch over the tracers so marked), which
+// locates such a point again with the canonical fp64 predicate of lcs_locate (info key "walk_fallbacks") and interpolates
+// in its owner: a tracer is never interpolated in a cell that does not hold it ("walk_cap_hits" stays 0 by construction),
+// and the rare path costs the hot kernel neither registers nor code.
+constexpr int kWalkCap = 24;
+template <int DIM, typename TV, typename TC, bool SLOW>
 __device__ __forceinline__ int simplex_velocity(const CellRec<DIM, TC> *__restrict__ crec, const int32_t *__restrict__ neigh,
                                                  const PairRec<DIM, TV> *__restrict__ vrec, TC tau, const TC *p, int32_t *cell,
-                                                 HeldSimplex<DIM, TV, TC> &h, TC *u)
+                                                 HeldSimplex<DIM, TV, TC> &h, const CanonCtx &cx, TC *u)
 {
     int32_t c = *cell;
     TC lam[DIM + 1];
     if (h.pair != (const void *)vrec) { h.vel = false; h.pair = vrec; }        // uniform: another snapshot pair
+    bool forced = false;
     for (int hop = 0;; ++hop) {
         if (h.cell != c) { load_cellrec<DIM, TC>(crec, c, h.r); h.cell = c; h.vel = false; }
         TC q[DIM];
@@ -581,8 +608,14 @@ __device__ __forceinline__ int simplex_velocity(const CellRec<DIM, TC> *__restri
 #pragma unroll
         for (int i = 1; i <= DIM; ++i)
             if (lam[i] < lmin) { lmin = lam[i]; jmin = i; }
-        if (lmin >= -WalkTol<TC>::eps) break;
-        if (hop >= kWalkCap) return 2;
+        if (lmin >= -WalkTol<TC>::eps || forced) break;
+        if (hop >= kWalkCap) {
+            if constexpr (!SLOW) return 2;
+            c = walk_fallback<DIM, TC>(cx, p);
+            if (c < 0) return 1;
+            forced = true;                       // weights of the canonical owner, whatever their rounding
+            continue;
+        }
         int32_t nb = __ldg(neigh + (int64_t)c * (DIM + 1) + jmin);
         if (nb < 0) return 1;
         c = nb;
@@ -603,120 +636,136 @@ __device__ __forceinline__ int simplex_velocity(const CellRec<DIM, TC> *__restri
     return 0;
 }
 
-template <int DIM, typename TV, typename TC>
-__global__ void __launch_bounds__(128, (sizeof(TC) == 4 ? 7 : 1))
+// Tracers whose walk gave up (simplex_velocity returned 2) are parked with flag 3 and their index appended to `pend`; the
+// SLOW instantiation, launched right after on the same stream, resumes each of them at the step it stopped in and finishes the
+// launch unit with the canonical re-location available.  No other kernel ever sees flag 3.
+struct Pending {
+    unsigned int *count;      // number of parked tracers of this launch unit (zeroed before the fast launch)
+    int32_t *index;           // their slots in the tracer array
+};
+
+template <int DIM, typename TV, typename TC, bool SLOW>
+__global__ void __launch_bounds__(128, (sizeof(TC) == 4 && !SLOW ? 7 : 1))
 simplex_window_kernel(const CellRec<DIM, TC> *__restrict__ crec, const int32_t *__restrict__ neigh, const PairRec<DIM, TV> *__restrict__ pa,
                       const PairRec<DIM, TV> *__restrict__ pb, const PairRec<DIM, TV> *__restrict__ pc, const TC *__restrict__ tau,
                       int nsteps, int first_step, int64_t n, SimplexTracer<DIM, TC> *__restrict__ st, TC h,
-                      unsigned long long *__restrict__ stats)
+                      const __grid_constant__ CanonCtx cx, Pending pend)
 {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    SimplexTracer<DIM, TC> t = load_tracer(st + i);
-    if ((t.meta >> 30) != 0) return;
-    TC x[DIM];
+    const int64_t stride = SLOW ? (int64_t)gridDim.x * blockDim.x : n;
+    const int64_t count = SLOW ? (int64_t)*pend.count : n;
+    for (; i < count; i += stride) {
+        const int64_t slot = SLOW ? (int64_t)pend.index[i] : i;
+        SimplexTracer<DIM, TC> t = load_tracer(st + slot);
+        if ((t.meta >> 30) != (SLOW ? 3u : 0u)) continue;
+        TC x[DIM];
 #pragma unroll
-    for (int k = 0; k < DIM; ++k) x[k] = t.x[k];
-    int32_t cell = t.cell;
-    int s = 0, rc = 0;
-    HeldSimplex<DIM, TV, TC> held;
-    for (; s < nsteps; ++s) {
-        const TC ta = __ldg(tau + 3 * s), tb = __ldg(tau + 3 * s + 1), tc = __ldg(tau + 3 * s + 2);
-        TC k1[DIM], k2[DIM], k3[DIM], k4[DIM], y[DIM];
-        int32_t c = cell;
-        rc = simplex_velocity<DIM, TV, TC>(crec, neigh, pa, ta, x, &c, held, k1);
-        if (rc) break;
+        for (int k = 0; k < DIM; ++k) x[k] = t.x[k];
+        int32_t cell = t.cell;
+        int s = SLOW ? (int)(t.meta & 0x3fffffffu) - first_step : 0, rc = 0;
+        HeldSimplex<DIM, TV, TC> held;
+        for (; s < nsteps; ++s) {
+            const TC ta = __ldg(tau + 3 * s), tb = __ldg(tau + 3 * s + 1), tc = __ldg(tau + 3 * s + 2);
+            TC k1[DIM], k2[DIM], k3[DIM], k4[DIM], y[DIM];
+            int32_t c = cell;
+            rc = simplex_velocity<DIM, TV, TC, SLOW>(crec, neigh, pa, ta, x, &c, held, cx, k1);
+            if (rc) break;
 #pragma unroll
-        for (int k = 0; k < DIM; ++k) y[k] = fma(TC(0.5) * h, k1[k], x[k]);
-        rc = simplex_velocity<DIM, TV, TC>(crec, neigh, pb, tb, y, &c, held, k2);
-        if (rc) break;
+            for (int k = 0; k < DIM; ++k) y[k] = fma(TC(0.5) * h, k1[k], x[k]);
+            rc = simplex_velocity<DIM, TV, TC, SLOW>(crec, neigh, pb, tb, y, &c, held, cx, k2);
+            if (rc) break;
 #pragma unroll
-        for (int k = 0; k < DIM; ++k) y[k] = fma(TC(0.5) * h, k2[k], x[k]);
-        rc = simplex_velocity<DIM, TV, TC>(crec, neigh, pb, tb, y, &c, held, k3);
-        if (rc) break;
+            for (int k = 0; k < DIM; ++k) y[k] = fma(TC(0.5) * h, k2[k], x[k]);
+            rc = simplex_velocity<DIM, TV, TC, SLOW>(crec, neigh, pb, tb, y, &c, held, cx, k3);
+            if (rc) break;
 #pragma unroll
-        for (int k = 0; k < DIM; ++k) y[k] = fma(h, k3[k], x[k]);
-        rc = simplex_velocity<DIM, TV, TC>(crec, neigh, pc, tc, y, &c, held, k4);
-        if (rc) break;
+            for (int k = 0; k < DIM; ++k) y[k] = fma(h, k3[k], x[k]);
+            rc = simplex_velocity<DIM, TV, TC, SLOW>(crec, neigh, pc, tc, y, &c, held, cx, k4);
+            if (rc) break;
 #pragma unroll
-        for (int k = 0; k < DIM; ++k) x[k] = fma(h * TC(1.0 / 6.0), (k1[k] + k4[k]) + TC(2) * (k2[k] + k3[k]), x[k]);
-        cell = c;
+            for (int k = 0; k < DIM; ++k) x[k] = fma(h * TC(1.0 / 6.0), (k1[k] + k4[k]) + TC(2) * (k2[k] + k3[k]), x[k]);
+            cell = c;
+        }
+#pragma unroll
+        for (int k = 0; k < DIM; ++k) t.x[k] = x[k];
+        t.cell = cell;
+        t.meta = rc ? ((uint32_t)(rc == 2 ? 3u : 1u) << 30) | (uint32_t)(first_step + s) : 0u;
+        if (!SLOW && rc == 2) pend.index[atomicAdd(pend.count, 1u)] = (int32_t)slot;
+        store_tracer(st + slot, t);
     }
-#pragma unroll
-    for (int k = 0; k < DIM; ++k) t.x[k] = x[k];
-    t.cell = cell;
-    if (rc) t.meta = (1u << 30) | (uint32_t)(first_step + s);
-    if (rc == 2) atomicAdd(stats + 4, 1ull);
-    store_tracer(st + i, t);
 }
 
 // Adams-Bashforth 4 with an RK4 start-up on simplicial meshes (row f4, reading #31): as simplex_window_kernel,
 // one velocity evaluation (walk + interpolation) per step after the first three; hist [n][3][DIM] as in cart_ab4_kernel.
-template <int DIM, typename TV, typename TC>
+template <int DIM, typename TV, typename TC, bool SLOW>
 __global__ void __launch_bounds__(128)
 simplex_ab4_kernel(const CellRec<DIM, TC> *__restrict__ crec, const int32_t *__restrict__ neigh, const PairRec<DIM, TV> *__restrict__ pa,
                    const PairRec<DIM, TV> *__restrict__ pb, const PairRec<DIM, TV> *__restrict__ pc, const TC *__restrict__ tau,
                    int nsteps, int first_step, int64_t n, SimplexTracer<DIM, TC> *__restrict__ st, TC *__restrict__ hist, TC h,
-                   unsigned long long *__restrict__ stats)
+                   const __grid_constant__ CanonCtx cx, Pending pend)
 {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    SimplexTracer<DIM, TC> t = load_tracer(st + i);
-    if ((t.meta >> 30) != 0) return;
-    TC x[DIM], h0[DIM], h1[DIM], h2[DIM];
+    const int64_t stride = SLOW ? (int64_t)gridDim.x * blockDim.x : n;
+    const int64_t count = SLOW ? (int64_t)*pend.count : n;
+    for (; i < count; i += stride) {
+        const int64_t slot = SLOW ? (int64_t)pend.index[i] : i;
+        SimplexTracer<DIM, TC> t = load_tracer(st + slot);
+        if ((t.meta >> 30) != (SLOW ? 3u : 0u)) continue;
+        int s = SLOW ? (int)(t.meta & 0x3fffffffu) - first_step : 0, rc = 0;
+        const bool have_hist = first_step + s > 0;
+        TC x[DIM], h0[DIM], h1[DIM], h2[DIM];
 #pragma unroll
-    for (int k = 0; k < DIM; ++k) {
-        x[k] = t.x[k];
-        h0[k] = first_step > 0 ? hist[(i * 3 + 0) * DIM + k] : TC(0);
-        h1[k] = first_step > 0 ? hist[(i * 3 + 1) * DIM + k] : TC(0);
-        h2[k] = first_step > 0 ? hist[(i * 3 + 2) * DIM + k] : TC(0);
-    }
-    int32_t cell = t.cell;
-    int s = 0;
-    int rc = 0;
-    HeldSimplex<DIM, TV, TC> held;
-    for (; s < nsteps; ++s) {
-        const TC ta = __ldg(tau + 3 * s), tb = __ldg(tau + 3 * s + 1), tc = __ldg(tau + 3 * s + 2);
-        TC k1[DIM], inc[DIM];
-        int32_t c = cell;
-        rc = simplex_velocity<DIM, TV, TC>(crec, neigh, pa, ta, x, &c, held, k1);
-        if (rc) break;
-        if (first_step + s < 3) {
-            TC k2[DIM], k3[DIM], k4[DIM], y[DIM];
-#pragma unroll
-            for (int k = 0; k < DIM; ++k) y[k] = fma(TC(0.5) * h, k1[k], x[k]);
-            rc = simplex_velocity<DIM, TV, TC>(crec, neigh, pb, tb, y, &c, held, k2);
+        for (int k = 0; k < DIM; ++k) {
+            x[k] = t.x[k];
+            h0[k] = have_hist ? hist[(slot * 3 + 0) * DIM + k] : TC(0);
+            h1[k] = have_hist ? hist[(slot * 3 + 1) * DIM + k] : TC(0);
+            h2[k] = have_hist ? hist[(slot * 3 + 2) * DIM + k] : TC(0);
+        }
+        int32_t cell = t.cell;
+        HeldSimplex<DIM, TV, TC> held;
+        for (; s < nsteps; ++s) {
+            const TC ta = __ldg(tau + 3 * s), tb = __ldg(tau + 3 * s + 1), tc = __ldg(tau + 3 * s + 2);
+            TC k1[DIM], inc[DIM];
+            int32_t c = cell;
+            rc = simplex_velocity<DIM, TV, TC, SLOW>(crec, neigh, pa, ta, x, &c, held, cx, k1);
             if (rc) break;
+            if (first_step + s < 3) {
+                TC k2[DIM], k3[DIM], k4[DIM], y[DIM];
 #pragma unroll
-            for (int k = 0; k < DIM; ++k) y[k] = fma(TC(0.5) * h, k2[k], x[k]);
-            rc = simplex_velocity<DIM, TV, TC>(crec, neigh, pb, tb, y, &c, held, k3);
-            if (rc) break;
+                for (int k = 0; k < DIM; ++k) y[k] = fma(TC(0.5) * h, k1[k], x[k]);
+                rc = simplex_velocity<DIM, TV, TC, SLOW>(crec, neigh, pb, tb, y, &c, held, cx, k2);
+                if (rc) break;
 #pragma unroll
-            for (int k = 0; k < DIM; ++k) y[k] = fma(h, k3[k], x[k]);
-            rc = simplex_velocity<DIM, TV, TC>(crec, neigh, pc, tc, y, &c, held, k4);
-            if (rc) break;
+                for (int k = 0; k < DIM; ++k) y[k] = fma(TC(0.5) * h, k2[k], x[k]);
+                rc = simplex_velocity<DIM, TV, TC, SLOW>(crec, neigh, pb, tb, y, &c, held, cx, k3);
+                if (rc) break;
 #pragma unroll
-            for (int k = 0; k < DIM; ++k) inc[k] = TC(1.0 / 6.0) * ((k1[k] + k4[k]) + TC(2) * (k2[k] + k3[k]));
-        } else {
+                for (int k = 0; k < DIM; ++k) y[k] = fma(h, k3[k], x[k]);
+                rc = simplex_velocity<DIM, TV, TC, SLOW>(crec, neigh, pc, tc, y, &c, held, cx, k4);
+                if (rc) break;
 #pragma unroll
-            for (int k = 0; k < DIM; ++k) inc[k] = TC(1.0 / 24.0) * (((TC(55) * k1[k] - TC(59) * h0[k]) + TC(37) * h1[k]) - TC(9) * h2[k]);
+                for (int k = 0; k < DIM; ++k) inc[k] = TC(1.0 / 6.0) * ((k1[k] + k4[k]) + TC(2) * (k2[k] + k3[k]));
+            } else {
+#pragma unroll
+                for (int k = 0; k < DIM; ++k) inc[k] = TC(1.0 / 24.0) * (((TC(55) * k1[k] - TC(59) * h0[k]) + TC(37) * h1[k]) - TC(9) * h2[k]);
+            }
+#pragma unroll
+            for (int k = 0; k < DIM; ++k) {
+                x[k] = fma(h, inc[k], x[k]);
+                h2[k] = h1[k]; h1[k] = h0[k]; h0[k] = k1[k];
+            }
+            cell = c;
         }
 #pragma unroll
         for (int k = 0; k < DIM; ++k) {
-            x[k] = fma(h, inc[k], x[k]);
-            h2[k] = h1[k]; h1[k] = h0[k]; h0[k] = k1[k];
+            t.x[k] = x[k];
+            hist[(slot * 3 + 0) * DIM + k] = h0[k]; hist[(slot * 3 + 1) * DIM + k] = h1[k]; hist[(slot * 3 + 2) * DIM + k] = h2[k];
         }
-        cell = c;
+        t.cell = cell;
+        t.meta = rc ? ((uint32_t)(rc == 2 ? 3u : 1u) << 30) | (uint32_t)(first_step + s) : 0u;
+        if (!SLOW && rc == 2) pend.index[atomicAdd(pend.count, 1u)] = (int32_t)slot;
+        store_tracer(st + slot, t);
     }
-#pragma unroll
-    for (int k = 0; k < DIM; ++k) {
-        t.x[k] = x[k];
-        hist[(i * 3 + 0) * DIM + k] = h0[k]; hist[(i * 3 + 1) * DIM + k] = h1[k]; hist[(i * 3 + 2) * DIM + k] = h2[k];
-    }
-    t.cell = cell;
-    if (rc) t.meta = (1u << 30) | (uint32_t)(first_step + s);
-    if (rc == 2) atomicAdd(stats + 4, 1ull);
-    store_tracer(st + i, t);
 }
 
 template <int DIM, typename TC>
@@ -766,8 +815,8 @@ template <int DIM> lcs_status build_impl(lcs_field *f, const double *vh, const i
     LCS_CUDA_OK(cudaMalloc((void **)&m.cells, (size_t)nf * 4));
     LCS_CUDA_OK(cudaMalloc((void **)&m.neigh, (size_t)nf * 4));
     LCS_CUDA_OK(cudaMalloc((void **)&m.oppside, (size_t)nc));
-    LCS_CUDA_OK(cudaMalloc((void **)&m.stats, 8 * sizeof(unsigned long long)));
-    LCS_CUDA_OK(cudaMemset(m.stats, 0, 8 * sizeof(unsigned long long)));
+    LCS_CUDA_OK(cudaMalloc((void **)&m.stats, 16 * sizeof(unsigned long long)));
+    LCS_CUDA_OK(cudaMemset(m.stats, 0, 16 * sizeof(unsigned long long)));
     LCS_CUDA_OK(cudaMemcpy(m.verts, vh, (size_t)nv * DIM * 8, cudaMemcpyHostToDevice));
     LCS_CUDA_OK(cudaMemcpy(m.cells, ch, (size_t)nf * 4, cudaMemcpyHostToDevice));
     LCS_CUDA_OK(cudaMemset(m.neigh, 0xff, (size_t)nf * 4));
@@ -869,7 +918,7 @@ struct SimplexLayout {
     bool ab4, do_bundle;
     int shift;
     int64_t nbins, ntiles;
-    size_t o_a, o_b, o_tau, o_hist, o_key, o_cnt, o_tile, total;
+    size_t o_a, o_b, o_tau, o_hist, o_key, o_cnt, o_tile, o_pend, total;
 };
 
 size_t simplex_tracer_bytes(const lcs_field *f)
@@ -908,6 +957,7 @@ SimplexLayout simplex_layout(const lcs_field *f, int64_t n, int64_t N)
     L.o_key = off; if (L.do_bundle) off = align_up(off + (size_t)n * 4);
     L.o_cnt = off; if (L.do_bundle) off = align_up(off + (size_t)L.nbins * 4);
     L.o_tile = off; if (L.do_bundle) off = align_up(off + (size_t)L.ntiles * 4);
+    L.o_pend = off; off = align_up(off + 256 + (size_t)n * 4);      // counter + slots of the tracers handed to the slow path
     L.total = off;
     return L;
 }
@@ -938,6 +988,7 @@ lcs_status simplex_advect_impl(lcs_field *f, int64_t n, const void *seeds_, doub
     TC *d_tau = (TC *)(base + L.o_tau);
     uint32_t *d_key = (uint32_t *)(base + L.o_key), *d_cnt = (uint32_t *)(base + L.o_cnt), *d_tile = (uint32_t *)(base + L.o_tile);
     BinGrid b = make_bins(f);
+    const CanonCtx cx{b, m.bins, m.verts, m.cells, m.neigh, m.oppside, m.nc, m.hop_cap, m.stats};
     LCS_LAUNCH((simplex_init_kernel<DIM, TC>), lcs_blocks(n, 128), 128, 0, st, b, m.bins, m.verts, m.cells, m.neigh, m.oppside, m.nc,
                m.hop_cap, seeds, n, cur, m.stats);
     const int block = f->opt_block ? (int)(f->opt_block > 128 ? 128 : f->opt_block) : 128;
@@ -970,14 +1021,26 @@ lcs_status simplex_advect_impl(lcs_field *f, int64_t n, const void *seeds_, doub
                 since_bundle = 0;
             }
             since_bundle += cnt;
-            WindowTimer timer(f, st);
+            const Pending pend{(unsigned int *)(base + L.o_pend), (int32_t *)(base + L.o_pend + 256)};
+            LCS_CUDA_OK(cudaMemsetAsync(pend.count, 0, 4, st));
+            {
+                WindowTimer timer(f, st);
+                if (ab4)
+                    LCS_LAUNCH((simplex_ab4_kernel<DIM, TV, TC, false>), lcs_blocks(n, block), block, 0, st, (const CellRec<DIM, TC> *)m.cellrec, m.neigh,
+                               (const VRec *)p[0], (const VRec *)p[1], (const VRec *)p[2], d_tau + 3 * (size_t)first, cnt, first, n, cur,
+                               (TC *)(base + L.o_hist), (TC)h, cx, pend);
+                else
+                    LCS_LAUNCH((simplex_window_kernel<DIM, TV, TC, false>), lcs_blocks(n, block), block, 0, st, (const CellRec<DIM, TC> *)m.cellrec, m.neigh,
+                               (const VRec *)p[0], (const VRec *)p[1], (const VRec *)p[2], d_tau + 3 * (size_t)first, cnt, first, n, cur, (TC)h, cx, pend);
+            }
+            // the tracers whose walk gave up (usually none): a small grid-stride launch over the parked slots
             if (ab4)
-                LCS_LAUNCH((simplex_ab4_kernel<DIM, TV, TC>), lcs_blocks(n, block), block, 0, st, (const CellRec<DIM, TC> *)m.cellrec, m.neigh,
+                LCS_LAUNCH((simplex_ab4_kernel<DIM, TV, TC, true>), 148, 128, 0, st, (const CellRec<DIM, TC> *)m.cellrec, m.neigh,
                            (const VRec *)p[0], (const VRec *)p[1], (const VRec *)p[2], d_tau + 3 * (size_t)first, cnt, first, n, cur,
-                           (TC *)(base + L.o_hist), (TC)h, m.stats);
+                           (TC *)(base + L.o_hist), (TC)h, cx, pend);
             else
-                LCS_LAUNCH((simplex_window_kernel<DIM, TV, TC>), lcs_blocks(n, block), block, 0, st, (const CellRec<DIM, TC> *)m.cellrec, m.neigh,
-                           (const VRec *)p[0], (const VRec *)p[1], (const VRec *)p[2], d_tau + 3 * (size_t)first, cnt, first, n, cur, (TC)h, m.stats);
+                LCS_LAUNCH((simplex_window_kernel<DIM, TV, TC, true>), 148, 128, 0, st, (const CellRec<DIM, TC> *)m.cellrec, m.neigh,
+                           (const VRec *)p[0], (const VRec *)p[1], (const VRec *)p[2], d_tau + 3 * (size_t)first, cnt, first, n, cur, (TC)h, cx, pend);
             if (lcs_early_due(f, (int64_t)first + cnt, N)) {         // row f1: evaluate C for the stencils that are still complete
                 LCS_LAUNCH((simplex_final_kernel<DIM, TC>), lcs_blocks(n, 256), 256, 0, st, n, cur, (int32_t)N, (TC *)f->early.flowmap,
                            f->early.flag, (int32_t *)nullptr);
