@@ -236,7 +236,7 @@ def reduce_over_ranks(elapsed_ms, seed_steps, seeds, device, world):
 
 
 # ------------------------------------------------------------------------------------------------
-def roofline_block(lcs, cfg, w, kernel_s, units_per_launch, share, win_launches, win_s_per_pass):
+def roofline_block(lcs, cfg, w, kernel_s, units_per_launch, share, win_launches, win_s_per_pass, options=()):
     """The roofline object of one config (see the module docstring)."""
     pk = measured_peaks(lcs)
     prof = profile_constants(cfg)
@@ -260,7 +260,9 @@ def roofline_block(lcs, cfg, w, kernel_s, units_per_launch, share, win_launches,
                                 "fields / held cell), so this is a statement about the method, not a utilisation"}
         delivered = prof.get("l1_bytes_to_registers_per_seed_step")
         kern = prof.get("kernel", "cart_xpair_kernel" if cart else "simplex_window_kernel")
-        staged = "tma" in kern
+        staged = cart and any(o.startswith("tma=") and o != "tma=0" for o in options)
+        if staged:                                           # the staged variant has no counter table of its own in roofline_cfgN.json
+            kern, delivered = "cart_xpair_tma_kernel", 256.0
         peak_key = "smem_records_swizzled_gbs" if staged else "l1_gather_line_gbs"
         if delivered:
             ach = delivered * rate / 1e9
@@ -407,7 +409,7 @@ def run_config(args, lcs, cfg, steps, warmup, rank, world, local, with_e2e, with
         kernel_s = win_ns * 1e-9 / max(win_launches, 1)                    # average launch duration of the dominant kernel
         units_per_launch = steps_per_pass * steps / max(win_launches, 1)
         share = (win_ns * 1e-9) / (elapsed_ms * 1e-3) if world == 1 else None
-        roofline = roofline_block(lcs, cfg, w, kernel_s, units_per_launch, share, win_launches, win_ns * 1e-9 / steps)
+        roofline = roofline_block(lcs, cfg, w, kernel_s, units_per_launch, share, win_launches, win_ns * 1e-9 / steps, args.option)
         l2_note = ("flushed: a 256 MB buffer is written between timed passes (working set %.1f MB < L2)" % (state_bytes / 1e6)) if flush else \
                   ("inputs larger than L2: tracer records, seeds, outputs and fields are %.0f MB per pass" % (state_bytes / 1e6))
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warmup,

@@ -105,11 +105,16 @@ lcs_status lcs_field_reserve(lcs_field *f, int64_t n_seeds, int64_t n_steps);
  * "bundle" -1 = auto, 0 = off, 1 = on: re-bundle tracers by cell (Morton order of the cell index) so that a
  * warp gathers from neighbouring cells; results are returned in the caller's order;
  * "bundle_steps" k = re-bundle every k RK4 steps (0 = once per snapshot window; unstructured meshes: every 160 steps);
- * "bundle_order" / "simplex_order" 0 = Morton, 1 = row-major (x fastest, default) sort key over cells / bins;
+ * "bundle_order" / "simplex_order" 0 = Morton, 1 = row-major (x fastest, default) sort key over cells / bins ("bundle_order" 2 = pairs of
+ * x-neighbouring cells split by sub-cell octant, 3 = bricks of 4 x 2 x 2 cells; both 3D Cartesian only);
  * "field_sets" m = keep the blended fields of the last m chunks resident (about 7 GB each for a 128^3 grid and 50-step chunks)
  * and reuse them when a later lcs_advect needs the same snapshot pair and stage times (FTLE time series: volumes released one
  * snapshot interval apart share most windows); "field_sets_clear" = forget them;
  * "preblend" -1/0/1 and "preblend_steps" k: 3D fp32 Cartesian grids gather from per-stage-time blended fields, k steps per launch;
+ * "tma" 0/1/2 (default 0): 3D fp32 grids that are periodic with power-of-two node counts on every axis: the pre-blended integrator
+ * stages the records of each block's bounding box through shared memory with TMA bulk copies (cp.async.bulk + mbarrier), tracers
+ * bundled in 4 x 2 x 2-cell bricks (2: in the order of "bundle_order"); bit-identical results; measured SLOWER than the global-memory
+ * gather on B200 (profiles/r2_cfg3_tma.md), hence off by default; "tma_cap" = records per shared-memory tile (default 704);
  * "ld256" 0/1 = gather each 32-byte node record with one 256-bit load; "block" = threads per block;
  * "time_windows" 0/1 = record CUDA events around the integrator launches (read with lcs_field_get_info). */
 lcs_status lcs_field_set_option(lcs_field *f, const char *key, int64_t value);

@@ -23,6 +23,7 @@
 //    last gathered cell stay in registers (cart_xpair_kernel below).
 //  * fused variant: one thread runs every RK4 step of a snapshot window; split variant (the paper's): one
 //    short kernel per RK4 stage with the stage state in global memory.
+#include <limits.h>
 #include <math.h>
 
 #include <algorithm>
@@ -280,6 +281,12 @@ __global__ void __launch_bounds__(256) cart_key_kernel(CartDev g, const CartTrac
             const uint32_t sub = ((t.w[DIM - 1] >= TC(0.5)) ? 8u : 0u) | ((t.w[1] >= TC(0.5)) ? 4u : 0u) | (((uint32_t)c[0] & 1u) << 1) |
                                  ((t.w[0] >= TC(0.5)) ? 1u : 0u);
             k = (((uint32_t)c[0] >> 1) + m0p * ((uint32_t)c[1] + (uint32_t)m1 * (uint32_t)c[DIM - 1])) * 16u + sub;
+        } else if (order == 3 && DIM == 3) {
+            // bricks of 4 x 2 x 2 cells, x fastest inside and across bricks: 256 consecutive tracers then sit in a box of about
+            // 8 x 2 x 2 cells, whose records the staged integrator copies into shared memory as one small tile
+            const uint32_t mb0 = (uint32_t)(m0 + 3) >> 2, mb1 = (uint32_t)(m1 + 1) >> 1;
+            const uint32_t sub = ((uint32_t)c[0] & 3u) | (((uint32_t)c[1] & 1u) << 2) | (((uint32_t)c[DIM - 1] & 1u) << 3);
+            k = (((uint32_t)c[0] >> 2) + mb0 * (((uint32_t)c[1] >> 1) + mb1 * ((uint32_t)c[DIM - 1] >> 1))) * 16u + sub;
         } else if (order >= 1) {
             k = (uint32_t)c[0] + (uint32_t)m0 * ((uint32_t)c[1] + (DIM == 3 ? (uint32_t)m1 * (uint32_t)c[DIM - 1] : 0u));
         } else {
@@ -511,6 +518,245 @@ cart_xpair_kernel(const __grid_constant__ CartDev g, const XPair *__restrict__ f
 }
 
 // ---------------------------------------------------------------------------------------------
+// Staged variant of the pre-blended integrator (BASELINE.json north_star, second subsystem: "the two bracketing snapshots
+// staged through L2 and shared memory via TMA or cp.async"; PAPER.md:61 the window of frames on the GPU, PAPER.md:109 bundles
+// "to improve memory coherence and shared-memory GPU performance").  A block owns 256 consecutive tracers of the brick-ordered
+// bundle (sort order 3), i.e. a box of about 8 x 2 x 2 cells.  Every RK4 step the block reduces the bounding box of its tracers'
+// cells (redux.sync + shared-memory atomics, one barrier), and warp 0 copies the records of that box, grown by the one cell a
+// stage point can move, of the two NEW stage-time fields of the step (tb, tc) into shared memory with the TMA engine's
+// non-tensor bulk copies (cp.async.bulk.shared.global, one per x-row segment, completion on an mbarrier per field).  Stages 2
+// and 4 then gather their 2 x 2 x-pair records from shared memory (8 LDS.128 per lane) instead of the L1; stage 1 and 3 reuse
+// the held cell as in cart_xpair_kernel and reload the few lanes that changed cell.  A box larger than the tile capacity
+// (a block that straddles the end of a brick row, or tracers that dispersed) and a stage point outside the box fall back to
+// the global-memory gather of cart_xpair_kernel, so the result is bit-identical to it in every case.
+// Only for grids that are periodic with power-of-two node counts on every axis (no exits; wrap by mask).
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, int count) { asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory"); }
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "LCS_WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra LCS_DONE_%=;\n"
+        "bra LCS_WAIT_%=;\n"
+        "LCS_DONE_%=:\n"
+        "}" ::"r"(bar), "r"(parity) : "memory");
+}
+// global -> shared bulk copy by the TMA engine (SASS UBLKCP), bytes a multiple of 16, completion counted on the mbarrier
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst), "l"(src), "r"(bytes), "r"(bar)
+                 : "memory");
+}
+__device__ __forceinline__ void lds_xpair(uint32_t addr, float4 &lo, float4 &hi)
+{
+    asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(lo.x), "=f"(lo.y), "=f"(lo.z), "=f"(lo.w) : "r"(addr));
+    asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(hi.x), "=f"(hi.y), "=f"(hi.z), "=f"(hi.w) : "r"(addr + 16u));
+}
+
+struct StageTile {
+    uint32_t addr;         // shared-memory address of the tile, 0 = this step is not staged
+    int o[3];              // cell coordinates (in the block's local frame) of record 0
+    int e[3];              // records per axis
+};
+
+__device__ __forceinline__ void set_held(HeldCell &hc, const float4 &l00, const float4 &h00, const float4 &l10, const float4 &h10, const float4 &l01,
+                                         const float4 &h01, const float4 &l11, const float4 &h11)
+{
+    hc.v[0][0] = l00.x; hc.v[0][1] = l00.y; hc.v[0][2] = l00.z;
+    hc.v[1][0] = h00.x; hc.v[1][1] = h00.y; hc.v[1][2] = h00.z;
+    hc.v[2][0] = l10.x; hc.v[2][1] = l10.y; hc.v[2][2] = l10.z;
+    hc.v[3][0] = h10.x; hc.v[3][1] = h10.y; hc.v[3][2] = h10.z;
+    hc.v[4][0] = l01.x; hc.v[4][1] = l01.y; hc.v[4][2] = l01.z;
+    hc.v[5][0] = h01.x; hc.v[5][1] = h01.y; hc.v[5][2] = h01.z;
+    hc.v[6][0] = l11.x; hc.v[6][1] = l11.y; hc.v[6][2] = l11.z;
+    hc.v[7][0] = h11.x; hc.v[7][1] = h11.y; hc.v[7][2] = h11.z;
+}
+
+// as cart_velocity_xpair<true, REUSE> with the gather served from the shared-memory tile when the cell lies inside it.
+// ci = cell in the block's local frame (wrapped once at load, then free-running), hc.idx = packed wrapped cell.
+template <bool REUSE>
+__device__ __forceinline__ void cart_velocity_staged(const CartDev &g, const XPair *__restrict__ field, const StageTile &tl, const int *ci,
+                                                     const float *xi, HeldCell &hc, float *u)
+{
+    int c[3];
+    float wl[3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        int ifl;
+        floor_split<float>(xi[a], ifl, wl[a]);
+        c[a] = ci[a] + ifl;
+    }
+    const int key = (c[0] & 1023) | ((c[1] & 1023) << 10) | ((c[2] & 1023) << 20);
+    if (!REUSE || key != hc.idx) {
+        const int j0 = c[0] - tl.o[0], j1 = c[1] - tl.o[1], j2 = c[2] - tl.o[2];
+        float4 l00, h00, l10, h10, l01, h01, l11, h11;
+        if (tl.addr != 0u && (unsigned)j0 < (unsigned)tl.e[0] && (unsigned)j1 < (unsigned)(tl.e[1] - 1) && (unsigned)j2 < (unsigned)(tl.e[2] - 1)) {
+            const uint32_t sy = (uint32_t)tl.e[0] * 32u, sz = sy * (uint32_t)tl.e[1];
+            const uint32_t b = tl.addr + (uint32_t)j0 * 32u + (uint32_t)j1 * sy + (uint32_t)j2 * sz;
+            lds_xpair(b, l00, h00);
+            lds_xpair(b + sy, l10, h10);
+            lds_xpair(b + sz, l01, h01);
+            lds_xpair(b + sz + sy, l11, h11);
+        } else {
+            const XPair *b = field + ((c[0] & (g.n[0] - 1)) + (c[1] & (g.n[1] - 1)) * g.np0 + (c[2] & (g.n[2] - 1)) * g.np01);
+            load_xpair(b, l00, h00);
+            load_xpair(b + g.np0, l10, h10);
+            load_xpair(b + g.np01, l01, h01);
+            load_xpair(b + g.np01 + g.np0, l11, h11);
+        }
+        set_held(hc, l00, h00, l10, h10, l01, h01, l11, h11);
+        hc.idx = key;
+    }
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        float a00 = fmaf(wl[0], hc.v[1][k], hc.v[0][k]);
+        float a10 = fmaf(wl[0], hc.v[3][k], hc.v[2][k]);
+        float a01 = fmaf(wl[0], hc.v[5][k], hc.v[4][k]);
+        float a11 = fmaf(wl[0], hc.v[7][k], hc.v[6][k]);
+        float b0 = fmaf(wl[1], a10 - a00, a00);
+        float b1 = fmaf(wl[1], a11 - a01, a01);
+        u[k] = fmaf(wl[2], b1 - b0, b0);
+    }
+}
+
+constexpr int kStageBlock = 256;
+
+__global__ void __launch_bounds__(kStageBlock, 4)
+cart_xpair_tma_kernel(const __grid_constant__ CartDev g, const XPair *__restrict__ fields, int64_t field_stride, int nsteps, int first_step,
+                      int64_t n, CartTracer<3, float> *__restrict__ st, float hs0, float hs1, float hs2, int cap)
+{
+    extern __shared__ __align__(128) unsigned char smem[];
+    // layout: tile of tb | tile of tc | 2 mbarriers | 3 bounding boxes {min[3], max[3], pad[2]}
+    const uint32_t tile_b = smem_u32(smem), tile_c = tile_b + (uint32_t)cap * 32u;
+    uint64_t *bars = reinterpret_cast<uint64_t *>(smem + (size_t)cap * 64);
+    int *sbox = reinterpret_cast<int *>(smem + (size_t)cap * 64 + 16);
+    const uint32_t bar_b = smem_u32(bars), bar_c = bar_b + 8u;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (tid == 0) {
+        mbar_init(bar_b, 32);
+        mbar_init(bar_c, 32);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+#pragma unroll
+        for (int k = 0; k < 3; ++k) { sbox[k] = INT_MAX; sbox[3 + k] = INT_MIN; }
+    }
+    __syncthreads();
+
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + tid;
+    CartTracer<3, float> t;
+    bool live = i < n;
+    if (live) { t = load_record(st + i); live = (t.meta >> 30) == 0; }
+    const float hs[3] = {hs0, hs1, hs2};
+    int ci[3] = {0, 0, 0};
+    float w[3] = {0.f, 0.f, 0.f};
+    if (live) {
+#pragma unroll
+        for (int a = 0; a < 3; ++a) { ci[a] = t.ci[a] & (g.n[a] - 1); w[a] = t.w[a]; }
+    }
+    HeldCell hc;
+    hc.idx = -1;
+    uint32_t uses = 0;                                          // staged steps so far: mbarrier phase parity
+    for (int s = 0; s < nsteps; ++s) {
+        const XPair *fa = fields + (int64_t)(2 * s) * field_stride;
+        const XPair *fb = fa + field_stride;
+        const XPair *fc = fb + field_stride;
+        // ---- bounding box of the block's cells at the start of the step
+        int *box = sbox + 8 * (s % 3);
+        {
+            const int lo0 = __reduce_min_sync(0xffffffffu, live ? ci[0] : INT_MAX), hi0 = __reduce_max_sync(0xffffffffu, live ? ci[0] : INT_MIN);
+            const int lo1 = __reduce_min_sync(0xffffffffu, live ? ci[1] : INT_MAX), hi1 = __reduce_max_sync(0xffffffffu, live ? ci[1] : INT_MIN);
+            const int lo2 = __reduce_min_sync(0xffffffffu, live ? ci[2] : INT_MAX), hi2 = __reduce_max_sync(0xffffffffu, live ? ci[2] : INT_MIN);
+            if (lane == 0) {
+                atomicMin(box + 0, lo0); atomicMin(box + 1, lo1); atomicMin(box + 2, lo2);
+                atomicMax(box + 3, hi0); atomicMax(box + 4, hi1); atomicMax(box + 5, hi2);
+            }
+            if (tid == 0) {
+                int *nxt = sbox + 8 * ((s + 1) % 3);
+#pragma unroll
+                for (int k = 0; k < 3; ++k) { nxt[k] = INT_MAX; nxt[3 + k] = INT_MIN; }
+            }
+        }
+        __syncthreads();                                        // box complete; every thread is done with the tiles of step s - 1
+        StageTile tb, tc;
+        {
+            const int lo0 = box[0], lo1 = box[1], lo2 = box[2], hi0 = box[3], hi1 = box[4], hi2 = box[5];
+            // a stage point is less than one cell from the start of the step (checked per lane): x needs cells lo-1 .. hi+1 (the
+            // x+1 node is inside the record), y and z need rows lo-1 .. hi+2
+            tb.o[0] = lo0 - 1; tb.o[1] = lo1 - 1; tb.o[2] = lo2 - 1;
+            tb.e[0] = hi0 - lo0 + 3; tb.e[1] = hi1 - lo1 + 4; tb.e[2] = hi2 - lo2 + 4;
+            const bool staged = hi0 >= lo0 && (int64_t)tb.e[0] * tb.e[1] * tb.e[2] <= (int64_t)cap && tb.e[0] <= g.n[0];
+            tb.addr = staged ? tile_b : 0u;
+            tc = tb;
+            tc.addr = staged ? tile_c : 0u;
+        }
+        const bool staged = tb.addr != 0u;
+        if (staged && warp == 0) {
+            // one bulk copy per x-row segment and field; a row that crosses the periodic seam in x takes two
+            const int rows = tb.e[1] * tb.e[2];
+            const int gx = tb.o[0] & (g.n[0] - 1);
+            const int n_a = min(tb.e[0], g.n[0] - gx), n_b = tb.e[0] - n_a;
+            int mine = 0;
+            for (int r = lane; r < rows; r += 32) ++mine;
+            const uint32_t bytes = (uint32_t)mine * (uint32_t)tb.e[0] * 32u;
+            mbar_arrive_expect_tx(bar_b, bytes);
+            mbar_arrive_expect_tx(bar_c, bytes);
+            for (int r = lane; r < rows; r += 32) {
+                const int jz = r / tb.e[1], jy = r - jz * tb.e[1];
+                const int64_t row = (int64_t)((tb.o[1] + jy) & (g.n[1] - 1)) * g.np0 + (int64_t)((tb.o[2] + jz) & (g.n[2] - 1)) * g.np01;
+                const uint32_t d = (uint32_t)r * (uint32_t)tb.e[0] * 32u;
+                bulk_g2s(tile_b + d, fb + row + gx, (uint32_t)n_a * 32u, bar_b);
+                if (n_b > 0) bulk_g2s(tile_b + d + (uint32_t)n_a * 32u, fb + row, (uint32_t)n_b * 32u, bar_b);
+                bulk_g2s(tile_c + d, fc + row + gx, (uint32_t)n_a * 32u, bar_c);
+                if (n_b > 0) bulk_g2s(tile_c + d + (uint32_t)n_a * 32u, fc + row, (uint32_t)n_b * 32u, bar_c);
+            }
+        }
+        const uint32_t parity = uses & 1u;
+        if (staged) ++uses;
+        StageTile none;
+        none.addr = 0u;
+        float k1[3], k2[3], k3[3], k4[3], xi[3];
+        // stage 1 reads the field stage 4 of the previous step read: held cell, else (first step, changed cell) global memory
+        if (live) {
+            cart_velocity_staged<true>(g, fa, none, ci, w, hc, k1);
+#pragma unroll
+            for (int a = 0; a < 3; ++a) xi[a] = fmaf(0.5f * hs[a], k1[a], w[a]);
+        }
+        if (staged) mbar_wait(bar_b, parity);
+        if (live) {
+            cart_velocity_staged<false>(g, fb, tb, ci, xi, hc, k2);
+#pragma unroll
+            for (int a = 0; a < 3; ++a) xi[a] = fmaf(0.5f * hs[a], k2[a], w[a]);
+            cart_velocity_staged<true>(g, fb, tb, ci, xi, hc, k3);
+#pragma unroll
+            for (int a = 0; a < 3; ++a) xi[a] = fmaf(hs[a], k3[a], w[a]);
+        }
+        if (staged) mbar_wait(bar_c, parity);
+        if (live) {
+            cart_velocity_staged<false>(g, fc, tc, ci, xi, hc, k4);
+#pragma unroll
+            for (int a = 0; a < 3; ++a) {
+                float wn = fmaf(hs[a] * (1.0f / 6.0f), (k1[a] + k4[a]) + 2.0f * (k2[a] + k3[a]), w[a]);
+                int ifl;
+                floor_split<float>(wn, ifl, w[a]);
+                ci[a] += ifl;
+            }
+        }
+    }
+    if (live) {
+        // the block's local frame differs from the stored (never wrapped) cell index by a multiple of n
+#pragma unroll
+        for (int a = 0; a < 3; ++a) { t.ci[a] = (t.ci[a] & ~(g.n[a] - 1)) + ci[a]; t.w[a] = w[a]; }
+        store_record(st + i, t);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
 // Adams-Bashforth 4 with an RK4 start-up (row f4; "Adams-Bashforth (multi-step)"; reading #31): one
 // velocity evaluation per step once three RK4 steps have filled the history.  hist: [n][3][DIM] physical velocities
 // f_{n-1}, f_{n-2}, f_{n-3} of each tracer, carried across launches (tracers are not re-bundled in this mode).
@@ -679,7 +925,7 @@ size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 // How lcs_advect carves the field's scratch for n tracers and N steps under the current options.  lcs_field_reserve sizes
 // the allocation with the same function (worst case over the windows of any [t0, tf]), so the hot call never allocates.
 struct CartLayout {
-    bool split, ab4, do_bundle, preblend;
+    bool split, ab4, do_bundle, preblend, tma;
     int shift, order, max_fields;
     int64_t nbins, ntiles;
     size_t o_a, o_b, o_xi, o_acc, o_hist, o_tau, o_key, o_cnt, o_tile, o_ftau, o_fields, total;
@@ -713,6 +959,18 @@ CartLayout cart_layout(const lcs_field *f, int64_t n, int64_t N)
     }
     L.order = (int)f->opt_bundle_order;
     int64_t nkeys = (int64_t)1 << (bits * DIM);
+    const bool can_blend = DIM == 3 && f->compute_dtype == LCS_F32 && f->vel_dtype == LCS_F32;
+    L.preblend = can_blend && !L.split && !L.ab4 && (f->opt_preblend == 1 || (f->opt_preblend < 0 && n >= (1 << 20)));
+    // staged (shared-memory) variant of the pre-blended integrator: periodic power-of-two grids of at most 1024 nodes per axis
+    // and at least 4 per axis, tracers bundled in brick order
+    bool fastwrap = true;
+    for (int a = 0; a < DIM; ++a) fastwrap = fastwrap && f->cart.periodic[a] && f->cart.pow2[a] && f->cart.n[a] <= 1024 && f->cart.n[a] >= 4;
+    L.tma = L.preblend && L.do_bundle && f->opt_tma != 0 && fastwrap && L.shift == 0;
+    if (L.tma && f->opt_tma == 1) L.order = 3;        // tma = 2: staged kernel on the sort order of option bundle_order (experiments)
+    if (L.order == 3) {
+        if (DIM == 3 && L.shift == 0) nkeys = (int64_t)((f->cart.n[0] + 3) / 4) * ((f->cart.n[1] + 1) / 2) * ((f->cart.n[2] + 1) / 2) * 16;
+        else L.order = 1;
+    }
     if (L.order == 2) {
         const int64_t sub = (int64_t)((f->cart.n[0] + 1) / 2) * f->cart.n[1] * f->cart.n[2] * 16;
         if (DIM == 3 && L.shift == 0 && sub <= (1 << 24)) nkeys = sub;
@@ -720,8 +978,6 @@ CartLayout cart_layout(const lcs_field *f, int64_t n, int64_t N)
     }
     L.nbins = L.do_bundle ? nkeys + 1 : 0;
     L.ntiles = (L.nbins + bundle::kScanTile - 1) / bundle::kScanTile;
-    const bool can_blend = DIM == 3 && f->compute_dtype == LCS_F32 && f->vel_dtype == LCS_F32;
-    L.preblend = can_blend && !L.split && !L.ab4 && (f->opt_preblend == 1 || (f->opt_preblend < 0 && n >= (1 << 20)));
     L.max_fields = L.preblend ? 2 * (int)(f->opt_preblend_steps < N ? f->opt_preblend_steps : N) + 1 : 0;
     size_t off = 0;
     L.o_a = off; off = align_up(off + (size_t)n * trb);
@@ -921,7 +1177,12 @@ lcs_status cart_advect_impl(lcs_field *f, int64_t n, const void *seeds_, double 
                 }
                 {
                     WindowTimer timer(f, st);
-                    if (fast)
+                    if (L.tma) {
+                        const int cap = (int)f->opt_tma_cap;
+                        const size_t smem = (size_t)cap * 64 + 16 + 3 * 8 * sizeof(int);
+                        LCS_LAUNCH(cart_xpair_tma_kernel, lcs_blocks(n, kStageBlock), kStageBlock, smem, st, g, (const XPair *)fields, f->nrec, u.count,
+                                   u.first, n, cur, hs[0], hs[1], hs[2], cap);
+                    } else if (fast)
                         LCS_LAUNCH((cart_xpair_kernel<true>), lcs_blocks(n, block), block, 0, st, g, (const XPair *)fields, f->nrec,
                                    u.count, u.first, n, cur, hs[0], hs[1], hs[2]);
                     else
@@ -973,6 +1234,13 @@ lcs_status cart_advect_impl(lcs_field *f, int64_t n, const void *seeds_, double 
 }  // namespace
 
 size_t lcs_cart_scratch_bytes(const lcs_field *f, int64_t n, int64_t N) { return cart_layout(f, n, N).total; }
+
+lcs_status lcs_cart_tma_configure(lcs_field *f)
+{
+    const size_t smem = (size_t)f->opt_tma_cap * 64 + 16 + 3 * 8 * sizeof(int);
+    if (smem > 48 * 1024) LCS_CUDA_OK(cudaFuncSetAttribute(cart_xpair_tma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    return LCS_OK;
+}
 
 size_t lcs_cart_field_set_bytes(const lcs_field *f, int64_t N)
 {

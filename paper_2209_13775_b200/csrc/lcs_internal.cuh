@@ -149,6 +149,8 @@ struct lcs_field {
     int64_t opt_preblend = -1;    // 3D fp32 Cartesian: gather from per-stage-time blended fields (-1 auto, 0 off, 1 on)
     int64_t opt_preblend_steps = 50; // RK4 steps per launch of the pre-blended integrator (2k+1 blended fields resident)
     int64_t opt_field_sets = 0;   // number of resident blended-field sets (0 = blend every chunk into scratch)
+    int64_t opt_tma = 0;          // 3D fp32 periodic power-of-two grids: stage the blended fields through shared memory with TMA bulk copies
+    int64_t opt_tma_cap = 704;    // records per shared-memory tile of the staged variant (2 tiles per block)
     int64_t opt_ld256 = 1;        // gather pair records with one 256-bit load instead of two 128-bit loads
     int64_t opt_block = 0;        // threads per block override (0 = default)
     int64_t opt_time_windows = 0; // record CUDA events around every window (hot) kernel launch
@@ -227,5 +229,6 @@ lcs_status lcs_fill_stage_tau(const lcs_field *f, double t0, double h, int64_t f
 // bytes lcs_advect carves out of the scratch for n seeds and N steps under the current options (the two integrators and
 // lcs_field_reserve use the same function, so a reservation always covers the call it was made for)
 size_t lcs_cart_scratch_bytes(const lcs_field *f, int64_t n, int64_t N);
+lcs_status lcs_cart_tma_configure(lcs_field *f);   // opts the staged kernel into the shared memory its tile capacity needs
 size_t lcs_simplex_scratch_bytes(const lcs_field *f, int64_t n, int64_t N);
 size_t lcs_cart_field_set_bytes(const lcs_field *f, int64_t N);     // one resident set of blended fields (0: not applicable)

@@ -538,6 +538,27 @@ def test_config3_variants_fp32(lcs, oracle, options):
         assert np.array_equal(cpu(F), cpu(F0))
 
 
+@pytest.mark.parametrize("options", [dict(tma=1), dict(tma=1, tma_cap=96), dict(tma=1, preblend_steps=5, bundle_steps=5), dict(tma=2, bundle_order=1)])
+def test_config3_staged_tma_variant_identical(lcs, oracle, options):
+    """Row (g): the pre-blended integrator with the stage-time fields staged through shared memory by TMA bulk copies
+    (option tma; BASELINE.json north_star, second subsystem).  Same arithmetic on the same records, so the flow map is
+    bit-identical to the global-memory gather in every mix of staged steps, steps whose box exceeds the tile capacity
+    (tma_cap=96) and re-bundling cadence; statistical gate against the oracle.  On a grid that is not periodic with
+    power-of-two node counts the option is ignored (the global-memory kernel runs)."""
+    w = I.config3(ngrid=48, nn=32, T=2.0, h=0.01, n_snap=9)
+    fo, Fo, flo, eso = oracle_run(oracle, w)
+    f0, sd0, F0, flag0, es0 = gpu_run(w, options=dict(bundle=1, preblend=1))
+    f, sd, F, flag, es = gpu_run(w, options=dict(bundle=1, preblend=1, **options))
+    assert np.array_equal(cpu(F), cpu(F0)) and np.array_equal(cpu(es), cpu(es0)) and int(cpu(flag).max()) == 0
+    cgo, fto, sto = oracle_cg(oracle, w, Fo, flo)
+    cgg, ftg, stg = gpu_cg(w, F, flag)
+    gate_statistical(cpu(F), Fo, cpu(ftg), fto, w.L, cpu(flag), flo)
+    w2 = I.config3(ngrid=24, nn=24, T=0.5, h=0.01, n_snap=3)            # 24 nodes per axis: not a power of two
+    fa, sa, Fa, fla, esa = gpu_run(w2, options=dict(bundle=1, preblend=1))
+    fb, sb, Fb, flb, esb = gpu_run(w2, options=dict(bundle=1, preblend=1, **options))
+    assert np.array_equal(cpu(Fa), cpu(Fb))
+
+
 @pytest.mark.parametrize("options", [dict(bundle=1, bundle_steps=5), dict(integrator=2, bundle=1)])
 def test_exit_handling_variants(lcs, oracle, options):
     """Exits (flags 0/1/2, exit_step) with re-bundling (finished tracers are parked in the last bin) and with the
