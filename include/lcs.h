@@ -100,7 +100,8 @@ void lcs_field_destroy(lcs_field *f);
 lcs_status lcs_field_reserve(lcs_field *f, int64_t n_seeds, int64_t n_steps);
 
 /* Integer options.  Keys: "integrator" 0 = auto, 1 = fused (one persistent per-seed loop per snapshot
- * window), 2 = split (one short kernel per RK4 stage, tracers advance synchronously: PAPER.md:85), 3 = 4-step
+ * window), 2 = split (the paper's design: tracers advance synchronously, one short kernel per RK4 stage on Cartesian grids, one per
+ * cell search and one per interpolation -- 8 launches per step -- on simplicial meshes: PAPER.md:85-87), 3 = 4-step
  * Adams-Bashforth with three RK4 start-up steps ("Adams-Bashforth (multi-step)"; one velocity evaluation per step);
  * "bundle" -1 = auto, 0 = off, 1 = on: re-bundle tracers by cell (Morton order of the cell index) so that a
  * warp gathers from neighbouring cells; results are returned in the caller's order;

@@ -768,6 +768,123 @@ simplex_ab4_kernel(const CellRec<DIM, TC> *__restrict__ crec, const int32_t *__r
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Split variant (the paper's design on unstructured grids: "the RK4 computation was divided into several
+// short kernels", each velocity evaluation "preceded by a cell search", i.e. 8 kernels per step; integrator option 2).  All
+// tracers advance one stage at a time; between the launches the stage point (xi), the running sum k1 + 2 k2 + 2 k3 (acc) and
+// the cell found for the stage point (scell) live in global memory as [n] arrays.  A tracer whose stage point leaves the mesh
+// gets its flag at once; its record (position and cell at the start of the step) is only rewritten by the last launch of a
+// step in which all four evaluations succeeded.  Same arithmetic per evaluation as the fused kernel (walk on the affine maps
+// with the canonical re-location when the walk gives up, P1 interpolation, time blend).
+template <int DIM, typename TC, int STAGE>
+__global__ void __launch_bounds__(128)
+simplex_search_kernel(const CellRec<DIM, TC> *__restrict__ crec, const int32_t *__restrict__ neigh, int step, int64_t n,
+                      SimplexTracer<DIM, TC> *__restrict__ st, const TC *__restrict__ xi_g, int32_t *__restrict__ scell,
+                      const __grid_constant__ CanonCtx cx)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    SimplexTracer<DIM, TC> t = load_tracer(st + i);
+    if ((t.meta >> 30) != 0) return;
+    TC p[DIM];
+#pragma unroll
+    for (int k = 0; k < DIM; ++k) p[k] = STAGE == 0 ? t.x[k] : xi_g[i * DIM + k];
+    int32_t c = STAGE == 0 ? t.cell : scell[i];
+    bool forced = false;
+    int rc = 0;
+    for (int hop = 0;; ++hop) {
+        CellRec<DIM, TC> r;
+        load_cellrec<DIM, TC>(crec, c, r);
+        TC q[DIM], lam[DIM + 1];
+#pragma unroll
+        for (int k = 0; k < DIM; ++k) q[k] = p[k] - r.v0[k];
+        TC sum = TC(0);
+#pragma unroll
+        for (int a = 0; a < DIM; ++a) {
+            TC l = TC(0);
+#pragma unroll
+            for (int k = 0; k < DIM; ++k) l = fma(r.M[a * DIM + k], q[k], l);
+            lam[a + 1] = l;
+            sum += l;
+        }
+        lam[0] = TC(1) - sum;
+        int jmin = 0;
+        TC lmin = lam[0];
+#pragma unroll
+        for (int a = 1; a <= DIM; ++a)
+            if (lam[a] < lmin) { lmin = lam[a]; jmin = a; }
+        if (lmin >= -WalkTol<TC>::eps || forced) break;
+        if (hop >= kWalkCap) {
+            c = walk_fallback<DIM, TC>(cx, p);
+            if (c < 0) { rc = 1; break; }
+            forced = true;
+            continue;
+        }
+        int32_t nb = __ldg(neigh + (int64_t)c * (DIM + 1) + jmin);
+        if (nb < 0) { rc = 1; break; }
+        c = nb;
+    }
+    if (rc) {
+        t.meta = (1u << 30) | (uint32_t)step;
+        store_tracer(st + i, t);
+        return;
+    }
+    scell[i] = c;
+}
+
+template <int DIM, typename TV, typename TC, int STAGE>
+__global__ void __launch_bounds__(128)
+simplex_interp_kernel(const CellRec<DIM, TC> *__restrict__ crec, const PairRec<DIM, TV> *__restrict__ vrec, TC tau, int64_t n,
+                      SimplexTracer<DIM, TC> *__restrict__ st, TC *__restrict__ xi_g, TC *__restrict__ acc_g,
+                      const int32_t *__restrict__ scell, TC h)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    SimplexTracer<DIM, TC> t = load_tracer(st + i);
+    if ((t.meta >> 30) != 0) return;
+    TC p[DIM];
+#pragma unroll
+    for (int k = 0; k < DIM; ++k) p[k] = STAGE == 0 ? t.x[k] : xi_g[i * DIM + k];
+    const int32_t c = scell[i];
+    CellRec<DIM, TC> r;
+    load_cellrec<DIM, TC>(crec, c, r);
+    TC q[DIM], lam[DIM + 1], u[DIM];
+#pragma unroll
+    for (int k = 0; k < DIM; ++k) q[k] = p[k] - r.v0[k];
+    TC sum = TC(0);
+#pragma unroll
+    for (int a = 0; a < DIM; ++a) {
+        TC l = TC(0);
+#pragma unroll
+        for (int k = 0; k < DIM; ++k) l = fma(r.M[a * DIM + k], q[k], l);
+        lam[a + 1] = l;
+        sum += l;
+    }
+    lam[0] = TC(1) - sum;
+#pragma unroll
+    for (int k = 0; k < DIM; ++k) u[k] = TC(0);
+#pragma unroll
+    for (int a = 0; a <= DIM; ++a) {
+        TC va[DIM], vd[DIM];
+        load_vertex<DIM, TV, TC>(vrec, r.vid[a], va, vd);
+#pragma unroll
+        for (int k = 0; k < DIM; ++k) u[k] = fma(lam[a], fma(tau, vd[k], va[k]), u[k]);
+    }
+    if constexpr (STAGE < 3) {
+        const TC cf = STAGE == 2 ? TC(1) : TC(0.5);
+#pragma unroll
+        for (int k = 0; k < DIM; ++k) {
+            xi_g[i * DIM + k] = fma(cf * h, u[k], t.x[k]);
+            acc_g[i * DIM + k] = STAGE == 0 ? u[k] : acc_g[i * DIM + k] + TC(2) * u[k];
+        }
+    } else {
+#pragma unroll
+        for (int k = 0; k < DIM; ++k) t.x[k] = fma(h * TC(1.0 / 6.0), acc_g[i * DIM + k] + u[k], t.x[k]);
+        t.cell = c;                                   // start of the next step's walk
+        store_tracer(st + i, t);
+    }
+}
+
 template <int DIM, typename TC>
 __global__ void __launch_bounds__(256) simplex_final_kernel(int64_t n, const SimplexTracer<DIM, TC> *__restrict__ st, int32_t N,
                                                              TC *__restrict__ flowmap, uint8_t *__restrict__ exit_flag,
@@ -915,10 +1032,10 @@ template <int DIM> lcs_status build_impl(lcs_field *f, const double *vh, const i
 
 // how lcs_advect carves the scratch on a simplicial mesh (shared with lcs_field_reserve, see CartLayout)
 struct SimplexLayout {
-    bool ab4, do_bundle;
+    bool ab4, split, do_bundle;
     int shift;
     int64_t nbins, ntiles;
-    size_t o_a, o_b, o_tau, o_hist, o_key, o_cnt, o_tile, o_pend, total;
+    size_t o_a, o_b, o_tau, o_hist, o_xi, o_acc, o_scell, o_key, o_cnt, o_tile, o_pend, total;
 };
 
 size_t simplex_tracer_bytes(const lcs_field *f)
@@ -936,6 +1053,7 @@ SimplexLayout simplex_layout(const lcs_field *f, int64_t n, int64_t N)
     const size_t tcb = lcs_esize(f->compute_dtype), trb = simplex_tracer_bytes(f);
     // re-bundling by bin (Morton or row-major order of the coarsened bin grid), histogram <= 2^24 bins
     L.ab4 = f->opt_integrator == 3;
+    L.split = f->opt_integrator == 2;
     L.do_bundle = !L.ab4 && (f->opt_bundle == 1 || (f->opt_bundle < 0 && n >= (1 << 18)));
     int bits = 0;
     for (L.shift = 0;; ++L.shift) {
@@ -954,6 +1072,9 @@ SimplexLayout simplex_layout(const lcs_field *f, int64_t n, int64_t N)
     L.o_b = off; if (L.do_bundle) off = align_up(off + (size_t)n * trb);
     L.o_tau = off; off = align_up(off + (size_t)3 * N * tcb);
     L.o_hist = off; if (L.ab4) off = align_up(off + (size_t)n * 3 * DIM * tcb);
+    L.o_xi = off; if (L.split) off = align_up(off + (size_t)n * DIM * tcb);
+    L.o_acc = off; if (L.split) off = align_up(off + (size_t)n * DIM * tcb);
+    L.o_scell = off; if (L.split) off = align_up(off + (size_t)n * 4);
     L.o_key = off; if (L.do_bundle) off = align_up(off + (size_t)n * 4);
     L.o_cnt = off; if (L.do_bundle) off = align_up(off + (size_t)L.nbins * 4);
     L.o_tile = off; if (L.do_bundle) off = align_up(off + (size_t)L.ntiles * 4);
@@ -971,10 +1092,6 @@ lcs_status simplex_advect_impl(lcs_field *f, int64_t n, const void *seeds_, doub
     TC *flowmap = (TC *)flowmap_;
     SimplexMesh &m = f->mesh;
     if (n >= (1LL << 31) || N >= (1LL << 24)) { lcs_set_error("too many seeds or steps for 32-bit tracer records"); return LCS_ERR_INVALID_ARG; }
-    if (f->opt_integrator == 2) {
-        lcs_set_error("integrator = 2 (split per-stage kernels) is not available on simplicial meshes in this build");
-        return LCS_ERR_INVALID_ARG;
-    }
     std::vector<StepWindow> windows;
     lcs_status rc = lcs_plan_windows(f, t0, h, N, windows);
     if (rc != LCS_OK) return rc;
@@ -1021,6 +1138,26 @@ lcs_status simplex_advect_impl(lcs_field *f, int64_t n, const void *seeds_, doub
                 since_bundle = 0;
             }
             since_bundle += cnt;
+            if (L.split) {
+                // the paper's 8 launches per RK4 step: search + interpolate for each of the four evaluations
+                WindowTimer timer(f, st);
+                TC *xi = (TC *)(base + L.o_xi), *acc = (TC *)(base + L.o_acc);
+                int32_t *scell = (int32_t *)(base + L.o_scell);
+                const CellRec<DIM, TC> *cr = (const CellRec<DIM, TC> *)m.cellrec;
+                const unsigned grid = lcs_blocks(n, block);
+                for (int sstep = first; sstep < first + cnt; ++sstep) {
+                    const TC t3[3] = {(TC)lcs_stage_tau(f, t0, h, sstep, 0, w.s[0]), (TC)lcs_stage_tau(f, t0, h, sstep, 1, w.s[1]),
+                                      (TC)lcs_stage_tau(f, t0, h, sstep, 2, w.s[2])};
+                    LCS_LAUNCH((simplex_search_kernel<DIM, TC, 0>), grid, block, 0, st, cr, m.neigh, sstep, n, cur, xi, scell, cx);
+                    LCS_LAUNCH((simplex_interp_kernel<DIM, TV, TC, 0>), grid, block, 0, st, cr, (const VRec *)p[0], t3[0], n, cur, xi, acc, scell, (TC)h);
+                    LCS_LAUNCH((simplex_search_kernel<DIM, TC, 1>), grid, block, 0, st, cr, m.neigh, sstep, n, cur, xi, scell, cx);
+                    LCS_LAUNCH((simplex_interp_kernel<DIM, TV, TC, 1>), grid, block, 0, st, cr, (const VRec *)p[1], t3[1], n, cur, xi, acc, scell, (TC)h);
+                    LCS_LAUNCH((simplex_search_kernel<DIM, TC, 2>), grid, block, 0, st, cr, m.neigh, sstep, n, cur, xi, scell, cx);
+                    LCS_LAUNCH((simplex_interp_kernel<DIM, TV, TC, 2>), grid, block, 0, st, cr, (const VRec *)p[1], t3[1], n, cur, xi, acc, scell, (TC)h);
+                    LCS_LAUNCH((simplex_search_kernel<DIM, TC, 3>), grid, block, 0, st, cr, m.neigh, sstep, n, cur, xi, scell, cx);
+                    LCS_LAUNCH((simplex_interp_kernel<DIM, TV, TC, 3>), grid, block, 0, st, cr, (const VRec *)p[2], t3[2], n, cur, xi, acc, scell, (TC)h);
+                }
+            } else {
             const Pending pend{(unsigned int *)(base + L.o_pend), (int32_t *)(base + L.o_pend + 256)};
             LCS_CUDA_OK(cudaMemsetAsync(pend.count, 0, 4, st));
             {
@@ -1041,6 +1178,7 @@ lcs_status simplex_advect_impl(lcs_field *f, int64_t n, const void *seeds_, doub
             else
                 LCS_LAUNCH((simplex_window_kernel<DIM, TV, TC, true>), 148, 128, 0, st, (const CellRec<DIM, TC> *)m.cellrec, m.neigh,
                            (const VRec *)p[0], (const VRec *)p[1], (const VRec *)p[2], d_tau + 3 * (size_t)first, cnt, first, n, cur, (TC)h, cx, pend);
+            }
             if (lcs_early_due(f, (int64_t)first + cnt, N)) {         // row f1: evaluate C for the stencils that are still complete
                 LCS_LAUNCH((simplex_final_kernel<DIM, TC>), lcs_blocks(n, 256), 256, 0, st, n, cur, (int32_t)N, (TC *)f->early.flowmap,
                            f->early.flag, (int32_t *)nullptr);

@@ -591,6 +591,31 @@ def test_preblend_nonperiodic_3d_fp32_with_exits(lcs, oracle):
     assert np.max(np.linalg.norm(cpu(F1)[same].astype(np.float64) - Fo[same], axis=1)) < 1e-3 * w.L
 
 
+@pytest.mark.parametrize("mesh", ["tri_f64", "tet_f32"])
+def test_simplex_split_stages_vs_oracle_and_fused(lcs, oracle, mesh):
+    """The paper's split design on unstructured meshes (one short kernel per cell search and per interpolation,
+    8 launches per RK4 step; integrator option 2): same per-evaluation arithmetic as the fused kernel, so the flow map equals
+    the fused one bit for bit wherever the walks end in the same cells (everywhere but within the walk tolerance of a face),
+    and passes the gate of its config against the oracle."""
+    if mesh == "tri_f64":
+        w = I.config2(ng=(96, 48), lattice=(40, 20), T=4.0)
+    else:
+        w = I.config4(ng=(20, 20, 36), delta=0.08, T=1.5, h=0.005, n_snap=10, length=4.0)
+    fo, Fo, flo, eso = oracle_run(oracle, w)
+    f1, sd1, F1, flag1, es1 = gpu_run(w, options=dict(integrator=1, bundle=0))
+    for opts in (dict(integrator=2, bundle=0), dict(integrator=2, bundle=1, bundle_steps=9)):
+        f2, sd2, F2, flag2, es2 = gpu_run(w, options=opts)
+        assert f2.info("walk_cap_hits") == 0 and f2.info("locate_fallbacks") == 0
+        assert np.mean(cpu(flag2) == cpu(flag1)) > 0.999
+        same = (cpu(flag2) == flo)
+        if mesh == "tri_f64":
+            assert same.mean() > 0.995 and np.max(np.abs(cpu(F2)[same] - Fo[same])) < 1e-9
+            assert np.max(np.abs(cpu(F2) - cpu(F1))[cpu(flag2) == cpu(flag1)]) < 1e-9
+        else:
+            err = np.linalg.norm(cpu(F2).astype(np.float64) - Fo, axis=1)
+            assert np.mean((err <= 1e-3 * w.L) & same) >= 0.999
+
+
 @pytest.mark.parametrize("options", [dict(bundle=1), dict(bundle=1, bundle_steps=7)])
 def test_simplex_bundled_identical_to_unbundled(lcs, oracle, options):
     """Re-bundling tracers by bin (triangles fp64, tets fp32 with flags 0/1/2): a tracer's arithmetic does not depend on
@@ -1007,7 +1032,7 @@ def test_random_cartesian_configs_all_variants(lcs, oracle):
 def test_random_simplex_configs_all_variants(lcs, oracle):
     """12 seeded random small simplicial workloads (jittered Delaunay triangles / tets, randomly permuted cell order and vertex
     order within cells so that orientation and local face numbering are arbitrary), fp64 or fp32, forward or backward, through the
-    unbundled, bundled and Adams-Bashforth variants.  lcs_locate is bit-exact against brute force on every seed; interior results
+    unbundled, bundled, Adams-Bashforth and split per-stage variants.  lcs_locate is bit-exact against brute force on every seed; interior results
     match to 1e-9 (fp64) where both sides agree on the exit flag, and flags agree on >= 98% of the seeds (the in-loop walk uses a
     tolerance at hull faces)."""
     import torch
@@ -1031,7 +1056,7 @@ def test_random_simplex_configs_all_variants(lcs, oracle):
         w = I.analytic_simplex(dim, I.linear_flow(A, b), V, Cc, np.arange(0.0, 2.01, 0.5), ng=ng, seed_lo=tuple(lo - 0.05 * ext),
                                seed_spacing=tuple(1.1 * ext / np.array(ng)), t0=t0, tf=t0 + (-h if backward else h) * nsteps,
                                h=(-h if backward else h), vel_dtype=dt, compute_dtype=dt)
-        variant = [dict(bundle=0), dict(bundle=1, bundle_steps=int(rng.integers(1, 9))), dict(integrator=3)][case % 3]
+        variant = [dict(bundle=0), dict(bundle=1, bundle_steps=int(rng.integers(1, 9))), dict(integrator=3), dict(integrator=2, bundle=case % 2)][case % 4]
         fo = oracle.OracleField.from_workload(w)
         s64 = w.seeds().astype(np.float64)
         f = lcs.Field.from_workload(w)
