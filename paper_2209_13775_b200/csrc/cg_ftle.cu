@@ -43,6 +43,46 @@ __device__ __forceinline__ double eigmax_sym3(double c11, double c12, double c13
     return q + 2.0 * p * cos(acos(r) / 3.0);
 }
 
+// Single-precision outputs (T = float): C and the algebra of the eigenvalue stay in fp64, but the fp64 library routines
+// (acos, cos, log: some hundred instructions each on the half-rate FP64 pipe, which made this HBM-streaming kernel FP64-bound
+// at 20% of the HBM peak) are replaced: the trigonometric step runs in fp32 and its result is polished by one Newton step on the
+// characteristic polynomial det(C - lambda I) in fp64 (taken only when it is a small correction: near a double root the
+// derivative vanishes and the fp32 estimate, already within 3e-7 lambda_max, is kept), and the logarithm of the float-rounded
+// lambda_max is taken in fp32.  The result differs from the fp64 closed form by less than the rounding of the float output
+// (tests: 2e-6 against the oracle).
+__device__ __forceinline__ double eigmax_sym3_mixed(double c11, double c12, double c13, double c22, double c23, double c33)
+{
+    // estimate: the trigonometric closed form in fp32 (the largest eigenvalue of a symmetric matrix is well conditioned: the
+    // estimate is within a few 1e-7 ||C||)
+    const double qd = (c11 + c22 + c33) * (1.0 / 3.0);
+    const float q = (float)qd;
+    const float f12 = (float)c12, f13 = (float)c13, f23 = (float)c23;
+    const float d1 = (float)(c11 - qd), d2 = (float)(c22 - qd), d3 = (float)(c33 - qd);
+    const float p2 = d1 * d1 + d2 * d2 + d3 * d3 + 2.0f * (f12 * f12 + f13 * f13 + f23 * f23);
+    if (!(p2 > 0.0f)) return qd;                               // multiple of the identity (or NaN, which propagates through qd)
+    const float ip = rsqrtf(p2 * (1.0f / 6.0f));
+    const float b11 = d1 * ip, b22 = d2 * ip, b33 = d3 * ip, b12 = f12 * ip, b13 = f13 * ip, b23 = f23 * ip;
+    const float det = b11 * (b22 * b33 - b23 * b23) - b12 * (b12 * b33 - b23 * b13) + b13 * (b12 * b23 - b22 * b13);
+    const float r = fminf(1.0f, fmaxf(-1.0f, 0.5f * det));
+    const float pf = p2 * (1.0f / 6.0f) * ip;                  // sqrt(p2 / 6)
+    double lam = qd + (double)(2.0f * pf * cosf(acosf(r) * (1.0f / 3.0f)));
+    // one Newton step on det(C - lambda I) in fp64
+    const double a11 = c11 - lam, a22 = c22 - lam, a33 = c33 - lam;
+    const double m1 = a22 * a33 - c23 * c23, m2 = a11 * a33 - c13 * c13, m3 = a11 * a22 - c12 * c12;
+    const double gv = a11 * m1 - c12 * (c12 * a33 - c23 * c13) + c13 * (c12 * c23 - a22 * c13);
+    const double gd = -(m1 + m2 + m3);
+    const double step = gv / gd;
+    if (fabs(step) <= 1e-4 * (double)pf) lam -= step;          // false for NaN as well
+    return lam;
+}
+template <typename T> __device__ __forceinline__ double log_for(double lam)
+{
+    if constexpr (sizeof(T) == 4) {
+        if (lam > 1e-30 && lam < 1e30) return (double)logf((float)lam);
+    }
+    return log(lam);
+}
+
 // EARLY (row f1, reading #29): the kernel runs at an evaluation point of lcs_advect_early_cg with the flags of
 // that moment (0 alive, 1 left, 2 never started).  A seed is (re-)evaluated only if it is alive and none of its grid
 // neighbours has left; neighbours that never started stay invalid neighbours (one-sided differences).  Seeds that are
@@ -53,11 +93,14 @@ __global__ void __launch_bounds__(256) cg_ftle_kernel(const __grid_constant__ Cg
                                                        T *__restrict__ ftle, uint8_t *__restrict__ status, int64_t n,
                                                        T *__restrict__ t_eff, double t_now)
 {
-    int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (idx >= n) return;
-    if (EARLY && flag[idx] != 0) return;
+    // launch geometry: x = position in the grid row, y / z = row and plane (no 64-bit division per seed: the index arithmetic of the
+    // one-thread-per-linear-index version cost more issue slots than the whole eigenvalue)
+    const int i0 = (int)(blockIdx.x * blockDim.x + threadIdx.x);
+    if (i0 >= g.ng[0]) return;
     const int64_t n0 = g.ng[0], n1 = g.ng[1];
-    int ijk[3] = {(int)(idx % n0), (int)((idx / n0) % n1), (int)(idx / (n0 * n1))};
+    const int ijk[3] = {i0, (int)blockIdx.y, (int)blockIdx.z};
+    const int64_t idx = i0 + n0 * (ijk[1] + n1 * (int64_t)ijk[2]);
+    if (EARLY && flag[idx] != 0) return;
     const int64_t stride[3] = {1, n0, n0 * n1};
     constexpr int NCG = (DIM == 2) ? 3 : 6;
     uint8_t st = 0;
@@ -111,15 +154,96 @@ __global__ void __launch_bounds__(256) cg_ftle_kernel(const __grid_constant__ Cg
         for (int b = 0; b < 3; ++b)
 #pragma unroll
             for (int c = b; c < 3; ++c) C[m++] = G[0][b] * G[0][c] + G[1][b] * G[1][c] + G[2][b] * G[2][c];
-        lam = eigmax_sym3(C[0], C[1], C[2], C[3], C[4], C[5]);
+        lam = sizeof(T) == 4 ? eigmax_sym3_mixed(C[0], C[1], C[2], C[3], C[4], C[5]) : eigmax_sym3(C[0], C[1], C[2], C[3], C[4], C[5]);
     }
     if (cg) {
+        if constexpr (sizeof(T) == 4 && NCG == 6) {
+            // 24 bytes per seed, 8-byte aligned: three 64-bit stores instead of six 32-bit ones
+            float2 *o = reinterpret_cast<float2 *>(cg + idx * NCG);
+            o[0] = make_float2((float)C[0], (float)C[1]);
+            o[1] = make_float2((float)C[2], (float)C[3]);
+            o[2] = make_float2((float)C[4], (float)C[5]);
+        } else {
 #pragma unroll
-        for (int i = 0; i < NCG; ++i) cg[idx * NCG + i] = (T)C[i];
+            for (int i = 0; i < NCG; ++i) cg[idx * NCG + i] = (T)C[i];
+        }
     }
-    ftle[idx] = (st & 1) ? (T)nan("") : (T)(log(lam) * g.inv_2T);
+    ftle[idx] = (st & 1) ? (T)nan("") : (T)(log_for<T>(lam) * g.inv_2T);
     if (status) status[idx] = st;
     if constexpr (EARLY) t_eff[idx] = (T)t_now;
+}
+
+// The hot instantiation (3D, float, plain evaluation: configs 3-5) written for issue slots: the generic kernel above spends 710
+// instructions per seed, a fifth of them on 64-bit index arithmetic and another tenth on branches, and runs at 20% of the HBM
+// peak although it moves 42 bytes per seed (ncu: issue slots 72%, DRAM 16%).  Here the neighbour offsets are 32-bit, validity is
+// carried in predicates (loads are issued for every in-grid neighbour whatever its flag), the selection between central and
+// one-sided differences happens on the float operands before ONE widening subtraction per entry, and C leaves in three 64-bit
+// stores.  Same rule (reading #12) and the same fp64 arithmetic for the differences, C and the eigenvalue algebra.
+// Requires 3 n < 2^31 (32-bit element offsets).
+__global__ void __launch_bounds__(256) cg_ftle3f_kernel(const __grid_constant__ CgGrid g, const float *__restrict__ F, const uint8_t *__restrict__ flag,
+                                                         float *__restrict__ cg, float *__restrict__ ftle, uint8_t *__restrict__ status)
+{
+    const int i0 = (int)(blockIdx.x * blockDim.x + threadIdx.x);
+    if (i0 >= g.ng[0]) return;
+    const int n0 = g.ng[0], n1 = g.ng[1], n2 = g.ng[2];
+    const int ijk[3] = {i0, (int)blockIdx.y, (int)blockIdx.z};
+    const int nn[3] = {n0, n1, n2};
+    const int stride[3] = {1, n0, n0 * n1};
+    const int idx = i0 + n0 * (ijk[1] + n1 * ijk[2]);
+    const float *Fc = F + 3 * idx;
+    const float F0[3] = {Fc[0], Fc[1], Fc[2]};
+    unsigned st = (flag && flag[idx] != 0) ? 1u : 0u;
+    double G[3][3];
+#pragma unroll
+    for (int b = 0; b < 3; ++b) {
+        // in-grid neighbours (by wrap on a periodic axis) and the period carried by a wrapped one
+        const bool atp = ijk[b] + 1 >= nn[b], atm = ijk[b] == 0;
+        bool okp = !atp || g.per[b], okm = !atm || g.per[b];
+        const int dp = (atp ? 1 - nn[b] : 1) * stride[b], dm = (atm ? nn[b] - 1 : -1) * stride[b];
+        const int jp = okp ? idx + dp : idx, jm = okm ? idx + dm : idx;        // a valid address in every case
+        const float *Pp = F + 3 * jp, *Pm = F + 3 * jm;
+        const float fp[3] = {Pp[0], Pp[1], Pp[2]}, fm[3] = {Pm[0], Pm[1], Pm[2]};
+        if (flag) { okp = okp && flag[jp] == 0; okm = okm && flag[jm] == 0; }
+        const double shift = ((okp && atp) ? g.period[b] : 0.0) + ((okm && atm) ? g.period[b] : 0.0);
+        const double scale = (okp && okm) ? 0.5 * g.inv_dx[b] : ((okp || okm) ? g.inv_dx[b] : 0.0);
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            const float hi = okp ? fp[a] : F0[a], lo = okm ? fm[a] : F0[a];
+            double d = (double)hi - (double)lo;
+            if (a == b) d += shift;
+            G[a][b] = d * scale;
+        }
+        if (!(st & 1u)) {
+            if (!okp && !okm) st |= 1u;
+            else if (!(okp && okm)) st |= 2u;
+        }
+    }
+    float c[6], ft;
+    if (st & 1u) {
+        const float q = __int_as_float(0x7fc00000);
+#pragma unroll
+        for (int i = 0; i < 6; ++i) c[i] = q;
+        ft = q;
+    } else {
+        double C[6];
+        int m = 0;
+#pragma unroll
+        for (int b = 0; b < 3; ++b)
+#pragma unroll
+            for (int k = b; k < 3; ++k) C[m++] = G[0][b] * G[0][k] + G[1][b] * G[1][k] + G[2][b] * G[2][k];
+        const double lam = eigmax_sym3_mixed(C[0], C[1], C[2], C[3], C[4], C[5]);
+        ft = (float)(log_for<float>(lam) * g.inv_2T);
+#pragma unroll
+        for (int i = 0; i < 6; ++i) c[i] = (float)C[i];
+    }
+    if (cg) {
+        float2 *o = reinterpret_cast<float2 *>(cg + 6 * (int64_t)idx);
+        o[0] = make_float2(c[0], c[1]);
+        o[1] = make_float2(c[2], c[3]);
+        o[2] = make_float2(c[4], c[5]);
+    }
+    ftle[idx] = ft;
+    if (status) status[idx] = (uint8_t)st;
 }
 
 // outputs of seeds that are never evaluated: NaN, t_eff = 0, status bit 0
@@ -177,13 +301,13 @@ __global__ void __launch_bounds__(256) cg_ftle_aux_kernel(const T *__restrict__ 
         for (int b = 0; b < 3; ++b)
 #pragma unroll
             for (int c = b; c < 3; ++c) C[m++] = G[0][b] * G[0][c] + G[1][b] * G[1][c] + G[2][b] * G[2][c];
-        lam = eigmax_sym3(C[0], C[1], C[2], C[3], C[4], C[5]);
+        lam = sizeof(T) == 4 ? eigmax_sym3_mixed(C[0], C[1], C[2], C[3], C[4], C[5]) : eigmax_sym3(C[0], C[1], C[2], C[3], C[4], C[5]);
     }
     if (cg) {
 #pragma unroll
         for (int k = 0; k < NCG; ++k) cg[i * NCG + k] = (T)C[k];
     }
-    ftle[i] = st ? (T)nan("") : (T)(log(lam) * inv_2T);
+    ftle[i] = st ? (T)nan("") : (T)(log_for<T>(lam) * inv_2T);
     if (status) status[i] = st;
 }
 
@@ -418,11 +542,15 @@ extern "C" lcs_status lcs_cg_ftle(int32_t dim, int32_t dtype, const int32_t ng[3
     g.inv_2T = 1.0 / (2.0 * fabs(T));
     if (n == 0) return LCS_OK;
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    const unsigned grid = lcs_blocks(n, 256);
-    if (dim == 2 && dtype == LCS_F64) LCS_LAUNCH((cg_ftle_kernel<2, double, false>), grid, 256, 0, st, g, (const double *)flowmap, exit_flag, (double *)cg, (double *)ftle, status, n, (double *)nullptr, 0.0);
-    else if (dim == 2) LCS_LAUNCH((cg_ftle_kernel<2, float, false>), grid, 256, 0, st, g, (const float *)flowmap, exit_flag, (float *)cg, (float *)ftle, status, n, (float *)nullptr, 0.0);
-    else if (dtype == LCS_F64) LCS_LAUNCH((cg_ftle_kernel<3, double, false>), grid, 256, 0, st, g, (const double *)flowmap, exit_flag, (double *)cg, (double *)ftle, status, n, (double *)nullptr, 0.0);
-    else LCS_LAUNCH((cg_ftle_kernel<3, float, false>), grid, 256, 0, st, g, (const float *)flowmap, exit_flag, (float *)cg, (float *)ftle, status, n, (float *)nullptr, 0.0);
+    // one thread per seed of a grid row; rows and planes on the y / z axes of the launch grid
+    if (g.ng[1] > 65535 || g.ng[2] > 65535) { lcs_set_error("seed grid too large on axis 1 or 2 (max 65535)"); return LCS_ERR_INVALID_ARG; }
+    const unsigned bx = (unsigned)(g.ng[0] >= 256 ? 256 : ((g.ng[0] + 31) / 32) * 32);
+    const dim3 block3(bx, 1, 1), grid3((unsigned)((g.ng[0] + bx - 1) / bx), (unsigned)g.ng[1], (unsigned)g.ng[2]);
+    if (dim == 2 && dtype == LCS_F64) LCS_LAUNCH((cg_ftle_kernel<2, double, false>), grid3, block3, 0, st, g, (const double *)flowmap, exit_flag, (double *)cg, (double *)ftle, status, n, (double *)nullptr, 0.0);
+    else if (dim == 2) LCS_LAUNCH((cg_ftle_kernel<2, float, false>), grid3, block3, 0, st, g, (const float *)flowmap, exit_flag, (float *)cg, (float *)ftle, status, n, (float *)nullptr, 0.0);
+    else if (dtype == LCS_F64) LCS_LAUNCH((cg_ftle_kernel<3, double, false>), grid3, block3, 0, st, g, (const double *)flowmap, exit_flag, (double *)cg, (double *)ftle, status, n, (double *)nullptr, 0.0);
+    else if (3 * n < (1LL << 31)) LCS_LAUNCH(cg_ftle3f_kernel, grid3, block3, 0, st, g, (const float *)flowmap, exit_flag, (float *)cg, (float *)ftle, status);
+    else LCS_LAUNCH((cg_ftle_kernel<3, float, false>), grid3, block3, 0, st, g, (const float *)flowmap, exit_flag, (float *)cg, (float *)ftle, status, n, (float *)nullptr, 0.0);
     LCS_CUDA_OK(cudaGetLastError());
     return LCS_OK;
 }
@@ -478,12 +606,15 @@ lcs_status lcs_early_cg_eval(lcs_field *f, int64_t m, cudaStream_t st)
     }
     const double t_now = (double)m * e.h;
     g.inv_2T = 1.0 / (2.0 * fabs(t_now));
-    const unsigned grid = lcs_blocks(n, 256);
+    // one thread per seed of a grid row; rows and planes on the y / z axes of the launch grid
+    if (g.ng[1] > 65535 || g.ng[2] > 65535) { lcs_set_error("seed grid too large on axis 1 or 2 (max 65535)"); return LCS_ERR_INVALID_ARG; }
+    const unsigned bx = (unsigned)(g.ng[0] >= 256 ? 256 : ((g.ng[0] + 31) / 32) * 32);
+    const dim3 block3(bx, 1, 1), grid3((unsigned)((g.ng[0] + bx - 1) / bx), (unsigned)g.ng[1], (unsigned)g.ng[2]);
     const bool f64 = f->compute_dtype == LCS_F64;
-    if (f->dim == 2 && f64) LCS_LAUNCH((cg_ftle_kernel<2, double, true>), grid, 256, 0, st, g, (const double *)e.flowmap, e.flag, (double *)e.cg, (double *)e.ftle, e.status, n, (double *)e.t_eff, t_now);
-    else if (f->dim == 2) LCS_LAUNCH((cg_ftle_kernel<2, float, true>), grid, 256, 0, st, g, (const float *)e.flowmap, e.flag, (float *)e.cg, (float *)e.ftle, e.status, n, (float *)e.t_eff, t_now);
-    else if (f64) LCS_LAUNCH((cg_ftle_kernel<3, double, true>), grid, 256, 0, st, g, (const double *)e.flowmap, e.flag, (double *)e.cg, (double *)e.ftle, e.status, n, (double *)e.t_eff, t_now);
-    else LCS_LAUNCH((cg_ftle_kernel<3, float, true>), grid, 256, 0, st, g, (const float *)e.flowmap, e.flag, (float *)e.cg, (float *)e.ftle, e.status, n, (float *)e.t_eff, t_now);
+    if (f->dim == 2 && f64) LCS_LAUNCH((cg_ftle_kernel<2, double, true>), grid3, block3, 0, st, g, (const double *)e.flowmap, e.flag, (double *)e.cg, (double *)e.ftle, e.status, n, (double *)e.t_eff, t_now);
+    else if (f->dim == 2) LCS_LAUNCH((cg_ftle_kernel<2, float, true>), grid3, block3, 0, st, g, (const float *)e.flowmap, e.flag, (float *)e.cg, (float *)e.ftle, e.status, n, (float *)e.t_eff, t_now);
+    else if (f64) LCS_LAUNCH((cg_ftle_kernel<3, double, true>), grid3, block3, 0, st, g, (const double *)e.flowmap, e.flag, (double *)e.cg, (double *)e.ftle, e.status, n, (double *)e.t_eff, t_now);
+    else LCS_LAUNCH((cg_ftle_kernel<3, float, true>), grid3, block3, 0, st, g, (const float *)e.flowmap, e.flag, (float *)e.cg, (float *)e.ftle, e.status, n, (float *)e.t_eff, t_now);
     LCS_CUDA_OK(cudaGetLastError());
     return LCS_OK;
 }
