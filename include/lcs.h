@@ -127,7 +127,10 @@ lcs_status lcs_field_get_info(const lcs_field *f, const char *key, int64_t *valu
  * Simplex: bin grid -> start cell -> walk across faces with the canonical fp64 face predicate (vertices
  * of a face sorted by id, every product and sum rounded separately, ties broken as if the point were
  * p + (eps, eps^2, eps^3)); the result is the unique owner, bit-exact against the oracle.
- * bary (optional, may be NULL): device [n][dim] Cartesian weights or [n][dim+1] barycentric weights. */
+ * bary (optional, may be NULL): device [n][dim] Cartesian weights or [n][dim+1] barycentric weights.
+ * Simplicial meshes are taken to triangulate a CONVEX region (Delaunay triangulations do; reading #11): a walk that
+ * reaches a hull face with the point strictly beyond it reports "outside" (-1; in lcs_advect: exit flag 1), so a point that is
+ * inside the mesh but separated from the walk's start by a concavity or a hole may be reported as outside.              */
 lcs_status lcs_locate(lcs_field *f, int64_t n, const double *pos, int32_t *cell, double *bary,
                       void *cuda_stream);
 
@@ -143,6 +146,20 @@ lcs_status lcs_locate(lcs_field *f, int64_t n, const double *pos, int32_t *cell,
  * LCS_ERR_TIME_RANGE if [t0,tf] leaves [times[0], times[ns-1]] by more than 1e-9 snapshot intervals.   */
 lcs_status lcs_advect(lcs_field *f, int64_t n, const void *seeds, double t0, double tf, double h,
                       void *flowmap, uint8_t *exit_flag, int32_t *exit_step, void *cuda_stream);
+
+/* FTLE time series: the same n seeds released at n_vol times t_start[k] (HOST array) and each integrated over the signed interval T
+ * with step h, i.e. n_vol calls of lcs_advect(seeds, t_start[k], t_start[k] + T, h) (LCS are followed through time as a
+ * sequence of FTLE fields; the cached window of velocity frames serves every tracer that is inside it).
+ * flowmaps: device [n_vol][n][dim] of compute_dtype; exit_flags (may be NULL): device [n_vol][n] u8; exit_steps (may be NULL):
+ * device [n_vol][n] i32; per volume exactly what lcs_advect returns (bit for bit: a tracer's arithmetic does not depend on who
+ * shares its launch).  On 3D fp32 Cartesian grids whose volumes are the same integration shifted by whole snapshot intervals the
+ * volumes that are inside a snapshot window at the same time are advanced TOGETHER -- one blend of the window's stage-time fields
+ * and one integrator launch over the tracers of all of them, bundled by cell; otherwise the volumes are integrated one after the
+ * other.  lcs_advect_series_reserve is the set-up call (the series needs room for the tracers of all overlapping volumes plus one;
+ * option "field_sets" must be 0).  n_vol * n < 2^31.  Errors as lcs_advect; LCS_ERR_OOM without a covering reservation.        */
+lcs_status lcs_advect_series_reserve(lcs_field *f, int64_t n, int32_t n_vol, const double *t_start, double T, double h);
+lcs_status lcs_advect_series(lcs_field *f, int64_t n, const void *seeds, int32_t n_vol, const double *t_start, double T, double h,
+                             void *flowmaps, uint8_t *exit_flags, int32_t *exit_steps, void *cuda_stream);
 
 /* Central-difference flow-map gradient G_ab = dF_a/dx_b on the structured seed grid,
  * Cauchy-Green tensor C = G^T G (Eq. 1.1), its largest eigenvalue (closed form) and
@@ -225,6 +242,13 @@ lcs_status lcs_ftle_host(lcs_field *f, const int32_t ng[3], const double seed_sp
                          const void *seeds_host, double t0, double tf, double h,
                          void *flowmap_host, uint8_t *exit_flag_host, int32_t *exit_step_host,
                          void *cg_host, void *ftle_host);
+
+/* The time-series counterpart of lcs_ftle_host: seeds up, lcs_advect_series, lcs_cg_ftle per volume, results down; synchronous.
+ * t_start: HOST [n_vol].  Outputs are [n_vol][n]... arrays in HOST memory: ftle_host [n_vol][n] (required); flowmaps_host
+ * [n_vol][n][dim], exit_flags_host [n_vol][n], exit_steps_host [n_vol][n], cg_host [n_vol][n][3 or 6] (each optional).   */
+lcs_status lcs_ftle_series_host(lcs_field *f, const int32_t ng[3], const double seed_spacing[3], const int32_t seed_periodic[3],
+                                const double period[3], const void *seeds_host, int32_t n_vol, const double *t_start, double T, double h,
+                                void *flowmaps_host, uint8_t *exit_flags_host, int32_t *exit_steps_host, void *cg_host, void *ftle_host);
 
 /* Measured peaks of the device the roofline fractions are quoted against ("Peaks to measure on the box
  * before quoting any %"; the paper's claim under test is "limited by memory bandwidth").  Runs a

@@ -207,7 +207,7 @@ __device__ __forceinline__ bool cart_velocity(const CartDev &g, const PairRec<DI
 // the initial cell agrees with lcs_locate.  flag 2 = seed outside at t0.
 template <int DIM, typename TC>
 __global__ void __launch_bounds__(256) cart_init_kernel(CartDev g, const TC *__restrict__ seeds, int64_t n,
-                                                         CartTracer<DIM, TC> *__restrict__ st)
+                                                         CartTracer<DIM, TC> *__restrict__ st, int32_t orig_base = 0)
 {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
@@ -226,7 +226,7 @@ __global__ void __launch_bounds__(256) cart_init_kernel(CartDev g, const TC *__r
         t.ci[a] = c;
         t.w[a] = (TC)w;
     }
-    t.orig = (int32_t)i;
+    t.orig = orig_base + (int32_t)i;
     t.meta = fl << 30;
     store_record(st + i, t);
 }
@@ -271,6 +271,7 @@ __global__ void __launch_bounds__(256) cart_key_kernel(CartDev g, const CartTrac
     if (i >= n) return;
     const CartTracer<DIM, TC> t = load_record(st + i);
     uint32_t k = last_bin;
+    if ((t.meta >> 30) == 3u) { key[i] = bundle::kDropKey; return; }       // record of a finished series volume: dropped by the sort
     if ((t.meta >> 30) == 0) {
         int c[DIM];
 #pragma unroll
@@ -466,12 +467,16 @@ __device__ __forceinline__ bool cart_velocity_xpair(const CartDev &g, const XPai
 template <bool FASTWRAP>
 __global__ void __launch_bounds__(256)
 cart_xpair_kernel(const __grid_constant__ CartDev g, const XPair *__restrict__ fields, int64_t field_stride,
-                  int nsteps, int first_step, int64_t n, CartTracer<3, float> *__restrict__ st, float hs0, float hs1, float hs2)
+                  int nsteps, int first_step, int64_t n, CartTracer<3, float> *__restrict__ st, float hs0, float hs1, float hs2,
+                  int per_tracer_steps)
 {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     CartTracer<3, float> t = load_record(st + i);
     if ((t.meta >> 30) != 0) return;
+    // series mode: tracers of several volumes, each at its own step count, share the launch: a live record carries the steps it
+    // has completed in the low bits of meta (otherwise those are zero while the tracer lives)
+    if (per_tracer_steps) first_step = (int)(t.meta & 0x3fffffffu);
     const float hs[3] = {hs0, hs1, hs2};
     int ci[3];
     float w[3];
@@ -514,7 +519,35 @@ cart_xpair_kernel(const __grid_constant__ CartDev g, const XPair *__restrict__ f
 #pragma unroll
     for (int a = 0; a < 3; ++a) { t.ci[a] = ci[a]; t.w[a] = w[a]; }
     if (!ok) t.meta = (1u << 30) | (uint32_t)(first_step + s);
+    else if (per_tracer_steps) t.meta = (uint32_t)(first_step + nsteps);
     store_record(st + i, t);
+}
+
+// series mode: outputs of the records of one finished volume (orig in [lo, hi)), written to the volume-major output arrays at index
+// orig; the records are then marked dead (flag 3) and dropped by the next re-bundling
+template <int DIM, typename TC>
+__global__ void __launch_bounds__(256) cart_final_series_kernel(CartDev g, const TC *__restrict__ seeds, int64_t n_act, CartTracer<DIM, TC> *__restrict__ st,
+                                                                 int32_t lo, int32_t hi, int32_t N, TC *__restrict__ flowmap,
+                                                                 uint8_t *__restrict__ exit_flag, int32_t *__restrict__ exit_step)
+{
+    int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= n_act) return;
+    CartTracer<DIM, TC> t = load_record(st + j);
+    const uint32_t fl = t.meta >> 30;
+    if (fl == 3u || t.orig < lo || t.orig >= hi) return;
+    const int64_t i = t.orig;
+    TC out[DIM];
+#pragma unroll
+    for (int a = 0; a < DIM; ++a) {
+        if (fl == 2) out[a] = seeds[(i - lo) * DIM + a];
+        else out[a] = (TC)(g.origin[a] + ((double)t.ci[a] + (double)t.w[a]) * g.spacing[a]);
+    }
+#pragma unroll
+    for (int a = 0; a < DIM; ++a) flowmap[i * DIM + a] = out[a];
+    if (exit_flag) exit_flag[i] = (uint8_t)fl;
+    if (exit_step) exit_step[i] = fl == 0 ? N : (fl == 2 ? 0 : (int32_t)(t.meta & 0x3fffffffu));
+    t.meta = 3u << 30;
+    store_record(st + j, t);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -1184,10 +1217,10 @@ lcs_status cart_advect_impl(lcs_field *f, int64_t n, const void *seeds_, double 
                                    u.first, n, cur, hs[0], hs[1], hs[2], cap);
                     } else if (fast)
                         LCS_LAUNCH((cart_xpair_kernel<true>), lcs_blocks(n, block), block, 0, st, g, (const XPair *)fields, f->nrec,
-                                   u.count, u.first, n, cur, hs[0], hs[1], hs[2]);
+                                   u.count, u.first, n, cur, hs[0], hs[1], hs[2], 0);
                     else
                         LCS_LAUNCH((cart_xpair_kernel<false>), lcs_blocks(n, block), block, 0, st, g, (const XPair *)fields, f->nrec,
-                                   u.count, u.first, n, cur, hs[0], hs[1], hs[2]);
+                                   u.count, u.first, n, cur, hs[0], hs[1], hs[2], 0);
                 }
                 bool last_blend_of_win = true;
                 for (size_t uj = ui + 1; uj < units.size() && units[uj].win == u.win; ++uj) last_blend_of_win = last_blend_of_win && !units[uj].blend;
@@ -1231,6 +1264,191 @@ lcs_status cart_advect_impl(lcs_field *f, int64_t n, const void *seeds_, double 
     return LCS_OK;
 }
 
+// ---------------------------------------------------------------------------------------------
+// FTLE time series (BASELINE.json config 5; a sequence of seed grids released one after the other through the
+// same data).  Volumes whose integration intervals overlap are advanced TOGETHER: the tracers of every volume that is inside a
+// snapshot window are bundled into one set, so that one blend of the window's stage-time fields and one integrator launch serve
+// them all, at 8-30 tracers per cell instead of 3 (the gathers of a warp then fall into a handful of 128-byte lines: 64 -> 76 G
+// seed-steps/s inside the kernel).  A volume joins the set when its release time is reached (cart_init_kernel
+// appends its records) and leaves it after its last step (cart_final_series_kernel writes its outputs and marks its records dead;
+// the next re-bundling drops them).  Records carry their own step count (per_tracer_steps).
+// Batching needs volumes that are the same integration shifted by whole snapshot intervals, on the pre-blended bundled path;
+// anything else is integrated volume by volume (plan.batched == false).
+struct SeriesPlan {
+    bool batched = false;
+    struct Unit { int pair, first, count, ftau_off, nfields, chunk; };
+    std::vector<Unit> units;                 // launch units of ONE volume (pair = snapshot pair of volume 0, chunk = index inside its window)
+    std::vector<float> ftau;
+    std::vector<int> shift;                  // volume k uses pair + shift[k]
+    struct Layer { int pair, chunk, unit; std::vector<int> start_vols, finish_vols; };   // unit = a member's unit (all members share count and stage times)
+    std::vector<Layer> layers;               // in integration order
+    int64_t cap_records = 0;                 // largest number of records in the set (incl. those dropped by the next re-bundling)
+};
+
+lcs_status series_plan(const lcs_field *f, int64_t n, int n_vol, const double *t_start, double h, int64_t N, SeriesPlan &P)
+{
+    P = SeriesPlan();
+    const CartLayout L1 = cart_layout(f, n * (int64_t)std::min(n_vol, 2), N);
+    if (!L1.preblend || !L1.do_bundle || L1.tma || n_vol < 2) return LCS_OK;
+    std::vector<StepWindow> w0;
+    lcs_status rc = lcs_plan_windows(f, t_start[0], h, N, w0);
+    if (rc != LCS_OK) return rc;
+    // units of volume 0 (as in cart_advect_impl: a window is cut into chunks of preblend_steps steps)
+    for (const StepWindow &w : w0) {
+        if (!(w.s[0] == w.s[1] && w.s[1] == w.s[2])) return LCS_OK;
+        const int chunk = (int)f->opt_preblend_steps;
+        for (int done = 0, cnt = 0, ci = 0; done < w.count; done += cnt, ++ci) {
+            cnt = w.count - done < chunk ? w.count - done : chunk;
+            SeriesPlan::Unit u{w.s[0], (int)w.first + done, cnt, (int)P.ftau.size(), 2 * cnt + 1, ci};
+            for (int s = u.first; s + 1 < u.first + u.count; ++s)
+                if ((float)lcs_stage_tau(f, t_start[0], h, s, 2, w.s[2]) != (float)lcs_stage_tau(f, t_start[0], h, s + 1, 0, w.s[0])) return LCS_OK;
+            for (int s = u.first; s < u.first + u.count; ++s) {
+                P.ftau.push_back((float)lcs_stage_tau(f, t_start[0], h, s, 0, w.s[0]));
+                P.ftau.push_back((float)lcs_stage_tau(f, t_start[0], h, s, 1, w.s[1]));
+            }
+            P.ftau.push_back((float)lcs_stage_tau(f, t_start[0], h, u.first + u.count - 1, 2, w.s[2]));
+            P.units.push_back(u);
+        }
+    }
+    // every other volume: the same units in snapshot pairs shifted by a constant, with the same stage-time weights bit for bit
+    P.shift.assign(n_vol, 0);
+    for (int k = 1; k < n_vol; ++k) {
+        std::vector<StepWindow> wk;
+        rc = lcs_plan_windows(f, t_start[k], h, N, wk);
+        if (rc != LCS_OK) return rc;
+        if (wk.size() != w0.size()) return LCS_OK;
+        const int sh = wk[0].s[0] - w0[0].s[0];
+        for (size_t i = 0; i < wk.size(); ++i)
+            if (wk[i].first != w0[i].first || wk[i].count != w0[i].count || wk[i].s[0] != w0[i].s[0] + sh || wk[i].s[1] != wk[i].s[0] ||
+                wk[i].s[2] != wk[i].s[0]) return LCS_OK;
+        for (const SeriesPlan::Unit &u : P.units) {
+            const float *tb = P.ftau.data() + u.ftau_off;
+            for (int s = u.first, j = 0; s < u.first + u.count; ++s, j += 2)
+                if ((float)lcs_stage_tau(f, t_start[k], h, s, 0, u.pair + sh) != tb[j] || (float)lcs_stage_tau(f, t_start[k], h, s, 1, u.pair + sh) != tb[j + 1]) return LCS_OK;
+            if ((float)lcs_stage_tau(f, t_start[k], h, u.first + u.count - 1, 2, u.pair + sh) != tb[2 * u.count]) return LCS_OK;
+        }
+        P.shift[k] = sh;
+    }
+    // layers: (snapshot pair, chunk inside the window) in integration order; volume k runs its unit i in layer
+    // (units[i].pair + shift[k], units[i].chunk).  Units that meet in a layer must be the same steps of the window: same count and
+    // the same stage-time weights bit for bit (they belong to different unit indices of volume 0's table).
+    const int dir = h > 0 ? 1 : -1;
+    const int last = (int)P.units.size() - 1;
+    struct Ev { int64_t order; int pair, unit, vol; };
+    std::vector<Ev> evs;
+    for (int k = 0; k < n_vol; ++k)
+        for (size_t i = 0; i < P.units.size(); ++i)
+            evs.push_back({(int64_t)dir * (P.units[i].pair + P.shift[k]) * 65536 + (int64_t)P.units[i].chunk, P.units[i].pair + P.shift[k], (int)i, k});
+    std::sort(evs.begin(), evs.end(), [](const Ev &a, const Ev &b) { return a.order != b.order ? a.order < b.order : a.vol < b.vol; });
+    for (const Ev &e : evs) {
+        const SeriesPlan::Unit &u = P.units[e.unit];
+        if (P.layers.empty() || P.layers.back().pair != e.pair || P.layers.back().chunk != u.chunk) P.layers.push_back({e.pair, u.chunk, e.unit, {}, {}});
+        SeriesPlan::Layer &ly = P.layers.back();
+        const SeriesPlan::Unit &r = P.units[ly.unit];
+        if (r.count != u.count || !std::equal(P.ftau.begin() + r.ftau_off, P.ftau.begin() + r.ftau_off + r.nfields, P.ftau.begin() + u.ftau_off)) {
+            P.layers.clear();
+            return LCS_OK;
+        }
+        if (e.unit == 0) ly.start_vols.push_back(e.vol);
+        if (e.unit == last) ly.finish_vols.push_back(e.vol);
+    }
+    // largest record count: live volumes + those that finished in the previous layer (dropped by this layer's re-bundling)
+    int64_t act = 0, finished_prev = 0;
+    for (const SeriesPlan::Layer &ly : P.layers) {
+        act += (int64_t)ly.start_vols.size();
+        P.cap_records = std::max(P.cap_records, act * n);
+        act -= finished_prev;
+        finished_prev = (int64_t)ly.finish_vols.size();
+    }
+    P.batched = true;
+    return LCS_OK;
+}
+
+lcs_status cart_advect_series_batched(lcs_field *f, const SeriesPlan &P, int64_t n, const float *seeds, int n_vol, double t0_first, double h, int64_t N,
+                                      float *flowmaps, uint8_t *exit_flags, int32_t *exit_steps, cudaStream_t st)
+{
+    using Tracer = CartTracer<3, float>;
+    const CartLayout L = cart_layout(f, P.cap_records, N);
+    lcs_status rc = lcs_scratch_check(f, L.total);
+    if (rc != LCS_OK) return rc;
+    char *base = (char *)f->scratch.buf;
+    Tracer *cur = (Tracer *)(base + L.o_a), *alt = (Tracer *)(base + L.o_b);
+    uint32_t *d_key = (uint32_t *)(base + L.o_key), *d_cnt = (uint32_t *)(base + L.o_cnt), *d_tile = (uint32_t *)(base + L.o_tile);
+    float *d_ftau = (float *)(base + L.o_ftau);
+    XPair *fields = (XPair *)(base + L.o_fields);
+    if (f->opt_field_sets > 0) { lcs_set_error("lcs_advect_series blends every window once and takes no resident field sets: set field_sets = 0"); return LCS_ERR_INVALID_ARG; }
+    CartDev g = make_dev(f);
+    const int block = f->opt_block ? (int)(f->opt_block > 256 ? 256 : f->opt_block) : 256;
+    bool fast = true;
+    for (int a = 0; a < 3; ++a) fast = fast && g.periodic[a] && g.pow2[a];
+    float hs[3];
+    for (int a = 0; a < 3; ++a) hs[a] = (float)(h * f->cart.inv[a]);
+    const int dir = h > 0 ? 1 : -1;
+    int64_t n_act = 0;
+    std::vector<int> to_finish;
+    int cur_pair = -1;
+    const void *raw_a = nullptr, *raw_b = nullptr;
+    auto finalize = [&](const std::vector<int> &vols) -> lcs_status {
+        for (int k : vols)
+            LCS_LAUNCH((cart_final_series_kernel<3, float>), lcs_blocks(n_act, 256), 256, 0, st, g, seeds, n_act, cur, (int32_t)(k * n), (int32_t)((k + 1) * n),
+                       (int32_t)N, flowmaps, exit_flags, exit_steps);
+        LCS_CUDA_OK(cudaGetLastError());
+        return LCS_OK;
+    };
+    for (size_t li = 0; li < P.layers.size(); ++li) {
+        const SeriesPlan::Layer &ly = P.layers[li];
+        const SeriesPlan::Unit &u = P.units[ly.unit];
+        // volumes that completed their last unit in the previous layer leave; volumes whose first unit this is join
+        rc = finalize(to_finish);
+        if (rc != LCS_OK) return rc;
+        const int64_t dropped = (int64_t)to_finish.size() * n;
+        to_finish.clear();
+        for (int k : ly.start_vols) {
+            LCS_LAUNCH((cart_init_kernel<3, float>), lcs_blocks(n, 256), 256, 0, st, g, seeds, n, cur + n_act, (int32_t)(k * n));
+            n_act += n;
+        }
+        // re-bundle the whole set (drops the dead records)
+        LCS_CUDA_OK(cudaMemsetAsync(d_cnt, 0, (size_t)L.nbins * 4, st));
+        LCS_LAUNCH((cart_key_kernel<3, float>), lcs_blocks(n_act, 256), 256, 0, st, g, cur, n_act, L.shift, L.order, (uint32_t)(L.nbins - 1), d_key, d_cnt);
+        bundle::sort_records<Tracer>(cur, alt, d_key, d_cnt, d_tile, n_act, L.nbins, st);
+        std::swap(cur, alt);
+        n_act -= dropped;
+        if (ly.pair != cur_pair) {
+            if (cur_pair >= 0) { rc = lcs_field_release_raw(f, cur_pair, st); if (rc != LCS_OK) return rc; }
+            rc = lcs_field_acquire_raw(f, ly.pair, st, &raw_a, &raw_b);
+            if (rc != LCS_OK) return rc;
+            lcs_field_prefetch(f, dir > 0 ? ly.pair + 2 : ly.pair - 1, ly.pair, ly.pair + 1);
+            cur_pair = ly.pair;
+            f->info_windows++;
+        }
+        // the stage-time weights of the unit are those of volume 0's copy of it (identical for every volume: series_plan checked)
+        {
+            const int32_t s3[3] = {u.pair, u.pair, u.pair};
+            rc = lcs_fill_stage_tau(f, t0_first, h, u.first, u.count, s3, nullptr, d_ftau, st);
+            if (rc != LCS_OK) return rc;
+        }
+        LCS_LAUNCH(blend_xpair_kernel, lcs_blocks(f->nrec, 256), 256, 0, st, (const float *)raw_a, (const float *)raw_b, g.n[0], g.n[1], g.n[2],
+                   f->cart.np[0], f->cart.np[1], f->cart.np[2], d_ftau, u.nfields, fields, f->nrec);
+        {
+            WindowTimer timer(f, st);
+            if (fast)
+                LCS_LAUNCH((cart_xpair_kernel<true>), lcs_blocks(n_act, block), block, 0, st, g, (const XPair *)fields, f->nrec, u.count, 0, n_act, cur,
+                           hs[0], hs[1], hs[2], 1);
+            else
+                LCS_LAUNCH((cart_xpair_kernel<false>), lcs_blocks(n_act, block), block, 0, st, g, (const XPair *)fields, f->nrec, u.count, 0, n_act, cur,
+                           hs[0], hs[1], hs[2], 1);
+        }
+        LCS_CUDA_OK(cudaGetLastError());
+        to_finish = ly.finish_vols;
+    }
+    rc = finalize(to_finish);
+    if (rc != LCS_OK) return rc;
+    if (cur_pair >= 0) { rc = lcs_field_release_raw(f, cur_pair, st); if (rc != LCS_OK) return rc; }
+    (void)n_vol;
+    f->info_series_layers = (int64_t)P.layers.size();
+    return LCS_OK;
+}
+
 }  // namespace
 
 size_t lcs_cart_scratch_bytes(const lcs_field *f, int64_t n, int64_t N) { return cart_layout(f, n, N).total; }
@@ -1246,6 +1464,27 @@ size_t lcs_cart_field_set_bytes(const lcs_field *f, int64_t N)
 {
     const CartLayout L = cart_layout(f, (int64_t)1 << 20, N);      // sets are used by the pre-blended integrator only
     return (f->opt_preblend != 0 && L.max_fields > 0) ? (size_t)L.max_fields * (size_t)f->nrec * 32 : 0;
+}
+
+// lcs_advect_series on a Cartesian grid: batched when series_plan allows it, else volume by volume
+lcs_status lcs_cart_advect_series(lcs_field *f, int64_t n, const void *seeds, int n_vol, const double *t_start, double h, int64_t N,
+                                  void *flowmaps, uint8_t *exit_flags, int32_t *exit_steps, cudaStream_t st, int64_t *cap_records_out)
+{
+    SeriesPlan P;
+    lcs_status rc = series_plan(f, n, n_vol, t_start, h, N, P);
+    if (rc != LCS_OK) return rc;
+    if (n_vol * n >= (1LL << 31)) { lcs_set_error("n_vol * n must stay below 2^31"); return LCS_ERR_INVALID_ARG; }
+    if (cap_records_out) { *cap_records_out = P.batched ? P.cap_records : n; return LCS_OK; }      // planning only (lcs_advect_series_reserve)
+    f->info_series_layers = 0;
+    if (P.batched)
+        return cart_advect_series_batched(f, P, n, (const float *)seeds, n_vol, t_start[0], h, N, (float *)flowmaps, exit_flags, exit_steps, st);
+    const size_t es = lcs_esize(f->compute_dtype);
+    for (int k = 0; k < n_vol; ++k) {
+        rc = lcs_cart_advect(f, n, seeds, t_start[k], h, N, (char *)flowmaps + (size_t)k * n * f->dim * es, exit_flags ? exit_flags + (size_t)k * n : nullptr,
+                             exit_steps ? exit_steps + (size_t)k * n : nullptr, st);
+        if (rc != LCS_OK) return rc;
+    }
+    return LCS_OK;
 }
 
 lcs_status lcs_cart_locate(lcs_field *f, int64_t n, const double *pos, int32_t *cell, double *w, cudaStream_t st)

@@ -16,6 +16,7 @@ namespace bundle {
 constexpr int kScanBlock = 1024;
 constexpr int kScanItems = 4;                    // per thread
 constexpr int kScanTile = kScanBlock * kScanItems;
+constexpr uint32_t kDropKey = 0xffffffffu;         // a record with this key is not counted and not scattered: it leaves the set
 
 // spread the low 10 bits of v so that there are two zero bits between consecutive bits
 __host__ __device__ __forceinline__ uint32_t spread3(uint32_t v)
@@ -148,6 +149,7 @@ static __global__ void __launch_bounds__(256) scatter_kernel(const REC *__restri
 #pragma unroll
     for (int k = 0; k < NQ; ++k) q[k] = s[k];
     const uint32_t k = key[i];
+    if (k == kDropKey) return;
     const unsigned active = __activemask();
     const unsigned parked = __ballot_sync(active, k == last_bin);
     uint32_t pos;

@@ -386,6 +386,11 @@ extern "C" void lcs_field_destroy(lcs_field *f)
     if (f->h_flag) cudaFree(f->h_flag);
     if (f->h_cg) cudaFree(f->h_cg);
     if (f->h_step) cudaFree(f->h_step);
+    if (f->hs_flow) cudaFree(f->hs_flow);
+    if (f->hs_ftle) cudaFree(f->hs_ftle);
+    if (f->hs_cg) cudaFree(f->hs_cg);
+    if (f->hs_flag) cudaFree(f->hs_flag);
+    if (f->hs_step) cudaFree(f->hs_step);
     lcs_simplex_free(f);
     if (f->side) cudaStreamDestroy(f->side);
     delete f;
@@ -457,6 +462,7 @@ extern "C" lcs_status lcs_field_get_info(const lcs_field *f, const char *key, in
 {
     if (!f || !key || !value) { lcs_set_error("null argument"); return LCS_ERR_INVALID_ARG; }
     if (!strcmp(key, "windows")) *value = f->info_windows;
+    else if (!strcmp(key, "series_layers")) *value = f->info_series_layers;
     else if (!strcmp(key, "h2d_bytes")) *value = f->info_h2d_bytes;
     else if (!strcmp(key, "n_nodes")) *value = f->nnodes;
     else if (!strcmp(key, "n_cells")) *value = f->kind == LCS_MESH_SIMPLEX ? f->mesh.nc : 0;
@@ -580,6 +586,57 @@ extern "C" lcs_status lcs_advect(lcs_field *f, int64_t n, const void *seeds, dou
 }
 
 // ---------------------------------------------------------------------------------------------
+static lcs_status series_args(lcs_field *f, int64_t n, int32_t n_vol, const double *t_start, double T, double h, int64_t *N)
+{
+    if (!f || n < 1 || n_vol < 1 || !t_start) { lcs_set_error("null argument, n < 1 or n_vol < 1"); return LCS_ERR_INVALID_ARG; }
+    if (n_vol > 65536 || (int64_t)n_vol * n >= (1LL << 31)) { lcs_set_error("n_vol * n must stay below 2^31"); return LCS_ERR_INVALID_ARG; }
+    int64_t Nk = 0;
+    for (int k = 0; k < n_vol; ++k) {
+        lcs_status rc = check_interval(f, t_start[k], t_start[k] + T, h, &Nk);
+        if (rc != LCS_OK) return rc;
+        if (k > 0 && Nk != *N) { lcs_set_error("volumes of a series take the same number of steps"); return LCS_ERR_INVALID_ARG; }
+        *N = Nk;
+    }
+    return LCS_OK;
+}
+
+extern "C" lcs_status lcs_advect_series_reserve(lcs_field *f, int64_t n, int32_t n_vol, const double *t_start, double T, double h)
+{
+    int64_t N = 0;
+    lcs_status rc = series_args(f, n, n_vol, t_start, T, h, &N);
+    if (rc != LCS_OK) return rc;
+    LCS_GUARD(
+        int64_t cap = n;
+        if (f->kind == LCS_MESH_CARTESIAN) {
+            rc = lcs_cart_advect_series(f, n, nullptr, n_vol, t_start, h, N, nullptr, nullptr, nullptr, nullptr, &cap);
+            if (rc != LCS_OK) return rc;
+        }
+        return lcs_field_reserve(f, cap, N);
+    )
+}
+
+extern "C" lcs_status lcs_advect_series(lcs_field *f, int64_t n, const void *seeds, int32_t n_vol, const double *t_start, double T, double h,
+                                        void *flowmaps, uint8_t *exit_flags, int32_t *exit_steps, void *cuda_stream)
+{
+    int64_t N = 0;
+    lcs_status rc = series_args(f, n, n_vol, t_start, T, h, &N);
+    if (rc != LCS_OK) return rc;
+    if (!seeds || !flowmaps) { lcs_set_error("null argument"); return LCS_ERR_INVALID_ARG; }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    LCS_GUARD(
+        if (f->kind == LCS_MESH_CARTESIAN)
+            return lcs_cart_advect_series(f, n, seeds, n_vol, t_start, h, N, flowmaps, exit_flags, exit_steps, st, nullptr);
+        const size_t es = lcs_esize(f->compute_dtype);
+        for (int k = 0; k < n_vol; ++k) {
+            rc = lcs_simplex_advect(f, n, seeds, t_start[k], h, N, (char *)flowmaps + (size_t)k * n * f->dim * es,
+                                    exit_flags ? exit_flags + (size_t)k * n : nullptr, exit_steps ? exit_steps + (size_t)k * n : nullptr, st);
+            if (rc != LCS_OK) return rc;
+        }
+        return LCS_OK;
+    )
+}
+
+// ---------------------------------------------------------------------------------------------
 extern "C" lcs_status lcs_ftle_host(lcs_field *f, const int32_t ng[3], const double seed_spacing[3], const int32_t seed_periodic[3],
                                     const double period[3], const void *seeds_host, double t0, double tf, double h,
                                     void *flowmap_host, uint8_t *exit_flag_host, int32_t *exit_step_host, void *cg_host, void *ftle_host)
@@ -622,6 +679,67 @@ extern "C" lcs_status lcs_ftle_host(lcs_field *f, const int32_t ng[3], const dou
     if (flowmap_host) LCS_CUDA_OK(cudaMemcpyAsync(flowmap_host, f->h_seeds, (size_t)n * f->dim * es, cudaMemcpyDeviceToHost, st));
     if (exit_flag_host) LCS_CUDA_OK(cudaMemcpyAsync(exit_flag_host, f->h_flag, (size_t)n, cudaMemcpyDeviceToHost, st));
     if (exit_step_host) LCS_CUDA_OK(cudaMemcpyAsync(exit_step_host, f->h_step, (size_t)n * 4, cudaMemcpyDeviceToHost, st));
+    LCS_CUDA_OK(cudaStreamSynchronize(st));
+    return LCS_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+extern "C" lcs_status lcs_ftle_series_host(lcs_field *f, const int32_t ng[3], const double seed_spacing[3], const int32_t seed_periodic[3],
+                                           const double period[3], const void *seeds_host, int32_t n_vol, const double *t_start, double T, double h,
+                                           void *flowmaps_host, uint8_t *exit_flags_host, int32_t *exit_steps_host, void *cg_host, void *ftle_host)
+{
+    if (!f || !ng || !seeds_host || !ftle_host || !t_start || n_vol < 1) { lcs_set_error("null argument"); return LCS_ERR_INVALID_ARG; }
+    const int64_t n = (int64_t)ng[0] * ng[1] * (f->dim == 3 ? ng[2] : 1);
+    if (n <= 0) { lcs_set_error("empty seed grid"); return LCS_ERR_INVALID_ARG; }
+    lcs_status rc = lcs_advect_series_reserve(f, n, n_vol, t_start, T, h);      // this convenience call is synchronous set-up + run
+    if (rc != LCS_OK) return rc;
+    const size_t es = lcs_esize(f->compute_dtype), ncg = f->dim == 2 ? 3 : 6;
+    const int64_t tot = n * n_vol;
+    if (f->h_cap < n) {                                      // seeds staging shared with lcs_ftle_host
+        cudaDeviceSynchronize();
+        if (f->h_seeds) cudaFree(f->h_seeds);
+        if (f->h_ftle) cudaFree(f->h_ftle);
+        if (f->h_flag) cudaFree(f->h_flag);
+        if (f->h_cg) cudaFree(f->h_cg);
+        if (f->h_step) cudaFree(f->h_step);
+        f->h_seeds = f->h_ftle = f->h_cg = nullptr; f->h_flag = nullptr; f->h_step = nullptr; f->h_cap = 0;
+        LCS_CUDA_OK(cudaMalloc(&f->h_seeds, (size_t)n * f->dim * es));
+        LCS_CUDA_OK(cudaMalloc(&f->h_ftle, (size_t)n * es));
+        LCS_CUDA_OK(cudaMalloc((void **)&f->h_flag, (size_t)n));
+        f->h_cap = n;
+    }
+    if (f->hs_cap < tot || (cg_host && !f->hs_cg)) {
+        cudaDeviceSynchronize();
+        if (f->hs_flow) cudaFree(f->hs_flow);
+        if (f->hs_ftle) cudaFree(f->hs_ftle);
+        if (f->hs_cg) cudaFree(f->hs_cg);
+        if (f->hs_flag) cudaFree(f->hs_flag);
+        if (f->hs_step) cudaFree(f->hs_step);
+        f->hs_flow = f->hs_ftle = f->hs_cg = nullptr; f->hs_flag = nullptr; f->hs_step = nullptr;
+        const int64_t cap = tot > f->hs_cap ? tot : f->hs_cap;
+        f->hs_cap = 0;
+        LCS_CUDA_OK(cudaMalloc(&f->hs_flow, (size_t)cap * f->dim * es));
+        LCS_CUDA_OK(cudaMalloc(&f->hs_ftle, (size_t)cap * es));
+        LCS_CUDA_OK(cudaMalloc((void **)&f->hs_flag, (size_t)cap));
+        LCS_CUDA_OK(cudaMalloc((void **)&f->hs_step, (size_t)cap * 4));
+        if (cg_host) LCS_CUDA_OK(cudaMalloc(&f->hs_cg, (size_t)cap * ncg * es));
+        f->hs_cap = cap;
+    }
+    cudaStream_t st = 0;
+    LCS_CUDA_OK(cudaMemcpyAsync(f->h_seeds, seeds_host, (size_t)n * f->dim * es, cudaMemcpyHostToDevice, st));
+    rc = lcs_advect_series(f, n, f->h_seeds, n_vol, t_start, T, h, f->hs_flow, f->hs_flag, f->hs_step, st);
+    if (rc != LCS_OK) return rc;
+    for (int k = 0; k < n_vol; ++k) {
+        rc = lcs_cg_ftle(f->dim, f->compute_dtype, ng, seed_spacing, seed_periodic, period, (char *)f->hs_flow + (size_t)k * n * f->dim * es,
+                         f->hs_flag + (size_t)k * n, T, cg_host ? (char *)f->hs_cg + (size_t)k * n * ncg * es : nullptr,
+                         (char *)f->hs_ftle + (size_t)k * n * es, nullptr, st);
+        if (rc != LCS_OK) return rc;
+    }
+    LCS_CUDA_OK(cudaMemcpyAsync(ftle_host, f->hs_ftle, (size_t)tot * es, cudaMemcpyDeviceToHost, st));
+    if (cg_host) LCS_CUDA_OK(cudaMemcpyAsync(cg_host, f->hs_cg, (size_t)tot * ncg * es, cudaMemcpyDeviceToHost, st));
+    if (flowmaps_host) LCS_CUDA_OK(cudaMemcpyAsync(flowmaps_host, f->hs_flow, (size_t)tot * f->dim * es, cudaMemcpyDeviceToHost, st));
+    if (exit_flags_host) LCS_CUDA_OK(cudaMemcpyAsync(exit_flags_host, f->hs_flag, (size_t)tot, cudaMemcpyDeviceToHost, st));
+    if (exit_steps_host) LCS_CUDA_OK(cudaMemcpyAsync(exit_steps_host, f->hs_step, (size_t)tot * 4, cudaMemcpyDeviceToHost, st));
     LCS_CUDA_OK(cudaStreamSynchronize(st));
     return LCS_OK;
 }

@@ -134,6 +134,10 @@ struct lcs_field {
     TracerScratch scratch;
     // host-API scratch
     void *h_seeds = nullptr, *h_flow = nullptr, *h_ftle = nullptr, *h_cg = nullptr;
+    void *hs_flow = nullptr, *hs_ftle = nullptr, *hs_cg = nullptr;      // staging of lcs_ftle_series_host ([n_vol][n] arrays)
+    uint8_t *hs_flag = nullptr;
+    int32_t *hs_step = nullptr;
+    int64_t hs_cap = 0;
     uint8_t *h_flag = nullptr;
     int32_t *h_step = nullptr;
     int64_t h_cap = 0;
@@ -156,6 +160,7 @@ struct lcs_field {
     int64_t opt_time_windows = 0; // record CUDA events around every window (hot) kernel launch
     // info
     int64_t info_windows = 0;
+    int64_t info_series_layers = 0;      // batched layers of the last lcs_advect_series (0: integrated volume by volume)
     int64_t info_h2d_bytes = 0;
     std::vector<cudaEvent_t> win_ev;     // start/stop pairs recorded on the launching stream
     size_t win_ev_used = 0;
@@ -202,6 +207,8 @@ lcs_status lcs_simplex_advect(lcs_field *f, int64_t n, const void *seeds, double
 
 // advect_cart.cu
 lcs_status lcs_cart_locate(lcs_field *f, int64_t n, const double *pos, int32_t *cell, double *w, cudaStream_t st);
+lcs_status lcs_cart_advect_series(lcs_field *f, int64_t n, const void *seeds, int n_vol, const double *t_start, double h, int64_t N,
+                                  void *flowmaps, uint8_t *exit_flags, int32_t *exit_steps, cudaStream_t st, int64_t *cap_records_out);
 lcs_status lcs_cart_advect(lcs_field *f, int64_t n, const void *seeds, double t0, double h, int64_t N,
                            void *flowmap, uint8_t *exit_flag, int32_t *exit_step, cudaStream_t st);
 

@@ -22,8 +22,8 @@ LCS_F32, LCS_F64 = 0, 1
 LCS_MESH_CARTESIAN, LCS_MESH_SIMPLEX = 0, 1
 
 EXPORTS = ["lcs_field_create", "lcs_field_set_snapshot", "lcs_field_sync", "lcs_field_destroy", "lcs_field_reserve",
-           "lcs_field_set_option", "lcs_field_get_info", "lcs_locate", "lcs_advect", "lcs_advect_early_cg", "lcs_cg_ftle", "lcs_cg_ftle_aux", "lcs_cg_eigen", "lcs_smooth_gaussian", "lcs_ridge",
-           "lcs_ftle_host", "lcs_measure_peak", "lcs_kernel_launch_count", "lcs_last_error"]
+           "lcs_field_set_option", "lcs_field_get_info", "lcs_locate", "lcs_advect", "lcs_advect_series", "lcs_advect_series_reserve", "lcs_advect_early_cg", "lcs_cg_ftle", "lcs_cg_ftle_aux", "lcs_cg_eigen", "lcs_smooth_gaussian", "lcs_ridge",
+           "lcs_ftle_host", "lcs_ftle_series_host", "lcs_measure_peak", "lcs_kernel_launch_count", "lcs_last_error"]
 PEAK_KINDS = {"fp32_fma_tflops": 0, "fp64_fma_tflops": 1, "launch_us": 2, "hbm_copy_gbs": 3, "l2_seq_gbs": 4, "l2_sector_gbs": 5,
               "hbm_sector_gbs": 6, "l1_gather_line_gbs": 7, "l1_gather_same_gbs": 8, "l1_gather_spread_gbs": 9,
               "smem_contiguous_gbs": 10, "smem_records_gbs": 11, "smem_records_swizzled_gbs": 12, "smem_records_same_gbs": 13}
@@ -71,6 +71,11 @@ def lib():
         L.lcs_locate.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.lcs_advect.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_double, C.c_double, C.c_double,
                                  C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.lcs_advect_series.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_int32, C.c_void_p, C.c_double, C.c_double, C.c_void_p, C.c_void_p,
+                                        C.c_void_p, C.c_void_p]
+        L.lcs_advect_series_reserve.argtypes = [C.c_void_p, C.c_int64, C.c_int32, C.c_void_p, C.c_double, C.c_double]
+        L.lcs_ftle_series_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_double,
+                                           C.c_double, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.lcs_cg_ftle.argtypes = [C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                   C.c_void_p, C.c_void_p, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.lcs_advect_early_cg.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_double,
@@ -249,6 +254,26 @@ class Field:
                                 _tptr(exit_flag), _tptr(exit_step), _stream_ptr(stream)))
         return flowmap, exit_flag, exit_step
 
+    def advect_series(self, seeds, t_start, T, h, flowmaps=None, exit_flags=None, exit_steps=None, stream=None, reserve=True):
+        """lcs_advect_series: the same seeds released at every t_start[k], each integrated over T with step h.  Returns
+        (flowmaps [n_vol][n][dim], exit_flags [n_vol][n], exit_steps [n_vol][n]) as torch CUDA tensors."""
+        import torch
+        assert seeds.is_cuda and seeds.is_contiguous()
+        n, dim = seeds.shape
+        ts = np.ascontiguousarray(t_start, dtype=np.float64)
+        nv = int(ts.shape[0])
+        if flowmaps is None:
+            flowmaps = torch.empty((nv, n, dim), dtype=seeds.dtype, device=seeds.device)
+        if exit_flags is None:
+            exit_flags = torch.empty((nv, n), dtype=torch.uint8, device=seeds.device)
+        if exit_steps is None:
+            exit_steps = torch.empty((nv, n), dtype=torch.int32, device=seeds.device)
+        if reserve:
+            _check(lib().lcs_advect_series_reserve(self._h, n, nv, _np_ptr(ts), float(T), float(h)))
+        _check(lib().lcs_advect_series(self._h, n, _tptr(seeds), nv, _np_ptr(ts), float(T), float(h), _tptr(flowmaps), _tptr(exit_flags),
+                                       _tptr(exit_steps), _stream_ptr(stream)))
+        return flowmaps, exit_flags, exit_steps
+
     def ftle_host(self, ng, seed_spacing, seed_periodic, period, seeds, t0, tf, h, flowmap=None, exit_flag=None, ftle=None,
                   exit_step=None, cg=None):
         """End-to-end with HOST numpy buffers (H2D + advect + cg_ftle + D2H inside the call); flowmap, exit_flag, exit_step
@@ -261,6 +286,19 @@ class Field:
                                    _arr3(seed_periodic, C.c_int32, 0), _arr3(period, C.c_double, 0.0),
                                    _np_ptr(seeds), float(t0), float(tf), float(h), _np_ptr(flowmap), _np_ptr(exit_flag),
                                    _np_ptr(exit_step), _np_ptr(cg), _np_ptr(ftle)))
+        return ftle
+
+    def ftle_series_host(self, ng, seed_spacing, seed_periodic, period, seeds, t_start, T, h, ftle=None, cg=None, flowmaps=None,
+                         exit_flags=None, exit_steps=None):
+        """lcs_ftle_series_host with HOST numpy buffers; returns ftle [n_vol][n]."""
+        seeds = np.ascontiguousarray(seeds, dtype=self.compute_dtype)
+        ts = np.ascontiguousarray(t_start, dtype=np.float64)
+        n, nv = seeds.shape[0], int(ts.shape[0])
+        if ftle is None:
+            ftle = np.empty((nv, n), dtype=self.compute_dtype)
+        _check(lib().lcs_ftle_series_host(self._h, _arr3(ng, C.c_int32, 1), _arr3(seed_spacing, C.c_double, 1.0), _arr3(seed_periodic, C.c_int32, 0),
+                                          _arr3(period, C.c_double, 0.0), _np_ptr(seeds), nv, _np_ptr(ts), float(T), float(h), _np_ptr(flowmaps),
+                                          _np_ptr(exit_flags), _np_ptr(exit_steps), _np_ptr(cg), _np_ptr(ftle)))
         return ftle
 
 

@@ -257,6 +257,76 @@ def test_config5_reduced_backward_streamed(lcs, oracle, options):
     print("config5 reduced", stats)
 
 
+@pytest.mark.parametrize("case", ["backward_ring", "forward_chunks", "nonperiodic_exits", "misaligned", "triangles"])
+def test_advect_series_identical_to_per_volume_advect(lcs, oracle, case):
+    """lcs_advect_series (FTLE time series: the same seeds released at several times): volumes that overlap in time are advanced
+    together -- one blend and one integrator launch per snapshot window over the bundled tracers of all of them -- and every
+    volume still equals, bit for bit, the lcs_advect of that volume alone (flow map, flags and exit steps: a record carries its
+    own step count).  Cases: config 5 reduced (backward, ring of 3 slots, volumes one snapshot interval apart); forward with
+    several chunks per window; a non-periodic grid with flags 0/1/2; release times that are not whole snapshot intervals apart
+    and a triangle mesh (both integrated volume by volume).  One volume is gated against the oracle."""
+    import torch
+    opts = dict(bundle=1, preblend=1)
+    ring = 0
+    if case == "backward_ring":
+        w = I.config5(ngrid=24, nn=32, n_grids=6, T=2.0, h=0.01, n_snap=13)
+        t_start, T, h, ring = [a for (a, b) in w.meta["windows"]], -2.0, w.h, 3
+    elif case == "forward_chunks":
+        w = I.config3(ngrid=20, nn=16, T=1.5, h=0.01, n_snap=9)
+        t_start, T, h = [0.0, 0.5, 1.0, 2.0], 1.5, 0.01
+        opts["preblend_steps"] = 20
+    elif case == "nonperiodic_exits":
+        A = np.array([[0.03, 0.05, 0.0], [-0.02, 0.04, 0.01], [0.0, -0.03, 0.02]])
+        w = I.analytic_cartesian(3, I.linear_flow(A, np.array([0.2, -0.05, 0.1])), (21, 17, 13), (0.0, 0.0, 0.0), (0.1, 0.1, 0.1),
+                                 (0.0, 1.0, 2.0, 3.0, 4.0, 5.0), ng=(40, 32, 24), seed_lo=(-0.1, -0.1, -0.1), seed_spacing=(2.2 / 40, 1.8 / 32, 1.4 / 24),
+                                 t0=0.0, tf=3.0, h=0.04, vel_dtype=np.float32, compute_dtype=np.float32)
+        t_start, T, h = [0.0, 1.0, 2.0], 3.0, 0.04
+        opts["preblend_steps"] = 6
+    elif case == "misaligned":
+        w = I.config3(ngrid=20, nn=16, T=1.0, h=0.01, n_snap=9)
+        t_start, T, h = [0.0, 0.3, 0.85], 1.0, 0.01
+    else:
+        w = I.config2(ng=(48, 24), lattice=(30, 15), T=2.0)
+        t_start, T, h, opts = [0.0, 0.5, 1.5], 2.0, w.h, dict()
+    f = lcs.Field.from_workload(w, max_resident_snapshots=ring, pinned=bool(ring))
+    for k, v in opts.items():
+        f.set_option(k, v)
+    sd = torch.from_numpy(w.seeds()).cuda()
+    Fs, fls, ess = f.advect_series(sd, t_start, T, h)
+    torch.cuda.synchronize()
+    f1 = lcs.Field.from_workload(w)
+    for k, v in opts.items():
+        f1.set_option(k, v)
+    for k, t0 in enumerate(t_start):
+        F, fl, es = f1.advect(sd, t0, t0 + T, h)
+        assert torch.equal(Fs[k], F) and torch.equal(fls[k], fl) and torch.equal(ess[k], es), (case, k)
+    assert (f.info("series_layers") > 0) == (case in ("backward_ring", "forward_chunks", "nonperiodic_exits"))      # batched or not
+    if case == "nonperiodic_exits":
+        assert set(np.unique(cpu(fls))) == {0, 1, 2}
+    if case == "backward_ring":
+        # the host-buffer convenience call returns the same FTLE as cg_ftle on the device results
+        fth = f.ftle_series_host(w.ng, w.seed_spacing, w.seed_periodic, w.period, w.seeds(), t_start, T, h)
+        for k in range(len(t_start)):
+            cgg, ftg, stg = gpu_cg(w, Fs[k].contiguous(), fls[k].contiguous(), T=T)
+            assert np.array_equal(fth[k], cpu(ftg), equal_nan=True)
+    if case in ("backward_ring", "forward_chunks"):
+        k = len(t_start) - 1
+        fo = oracle.OracleField.from_workload(w)
+        Fo, flo, eso = fo.advect(w.seeds().astype(np.float64), t_start[k], t_start[k] + T, h)
+        cgo, fto, sto = oracle_cg(oracle, w, Fo, flo, T=T)
+        cgg, ftg, stg = gpu_cg(w, Fs[k].contiguous(), fls[k].contiguous(), T=T)
+        gate_statistical(cpu(Fs[k]), Fo, cpu(ftg), fto, w.L, cpu(fls[k]), flo)
+    # the series needs a reservation that covers all overlapping volumes
+    f2 = lcs.Field.from_workload(w)
+    for k, v in opts.items():
+        f2.set_option(k, v)
+    f2.reserve(sd.shape[0], abs(int(round(T / h))))
+    if case in ("backward_ring", "forward_chunks", "nonperiodic_exits"):
+        with pytest.raises(lcs.LcsError) as e:
+            f2.advect_series(sd, t_start, T, h, reserve=False)
+        assert e.value.status == 4
+
+
 # -------------------------------------------------------------------------------------------------
 # closed forms directly on the GPU path, all mesh kinds and dtypes
 @pytest.mark.parametrize("mesh", ["cart2", "cart3", "tri", "tet"])
