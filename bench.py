@@ -293,8 +293,9 @@ def run_config(args, lcs, cfg, steps, warmup, rank, world, local, with_e2e, with
     w, runs = make_workload(cfg, rank)
     ring = 4 if cfg == 5 else 0
     field = lcs.Field.from_workload(w, max_resident_snapshots=ring, pinned=True)
-    if cfg == 5:
-        field.set_option("field_sets", 12)               # time series: consecutive volumes share 9 of their 10 windows
+    series = cfg == 5 and args.cfg5_mode == "series"     # the 16 volumes advanced together through every window (lcs_advect_series)
+    if cfg == 5 and not series:
+        field.set_option("field_sets", 12)               # volume by volume: consecutive volumes share 9 of their 10 windows
     for kv in args.option:
         k, v = kv.split("=")
         field.set_option(k, int(v))
@@ -307,10 +308,25 @@ def run_config(args, lcs, cfg, steps, warmup, rank, world, local, with_e2e, with
     es = torch.empty(n, dtype=torch.int32, device="cuda")
     stream = torch.cuda.current_stream()
     # set-up: everything lcs_advect needs is allocated here, once (the hot calls never allocate)
-    field.reserve(n, max(int(round((tf - t0) / h)) for (t0, tf, h) in runs))
+    if series:
+        t_starts = [t0 for (t0, tf, h) in runs]
+        T_ser, h_ser = runs[0][1] - runs[0][0], runs[0][2]
+        flows = torch.empty((len(runs), n, w.dim), dtype=tdt, device="cuda")
+        flags = torch.empty((len(runs), n), dtype=torch.uint8, device="cuda")
+        ess = torch.empty((len(runs), n), dtype=torch.int32, device="cuda")
+        field.advect_series(seeds_d, t_starts, T_ser, h_ser, flowmaps=flows, exit_flags=flags, exit_steps=ess)      # reserves
+    else:
+        field.reserve(n, max(int(round((tf - t0) / h)) for (t0, tf, h) in runs))
 
     def one_pass(count=None):
         """All rows of the hot path over one batch: flow map(s) -> CG -> FTLE."""
+        if series:
+            field.advect_series(seeds_d, t_starts, T_ser, h_ser, flowmaps=flows, exit_flags=flags, exit_steps=ess, reserve=False)
+            for k in range(len(runs)):
+                lcs.cg_ftle(w.dim, w.ng, w.seed_spacing, w.seed_periodic, w.period, flows[k], flags[k], T_ser, want_cg=True, want_status=False)
+            if count is not None:
+                count.append(float(ess.sum(dtype=torch.int64).item()))
+            return
         if cfg == 5:
             field.set_option("field_sets_clear", 0)      # every pass starts without resident blended fields: reuse only WITHIN a pass
         for (t0, tf, h) in runs:
@@ -379,7 +395,15 @@ def run_config(args, lcs, cfg, steps, warmup, rank, world, local, with_e2e, with
         esz = seeds_h.element_size()
         e_steps = steps if cfg == args.config else min(steps, 5)
 
+        if series:
+            ftle_h = torch.empty((len(runs), n), dtype=tdt).pin_memory()
+            cg_h = torch.empty((len(runs), n, ncg), dtype=tdt).pin_memory()
+
         def e2e_pass():
+            if series:
+                field.ftle_series_host(w.ng, w.seed_spacing, w.seed_periodic, w.period, seeds_h.numpy(), t_starts, T_ser, h_ser,
+                                       ftle=ftle_h.numpy(), cg=cg_h.numpy())
+                return
             if cfg == 5:
                 field.set_option("field_sets_clear", 0)
             for (t0, tf, h) in runs:
@@ -417,7 +441,8 @@ def run_config(args, lcs, cfg, steps, warmup, rank, world, local, with_e2e, with
                 "dtype": "f32" if w.compute_dtype == np.float32 else "f64", "data": "synthetic",
                 "config": {"workload": w.name, "baseline_config": cfg, "seeds": n * len(runs), "rk4_steps": w.n_steps,
                            "seed_steps_per_pass": steps_per_pass, "parallelism": "independent FTLE volumes per rank, no collective",
-                           "options": dict(kv.split("=") for kv in args.option), "l2": l2_note},
+                           "options": dict(kv.split("=") for kv in args.option), "l2": l2_note,
+                           **({"series": "lcs_advect_series: %d volumes, overlapping ones advanced together" % len(runs)} if series else {})},
                 "seeds_per_s_to_ftle": seeds_all / sec_per_step, "roofline": roofline, "clocks": clocks, "gpu_launches": int(launches),
                 "e2e": e2e}
         if with_cpu and world == 1:
@@ -440,6 +465,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--option", action="append", default=[], help="library option key=value (e.g. integrator=2)")
+    ap.add_argument("--cfg5-mode", default="series", choices=["series", "volumes"],
+                    help="config 5: lcs_advect_series (overlapping volumes advanced together) or one lcs_advect per volume with resident field sets")
     args = ap.parse_args()
     if args.impl == "reference":
         return reference_arm(args)
