@@ -792,6 +792,42 @@ def test_config5_full_size_series_with_field_sets(lcs, oracle):
     assert frac >= 0.999 and np.median(rel) <= 1e-3
 
 
+@pytest.mark.slow
+def test_config5_full_size_advect_series(lcs, oracle):
+    """Config 5 at full size as bench.py times it by default: lcs_advect_series on a ring of 4 device slots fed from pinned host
+    memory.  Four consecutive volumes (192^3 seeds each, backward 500 steps, released one snapshot interval apart) advanced
+    together: up to four volumes share a launch.  The first and the last volume must equal, bit for bit, the lcs_advect of that
+    volume alone on a fresh field; the last one passes the statistical gate against 6 seeded 18^3 oracle blocks, one of them
+    across the periodic seam."""
+    import torch
+    w = I.config5()
+    f = lcs.Field.from_workload(w, max_resident_snapshots=4, pinned=True)
+    sd = torch.from_numpy(w.seeds()).cuda()
+    vols = w.meta["windows"][5:9]
+    t_start = [a for (a, b) in vols]
+    T = vols[0][1] - vols[0][0]
+    Fs, fls, ess = f.advect_series(sd, t_start, T, w.h)
+    torch.cuda.synchronize()
+    assert f.info("series_layers") == 13 and f.info("ring") == 1 and f.info("h2d_bytes") > 0 and int(fls.max()) == 0
+    f0 = lcs.Field.from_workload(w, max_resident_snapshots=4, pinned=True)
+    for k in (0, 3):
+        F0, flag0, es0 = f0.advect(sd, t_start[k], t_start[k] + T, w.h)
+        assert torch.equal(F0, Fs[k]) and torch.equal(flag0, fls[k]) and torch.equal(es0, ess[k]), k
+    f0.close()
+    F, flag = Fs[3].contiguous(), fls[3].contiguous()
+    cgg, ftg, stg = gpu_cg(w, F, flag, T=T)
+    fo = oracle.OracleField.from_workload(w)
+    rng = np.random.default_rng(56)
+    B = 18
+    n = w.ng[0]
+    blocks = [tuple(int(v) for v in rng.integers(0, n - B, 3)) for _ in range(5)] + [(n - 9, n - 5, n - 12)]
+    err, rel = compare_periodic_blocks(oracle, w, fo, F, ftg, blocks, B, t_start[3], t_start[3] + T, w.h)
+    frac = np.mean(err <= 1e-3 * w.L)
+    print("config5 full (lcs_advect_series, volume 8 of 4): frac_ok %.5f median FTLE rel %.3e mean err %.3e max %.3e" % (frac, np.median(rel), err.mean(), err.max()))
+    assert frac >= 0.999 and np.median(rel) <= 1e-3
+    f.close()
+
+
 # -------------------------------------------------------------------------------------------------
 # row f2: full eigen-decomposition of C
 @pytest.mark.parametrize("dim", [2, 3])
