@@ -654,7 +654,8 @@ simplex_window_kernel(const CellRec<DIM, TC> *__restrict__ crec, const int32_t *
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const int64_t stride = SLOW ? (int64_t)gridDim.x * blockDim.x : n;
     const int64_t count = SLOW ? (int64_t)*pend.count : n;
-    for (; i < count; i += stride) {
+    if (i >= count) return;
+    do {
         const int64_t slot = SLOW ? (int64_t)pend.index[i] : i;
         SimplexTracer<DIM, TC> t = load_tracer(st + slot);
         if ((t.meta >> 30) != (SLOW ? 3u : 0u)) continue;
@@ -692,7 +693,7 @@ simplex_window_kernel(const CellRec<DIM, TC> *__restrict__ crec, const int32_t *
         t.meta = rc ? ((uint32_t)(rc == 2 ? 3u : 1u) << 30) | (uint32_t)(first_step + s) : 0u;
         if (!SLOW && rc == 2) pend.index[atomicAdd(pend.count, 1u)] = (int32_t)slot;
         store_tracer(st + slot, t);
-    }
+    } while (SLOW && (i += stride) < count);
 }
 
 // Adams-Bashforth 4 with an RK4 start-up on simplicial meshes (row f4, reading #31): as simplex_window_kernel,
@@ -707,7 +708,8 @@ simplex_ab4_kernel(const CellRec<DIM, TC> *__restrict__ crec, const int32_t *__r
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const int64_t stride = SLOW ? (int64_t)gridDim.x * blockDim.x : n;
     const int64_t count = SLOW ? (int64_t)*pend.count : n;
-    for (; i < count; i += stride) {
+    if (i >= count) return;
+    do {
         const int64_t slot = SLOW ? (int64_t)pend.index[i] : i;
         SimplexTracer<DIM, TC> t = load_tracer(st + slot);
         if ((t.meta >> 30) != (SLOW ? 3u : 0u)) continue;
@@ -765,7 +767,7 @@ simplex_ab4_kernel(const CellRec<DIM, TC> *__restrict__ crec, const int32_t *__r
         t.meta = rc ? ((uint32_t)(rc == 2 ? 3u : 1u) << 30) | (uint32_t)(first_step + s) : 0u;
         if (!SLOW && rc == 2) pend.index[atomicAdd(pend.count, 1u)] = (int32_t)slot;
         store_tracer(st + slot, t);
-    }
+    } while (SLOW && (i += stride) < count);
 }
 
 // ---------------------------------------------------------------------------------------------
