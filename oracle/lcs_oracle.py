@@ -2,7 +2,10 @@
 
 Allowed users of this module: tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
 --impl reference legs, nothing else.  The CUDA binding (paper_2209_13775_b200.lcs) is never loaded
-from here and no code is shared with it.  Argument marshalling only: all arithmetic is in lcs_oracle.c.
+from here and no code is shared with it.  Argument marshalling only: the arithmetic is in lcs_oracle.c, with one exception:
+the update rule of oracle rule O10 (early Cauchy-Green evaluation: which seeds are re-evaluated at an evaluation point and which
+keep their last result) is the numpy mask bookkeeping of `advect_early_cg` below, written from DESIGN.md reading #29; every
+evaluation it triggers is the C routine orc_cg_ftle.
 """
 from __future__ import annotations
 
