@@ -444,6 +444,28 @@ def test_argument_errors_and_empty(lcs):
     assert e.value.status == 6
 
 
+def test_advect_series_arguments_and_single_volume(lcs):
+    """lcs_advect_series: argument errors (sign of h against T, interval outside the snapshot times, empty series, resident
+    field sets), and a one-volume series, which is lcs_advect."""
+    import torch
+    w = I.config3(ngrid=16, nn=16, T=1.0, h=0.01, n_snap=5)
+    f = lcs.Field.from_workload(w)
+    for k, v in dict(bundle=1, preblend=1).items():
+        f.set_option(k, v)
+    sd = torch.from_numpy(w.seeds()).cuda()
+    for (ts, T, h, status) in (([0.0, 0.5], 1.0, -0.01, 1), ([0.0, 0.5], 1.0, 0.0, 1), ([0.0, 1.5], 1.0, 0.01, 2), ([], 1.0, 0.01, 1)):
+        with pytest.raises(lcs.LcsError) as e:
+            f.advect_series(sd, ts, T, h)
+        assert e.value.status == status, (ts, T, h, str(e.value))
+    Fs, fls, ess = f.advect_series(sd, [0.5], 1.0, 0.01)
+    F, fl, es = f.advect(sd, 0.5, 1.5, 0.01)
+    assert f.info("series_layers") == 0 and torch.equal(Fs[0], F) and torch.equal(ess[0], es)
+    f.set_option("field_sets", 2)
+    with pytest.raises(lcs.LcsError) as e:
+        f.advect_series(sd, [0.0, 0.5], 1.0, 0.01)
+    assert e.value.status == 1
+
+
 def test_aliasing_and_host_api(lcs, oracle):
     """flowmap may alias seeds; lcs_ftle_host (host buffers, copies inside the call) equals the device path."""
     import torch
