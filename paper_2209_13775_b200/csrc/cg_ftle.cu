@@ -185,37 +185,64 @@ __global__ void __launch_bounds__(256) cg_ftle3f_kernel(const __grid_constant__ 
 {
     const int i0 = (int)(blockIdx.x * blockDim.x + threadIdx.x);
     if (i0 >= g.ng[0]) return;
+    const unsigned lanes = __activemask();
     const int n0 = g.ng[0], n1 = g.ng[1], n2 = g.ng[2];
     const int ijk[3] = {i0, (int)blockIdx.y, (int)blockIdx.z};
     const int nn[3] = {n0, n1, n2};
     const int stride[3] = {1, n0, n0 * n1};
     const int idx = i0 + n0 * (ijk[1] + n1 * ijk[2]);
-    const float *Fc = F + 3 * idx;
-    const float F0[3] = {Fc[0], Fc[1], Fc[2]};
-    unsigned st = (flag && flag[idx] != 0) ? 1u : 0u;
-    double G[3][3];
+    // in-grid neighbours (by wrap on a periodic axis), their flags
+    bool atp[3], atm[3], okp[3], okm[3];
+    int jp[3], jm[3];
+    bool all_ok = !(flag && flag[idx] != 0);
 #pragma unroll
     for (int b = 0; b < 3; ++b) {
-        // in-grid neighbours (by wrap on a periodic axis) and the period carried by a wrapped one
-        const bool atp = ijk[b] + 1 >= nn[b], atm = ijk[b] == 0;
-        bool okp = !atp || g.per[b], okm = !atm || g.per[b];
-        const int dp = (atp ? 1 - nn[b] : 1) * stride[b], dm = (atm ? nn[b] - 1 : -1) * stride[b];
-        const int jp = okp ? idx + dp : idx, jm = okm ? idx + dm : idx;        // a valid address in every case
-        const float *Pp = F + 3 * jp, *Pm = F + 3 * jm;
-        const float fp[3] = {Pp[0], Pp[1], Pp[2]}, fm[3] = {Pm[0], Pm[1], Pm[2]};
-        if (flag) { okp = okp && flag[jp] == 0; okm = okm && flag[jm] == 0; }
-        const double shift = ((okp && atp) ? g.period[b] : 0.0) + ((okm && atm) ? g.period[b] : 0.0);
-        const double scale = (okp && okm) ? 0.5 * g.inv_dx[b] : ((okp || okm) ? g.inv_dx[b] : 0.0);
+        atp[b] = ijk[b] + 1 >= nn[b];
+        atm[b] = ijk[b] == 0;
+        okp[b] = !atp[b] || g.per[b];
+        okm[b] = !atm[b] || g.per[b];
+        jp[b] = okp[b] ? idx + (atp[b] ? 1 - nn[b] : 1) * stride[b] : idx;        // a valid address in every case
+        jm[b] = okm[b] ? idx + (atm[b] ? nn[b] - 1 : -1) * stride[b] : idx;
+        if (flag) { okp[b] = okp[b] && flag[jp[b]] == 0; okm[b] = okm[b] && flag[jm[b]] == 0; }
+        all_ok = all_ok && okp[b] && okm[b];
+    }
+    double G[3][3];
+    unsigned st = 0;
+    if (__all_sync(lanes, all_ok)) {
+        // every seed of the warp has its full stencil (the whole of configs 3 and 5): central differences without selects
 #pragma unroll
-        for (int a = 0; a < 3; ++a) {
-            const float hi = okp ? fp[a] : F0[a], lo = okm ? fm[a] : F0[a];
-            double d = (double)hi - (double)lo;
-            if (a == b) d += shift;
-            G[a][b] = d * scale;
+        for (int b = 0; b < 3; ++b) {
+            const float *Pp = F + 3 * jp[b], *Pm = F + 3 * jm[b];
+            const double shift = (atp[b] ? g.period[b] : 0.0) + (atm[b] ? g.period[b] : 0.0);
+            const double scale = 0.5 * g.inv_dx[b];
+#pragma unroll
+            for (int a = 0; a < 3; ++a) {
+                double d = (double)Pp[a] - (double)Pm[a];
+                if (a == b) d += shift;
+                G[a][b] = d * scale;
+            }
         }
-        if (!(st & 1u)) {
-            if (!okp && !okm) st |= 1u;
-            else if (!(okp && okm)) st |= 2u;
+    } else {
+        const float *Fc = F + 3 * idx;
+        const float F0[3] = {Fc[0], Fc[1], Fc[2]};
+        st = (flag && flag[idx] != 0) ? 1u : 0u;
+#pragma unroll
+        for (int b = 0; b < 3; ++b) {
+            const float *Pp = F + 3 * jp[b], *Pm = F + 3 * jm[b];
+            const float fp[3] = {Pp[0], Pp[1], Pp[2]}, fm[3] = {Pm[0], Pm[1], Pm[2]};
+            const double shift = ((okp[b] && atp[b]) ? g.period[b] : 0.0) + ((okm[b] && atm[b]) ? g.period[b] : 0.0);
+            const double scale = (okp[b] && okm[b]) ? 0.5 * g.inv_dx[b] : ((okp[b] || okm[b]) ? g.inv_dx[b] : 0.0);
+#pragma unroll
+            for (int a = 0; a < 3; ++a) {
+                const float hi = okp[b] ? fp[a] : F0[a], lo = okm[b] ? fm[a] : F0[a];
+                double d = (double)hi - (double)lo;
+                if (a == b) d += shift;
+                G[a][b] = d * scale;
+            }
+            if (!(st & 1u)) {
+                if (!okp[b] && !okm[b]) st |= 1u;
+                else if (!(okp[b] && okm[b])) st |= 2u;
+            }
         }
     }
     float c[6], ft;
