@@ -309,9 +309,10 @@ template <int DIM>
 __device__ __forceinline__ int32_t locate_canonical(const BinGrid &b, const int32_t *__restrict__ bins, const double *__restrict__ verts,
                                                     const int32_t *__restrict__ cells, const int32_t *__restrict__ neigh,
                                                     const uint8_t *__restrict__ oppside, int64_t nc, int64_t hop_cap, const double *p,
-                                                    unsigned long long *__restrict__ stats)
+                                                    unsigned long long *__restrict__ stats, int64_t start = -1)
 {
-    int64_t c = bins[bin_of<DIM>(b, p)];
+    // the owner is unique, so any start cell gives the same answer; the bin grid is the default
+    int64_t c = start >= 0 ? start : (int64_t)bins[bin_of<DIM>(b, p)];
     if (c < 0) c = 0;
     for (int64_t hop = 0; hop < hop_cap; ++hop) {
         bool beyond;
@@ -432,26 +433,6 @@ template <typename REC> __device__ __forceinline__ void store_tracer(REC *p, con
     for (int k = 0; k < NQ; ++k) d[k] = s[k];
 }
 
-template <int DIM, typename TC>
-__global__ void __launch_bounds__(128) simplex_init_kernel(BinGrid b, const int32_t *__restrict__ bins, const double *__restrict__ verts,
-                                                            const int32_t *__restrict__ cells, const int32_t *__restrict__ neigh,
-                                                            const uint8_t *__restrict__ oppside, int64_t nc, int64_t hop_cap,
-                                                            const TC *__restrict__ seeds, int64_t n, SimplexTracer<DIM, TC> *__restrict__ st,
-                                                            unsigned long long *__restrict__ stats)
-{
-    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    SimplexTracer<DIM, TC> t;
-    double p[DIM];
-#pragma unroll
-    for (int k = 0; k < DIM; ++k) { TC v = seeds[i * DIM + k]; t.x[k] = v; p[k] = (double)v; }
-    int32_t c = locate_canonical<DIM>(b, bins, verts, cells, neigh, oppside, nc, hop_cap, p, stats);
-    t.cell = c;
-    t.orig = (int32_t)i;
-    t.meta = c < 0 ? (2u << 30) : 0u;
-    store_tracer(st + i, t);
-}
-
 // sort key: Morton code of the tracer's bin (bin grid coarsened by `shift`); finished tracers go to the last bin so
 // that live tracers stay compacted at the front and whole warps of finished ones retire at once
 template <int DIM, typename TC>
@@ -547,6 +528,81 @@ __device__ __forceinline__ void load_vertex(const PairRec<DIM, TV> *__restrict__
     load_words<NB>(rec + v, w);
 #pragma unroll
     for (int k = 0; k < DIM; ++k) { a[k] = (TC)word_value<TV>(w, k); d[k] = (TC)word_value<TV>(w, P + k); }
+}
+
+// Seeds -> tracer records with their canonical cells (flag 2 = outside at t0).  The owner is decided by the canonical fp64
+// predicate, as in lcs_locate; to get there cheaply the walk first runs on the per-cell affine maps in the compute type (one
+// 64-byte record and a dozen FMAs per hop instead of four fp64 face predicates on gathered vertex coordinates) and hands its
+// last cell to the canonical walk; a seed that the affine map places strictly inside its cell, by more than the rounding-error
+// bound of its weights, needs no canonical probe at all (the owner is the same: there is no tie to break).
+template <int DIM, typename TC>
+__global__ void __launch_bounds__(128) simplex_init_kernel(BinGrid b, const int32_t *__restrict__ bins, const double *__restrict__ verts,
+                                                            const int32_t *__restrict__ cells, const int32_t *__restrict__ neigh,
+                                                            const uint8_t *__restrict__ oppside, const CellRec<DIM, TC> *__restrict__ crec,
+                                                            int64_t nc, int64_t hop_cap, const TC *__restrict__ seeds, int64_t n,
+                                                            SimplexTracer<DIM, TC> *__restrict__ st, unsigned long long *__restrict__ stats)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    SimplexTracer<DIM, TC> t;
+    double p[DIM];
+    TC pc[DIM];
+#pragma unroll
+    for (int k = 0; k < DIM; ++k) { TC v = seeds[i * DIM + k]; t.x[k] = v; pc[k] = v; p[k] = (double)v; }
+    int32_t c = bins[bin_of<DIM>(b, p)];
+    if (c < 0) c = 0;
+    bool certain = false;
+    for (int hop = 0; hop < 16; ++hop) {
+        CellRec<DIM, TC> r;
+        load_cellrec<DIM, TC>(crec, c, r);
+        TC q[DIM], sum = TC(0), lmin;
+#pragma unroll
+        for (int k = 0; k < DIM; ++k) q[k] = pc[k] - r.v0[k];
+        int jmin = 0;
+        TC lam[DIM + 1];
+#pragma unroll
+        for (int a = 0; a < DIM; ++a) {
+            TC l = TC(0);
+#pragma unroll
+            for (int k = 0; k < DIM; ++k) l = fma(r.M[a * DIM + k], q[k], l);
+            lam[a + 1] = l;
+            sum += l;
+        }
+        lam[0] = TC(1) - sum;
+        lmin = lam[0];
+#pragma unroll
+        for (int a = 1; a <= DIM; ++a)
+            if (lam[a] < lmin) { lmin = lam[a]; jmin = a; }
+        if (lmin >= TC(0)) {
+            // Certainly the owner?  Rounding-error bound of the weights computed above: the map entries and v0 are roundings of
+            // exact values (relative eps each), q and the FMA chain add a few eps of the term magnitudes:
+            // |lam_i - exact| <= 8 eps sum_k |M_ik| (|q_k| + |v0_k|) for i >= 1, their sum (+ eps) for lam_0.  A point whose weights
+            // all exceed four times their bounds is strictly inside this cell, so the canonical predicate (which has no tie to break
+            // there) names the same owner and is skipped; everything nearer to a face goes through it.
+            const TC eps = sizeof(TC) == 4 ? TC(5.9604645e-8) : TC(1.1102230246251565e-16);
+            TC e0 = eps;
+            certain = true;
+#pragma unroll
+            for (int a = 0; a < DIM; ++a) {
+                TC e = TC(0);
+#pragma unroll
+                for (int k = 0; k < DIM; ++k) e = fma(fabs(r.M[a * DIM + k]), fabs(q[k]) + fabs(r.v0[k]), e);
+                e *= TC(8) * eps;
+                e0 += e;
+                certain = certain && lam[a + 1] > TC(4) * e;
+            }
+            certain = certain && lam[0] > TC(4) * e0;
+            break;
+        }
+        const int32_t nb = __ldg(neigh + (int64_t)c * (DIM + 1) + jmin);
+        if (nb < 0) break;
+        c = nb;
+    }
+    if (!certain) c = locate_canonical<DIM>(b, bins, verts, cells, neigh, oppside, nc, hop_cap, p, stats, c);
+    t.cell = c;
+    t.orig = (int32_t)i;
+    t.meta = c < 0 ? (2u << 30) : 0u;
+    store_tracer(st + i, t);
 }
 
 // What the in-advect walk needs when it gives up: the canonical (fp64) locator of lcs_locate.
@@ -1108,8 +1164,8 @@ lcs_status simplex_advect_impl(lcs_field *f, int64_t n, const void *seeds_, doub
     uint32_t *d_key = (uint32_t *)(base + L.o_key), *d_cnt = (uint32_t *)(base + L.o_cnt), *d_tile = (uint32_t *)(base + L.o_tile);
     BinGrid b = make_bins(f);
     const CanonCtx cx{b, m.bins, m.verts, m.cells, m.neigh, m.oppside, m.nc, m.hop_cap, m.stats};
-    LCS_LAUNCH((simplex_init_kernel<DIM, TC>), lcs_blocks(n, 128), 128, 0, st, b, m.bins, m.verts, m.cells, m.neigh, m.oppside, m.nc,
-               m.hop_cap, seeds, n, cur, m.stats);
+    LCS_LAUNCH((simplex_init_kernel<DIM, TC>), lcs_blocks(n, 128), 128, 0, st, b, m.bins, m.verts, m.cells, m.neigh, m.oppside,
+               (const CellRec<DIM, TC> *)m.cellrec, m.nc, m.hop_cap, seeds, n, cur, m.stats);
     const int block = f->opt_block ? (int)(f->opt_block > 128 ? 128 : f->opt_block) : 128;
     const int dir = h > 0 ? 1 : -1;
     using VRec = PairRec<DIM, TV>;
