@@ -291,7 +291,7 @@ def run_config(args, lcs, cfg, steps, warmup, rank, world, local, with_e2e, with
     import torch
     import torch.distributed as dist
     w, runs = make_workload(cfg, rank)
-    ring = 4 if cfg == 5 else 0
+    ring = args.cfg5_ring if cfg == 5 else 0          # config 5 streams its snapshots from pinned host memory through a ring of device slots
     field = lcs.Field.from_workload(w, max_resident_snapshots=ring, pinned=True)
     series = cfg == 5 and args.cfg5_mode == "series"     # the 16 volumes advanced together through every window (lcs_advect_series)
     if cfg == 5 and not series:
@@ -442,7 +442,8 @@ def run_config(args, lcs, cfg, steps, warmup, rank, world, local, with_e2e, with
                 "config": {"workload": w.name, "baseline_config": cfg, "seeds": n * len(runs), "rk4_steps": w.n_steps,
                            "seed_steps_per_pass": steps_per_pass, "parallelism": "independent FTLE volumes per rank, no collective",
                            "options": dict(kv.split("=") for kv in args.option), "l2": l2_note,
-                           **({"series": "lcs_advect_series: %d volumes, overlapping ones advanced together" % len(runs)} if series else {})},
+                           **({"series": "lcs_advect_series: %d volumes, overlapping ones advanced together" % len(runs)} if series else {}),
+                           **({"snapshot_ring_slots": ring, "h2d_snapshot_bytes_total": int(field.info("h2d_bytes"))} if cfg == 5 else {})},
                 "seeds_per_s_to_ftle": seeds_all / sec_per_step, "roofline": roofline, "clocks": clocks, "gpu_launches": int(launches),
                 "e2e": e2e}
         if with_cpu and world == 1:
@@ -465,6 +466,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--option", action="append", default=[], help="library option key=value (e.g. integrator=2)")
+    ap.add_argument("--cfg5-ring", type=int, default=4, help="config 5: device slots of the snapshot ring (0 = every snapshot resident, no streaming)")
     ap.add_argument("--cfg5-mode", default="series", choices=["series", "volumes"],
                     help="config 5: lcs_advect_series (overlapping volumes advanced together) or one lcs_advect per volume with resident field sets")
     args = ap.parse_args()
