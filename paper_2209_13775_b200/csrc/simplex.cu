@@ -645,7 +645,13 @@ __device__ __forceinline__ int simplex_velocity(const CellRec<DIM, TC> *__restri
     if (h.pair != (const void *)vrec) { h.vel = false; h.pair = vrec; }        // uniform: another snapshot pair
     bool forced = false;
     for (int hop = 0;; ++hop) {
-        if (h.cell != c) { load_cellrec<DIM, TC>(crec, c, h.r); h.cell = c; h.vel = false; }
+        if (h.cell != c) {
+            load_cellrec<DIM, TC>(crec, c, h.r);
+            // the neighbour row of the new cell will be wanted by the next hop out of it: bring its line into L1 now
+            asm volatile("prefetch.global.L1 [%0];" ::"l"(neigh + (int64_t)c * (DIM + 1)));
+            h.cell = c;
+            h.vel = false;
+        }
         TC q[DIM];
 #pragma unroll
         for (int k = 0; k < DIM; ++k) q[k] = p[k] - h.r.v0[k];
