@@ -635,15 +635,19 @@ template <int DIM, typename TC> __device__ __forceinline__ int32_t walk_fallback
 // in its owner: a tracer is never interpolated in a cell that does not hold it ("walk_cap_hits" stays 0 by construction),
 // and the rare path costs the hot kernel neither registers nor code.
 constexpr int kWalkCap = 24;
-template <int DIM, typename TV, typename TC, bool SLOW>
+template <int DIM, typename TV, typename TC, bool SLOW, bool ONE_PAIR = false>
 __device__ __forceinline__ int simplex_velocity(const CellRec<DIM, TC> *__restrict__ crec, const int32_t *__restrict__ neigh,
                                                  const PairRec<DIM, TV> *__restrict__ vrec, TC tau, const TC *p, int32_t *cell,
                                                  HeldSimplex<DIM, TV, TC> &h, const CanonCtx &cx, TC *u)
 {
     int32_t c = *cell;
     TC lam[DIM + 1];
-    if (h.pair != (const void *)vrec) { h.vel = false; h.pair = vrec; }        // uniform: another snapshot pair
-    bool forced = false;
+    // ONE_PAIR: every stage of the launch reads the same snapshot pair (the usual window), so the held vertex records can only
+    // be stale right after a cell change inside this call: no pair bookkeeping, and the vertex ids die with the reload
+    if constexpr (!ONE_PAIR) {
+        if (h.pair != (const void *)vrec) { h.vel = false; h.pair = vrec; }    // uniform: another snapshot pair
+    }
+    bool forced = false, fresh = false;
     for (int hop = 0;; ++hop) {
         if (h.cell != c) {
             load_cellrec<DIM, TC>(crec, c, h.r);
@@ -651,6 +655,7 @@ __device__ __forceinline__ int simplex_velocity(const CellRec<DIM, TC> *__restri
             asm volatile("prefetch.global.L1 [%0];" ::"l"(neigh + (int64_t)c * (DIM + 1)));
             h.cell = c;
             h.vel = false;
+            fresh = true;
         }
         TC q[DIM];
 #pragma unroll
@@ -683,7 +688,7 @@ __device__ __forceinline__ int simplex_velocity(const CellRec<DIM, TC> *__restri
         c = nb;
     }
     *cell = c;
-    if (!h.vel) {
+    if (ONE_PAIR ? fresh : !h.vel) {
 #pragma unroll
         for (int i = 0; i <= DIM; ++i) load_vertex<DIM, TV, TC>(vrec, h.r.vid[i], h.a[i], h.d[i]);
         h.vel = true;
@@ -706,7 +711,7 @@ struct Pending {
     int32_t *index;           // their slots in the tracer array
 };
 
-template <int DIM, typename TV, typename TC, bool SLOW>
+template <int DIM, typename TV, typename TC, bool SLOW, bool ONE_PAIR = false>
 __global__ void __launch_bounds__(128, (sizeof(TC) == 4 && !SLOW ? 7 : 1))
 simplex_window_kernel(const CellRec<DIM, TC> *__restrict__ crec, const int32_t *__restrict__ neigh, const PairRec<DIM, TV> *__restrict__ pa,
                       const PairRec<DIM, TV> *__restrict__ pb, const PairRec<DIM, TV> *__restrict__ pc, const TC *__restrict__ tau,
@@ -732,19 +737,19 @@ simplex_window_kernel(const CellRec<DIM, TC> *__restrict__ crec, const int32_t *
             // the running sum k1 + 2 k2 + 2 k3 instead of the four slopes: six registers fewer live at stage 4
             TC acc[DIM], u[DIM], y[DIM];
             int32_t c = cell;
-            rc = simplex_velocity<DIM, TV, TC, SLOW>(crec, neigh, pa, ta, x, &c, held, cx, acc);
+            rc = simplex_velocity<DIM, TV, TC, SLOW, ONE_PAIR>(crec, neigh, pa, ta, x, &c, held, cx, acc);
             if (rc) break;
 #pragma unroll
             for (int k = 0; k < DIM; ++k) y[k] = fma(TC(0.5) * h, acc[k], x[k]);
-            rc = simplex_velocity<DIM, TV, TC, SLOW>(crec, neigh, pb, tb, y, &c, held, cx, u);
+            rc = simplex_velocity<DIM, TV, TC, SLOW, ONE_PAIR>(crec, neigh, pb, tb, y, &c, held, cx, u);
             if (rc) break;
 #pragma unroll
             for (int k = 0; k < DIM; ++k) { y[k] = fma(TC(0.5) * h, u[k], x[k]); acc[k] = fma(TC(2), u[k], acc[k]); }
-            rc = simplex_velocity<DIM, TV, TC, SLOW>(crec, neigh, pb, tb, y, &c, held, cx, u);
+            rc = simplex_velocity<DIM, TV, TC, SLOW, ONE_PAIR>(crec, neigh, pb, tb, y, &c, held, cx, u);
             if (rc) break;
 #pragma unroll
             for (int k = 0; k < DIM; ++k) { y[k] = fma(h, u[k], x[k]); acc[k] = fma(TC(2), u[k], acc[k]); }
-            rc = simplex_velocity<DIM, TV, TC, SLOW>(crec, neigh, pc, tc, y, &c, held, cx, u);
+            rc = simplex_velocity<DIM, TV, TC, SLOW, ONE_PAIR>(crec, neigh, pc, tc, y, &c, held, cx, u);
             if (rc) break;
 #pragma unroll
             for (int k = 0; k < DIM; ++k) x[k] = fma(h * TC(1.0 / 6.0), acc[k] + u[k], x[k]);
@@ -1231,6 +1236,9 @@ lcs_status simplex_advect_impl(lcs_field *f, int64_t n, const void *seeds_, doub
                     LCS_LAUNCH((simplex_ab4_kernel<DIM, TV, TC, false>), lcs_blocks(n, block), block, 0, st, (const CellRec<DIM, TC> *)m.cellrec, m.neigh,
                                (const VRec *)p[0], (const VRec *)p[1], (const VRec *)p[2], d_tau + 3 * (size_t)first, cnt, first, n, cur,
                                (TC *)(base + L.o_hist), (TC)h, cx, pend);
+                else if (p[0] == p[1] && p[1] == p[2])
+                    LCS_LAUNCH((simplex_window_kernel<DIM, TV, TC, false, true>), lcs_blocks(n, block), block, 0, st, (const CellRec<DIM, TC> *)m.cellrec, m.neigh,
+                               (const VRec *)p[0], (const VRec *)p[1], (const VRec *)p[2], d_tau + 3 * (size_t)first, cnt, first, n, cur, (TC)h, cx, pend);
                 else
                     LCS_LAUNCH((simplex_window_kernel<DIM, TV, TC, false>), lcs_blocks(n, block), block, 0, st, (const CellRec<DIM, TC> *)m.cellrec, m.neigh,
                                (const VRec *)p[0], (const VRec *)p[1], (const VRec *)p[2], d_tau + 3 * (size_t)first, cnt, first, n, cur, (TC)h, cx, pend);
