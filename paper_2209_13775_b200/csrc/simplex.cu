@@ -712,7 +712,7 @@ struct Pending {
 };
 
 template <int DIM, typename TV, typename TC, bool SLOW, bool ONE_PAIR = false>
-__global__ void __launch_bounds__(128, (sizeof(TC) == 4 && !SLOW ? 7 : 1))
+__global__ void __launch_bounds__(128, (SLOW ? 1 : (sizeof(TC) == 4 ? 7 : (DIM == 2 ? 5 : 1))))
 simplex_window_kernel(const CellRec<DIM, TC> *__restrict__ crec, const int32_t *__restrict__ neigh, const PairRec<DIM, TV> *__restrict__ pa,
                       const PairRec<DIM, TV> *__restrict__ pb, const PairRec<DIM, TV> *__restrict__ pc, const TC *__restrict__ tau,
                       int nsteps, int first_step, int64_t n, SimplexTracer<DIM, TC> *__restrict__ st, TC h,
