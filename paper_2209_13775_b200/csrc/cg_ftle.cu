@@ -47,9 +47,14 @@ __device__ __forceinline__ double eigmax_sym3(double c11, double c12, double c13
 // (acos, cos, log: some hundred instructions each on the half-rate FP64 pipe, which made this HBM-streaming kernel FP64-bound
 // at 20% of the HBM peak) are replaced: the trigonometric step runs in fp32 and its result is polished by one Newton step on the
 // characteristic polynomial det(C - lambda I) in fp64 (taken only when it is a small correction: near a double root the
-// derivative vanishes and the fp32 estimate, already within 3e-7 lambda_max, is kept), and the logarithm of the float-rounded
+// determinant form is ill-conditioned and the kernel falls back to the fp64 closed form), and the logarithm of the float-rounded
 // lambda_max is taken in fp32.  The result differs from the fp64 closed form by less than the rounding of the float output
 // (tests: 2e-6 against the oracle).
+// out of line: the rare fallback of eigmax_sym3_mixed must not cost the hot kernel registers (fp64 acos / cos are large)
+__device__ __noinline__ double eigmax_sym3_rare(double c11, double c12, double c13, double c22, double c23, double c33)
+{
+    return eigmax_sym3(c11, c12, c13, c22, c23, c33);
+}
 __device__ __forceinline__ double eigmax_sym3_mixed(double c11, double c12, double c13, double c22, double c23, double c33)
 {
     // estimate: the trigonometric closed form in fp32 (the largest eigenvalue of a symmetric matrix is well conditioned: the
@@ -72,8 +77,12 @@ __device__ __forceinline__ double eigmax_sym3_mixed(double c11, double c12, doub
     const double gv = a11 * m1 - c12 * (c12 * a33 - c23 * c13) + c13 * (c12 * c23 - a22 * c13);
     const double gd = -(m1 + m2 + m3);
     const double step = gv / gd;
-    if (fabs(step) <= 1e-4 * (double)pf) lam -= step;          // false for NaN as well
-    return lam;
+    // The step measures the error e0 of the estimate: a few 1e-7 p far from a double root, about 1e-8 p / gap when the two largest
+    // eigenvalues nearly coincide (the determinant form loses digits there), and the polished value is then off by e0^2 / gap.  Up to
+    // e0 = 2e-5 p (relative gap above about 1e-3) that is below 5e-7 p, i.e. below the rounding of the float output; anything beyond
+    // takes the fp64 closed form (rare: FTLE near zero).  NaN fails the comparison and takes it too (and stays NaN).
+    if (fabs(step) <= 2e-5 * (double)pf) return lam - step;
+    return eigmax_sym3_rare(c11, c12, c13, c22, c23, c33);
 }
 template <typename T> __device__ __forceinline__ double log_for(double lam)
 {

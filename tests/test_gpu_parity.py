@@ -599,6 +599,33 @@ def test_cg_ftle_patterns_vs_oracle(lcs, oracle):
         assert cgn is None and np.allclose(cpu(ftn), fto, rtol=1e-12, atol=1e-12, equal_nan=True)
 
 
+def test_cg_ftle_float_near_double_root(lcs, oracle):
+    """DESIGN.md reading #35: for fp32 outputs the largest eigenvalue comes from an fp32 closed form polished by one fp64 Newton
+    step, which is ill-conditioned when the two largest eigenvalues of C nearly coincide; such seeds must take the fp64 closed
+    form.  Linear flow maps x -> R diag(s, s (1 + d), s3) x with relative gaps d from 1e-6 to 1e-1 (and an exact double and
+    triple root): FTLE within 2e-6 of the oracle on the same float flow map."""
+    import torch
+    ng = (12, 10, 8)
+    dx = (0.05, 0.04, 0.03)
+    k, j, i = np.meshgrid(np.arange(ng[2]), np.arange(ng[1]), np.arange(ng[0]), indexing="ij")
+    X = np.stack([i * dx[0], j * dx[1], k * dx[2]], axis=-1).reshape(-1, 3)
+    rng = np.random.default_rng(35)
+    worst = 0.0
+    for d in (0.0, 1e-6, 1e-5, 1e-4, 1e-3, 1e-2, 1e-1):
+        for s3 in (0.5, 1.0 if d == 0.0 else 0.9):
+            Q, _ = np.linalg.qr(rng.standard_normal((3, 3)))
+            A = Q @ np.diag([1.7, 1.7 * (1.0 + d), 1.7 * s3]) @ np.linalg.qr(rng.standard_normal((3, 3)))[0].T
+            F = (X @ A.T).astype(np.float32)
+            cgo, fto, sto = oracle.cg_ftle(3, ng, dx, (0, 0, 0), (0.0, 0.0, 0.0), F.astype(np.float64), None, 4.0)
+            cgg, ftg, stg = lcs.cg_ftle(3, ng, dx, (0, 0, 0), (0.0, 0.0, 0.0), torch.from_numpy(F).cuda(), None, 4.0)
+            ok = np.isfinite(fto)
+            assert np.array_equal(np.isfinite(cpu(ftg)), ok)
+            err = np.max(np.abs(cpu(ftg)[ok].astype(np.float64) - fto[ok]))
+            worst = max(worst, err)
+            assert np.allclose(cpu(ftg)[ok], fto[ok], rtol=2e-6, atol=2e-6), (d, s3, err)
+    print("cg_ftle float near a double root: worst |dFTLE| = %.2e" % worst)
+
+
 # -------------------------------------------------------------------------------------------------
 # integrator variants: re-bundled tracers and the paper's split (one kernel per RK4 stage) design
 @pytest.mark.parametrize("options", [dict(bundle=1), dict(bundle=1, bundle_steps=7), dict(bundle=1, ld256=0),
