@@ -132,7 +132,7 @@ lcs_status lcs_field_require_pair(lcs_field *f, int s, cudaStream_t st, const vo
 {
     if (s < 0 || s + 1 >= f->ns) { lcs_set_error("pair %d out of range", s); return LCS_ERR_INVALID_ARG; }
     f->pair_clock++;
-    for (int k = 0; k < lcs_field::kPairCache; ++k)
+    for (int k = 0; k < f->n_pair_cache; ++k)
         if (f->pair_snap[k] == s && f->pair_buf[k]) { f->pair_age[k] = f->pair_clock; *pair = f->pair_buf[k]; return LCS_OK; }
     int s0, s1;
     lcs_status rc = ensure_slot(f, s, s, s + 1, &s0);
@@ -140,7 +140,7 @@ lcs_status lcs_field_require_pair(lcs_field *f, int s, cudaStream_t st, const vo
     rc = ensure_slot(f, s + 1, s, s + 1, &s1);
     if (rc != LCS_OK) return rc;
     int k = 0;
-    for (int j = 1; j < lcs_field::kPairCache; ++j)
+    for (int j = 1; j < f->n_pair_cache; ++j)
         if (f->pair_age[j] < f->pair_age[k]) k = j;
     LCS_CUDA_OK(cudaStreamWaitEvent(st, f->slot_ready[s0], 0));
     LCS_CUDA_OK(cudaStreamWaitEvent(st, f->slot_ready[s1], 0));
@@ -359,7 +359,8 @@ extern "C" lcs_status lcs_field_create(const lcs_field_desc *d, lcs_field **out)
     if (e != cudaSuccess) { lcs_set_error("stream/event creation failed: %s", cudaGetErrorString(e)); lcs_field_destroy(f); return LCS_ERR_CUDA; }
     // the snapshot window and the pair-record cache are allocated here, once: the hot calls never allocate
     for (int k = 0; k < f->nslots && e == cudaSuccess; ++k) e = cudaMalloc(&f->slot[k], raw_bytes(f));
-    for (int k = 0; k < lcs_field::kPairCache && e == cudaSuccess; ++k) e = cudaMalloc(&f->pair_buf[k], pair_bytes(f));
+    if (!f->ring && f->ns - 1 <= lcs_field::kMaxPairCache && (size_t)(f->ns - 1) * pair_bytes(f) <= ((size_t)256 << 20)) f->n_pair_cache = f->ns - 1 > 4 ? f->ns - 1 : 4;
+    for (int k = 0; k < f->n_pair_cache && e == cudaSuccess; ++k) e = cudaMalloc(&f->pair_buf[k], pair_bytes(f));
     if (e != cudaSuccess) {
         lcs_set_error("allocating the snapshot window failed: %s", cudaGetErrorString(e));
         lcs_field_destroy(f);
@@ -377,7 +378,7 @@ extern "C" void lcs_field_destroy(lcs_field *f)
     for (cudaEvent_t ev : f->slot_ready) if (ev) cudaEventDestroy(ev);
     for (cudaEvent_t ev : f->slot_free) if (ev) cudaEventDestroy(ev);
     for (cudaEvent_t ev : f->win_ev) cudaEventDestroy(ev);
-    for (int k = 0; k < lcs_field::kPairCache; ++k) if (f->pair_buf[k]) cudaFree(f->pair_buf[k]);
+    for (int k = 0; k < f->n_pair_cache; ++k) if (f->pair_buf[k]) cudaFree(f->pair_buf[k]);
     if (f->scratch.buf) cudaFree(f->scratch.buf);
     for (FieldSet &fs : f->field_sets) if (fs.buf) cudaFree(fs.buf);
     if (f->h_seeds) cudaFree(f->h_seeds);
@@ -401,7 +402,7 @@ extern "C" lcs_status lcs_field_set_snapshot(lcs_field *f, int32_t s, const void
     if (!f || !vel) { lcs_set_error("null argument"); return LCS_ERR_INVALID_ARG; }
     if (s < 0 || s >= f->ns) { lcs_set_error("snapshot index %d out of range", s); return LCS_ERR_INVALID_ARG; }
     // any cached pair built from the old contents is stale
-    for (int k = 0; k < lcs_field::kPairCache; ++k)
+    for (int k = 0; k < f->n_pair_cache; ++k)
         if (f->pair_snap[k] == s || f->pair_snap[k] == s - 1) f->pair_snap[k] = -1;
     for (FieldSet &fs : f->field_sets)
         if (fs.pair == s || fs.pair == s - 1) { fs.pair = -1; fs.tau.clear(); }

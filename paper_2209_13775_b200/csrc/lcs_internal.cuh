@@ -103,6 +103,7 @@ struct FieldSet {
 };
 
 struct lcs_field {
+    lcs_field() { for (int k = 0; k < kMaxPairCache; ++k) pair_snap[k] = -1; }
     int dim = 0, kind = 0;
     int vel_dtype = 0, compute_dtype = 0;
     int P = 2;                    // padded components
@@ -125,10 +126,13 @@ struct lcs_field {
     std::vector<char> snap_set;
     std::vector<const void *> host_src;  // ring mode: retained host pointers
     // pair-record cache (built on the compute stream from two raw slots)
-    static constexpr int kPairCache = 4;
-    void *pair_buf[kPairCache] = {nullptr, nullptr, nullptr, nullptr};
-    int pair_snap[kPairCache] = {-1, -1, -1, -1};
-    int64_t pair_age[kPairCache] = {0, 0, 0, 0};
+    // 4 entries (a window and its neighbours), or one per snapshot pair when the whole series of pair records fits 256 MB
+    // (small fields: configs 1 and 2 then build every pair once instead of once per pass)
+    static constexpr int kMaxPairCache = 64;
+    int n_pair_cache = 4;
+    void *pair_buf[kMaxPairCache] = {};
+    int pair_snap[kMaxPairCache];
+    int64_t pair_age[kMaxPairCache] = {};
     int64_t pair_clock = 0;
     cudaStream_t side = nullptr;
     TracerScratch scratch;
