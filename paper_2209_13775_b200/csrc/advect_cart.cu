@@ -205,9 +205,43 @@ __device__ __forceinline__ bool cart_velocity(const CartDev &g, const PairRec<DI
 // ---------------------------------------------------------------------------------------------
 // seeds (physical, compute dtype) -> (cell, offset) state.  fp64 arithmetic, the oracle's O2 formula, so
 // the initial cell agrees with lcs_locate.  flag 2 = seed outside at t0.
+// sort key of a live tracer (the orders are described at cart_key_kernel below)
+template <int DIM, typename TC>
+__device__ __forceinline__ uint32_t cart_key_of(const CartDev &g, const int *ci, const TC *w, int shift, int order, uint32_t last_bin)
+{
+    int c[DIM];
+#pragma unroll
+    for (int a = 0; a < DIM; ++a) c[a] = (g.periodic[a] ? wrap_index(ci[a], g.n[a], g.pow2[a]) : ci[a]) >> shift;
+    const int m0 = ((g.n[0] - 1) >> shift) + 1, m1 = ((g.n[1] - 1) >> shift) + 1;
+    uint32_t k;
+    if (order == 2 && DIM == 3) {
+        const uint32_t m0p = (uint32_t)(m0 + 1) >> 1;
+        const uint32_t sub = ((w[DIM - 1] >= TC(0.5)) ? 8u : 0u) | ((w[1] >= TC(0.5)) ? 4u : 0u) | (((uint32_t)c[0] & 1u) << 1) |
+                             ((w[0] >= TC(0.5)) ? 1u : 0u);
+        k = (((uint32_t)c[0] >> 1) + m0p * ((uint32_t)c[1] + (uint32_t)m1 * (uint32_t)c[DIM - 1])) * 16u + sub;
+    } else if (order == 3 && DIM == 3) {
+        // bricks of 4 x 2 x 2 cells, x fastest inside and across bricks: 256 consecutive tracers then sit in a box of about
+        // 8 x 2 x 2 cells, whose records the staged integrator copies into shared memory as one small tile
+        const uint32_t mb0 = (uint32_t)(m0 + 3) >> 2, mb1 = (uint32_t)(m1 + 1) >> 1;
+        const uint32_t sub = ((uint32_t)c[0] & 3u) | (((uint32_t)c[1] & 1u) << 2) | (((uint32_t)c[DIM - 1] & 1u) << 3);
+        k = (((uint32_t)c[0] >> 2) + mb0 * (((uint32_t)c[1] >> 1) + mb1 * ((uint32_t)c[DIM - 1] >> 1))) * 16u + sub;
+    } else if (order >= 1) {
+        k = (uint32_t)c[0] + (uint32_t)m0 * ((uint32_t)c[1] + (DIM == 3 ? (uint32_t)m1 * (uint32_t)c[DIM - 1] : 0u));
+    } else {
+        k = bundle::morton<DIM>(c);
+    }
+    return k > last_bin - 1 ? last_bin - 1 : k;
+}
+
+struct KeyOut {                 // where a kernel leaves the sort key of its record for the NEXT re-bundling (key == nullptr: nowhere)
+    uint32_t *key, *cnt;
+    int shift, order;
+    uint32_t last_bin;
+};
+
 template <int DIM, typename TC>
 __global__ void __launch_bounds__(256) cart_init_kernel(CartDev g, const TC *__restrict__ seeds, int64_t n,
-                                                         CartTracer<DIM, TC> *__restrict__ st, int32_t orig_base = 0)
+                                                         CartTracer<DIM, TC> *__restrict__ st, int32_t orig_base = 0, KeyOut ko = KeyOut{})
 {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
@@ -229,6 +263,11 @@ __global__ void __launch_bounds__(256) cart_init_kernel(CartDev g, const TC *__r
     t.orig = orig_base + (int32_t)i;
     t.meta = fl << 30;
     store_record(st + i, t);
+    if (ko.key) {
+        const uint32_t k = fl ? ko.last_bin : cart_key_of<DIM, TC>(g, t.ci, t.w, ko.shift, ko.order, ko.last_bin);
+        ko.key[i] = k;
+        bundle::count_key(ko.cnt, k, ko.last_bin);
+    }
 }
 
 // (cell, offset) -> physical flow map + flags, scattered back to the caller's seed order
@@ -272,29 +311,7 @@ __global__ void __launch_bounds__(256) cart_key_kernel(CartDev g, const CartTrac
     const CartTracer<DIM, TC> t = load_record(st + i);
     uint32_t k = last_bin;
     if ((t.meta >> 30) == 3u) { key[i] = bundle::kDropKey; return; }       // record of a finished series volume: dropped by the sort
-    if ((t.meta >> 30) == 0) {
-        int c[DIM];
-#pragma unroll
-        for (int a = 0; a < DIM; ++a) c[a] = (g.periodic[a] ? wrap_index(t.ci[a], g.n[a], g.pow2[a]) : t.ci[a]) >> shift;
-        const int m0 = ((g.n[0] - 1) >> shift) + 1, m1 = ((g.n[1] - 1) >> shift) + 1;
-        if (order == 2 && DIM == 3) {
-            const uint32_t m0p = (uint32_t)(m0 + 1) >> 1;
-            const uint32_t sub = ((t.w[DIM - 1] >= TC(0.5)) ? 8u : 0u) | ((t.w[1] >= TC(0.5)) ? 4u : 0u) | (((uint32_t)c[0] & 1u) << 1) |
-                                 ((t.w[0] >= TC(0.5)) ? 1u : 0u);
-            k = (((uint32_t)c[0] >> 1) + m0p * ((uint32_t)c[1] + (uint32_t)m1 * (uint32_t)c[DIM - 1])) * 16u + sub;
-        } else if (order == 3 && DIM == 3) {
-            // bricks of 4 x 2 x 2 cells, x fastest inside and across bricks: 256 consecutive tracers then sit in a box of about
-            // 8 x 2 x 2 cells, whose records the staged integrator copies into shared memory as one small tile
-            const uint32_t mb0 = (uint32_t)(m0 + 3) >> 2, mb1 = (uint32_t)(m1 + 1) >> 1;
-            const uint32_t sub = ((uint32_t)c[0] & 3u) | (((uint32_t)c[1] & 1u) << 2) | (((uint32_t)c[DIM - 1] & 1u) << 3);
-            k = (((uint32_t)c[0] >> 2) + mb0 * (((uint32_t)c[1] >> 1) + mb1 * ((uint32_t)c[DIM - 1] >> 1))) * 16u + sub;
-        } else if (order >= 1) {
-            k = (uint32_t)c[0] + (uint32_t)m0 * ((uint32_t)c[1] + (DIM == 3 ? (uint32_t)m1 * (uint32_t)c[DIM - 1] : 0u));
-        } else {
-            k = bundle::morton<DIM>(c);
-        }
-        if (k > last_bin - 1) k = last_bin - 1;
-    }
+    if ((t.meta >> 30) == 0) k = cart_key_of<DIM, TC>(g, t.ci, t.w, shift, order, last_bin);
     key[i] = k;
     bundle::count_key(cnt, k, last_bin);
 }
@@ -462,21 +479,55 @@ __device__ __forceinline__ bool cart_velocity_xpair(const CartDev &g, const XPai
     return true;
 }
 
+// What the integrator does for a time series (lcs_advect_series) beyond integrating: records carry their own step count, every
+// record leaves its sort key for the next re-bundling (no separate key kernel over the set), and the records of the volume that
+// finishes with this launch (orig in [fin_lo, fin_hi)) write their outputs and drop out (no separate scan of the set).
+struct SeriesTail {
+    KeyOut ko;
+    int32_t fin_lo, fin_hi, N;
+    const float *seeds;
+    float *flowmap;
+    uint8_t *exit_flag;
+    int32_t *exit_step;
+};
+
+__device__ __forceinline__ void series_finish(const CartDev &g, const SeriesTail &sr, const CartTracer<3, float> &t)
+{
+    const uint32_t fl = t.meta >> 30;
+    const int64_t i = t.orig;
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+        sr.flowmap[i * 3 + a] = fl == 2 ? sr.seeds[(i - sr.fin_lo) * 3 + a] : (float)(g.origin[a] + ((double)t.ci[a] + (double)t.w[a]) * g.spacing[a]);
+    if (sr.exit_flag) sr.exit_flag[i] = (uint8_t)fl;
+    if (sr.exit_step) sr.exit_step[i] = fl == 0 ? sr.N : (fl == 2 ? 0 : (int32_t)(t.meta & 0x3fffffffu));
+}
+
 // Step s of the chunk reads the blended fields 2s (ta), 2s+1 (tb), 2s+2 (tc = ta of step s+1): the host only uses this
 // kernel for chunks whose stage times have exactly that structure, so the field addresses are warp-uniform arithmetic.
-template <bool FASTWRAP>
+template <bool FASTWRAP, bool SERIES>
 __global__ void __launch_bounds__(256)
 cart_xpair_kernel(const __grid_constant__ CartDev g, const XPair *__restrict__ fields, int64_t field_stride,
                   int nsteps, int first_step, int64_t n, CartTracer<3, float> *__restrict__ st, float hs0, float hs1, float hs2,
-                  int per_tracer_steps)
+                  const __grid_constant__ SeriesTail sr)
 {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     CartTracer<3, float> t = load_record(st + i);
-    if ((t.meta >> 30) != 0) return;
+    if ((t.meta >> 30) != 0) {
+        if constexpr (SERIES) {                                // a parked record of the set: it still needs its key, or its exit
+            if (sr.ko.key) {
+                const bool fin = t.orig >= sr.fin_lo && t.orig < sr.fin_hi;
+                if (fin) series_finish(g, sr, t);
+                const uint32_t k = fin ? bundle::kDropKey : sr.ko.last_bin;
+                sr.ko.key[i] = k;
+                if (!fin) bundle::count_key(sr.ko.cnt, k, sr.ko.last_bin);
+            }
+        }
+        return;
+    }
     // series mode: tracers of several volumes, each at its own step count, share the launch: a live record carries the steps it
     // has completed in the low bits of meta (otherwise those are zero while the tracer lives)
-    if (per_tracer_steps) first_step = (int)(t.meta & 0x3fffffffu);
+    if constexpr (SERIES) first_step = (int)(t.meta & 0x3fffffffu);
     const float hs[3] = {hs0, hs1, hs2};
     int ci[3];
     float w[3];
@@ -519,7 +570,20 @@ cart_xpair_kernel(const __grid_constant__ CartDev g, const XPair *__restrict__ f
 #pragma unroll
     for (int a = 0; a < 3; ++a) { t.ci[a] = ci[a]; t.w[a] = w[a]; }
     if (!ok) t.meta = (1u << 30) | (uint32_t)(first_step + s);
-    else if (per_tracer_steps) t.meta = (uint32_t)(first_step + nsteps);
+    else if (SERIES) t.meta = (uint32_t)(first_step + nsteps);
+    if constexpr (SERIES) {
+        if (sr.ko.key) {
+            const bool fin = t.orig >= sr.fin_lo && t.orig < sr.fin_hi;
+            if (fin) {
+                series_finish(g, sr, t);
+                sr.ko.key[i] = bundle::kDropKey;
+                return;                                        // the record is not needed any more
+            }
+            const uint32_t k = ok ? cart_key_of<3, float>(g, ci, w, sr.ko.shift, sr.ko.order, sr.ko.last_bin) : sr.ko.last_bin;
+            sr.ko.key[i] = k;
+            bundle::count_key(sr.ko.cnt, k, sr.ko.last_bin);
+        }
+    }
     store_record(st + i, t);
 }
 
@@ -1216,11 +1280,11 @@ lcs_status cart_advect_impl(lcs_field *f, int64_t n, const void *seeds_, double 
                         LCS_LAUNCH(cart_xpair_tma_kernel, lcs_blocks(n, kStageBlock), kStageBlock, smem, st, g, (const XPair *)fields, f->nrec, u.count,
                                    u.first, n, cur, hs[0], hs[1], hs[2], cap);
                     } else if (fast)
-                        LCS_LAUNCH((cart_xpair_kernel<true>), lcs_blocks(n, block), block, 0, st, g, (const XPair *)fields, f->nrec,
-                                   u.count, u.first, n, cur, hs[0], hs[1], hs[2], 0);
+                        LCS_LAUNCH((cart_xpair_kernel<true, false>), lcs_blocks(n, block), block, 0, st, g, (const XPair *)fields, f->nrec,
+                                   u.count, u.first, n, cur, hs[0], hs[1], hs[2], SeriesTail{});
                     else
-                        LCS_LAUNCH((cart_xpair_kernel<false>), lcs_blocks(n, block), block, 0, st, g, (const XPair *)fields, f->nrec,
-                                   u.count, u.first, n, cur, hs[0], hs[1], hs[2], 0);
+                        LCS_LAUNCH((cart_xpair_kernel<false, false>), lcs_blocks(n, block), block, 0, st, g, (const XPair *)fields, f->nrec,
+                                   u.count, u.first, n, cur, hs[0], hs[1], hs[2], SeriesTail{});
                 }
                 bool last_blend_of_win = true;
                 for (size_t uj = ui + 1; uj < units.size() && units[uj].win == u.win; ++uj) last_blend_of_win = last_blend_of_win && !units[uj].blend;
@@ -1395,24 +1459,41 @@ lcs_status cart_advect_series_batched(lcs_field *f, const SeriesPlan &P, int64_t
         LCS_CUDA_OK(cudaGetLastError());
         return LCS_OK;
     };
+    // fused bookkeeping (the usual series: at most one volume finishes per layer): the integrator leaves every record's sort key
+    // for the next re-bundling and writes the outputs of the finishing volume itself; otherwise a key kernel per layer and a scan of
+    // the set per finished volume
+    bool fused = true;
+    for (const SeriesPlan::Layer &ly : P.layers) fused = fused && ly.finish_vols.size() <= 1;
+    const KeyOut ko{d_key, d_cnt, L.shift, L.order, (uint32_t)(L.nbins - 1)};
+    if (fused) LCS_CUDA_OK(cudaMemsetAsync(d_cnt, 0, (size_t)L.nbins * 4, st));
     for (size_t li = 0; li < P.layers.size(); ++li) {
         const SeriesPlan::Layer &ly = P.layers[li];
         const SeriesPlan::Unit &u = P.units[ly.unit];
         // volumes that completed their last unit in the previous layer leave; volumes whose first unit this is join
-        rc = finalize(to_finish);
-        if (rc != LCS_OK) return rc;
-        const int64_t dropped = (int64_t)to_finish.size() * n;
-        to_finish.clear();
+        int64_t dropped = 0;
+        if (!fused) {
+            rc = finalize(to_finish);
+            if (rc != LCS_OK) return rc;
+            dropped = (int64_t)to_finish.size() * n;
+            to_finish.clear();
+        } else if (li > 0) {
+            dropped = (int64_t)P.layers[li - 1].finish_vols.size() * n;
+        }
         for (int k : ly.start_vols) {
-            LCS_LAUNCH((cart_init_kernel<3, float>), lcs_blocks(n, 256), 256, 0, st, g, seeds, n, cur + n_act, (int32_t)(k * n));
+            KeyOut kn = ko;
+            kn.key = fused ? d_key + n_act : nullptr;
+            LCS_LAUNCH((cart_init_kernel<3, float>), lcs_blocks(n, 256), 256, 0, st, g, seeds, n, cur + n_act, (int32_t)(k * n), kn);
             n_act += n;
         }
         // re-bundle the whole set (drops the dead records)
-        LCS_CUDA_OK(cudaMemsetAsync(d_cnt, 0, (size_t)L.nbins * 4, st));
-        LCS_LAUNCH((cart_key_kernel<3, float>), lcs_blocks(n_act, 256), 256, 0, st, g, cur, n_act, L.shift, L.order, (uint32_t)(L.nbins - 1), d_key, d_cnt);
+        if (!fused) {
+            LCS_CUDA_OK(cudaMemsetAsync(d_cnt, 0, (size_t)L.nbins * 4, st));
+            LCS_LAUNCH((cart_key_kernel<3, float>), lcs_blocks(n_act, 256), 256, 0, st, g, cur, n_act, L.shift, L.order, (uint32_t)(L.nbins - 1), d_key, d_cnt);
+        }
         bundle::sort_records<Tracer>(cur, alt, d_key, d_cnt, d_tile, n_act, L.nbins, st);
         std::swap(cur, alt);
         n_act -= dropped;
+        if (fused) LCS_CUDA_OK(cudaMemsetAsync(d_cnt, 0, (size_t)L.nbins * 4, st));      // histogram of the NEXT re-bundling
         if (ly.pair != cur_pair) {
             if (cur_pair >= 0) { rc = lcs_field_release_raw(f, cur_pair, st); if (rc != LCS_OK) return rc; }
             rc = lcs_field_acquire_raw(f, ly.pair, st, &raw_a, &raw_b);
@@ -1429,17 +1510,25 @@ lcs_status cart_advect_series_batched(lcs_field *f, const SeriesPlan &P, int64_t
         }
         LCS_LAUNCH(blend_xpair_kernel, lcs_blocks(f->nrec, 256), 256, 0, st, (const float *)raw_a, (const float *)raw_b, g.n[0], g.n[1], g.n[2],
                    f->cart.np[0], f->cart.np[1], f->cart.np[2], d_ftau, u.nfields, fields, f->nrec);
+        SeriesTail sr{};
+        sr.N = (int32_t)N;
+        if (fused) {
+            sr.ko = ko;
+            sr.fin_lo = sr.fin_hi = 0;
+            if (!ly.finish_vols.empty()) { sr.fin_lo = (int32_t)(ly.finish_vols[0] * n); sr.fin_hi = (int32_t)((ly.finish_vols[0] + 1) * n); }
+            sr.seeds = seeds; sr.flowmap = flowmaps; sr.exit_flag = exit_flags; sr.exit_step = exit_steps;
+        }
         {
             WindowTimer timer(f, st);
             if (fast)
-                LCS_LAUNCH((cart_xpair_kernel<true>), lcs_blocks(n_act, block), block, 0, st, g, (const XPair *)fields, f->nrec, u.count, 0, n_act, cur,
-                           hs[0], hs[1], hs[2], 1);
+                LCS_LAUNCH((cart_xpair_kernel<true, true>), lcs_blocks(n_act, block), block, 0, st, g, (const XPair *)fields, f->nrec, u.count, 0, n_act, cur,
+                           hs[0], hs[1], hs[2], sr);
             else
-                LCS_LAUNCH((cart_xpair_kernel<false>), lcs_blocks(n_act, block), block, 0, st, g, (const XPair *)fields, f->nrec, u.count, 0, n_act, cur,
-                           hs[0], hs[1], hs[2], 1);
+                LCS_LAUNCH((cart_xpair_kernel<false, true>), lcs_blocks(n_act, block), block, 0, st, g, (const XPair *)fields, f->nrec, u.count, 0, n_act, cur,
+                           hs[0], hs[1], hs[2], sr);
         }
         LCS_CUDA_OK(cudaGetLastError());
-        to_finish = ly.finish_vols;
+        if (!fused) to_finish = ly.finish_vols;
     }
     rc = finalize(to_finish);
     if (rc != LCS_OK) return rc;
