@@ -119,6 +119,14 @@ lcs_status lcs_field_reserve(lcs_field *f, int64_t n_seeds, int64_t n_steps);
  * "ld256" 0/1 = gather each 32-byte node record with one 256-bit load; "block" = threads per block;
  * "time_windows" 0/1 = record CUDA events around the integrator launches (read with lcs_field_get_info). */
 lcs_status lcs_field_set_option(lcs_field *f, const char *key, int64_t value);
+/* Counters and sizes.  Keys: "n_nodes", "n_cells", "n_bins", "n_boundary_faces" (mesh); "ring", "windows" (snapshot windows visited),
+ * "h2d_bytes" (snapshot bytes uploaded so far), "scratch_bytes" (reserved tracer scratch); "locate_fallbacks", "locate_random_walks",
+ * "locate_hops", "locate_max_hops" (canonical walks of lcs_locate and of the seeds; the first two stay 0 on the seeded inputs),
+ * "walk_fallbacks" (in-advect walks that gave up and were re-located with the canonical predicate), "walk_cap_hits" (tracers
+ * interpolated in a cell that does not hold them: 0 by construction); "field_set_hits", "field_set_misses"; "series_layers" (batched
+ * layers of the last lcs_advect_series, 0 = integrated volume by volume); "window_launches", "window_time_ns" (with option
+ * "time_windows": integrator launches bracketed by CUDA events and their summed duration; reading the latter synchronises).
+ * Errors: LCS_ERR_INVALID_ARG for an unknown key.                                                                            */
 lcs_status lcs_field_get_info(const lcs_field *f, const char *key, int64_t *value);
 
 /* Cell containing each position ("computes which cell ... each seed point is located in";
