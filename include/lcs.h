@@ -277,7 +277,10 @@ typedef enum {
     LCS_PEAK_SMEM_CONTIGUOUS = 10,    /* shared memory, LDS.128, lane L reads chunk base + L (conflict-free)        */
     LCS_PEAK_SMEM_RECORDS = 11,       /* shared memory, lane L reads the 32-byte record base + L as 2 x LDS.128     */
     LCS_PEAK_SMEM_RECORDS_SWIZZLED = 12, /* ... with the 16-byte chunks laid out as TMA's 32-byte swizzle does      */
-    LCS_PEAK_SMEM_RECORDS_SAME = 13   /* ... swizzled, the 4 lanes of a group read the same record (broadcast)      */
+    LCS_PEAK_SMEM_RECORDS_SAME = 13,  /* ... swizzled, the 4 lanes of a group read the same record (broadcast)      */
+    LCS_PEAK_L1_GATHER_WARP_SAME = 14,   /* L1-resident 256-bit gathers, the whole warp reads one record             */
+    LCS_PEAK_L1_GATHER_WARP_LINE = 15,   /* ... the whole warp reads the four records of one 128-byte line           */
+    LCS_PEAK_L1_GATHER_WARP_2LINES = 16  /* ... two lines, 16 lanes each                                             */
 } lcs_peak_kind;
 lcs_status lcs_measure_peak(int32_t kind, double *value);
 

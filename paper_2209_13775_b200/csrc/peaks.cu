@@ -88,7 +88,10 @@ template <int MODE> __global__ void __launch_bounds__(256) l1_gather_kernel(cons
             uint32_t r;
             if (MODE == 0) r = ((hash32(r0 + (lane >> 2)) << 2) + (lane & 3)) & kRecMask;
             else if (MODE == 1) r = (hash32(r0 + (lane >> 2)) << 2) & kRecMask;
-            else r = ((hash32(r0 + lane) << 2)) & kRecMask;
+            else if (MODE == 2) r = ((hash32(r0 + lane) << 2)) & kRecMask;
+            else if (MODE == 3) r = (r0 << 2) & kRecMask;                                    // the whole warp reads one record
+            else if (MODE == 4) r = ((r0 << 2) + (lane & 3)) & kRecMask;                     // ... the 4 records of one line
+            else r = ((hash32(r0 + (lane >> 4)) << 2) + (lane & 3)) & kRecMask;             // ... two lines, 16 lanes each
             asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
                          : "=f"(v[u][0]), "=f"(v[u][1]), "=f"(v[u][2]), "=f"(v[u][3]), "=f"(v[u][4]), "=f"(v[u][5]), "=f"(v[u][6]), "=f"(v[u][7])
                          : "l"(rec + 8 * r));
@@ -229,13 +232,19 @@ extern "C" lcs_status lcs_measure_peak(int32_t kind, double *value)
     }
     case LCS_PEAK_L1_GATHER_LINE:
     case LCS_PEAK_L1_GATHER_SAME:
-    case LCS_PEAK_L1_GATHER_SPREAD: {
+    case LCS_PEAK_L1_GATHER_SPREAD:
+    case LCS_PEAK_L1_GATHER_WARP_SAME:
+    case LCS_PEAK_L1_GATHER_WARP_LINE:
+    case LCS_PEAK_L1_GATHER_WARP_2LINES: {
         const int iters = 2000, blocks = kSMs * 8;
         if (cudaMalloc(&buf, 64 << 10) != cudaSuccess) { lcs_set_error("out of memory"); return done(LCS_ERR_OOM); }
         cudaMemset(buf, 0, 64 << 10);
         if (kind == LCS_PEAK_L1_GATHER_LINE) rc = time_best([&] { LCS_LAUNCH((l1_gather_kernel<0>), blocks, 256, 0, 0, (const float *)buf, out, iters); }, &ms);
         else if (kind == LCS_PEAK_L1_GATHER_SAME) rc = time_best([&] { LCS_LAUNCH((l1_gather_kernel<1>), blocks, 256, 0, 0, (const float *)buf, out, iters); }, &ms);
-        else rc = time_best([&] { LCS_LAUNCH((l1_gather_kernel<2>), blocks, 256, 0, 0, (const float *)buf, out, iters); }, &ms);
+        else if (kind == LCS_PEAK_L1_GATHER_SPREAD) rc = time_best([&] { LCS_LAUNCH((l1_gather_kernel<2>), blocks, 256, 0, 0, (const float *)buf, out, iters); }, &ms);
+        else if (kind == LCS_PEAK_L1_GATHER_WARP_SAME) rc = time_best([&] { LCS_LAUNCH((l1_gather_kernel<3>), blocks, 256, 0, 0, (const float *)buf, out, iters); }, &ms);
+        else if (kind == LCS_PEAK_L1_GATHER_WARP_LINE) rc = time_best([&] { LCS_LAUNCH((l1_gather_kernel<4>), blocks, 256, 0, 0, (const float *)buf, out, iters); }, &ms);
+        else rc = time_best([&] { LCS_LAUNCH((l1_gather_kernel<5>), blocks, 256, 0, 0, (const float *)buf, out, iters); }, &ms);
         *value = 32.0 * blocks * 256 * iters / (ms * 1e-3) / 1e9;
         break;
     }

@@ -26,7 +26,8 @@ EXPORTS = ["lcs_field_create", "lcs_field_set_snapshot", "lcs_field_sync", "lcs_
            "lcs_ftle_host", "lcs_ftle_series_host", "lcs_measure_peak", "lcs_kernel_launch_count", "lcs_last_error"]
 PEAK_KINDS = {"fp32_fma_tflops": 0, "fp64_fma_tflops": 1, "launch_us": 2, "hbm_copy_gbs": 3, "l2_seq_gbs": 4, "l2_sector_gbs": 5,
               "hbm_sector_gbs": 6, "l1_gather_line_gbs": 7, "l1_gather_same_gbs": 8, "l1_gather_spread_gbs": 9,
-              "smem_contiguous_gbs": 10, "smem_records_gbs": 11, "smem_records_swizzled_gbs": 12, "smem_records_same_gbs": 13}
+              "smem_contiguous_gbs": 10, "smem_records_gbs": 11, "smem_records_swizzled_gbs": 12, "smem_records_same_gbs": 13,
+              "l1_gather_warp_same_gbs": 14, "l1_gather_warp_line_gbs": 15, "l1_gather_warp_2lines_gbs": 16}
 
 
 class LcsError(RuntimeError):
