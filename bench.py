@@ -300,9 +300,17 @@ def run_config(args, lcs, cfg, steps, warmup, rank, world, local, with_e2e, with
         k, v = kv.split("=")
         field.set_option(k, int(v))
     tdt = torch.float32 if w.compute_dtype == np.float32 else torch.float64
-    seeds_h = torch.from_numpy(w.seeds()).pin_memory()
+    slab = args.shard == "volume" and cfg in (3, 4)      # ONE volume across the ranks: seed slabs along the slowest axis + a halo layer
+    seeds_all = w.seeds()
+    if slab:
+        from paper_2209_13775_b200 import shard
+        runs = [make_workload(cfg, 0)[1][0]]             # every rank works on the same volume
+        plane = int(w.ng[0]) * (int(w.ng[1]) if w.dim == 3 else 1)
+        k0, k1 = shard.slab_range(int(w.ng[w.dim - 1]), rank, world)
+        seeds_all = np.ascontiguousarray(seeds_all[k0 * plane:k1 * plane])
+    seeds_h = torch.from_numpy(seeds_all).pin_memory()
     seeds_d = seeds_h.cuda()
-    n = w.n_seeds
+    n = seeds_h.shape[0]
     flow = torch.empty_like(seeds_d)
     flag = torch.empty(n, dtype=torch.uint8, device="cuda")
     es = torch.empty(n, dtype=torch.int32, device="cuda")
@@ -331,7 +339,10 @@ def run_config(args, lcs, cfg, steps, warmup, rank, world, local, with_e2e, with
             field.set_option("field_sets_clear", 0)      # every pass starts without resident blended fields: reuse only WITHIN a pass
         for (t0, tf, h) in runs:
             field.advect(seeds_d, t0, tf, h, flowmap=flow, exit_flag=flag, exit_step=es, reserve=False)
-            lcs.cg_ftle(w.dim, w.ng, w.seed_spacing, w.seed_periodic, w.period, flow, flag, tf - t0, want_cg=True, want_status=False)
+            if slab:
+                shard.cg_ftle_slab(lcs, w.dim, w.ng, w.seed_spacing, w.seed_periodic, w.period, flow, flag, tf - t0, rank, world, want_cg=True)
+            else:
+                lcs.cg_ftle(w.dim, w.ng, w.seed_spacing, w.seed_periodic, w.period, flow, flag, tf - t0, want_cg=True, want_status=False)
             if count is not None:
                 count.append(float(es.sum(dtype=torch.int64).item()))
 
@@ -388,7 +399,7 @@ def run_config(args, lcs, cfg, steps, warmup, rank, world, local, with_e2e, with
     # end to end through the C-ABI with HOST buffers: H2D of the seeds, D2H of the Cauchy-Green tensor and the FTLE inside the
     # timed region (the same outputs the device-timed pass writes)
     e2e = None
-    if with_e2e:
+    if with_e2e and not slab:                            # (--shard volume: the host-buffer call has no halo exchange; device-timed only)
         ncg = 3 if w.dim == 2 else 6
         ftle_h = torch.empty(n, dtype=tdt).pin_memory()
         cg_h = torch.empty((n, ncg), dtype=tdt).pin_memory()
@@ -437,10 +448,11 @@ def run_config(args, lcs, cfg, steps, warmup, rank, world, local, with_e2e, with
         l2_note = ("flushed: a 256 MB buffer is written between timed passes (working set %.1f MB < L2)" % (state_bytes / 1e6)) if flush else \
                   ("inputs larger than L2: tracer records, seeds, outputs and fields are %.0f MB per pass" % (state_bytes / 1e6))
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warmup,
-                "ms_per_step": sec_per_step * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "ms_per_step": sec_per_step * 1e3, "higher_is_better": True, "scaling": "strong" if slab else "weak", "vs_baseline": None,
                 "dtype": "f32" if w.compute_dtype == np.float32 else "f64", "data": "synthetic",
                 "config": {"workload": w.name, "baseline_config": cfg, "seeds": n * len(runs), "rk4_steps": w.n_steps,
-                           "seed_steps_per_pass": steps_per_pass, "parallelism": "independent FTLE volumes per rank, no collective",
+                           "seed_steps_per_pass": steps_per_pass, "parallelism": ("one volume in %d seed slabs, one halo layer of flow map exchanged before lcs_cg_ftle" % world) if slab else
+                                          "independent FTLE volumes per rank, no collective",
                            "options": dict(kv.split("=") for kv in args.option), "l2": l2_note,
                            **({"series": "lcs_advect_series: %d volumes, overlapping ones advanced together" % len(runs)} if series else {}),
                            **({"snapshot_ring_slots": ring, "h2d_snapshot_bytes_total": int(field.info("h2d_bytes"))} if cfg == 5 else {})},
@@ -466,6 +478,9 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--option", action="append", default=[], help="library option key=value (e.g. integrator=2)")
+    ap.add_argument("--shard", default="volumes", choices=["volumes", "volume"],
+                    help="N > 1: 'volumes' = an independent FTLE volume per rank (weak scaling, no collective); 'volume' = ONE volume of "
+                         "config 3 / 4 split into seed slabs with a halo exchange of the flow map before lcs_cg_ftle (strong scaling)")
     ap.add_argument("--cfg5-ring", type=int, default=4, help="config 5: device slots of the snapshot ring (0 = every snapshot resident, no streaming)")
     ap.add_argument("--cfg5-mode", default="series", choices=["series", "volumes"],
                     help="config 5: lcs_advect_series (overlapping volumes advanced together) or one lcs_advect per volume with resident field sets")

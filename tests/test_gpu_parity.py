@@ -626,6 +626,56 @@ def test_cg_ftle_float_near_double_root(lcs, oracle):
     print("cg_ftle float near a double root: worst |dFTLE| = %.2e" % worst)
 
 
+@pytest.mark.parametrize("case", ["periodic3d_f32", "open3d_f32_flags", "open2d_f64"])
+def test_cg_ftle_slabs_with_halo_equal_the_whole_grid(lcs, oracle, case, monkeypatch):
+    """One volume across ranks (paper_2209_13775_b200/shard.py): every rank's lcs_cg_ftle on its seed slab extended
+    by one halo layer of flow map and flags equals the whole-grid lcs_cg_ftle on the rank's own seeds -- bit for bit on open axes
+    (flags 0/1/2 included), to the rounding of F + period in the flow map's type for the layers at a periodic seam.  The ranks are
+    emulated one after the other on one GPU: the exchange is replaced by cuts from the global arrays (the exchange itself is
+    tested with gloo in tests/test_multi_rank.py)."""
+    import torch
+    from paper_2209_13775_b200 import shard
+    rng = np.random.default_rng(81)
+    if case == "periodic3d_f32":
+        dim, ng, per, period, dt = 3, (12, 10, 9), (1, 1, 1), (1.2, 1.0, 0.9), np.float32
+    elif case == "open3d_f32_flags":
+        dim, ng, per, period, dt = 3, (11, 9, 8), (0, 0, 0), (0.0, 0.0, 0.0), np.float32
+    else:
+        dim, ng, per, period, dt = 2, (16, 13), (0, 0), (0.0, 0.0), np.float64
+    dx = tuple(0.1 for _ in range(dim))
+    n = int(np.prod(ng))
+    idx = np.stack(np.meshgrid(*[np.arange(m) for m in ng[::-1]], indexing="ij"), -1).reshape(-1, dim)[:, ::-1]
+    F = (idx * 0.1 + 0.05 * np.sin(3.0 * idx * 0.1 + 0.3) + 0.01 * rng.standard_normal((n, dim))).astype(dt)
+    flag = (rng.random(n) < (0.15 if "flags" in case else 0.0)).astype(np.uint8) * rng.integers(1, 3, n).astype(np.uint8)
+    Fd, fd = torch.from_numpy(F).cuda(), torch.from_numpy(flag).cuda()
+    cg0, ft0, st0 = lcs.cg_ftle(dim, ng, dx, per, period, Fd, fd, 2.0, want_cg=True, want_status=True)
+    plane = n // ng[dim - 1]
+    F3, f3 = Fd.view(ng[dim - 1], plane, dim), fd.view(ng[dim - 1], plane)
+    for world in (1, 2, 3):
+        for rank in range(world):
+            k0, k1 = shard.slab_range(ng[dim - 1], rank, world)
+
+            def fake_exchange(Fs, fs, r, w, periodic, group=None, k0=k0, k1=k1):
+                nz = ng[dim - 1]
+                lo = (F3[(k0 - 1) % nz], f3[(k0 - 1) % nz]) if (periodic or k0 > 0) else None
+                hi = (F3[k1 % nz], f3[k1 % nz]) if (periodic or k1 < nz) else None
+                return lo, hi
+            monkeypatch.setattr(shard, "exchange_halo", fake_exchange)
+            cg, ft, st = shard.cg_ftle_slab(lcs, dim, ng, dx, per, period, F3[k0:k1].reshape(-1, dim).contiguous(), f3[k0:k1].reshape(-1).contiguous(),
+                                            2.0, rank, world, want_cg=True, want_status=True)
+            a, b = k0 * plane, k1 * plane
+            assert torch.equal(st, st0[a:b]), (case, world, rank)
+            if per[dim - 1]:
+                ok = torch.isfinite(ft0[a:b])
+                assert torch.allclose(ft[ok], ft0[a:b][ok], rtol=2e-5, atol=2e-6) and torch.allclose(cg[ok], cg0[a:b][ok], rtol=2e-4, atol=2e-5)
+                inner = slice(plane, (k1 - k0 - 1) * plane)                # layers that do not touch the seam-shifted halo
+                if rank not in (0, world - 1) and k1 - k0 > 2:
+                    assert torch.equal(ft[inner], ft0[a:b][inner])
+            else:
+                assert torch.equal(torch.nan_to_num(ft, nan=-1.0), torch.nan_to_num(ft0[a:b], nan=-1.0)), (case, world, rank)
+                assert torch.equal(torch.nan_to_num(cg, nan=-1.0), torch.nan_to_num(cg0[a:b], nan=-1.0))
+
+
 # -------------------------------------------------------------------------------------------------
 # integrator variants: re-bundled tracers and the paper's split (one kernel per RK4 stage) design
 @pytest.mark.parametrize("options", [dict(bundle=1), dict(bundle=1, bundle_steps=7), dict(bundle=1, ld256=0),

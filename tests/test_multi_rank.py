@@ -68,3 +68,64 @@ def test_rank_shards_are_independent_volumes_of_equal_size(monkeypatch):
         tiny = getattr(I, name)(ng=(8, 4)) if cfg == 1 else I.config2(ng=(8, 4), lattice=(9, 5))
         monkeypatch.setattr(I, name, lambda *a, _t=tiny, **k: _t)
         assert bench.make_workload(cfg, 0)[1] == bench.make_workload(cfg, 5)[1]
+
+
+# -------------------------------------------------------------------------------------------------
+# one volume across ranks: seed slabs + one halo layer of the flow map (paper_2209_13775_b200/shard.py)
+def test_slab_ranges_and_neighbours():
+    sys.path.insert(0, ROOT)
+    from paper_2209_13775_b200 import shard
+    for n, world in ((256, 8), (10, 3), (7, 7), (5, 2)):
+        r = [shard.slab_range(n, k, world) for k in range(world)]
+        assert r[0][0] == 0 and r[-1][1] == n and all(r[k][1] == r[k + 1][0] for k in range(world - 1))
+        sizes = [b - a for a, b in r]
+        assert min(sizes) >= 1 and max(sizes) - min(sizes) <= 1
+    assert shard.neighbours(0, 4, False) == (None, 1) and shard.neighbours(3, 4, False) == (2, None)
+    assert shard.neighbours(0, 4, True) == (3, 1) and shard.neighbours(3, 4, True) == (2, 0) and shard.neighbours(0, 1, True) == (0, 0)
+
+
+def _halo_worker(rank, world, port, periodic, out):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    sys.path.insert(0, ROOT)
+    import torch
+    import torch.distributed as dist
+    from paper_2209_13775_b200 import shard
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        nz, plane, dim, period = 7, 12, 3, 6.5
+        g = torch.Generator().manual_seed(7)
+        F = torch.rand((nz, plane, dim), generator=g, dtype=torch.float32)          # the global flow map, same on every rank
+        flag = (torch.rand((nz, plane), generator=g) < 0.2).to(torch.uint8)
+        k0, k1 = shard.slab_range(nz, rank, world)
+        lo, hi = shard.exchange_halo(F[k0:k1].contiguous(), flag[k0:k1].contiguous(), rank, world, periodic)
+        Fe, fe, n_lo = shard.extend_with_halo(F[k0:k1], flag[k0:k1], lo, hi, dim - 1, period, periodic and rank == 0, periodic and rank == world - 1)
+        # what the extended slab must be, cut from the global arrays
+        idx = list(range(k0 - 1, k1 + 1))
+        keep = [k for k in idx if periodic or 0 <= k < nz]
+        ref_F = torch.stack([F[k % nz].clone() for k in keep])
+        for j, k in enumerate(keep):
+            if k < 0: ref_F[j, :, dim - 1] -= period
+            if k >= nz: ref_F[j, :, dim - 1] += period
+        ref_f = torch.stack([flag[k % nz] for k in keep])
+        ok = bool(torch.equal(Fe, ref_F) and torch.equal(fe, ref_f) and n_lo == (1 if keep[0] == k0 - 1 else 0))
+        out.put((rank, ok, tuple(Fe.shape)))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("world,periodic", [(2, False), (2, True), (3, True)])
+def test_halo_exchange_gloo(world, periodic):
+    """Every rank's slab, extended by the layers it receives, equals the same layers cut from the global flow map (with the
+    period added across the seam): world 2 open, world 2 periodic (both neighbours are the same rank), world 3 periodic."""
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 31500 + (os.getpid() + 17 * world + int(periodic)) % 2000
+    procs = [ctx.Process(target=_halo_worker, args=(r, world, port, periodic, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    res = sorted(q.get(timeout=120) for _ in procs)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert all(ok for _, ok, _ in res), res
