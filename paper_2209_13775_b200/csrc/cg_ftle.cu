@@ -189,7 +189,7 @@ __global__ void __launch_bounds__(256) cg_ftle_kernel(const __grid_constant__ Cg
 // one-sided differences happens on the float operands before ONE widening subtraction per entry, and C leaves in three 64-bit
 // stores.  Same rule (reading #12) and the same fp64 arithmetic for the differences, C and the eigenvalue algebra.
 // Requires 3 n < 2^31 (32-bit element offsets).
-__global__ void __launch_bounds__(256) cg_ftle3f_kernel(const __grid_constant__ CgGrid g, const float *__restrict__ F, const uint8_t *__restrict__ flag,
+__global__ void __launch_bounds__(256, 6) cg_ftle3f_kernel(const __grid_constant__ CgGrid g, const float *__restrict__ F, const uint8_t *__restrict__ flag,
                                                          float *__restrict__ cg, float *__restrict__ ftle, uint8_t *__restrict__ status)
 {
     const int i0 = (int)(blockIdx.x * blockDim.x + threadIdx.x);
