@@ -189,7 +189,7 @@ __global__ void __launch_bounds__(256) cg_ftle_kernel(const __grid_constant__ Cg
 // one-sided differences happens on the float operands before ONE widening subtraction per entry, and C leaves in three 64-bit
 // stores.  Same rule (reading #12) and the same fp64 arithmetic for the differences, C and the eigenvalue algebra.
 // Requires 3 n < 2^31 (32-bit element offsets).
-__global__ void __launch_bounds__(256, 6) cg_ftle3f_kernel(const __grid_constant__ CgGrid g, const float *__restrict__ F, const uint8_t *__restrict__ flag,
+template <bool PER_ALL> __global__ void __launch_bounds__(256, 6) cg_ftle3f_kernel(const __grid_constant__ CgGrid g, const float *__restrict__ F, const uint8_t *__restrict__ flag,
                                                          float *__restrict__ cg, float *__restrict__ ftle, uint8_t *__restrict__ status)
 {
     const int i0 = (int)(blockIdx.x * blockDim.x + threadIdx.x);
@@ -208,8 +208,8 @@ __global__ void __launch_bounds__(256, 6) cg_ftle3f_kernel(const __grid_constant
     for (int b = 0; b < 3; ++b) {
         atp[b] = ijk[b] + 1 >= nn[b];
         atm[b] = ijk[b] == 0;
-        okp[b] = !atp[b] || g.per[b];
-        okm[b] = !atm[b] || g.per[b];
+        okp[b] = PER_ALL || !atp[b] || g.per[b];               // PER_ALL: every axis wraps, every neighbour is in the grid
+        okm[b] = PER_ALL || !atm[b] || g.per[b];
         jp[b] = okp[b] ? idx + (atp[b] ? 1 - nn[b] : 1) * stride[b] : idx;        // a valid address in every case
         jm[b] = okm[b] ? idx + (atm[b] ? nn[b] - 1 : -1) * stride[b] : idx;
         if (flag) { okp[b] = okp[b] && flag[jp[b]] == 0; okm[b] = okm[b] && flag[jm[b]] == 0; }
@@ -585,7 +585,9 @@ extern "C" lcs_status lcs_cg_ftle(int32_t dim, int32_t dtype, const int32_t ng[3
     if (dim == 2 && dtype == LCS_F64) LCS_LAUNCH((cg_ftle_kernel<2, double, false>), grid3, block3, 0, st, g, (const double *)flowmap, exit_flag, (double *)cg, (double *)ftle, status, n, (double *)nullptr, 0.0);
     else if (dim == 2) LCS_LAUNCH((cg_ftle_kernel<2, float, false>), grid3, block3, 0, st, g, (const float *)flowmap, exit_flag, (float *)cg, (float *)ftle, status, n, (float *)nullptr, 0.0);
     else if (dtype == LCS_F64) LCS_LAUNCH((cg_ftle_kernel<3, double, false>), grid3, block3, 0, st, g, (const double *)flowmap, exit_flag, (double *)cg, (double *)ftle, status, n, (double *)nullptr, 0.0);
-    else if (3 * n < (1LL << 31)) LCS_LAUNCH(cg_ftle3f_kernel, grid3, block3, 0, st, g, (const float *)flowmap, exit_flag, (float *)cg, (float *)ftle, status);
+    else if (3 * n < (1LL << 31) && g.per[0] && g.per[1] && g.per[2])
+        LCS_LAUNCH(cg_ftle3f_kernel<true>, grid3, block3, 0, st, g, (const float *)flowmap, exit_flag, (float *)cg, (float *)ftle, status);
+    else if (3 * n < (1LL << 31)) LCS_LAUNCH(cg_ftle3f_kernel<false>, grid3, block3, 0, st, g, (const float *)flowmap, exit_flag, (float *)cg, (float *)ftle, status);
     else LCS_LAUNCH((cg_ftle_kernel<3, float, false>), grid3, block3, 0, st, g, (const float *)flowmap, exit_flag, (float *)cg, (float *)ftle, status, n, (float *)nullptr, 0.0);
     LCS_CUDA_OK(cudaGetLastError());
     return LCS_OK;
