@@ -266,7 +266,12 @@ def roofline_block(lcs, cfg, w, kernel_s, units_per_launch, share, win_launches,
         peak_key = "smem_records_swizzled_gbs" if staged else "l1_gather_line_gbs"
         if delivered:
             ach = delivered * rate / 1e9
+            busy = prof.get("l1_data_pipe_pct")
             return {"bound": "l1", "kernel": kern, "achieved": ach, "peak": pk[peak_key], "unit": "GB/s", "frac": ach / pk[peak_key],
+                    "binding_resource_busy": (max(busy) / 100.0 if busy and not staged else None),
+                    "binding_resource_busy_note": "l1tex__data_pipe_lsu_wavefronts, % of peak, from the committed ncu table of this kernel "
+                                                  "(SURVEY.md 8.3: the binding roofline is the resource with the highest % of its peak); `frac` "
+                                                  "counts only the bytes the gathers usefully deliver",
                     "bytes_to_registers_per_seed_step": delivered,
                     "note": "L1 / shared-memory data pipe (128 B per clock per SM into registers): bytes the kernel's gathers actually deliver to "
                             "registers per seed-step (ncu request counts, profiles/) x rate, over the measured best-case gather rate (%s)" % peak_key,
