@@ -106,7 +106,8 @@ lcs_status lcs_field_reserve(lcs_field *f, int64_t n_seeds, int64_t n_steps);
  * "bundle" -1 = auto, 0 = off, 1 = on: re-bundle tracers by cell (Morton order of the cell index) so that a
  * warp gathers from neighbouring cells; results are returned in the caller's order;
  * "bundle_steps" k = re-bundle every k RK4 steps (0 = once per snapshot window; unstructured meshes: every 160 steps);
- * "bundle_order" / "simplex_order" 0 = Morton, 1 = row-major (x fastest, default) sort key over cells / bins ("bundle_order" 2 = pairs of
+ * "bundle_order" / "simplex_order" 0 = Morton, 1 = row-major (x fastest) sort key over cells / bins; "bundle_order" -1 (default) = Morton for the
+ * pre-blended integrator, row-major otherwise; "simplex_order" defaults to 1 ("bundle_order" 2 = pairs of
  * x-neighbouring cells split by sub-cell octant, 3 = bricks of 4 x 2 x 2 cells; both 3D Cartesian only);
  * "field_sets" m = keep the blended fields of the last m chunks resident (about 7 GB each for a 128^3 grid and 50-step chunks)
  * and reuse them when a later lcs_advect needs the same snapshot pair and stage times (FTLE time series: volumes released one

@@ -435,7 +435,7 @@ extern "C" lcs_status lcs_field_set_option(lcs_field *f, const char *key, int64_
     if (!strcmp(key, "integrator") && value >= 0 && value <= 3) f->opt_integrator = value;
     else if (!strcmp(key, "bundle") && value >= -1 && value <= 1) f->opt_bundle = value;
     else if (!strcmp(key, "bundle_steps") && value >= 0) f->opt_bundle_steps = value;
-    else if (!strcmp(key, "bundle_order") && value >= 0 && value <= 3) f->opt_bundle_order = value;
+    else if (!strcmp(key, "bundle_order") && value >= -1 && value <= 3) f->opt_bundle_order = value;
     else if (!strcmp(key, "simplex_order") && (value == 0 || value == 1)) f->opt_simplex_order = value;
     else if (!strcmp(key, "tma") && value >= 0 && value <= 2) f->opt_tma = value;
     else if (!strcmp(key, "tma_cap") && value >= 64 && value <= 3500) {

@@ -151,7 +151,8 @@ struct lcs_field {
     // options
     int64_t opt_integrator = 0;   // 0 auto, 1 fused, 2 split
     int64_t opt_bundle = -1;      // re-bundle tracers by cell: -1 auto (large seed sets), 0 off, 1 on
-    int64_t opt_bundle_order = 1; // Cartesian sort key: 0 = Morton code of the cell, 1 = row-major cell index (x fastest; +8% on config 3)
+    int64_t opt_bundle_order = -1; // Cartesian sort key: -1 = auto (Morton for the pre-blended integrator, whose gathers bypass L1 allocation and live on L2
+                                   // locality; row-major otherwise), 0 = Morton code of the cell, 1 = row-major cell index (x fastest), 2 / 3: see lcs.h
     int64_t opt_simplex_order = 1; // simplex sort key over the bin grid: 0 = Morton, 1 = row-major
     int64_t opt_bundle_steps = 0; // RK4 steps between re-bundlings (0 = once per snapshot window)
     int64_t opt_preblend = -1;    // 3D fp32 Cartesian: gather from per-stage-time blended fields (-1 auto, 0 off, 1 on)
