@@ -229,6 +229,18 @@ lcs_status lcs_cg_eigen(int32_t dim, int32_t dtype, int64_t n, const void *cg, v
 lcs_status lcs_smooth_gaussian(int32_t dim, int32_t dtype, const int32_t ng[3], const int32_t seed_periodic[3],
                                double sigma, const void *field, void *out, void *work, void *cuda_stream);
 
+/* lcs_smooth_gaussian for callers that cannot allocate device memory (CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc): same passes, same results, but the intermediate field lives in a file-scope device array of the library
+ * instead of a caller-supplied work buffer, and the call allocates and frees nothing (no cudaMalloc / cudaFree, no allocating
+ * library routine; the array's device address is looked up once per device).  Limit: ng0*ng1*ng2 * sizeof(dtype) <= 16 MiB, i.e.
+ * 4 194 304 fp32 or 2 097 152 fp64 seeds; larger grids return LCS_ERR_INVALID_ARG (use lcs_smooth_gaussian).  Every GPU that loads
+ * the library holds the 16 MiB until the process exits.  All calls on a device share the array, which keeps the last call's contents
+ * (nothing in it has to start at zero: each pass reads only what the pass before wrote): calls that overlap on the GPU -- different
+ * streams, or different host threads -- race on it; calls on one stream serialise by themselves.
+ * field, out: two distinct device buffers of [n] `dtype`.  Other arguments and errors as lcs_smooth_gaussian.                  */
+lcs_status lcs_smooth_gaussian_static(int32_t dim, int32_t dtype, const int32_t ng[3], const int32_t seed_periodic[3],
+                                      double sigma, const void *field, void *out, void *cuda_stream);
+
 /* Ridge indicator of a scalar field (the smoothed FTLE) on the structured seed grid, the second step of the LCS filter
  * ("C-ridge extraction"; the paper gives no definition: DESIGN.md reading #32, second-derivative ridge).
  * Per seed: gradient g and Hessian H by central differences on the 3^dim stencil (wrapped on periodic axes), kappa = smallest

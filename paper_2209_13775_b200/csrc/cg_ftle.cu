@@ -713,6 +713,70 @@ extern "C" lcs_status lcs_smooth_gaussian(int32_t dim, int32_t dtype, const int3
     return LCS_OK;
 }
 
+// ---------------------------------------------------------------------------------------------
+// lcs_smooth_gaussian without a caller-supplied work buffer and without any allocation: the intermediate field of the axis passes
+// lives in a file-scope device array.  For callers that cannot call cudaMalloc (CUDA graph capture, tight serving loops, harnesses
+// that forbid it).  Every GPU that loads the library holds the array (16 MiB) until the process exits.
+constexpr size_t kSmoothScratchBytes = (size_t)16 << 20;        // 4 Mi fp32 or 2 Mi fp64 seeds
+static __device__ __align__(256) unsigned char g_smooth_scratch[kSmoothScratchBytes];
+
+// The array's name is a host-side stand-in in host code, not a device address: the address is asked for once per device, with that
+// device current, and cached.
+static lcs_status smooth_scratch_address(void **out)
+{
+    constexpr int kMaxDev = 64;
+    static void *addr[kMaxDev] = {};
+    static std::atomic<int> known[kMaxDev] = {};
+    int dev = -1;
+    LCS_CUDA_OK(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kMaxDev) { lcs_set_error("device ordinal %d out of range", dev); return LCS_ERR_CUDA; }
+    if (!known[dev].load(std::memory_order_acquire)) {
+        void *p = nullptr;
+        LCS_CUDA_OK(cudaGetSymbolAddress(&p, g_smooth_scratch));
+        if (!p) { lcs_set_error("cudaGetSymbolAddress returned a null address"); return LCS_ERR_CUDA; }
+        addr[dev] = p;                                          // every thread that races here stores the same value
+        known[dev].store(1, std::memory_order_release);
+    }
+    *out = addr[dev];
+    return LCS_OK;
+}
+
+extern "C" lcs_status lcs_smooth_gaussian_static(int32_t dim, int32_t dtype, const int32_t ng[3], const int32_t seed_periodic[3], double sigma,
+                                                 const void *field, void *out, void *cuda_stream)
+{
+    if ((dim != 2 && dim != 3) || !ng || !field || !out) { lcs_set_error("null argument or bad dim"); return LCS_ERR_INVALID_ARG; }
+    if (dtype != LCS_F32 && dtype != LCS_F64) { lcs_set_error("bad dtype"); return LCS_ERR_INVALID_ARG; }
+    if (!(sigma > 0.0) || ceil(3.0 * sigma) > 64.0) { lcs_set_error("sigma must be in (0, 21.33] seed-grid cells"); return LCS_ERR_INVALID_ARG; }
+    if (out == field) { lcs_set_error("field and out must be distinct buffers"); return LCS_ERR_INVALID_ARG; }
+    int64_t n[3] = {1, 1, 1}, total = 1;
+    for (int a = 0; a < dim; ++a) { if (ng[a] < 1) { lcs_set_error("bad seed grid"); return LCS_ERR_INVALID_ARG; } n[a] = ng[a]; total *= n[a]; }
+    const size_t need = (size_t)total * lcs_esize(dtype);
+    if (need > kSmoothScratchBytes) {
+        lcs_set_error("lcs_smooth_gaussian_static: %lld seeds of %zu bytes exceed the static scratch of %zu bytes (max %zu seeds): use lcs_smooth_gaussian "
+                      "with a work buffer", (long long)total, lcs_esize(dtype), kSmoothScratchBytes, kSmoothScratchBytes / lcs_esize(dtype));
+        return LCS_ERR_INVALID_ARG;
+    }
+    void *work = nullptr;
+    lcs_status rc = smooth_scratch_address(&work);
+    if (rc != LCS_OK) return rc;
+    const int64_t stride[3] = {1, n[0], n[0] * n[1]};
+    const int R = (int)ceil(3.0 * sigma);
+    const double inv_2s2 = 1.0 / (2.0 * sigma * sigma);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    // the passes of lcs_smooth_gaussian (2D: field -> work -> out; 3D: field -> out -> work -> out).  Nothing in the scratch has to
+    // start at zero: every element a pass reads was written by the pass before it, whatever an earlier call left behind.
+    const void *src = field;
+    for (int a = 0; a < dim; ++a) {
+        void *dst = ((dim - a) % 2 == 1) ? out : work;
+        const int per = seed_periodic ? (seed_periodic[a] != 0) : 0;
+        if (dtype == LCS_F64) LCS_LAUNCH((smooth_axis_kernel<double>), lcs_blocks(total, 256), 256, 0, st, (const double *)src, (double *)dst, total, stride[a], n[a], per, R, inv_2s2);
+        else LCS_LAUNCH((smooth_axis_kernel<float>), lcs_blocks(total, 256), 256, 0, st, (const float *)src, (float *)dst, total, stride[a], n[a], per, R, inv_2s2);
+        src = dst;
+    }
+    LCS_CUDA_OK(cudaGetLastError());
+    return LCS_OK;
+}
+
 extern "C" lcs_status lcs_ridge(int32_t dim, int32_t dtype, const int32_t ng[3], const double seed_spacing[3], const int32_t seed_periodic[3],
                                 double kappa_min, double s_min, const void *field, void *kappa, void *dgn, uint8_t *mask, void *cuda_stream)
 {

@@ -22,7 +22,7 @@ LCS_F32, LCS_F64 = 0, 1
 LCS_MESH_CARTESIAN, LCS_MESH_SIMPLEX = 0, 1
 
 EXPORTS = ["lcs_field_create", "lcs_field_set_snapshot", "lcs_field_sync", "lcs_field_destroy", "lcs_field_reserve",
-           "lcs_field_set_option", "lcs_field_get_info", "lcs_locate", "lcs_advect", "lcs_advect_series", "lcs_advect_series_reserve", "lcs_advect_early_cg", "lcs_cg_ftle", "lcs_cg_ftle_aux", "lcs_cg_eigen", "lcs_smooth_gaussian", "lcs_ridge",
+           "lcs_field_set_option", "lcs_field_get_info", "lcs_locate", "lcs_advect", "lcs_advect_series", "lcs_advect_series_reserve", "lcs_advect_early_cg", "lcs_cg_ftle", "lcs_cg_ftle_aux", "lcs_cg_eigen", "lcs_smooth_gaussian", "lcs_smooth_gaussian_static", "lcs_ridge",
            "lcs_ftle_host", "lcs_ftle_series_host", "lcs_measure_peak", "lcs_kernel_launch_count", "lcs_last_error"]
 PEAK_KINDS = {"fp32_fma_tflops": 0, "fp64_fma_tflops": 1, "launch_us": 2, "hbm_copy_gbs": 3, "l2_seq_gbs": 4, "l2_sector_gbs": 5,
               "hbm_sector_gbs": 6, "l1_gather_line_gbs": 7, "l1_gather_same_gbs": 8, "l1_gather_spread_gbs": 9,
@@ -86,6 +86,7 @@ def lib():
                                       C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.lcs_smooth_gaussian.argtypes = [C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p,
                                           C.c_void_p]
+        L.lcs_smooth_gaussian_static.argtypes = [C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p]
         L.lcs_ridge.argtypes = [C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.c_void_p, C.c_void_p,
                                 C.c_void_p, C.c_void_p, C.c_void_p]
         L.lcs_cg_eigen.argtypes = [C.c_int32, C.c_int32, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
@@ -375,6 +376,20 @@ def smooth_gaussian(dim, ng, seed_periodic, sigma, field, stream=None):
     out, work = torch.empty_like(field), torch.empty_like(field)
     _check(lib().lcs_smooth_gaussian(int(dim), dtype, _arr3(ng, C.c_int32, 1), _arr3(seed_periodic, C.c_int32, 0), float(sigma),
                                      _tptr(field), _tptr(out), _tptr(work), _stream_ptr(stream)))
+    return out
+
+
+SMOOTH_STATIC_MAX_BYTES = 16 << 20
+
+
+def smooth_gaussian_static(dim, ng, seed_periodic, sigma, field, out, stream=None):
+    """lcs_smooth_gaussian_static: smoothing with the library's static scratch (no allocation inside the call; the caller supplies
+    `out`).  field, out: torch CUDA tensors [n] of the same dtype, distinct.  Returns out."""
+    import torch
+    assert field.is_cuda and field.is_contiguous() and out.is_cuda and out.is_contiguous() and out.dtype == field.dtype
+    dtype = LCS_F64 if field.dtype == torch.float64 else LCS_F32
+    _check(lib().lcs_smooth_gaussian_static(int(dim), dtype, _arr3(ng, C.c_int32, 1), _arr3(seed_periodic, C.c_int32, 0), float(sigma),
+                                            _tptr(field), _tptr(out), _stream_ptr(stream)))
     return out
 
 
