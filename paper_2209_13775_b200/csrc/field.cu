@@ -26,6 +26,11 @@ void lcs_set_error(const char *fmt, ...)
     va_end(ap);
 }
 
+// no C++ exception crosses the boundary (std::vector storage of the window plan, of the field-set keys, ...)
+#define LCS_GUARD(...)                                                                           \
+    try { __VA_ARGS__ } catch (const std::bad_alloc &) { lcs_set_error("host allocation failed"); return LCS_ERR_OOM; } \
+    catch (...) { lcs_set_error("unexpected C++ exception"); return LCS_ERR_CUDA; }
+
 extern "C" const char *lcs_last_error(void) { return g_err; }
 extern "C" int64_t lcs_kernel_launch_count(void) { return g_lcs_launches.load(); }
 
@@ -278,7 +283,13 @@ lcs_status lcs_plan_windows(const lcs_field *f, double t0, double h, int64_t N, 
 }
 
 // ---------------------------------------------------------------------------------------------
+static lcs_status field_create_impl(const lcs_field_desc *d, lcs_field **out);
 extern "C" lcs_status lcs_field_create(const lcs_field_desc *d, lcs_field **out)
+{
+    LCS_GUARD(return field_create_impl(d, out);)
+}
+
+static lcs_status field_create_impl(const lcs_field_desc *d, lcs_field **out)
 {
     if (out) *out = nullptr;
     if (!d || !out) { lcs_set_error("null argument"); return LCS_ERR_INVALID_ARG; }
@@ -459,7 +470,13 @@ extern "C" lcs_status lcs_field_set_option(lcs_field *f, const char *key, int64_
     return LCS_OK;
 }
 
+static lcs_status field_get_info_impl(const lcs_field *f, const char *key, int64_t *value);
 extern "C" lcs_status lcs_field_get_info(const lcs_field *f, const char *key, int64_t *value)
+{
+    LCS_GUARD(return field_get_info_impl(f, key, value);)
+}
+
+static lcs_status field_get_info_impl(const lcs_field *f, const char *key, int64_t *value)
 {
     if (!f || !key || !value) { lcs_set_error("null argument"); return LCS_ERR_INVALID_ARG; }
     if (!strcmp(key, "windows")) *value = f->info_windows;
@@ -534,11 +551,6 @@ static lcs_status check_interval(const lcs_field *f, double t0, double tf, doubl
     *N = n;
     return LCS_OK;
 }
-
-// no C++ exception crosses the boundary (std::vector storage of the window plan, of the field-set keys, ...)
-#define LCS_GUARD(...)                                                                           \
-    try { __VA_ARGS__ } catch (const std::bad_alloc &) { lcs_set_error("host allocation failed"); return LCS_ERR_OOM; } \
-    catch (...) { lcs_set_error("unexpected C++ exception"); return LCS_ERR_CUDA; }
 
 extern "C" lcs_status lcs_field_reserve(lcs_field *f, int64_t n_seeds, int64_t n_steps)
 {
